@@ -1,0 +1,145 @@
+/*
+ * genga.h -- C-ABI of the B200-native hybrid symplectic integrator
+ * (Grimm & Stadel, "The GENGA code", arxiv 1404.2324; line numbers refer to PAPER.md).
+ *
+ * One context = one simulation in one of the paper's three modes:
+ *   mode 0  up to 2048 massive bodies about one central mass,
+ *   mode 1  up to 32 massive bodies plus up to 10^6 massless test particles (L334-342),
+ *   mode 2  up to 100000 independent systems of up to 16 bodies each (L344-376).
+ * Every step of the method runs in CUDA kernels on the stream given at creation; this
+ * library never falls back to the CPU.  It needs an sm_100a device.
+ *
+ * Body layout (all modes): SoA, Ntot = n_massive + n_test (modes 0,1) or
+ * n_systems * n_massive (mode 2; body index = system * n_massive + k).
+ * 3-vectors are stored as x[c * Ntot + i], c = 0,1,2.  Massive bodies come first.
+ *
+ * Coordinates at the boundary are HELIOCENTRIC positions and HELIOCENTRIC velocities;
+ * internally the integrator works in democratic coordinates (heliocentric positions,
+ * barycentric velocities, L69).  Units: whatever makes G the value given in the config
+ * (G = 1 with AU, M_sun, day/k).
+ *
+ * Ownership: the caller owns every buffer, including the workspace and the stream; the
+ * context owns only a small host structure.  "device" / "host" below says where a
+ * pointer must point.  Buffers passed to a call may be reused once the work the call
+ * enqueued has completed on the stream (the *_host variants and genga_energy /
+ * genga_encounters / genga_status synchronise the stream before returning).
+ *
+ * Errors: every call returns 0 or a negative genga_error.  Conditions detected on the
+ * device during genga_step (Kepler or Bulirsch-Stoer non-convergence, pair list
+ * overflow) are latched in a device word and returned by the next synchronising call
+ * (genga_status, genga_get_state_host, genga_energy, genga_encounters).
+ */
+#ifndef GENGA_H
+#define GENGA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct genga_ctx genga_ctx;
+
+typedef enum {
+    GENGA_OK = 0,
+    GENGA_EINVAL = -1,    /* bad mode / sizes / order / dt == 0 / NULL pointer / workspace too small */
+    GENGA_ECAPACITY = -2, /* candidate or encounter pair list exceeded max_pairs */
+    GENGA_EKEPLER = -3,   /* universal-variable Kepler solver did not converge */
+    GENGA_EBS = -4,       /* Bulirsch-Stoer step size underflow */
+    GENGA_ECUDA = -5      /* a CUDA runtime call failed (see genga_last_cuda_error) */
+} genga_error;
+
+enum { GENGA_MODE_MASSIVE = 0, GENGA_MODE_TEST_PARTICLE = 1, GENGA_MODE_MULTI_SYSTEM = 2 };
+
+typedef struct {
+    int32_t mode;       /* GENGA_MODE_*                                                      */
+    int32_t n_massive;  /* per system: 1..2048 (mode 0), 1..32 (mode 1), 1..16 (mode 2); L188  */
+    int64_t n_test;     /* mode 1 only: 0..10^6 test particles; else 0                        */
+    int32_t n_systems;  /* mode 2 only: 1..100000; else 1                                     */
+    int32_t flags;      /* bit 0: do not merge the closing and the next opening kick (L144,
+                           L266); the result is the same map, this only selects the schedule  */
+    double G;           /* gravitational constant                                            */
+    double n1, n2;      /* critical-radius parameters of Eq. 6 (L94-96); usually 3 and 0.4   */
+    double bs_eps;      /* Bulirsch-Stoer relative tolerance (L116 "machine precision")      */
+    int64_t max_pairs;  /* capacity of the candidate list and of the encounter list          */
+    void *workspace;    /* device memory, >= genga_workspace_bytes(), 256-byte aligned        */
+    size_t workspace_bytes;
+    void *stream;       /* cudaStream_t; NULL = the legacy default stream                     */
+} genga_config;
+
+/* Bytes of device workspace a context with this config needs (workspace fields ignored).
+ * Returns 0 if the config is invalid. */
+size_t genga_workspace_bytes(const genga_config *cfg);
+
+/* Create / destroy a context.  genga_create does not touch the device state arrays;
+ * call genga_set_state before anything else. */
+int genga_create(const genga_config *cfg, genga_ctx **out);
+int genga_destroy(genga_ctx *ctx);
+
+/* Load the state (problem statement: L69, L188, L316-324, L352).
+ *   m0[n_systems]  central masses; m[Ntot] masses (0 for test particles); radius[Ntot]
+ *   physical radii (stored; collisions are not on this path); x[3*Ntot], v[3*Ntot]
+ *   heliocentric positions / velocities.
+ * genga_set_state: all pointers DEVICE.  genga_set_state_host: all pointers HOST (pinned
+ * or pageable); the copies are enqueued on the stream and the call returns after they and
+ * the conversion to democratic coordinates have completed. */
+int genga_set_state(genga_ctx *ctx, const double *m0, const double *m, const double *radius,
+                    const double *x, const double *v);
+int genga_set_state_host(genga_ctx *ctx, const double *m0, const double *m, const double *radius,
+                         const double *x, const double *v);
+
+/* Advance n_steps time steps of length dt (dt < 0 integrates backwards) with the hybrid
+ * symplectic scheme of order 2 (Eq. 7; per-step algorithm), 4 or 6
+ * (Yoshida compositions, L168-170).  Each step: critical radii (Eq. 6), kick with the
+ * changeover weight and prechecker (Eq. 2), Sun kick (Eq. 3), Kepler drift (Eq. 9),
+ * encounter search (Eq. 10-12), grouping (Appendix), Bulirsch-Stoer on the groups (L116),
+ * Sun kick, kick.  Work is enqueued on the stream; the call does not synchronise. */
+int genga_step(genga_ctx *ctx, int64_t n_steps, double dt, int order);
+
+/* Read the state back as heliocentric x[3*Ntot], v[3*Ntot].  DEVICE pointers (enqueued,
+ * no sync) or HOST pointers (synchronises; returns a latched device error if any). */
+int genga_get_state(genga_ctx *ctx, double *x, double *v);
+int genga_get_state_host(genga_ctx *ctx, double *x, double *v);
+
+/* Total energy E[n_systems] and angular momentum L[3*n_systems] (x,y,z per system) of the
+ * current state, Eq. 1-3 summed (L73-80).  HOST pointers; synchronises.  L may be NULL. */
+int genga_energy(genga_ctx *ctx, double *E, double *L);
+
+/* Close-encounter data of the LAST drift substep executed (L118-142, L276-284):
+ *   pairs[2*cap]  confirmed pairs (i, j), i < j, global body indices, sorted by (i, j);
+ *                 at most cap are written;   *n_pairs = number confirmed;
+ *   *n_candidates = number of prechecker candidates of that substep;
+ *   group_label[Ntot] (or NULL): lowest body index of the body's encounter group, the
+ *                 body's own index if it is in no group.
+ * HOST pointers; synchronises. */
+int genga_encounters(genga_ctx *ctx, int32_t *pairs, int64_t cap, int64_t *n_pairs,
+                     int64_t *n_candidates, int32_t *group_label);
+
+/* Synchronise the stream and return (and clear) the latched device error, or GENGA_OK. */
+int genga_status(genga_ctx *ctx);
+
+/* ---- auxiliary entry points: single operators of the path, for tests and kernel timing ---- */
+
+/* Critical radii for a step dt at the current state (Eq. 6) and the kick accelerations
+ * a[3*Ntot] of operator B there (Eq. 2 with the changeover weight); also refreshes the
+ * candidate list.  a, rcrit DEVICE pointers (rcrit may be NULL).  Enqueues, no sync. */
+int genga_accelerations(genga_ctx *ctx, double dt, double *a, double *rcrit);
+
+/* Kepler drift (Eq. 9, universal variables) of n independent bodies about mu for time h:
+ * x[3*n], v[3*n] DEVICE, updated in place.  Stand-alone: needs no state in the context. */
+int genga_kepler_drift(genga_ctx *ctx, int64_t n, double mu, double h, double *x, double *v);
+
+/* Counters accumulated since genga_create, HOST out[8]:
+ *  0 steps, 1 force evaluations, 2 ordered pair interactions evaluated, 3 kernel launches,
+ *  4 groups integrated, 5 largest group, 6 BS steps accepted, 7 candidates seen.
+ * Synchronises. */
+int genga_counters(genga_ctx *ctx, int64_t *out);
+
+const char *genga_strerror(int code);
+const char *genga_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GENGA_H */

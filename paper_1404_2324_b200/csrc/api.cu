@@ -1,0 +1,471 @@
+// C-ABI of the library (include/genga.h): context, workspace carving, the per-step kernel
+// sequence captured once into a CUDA graph and replayed, so that a step
+// never returns to the host (the paper's Sync/Copy overheads, L204/L274, are designed out:
+// every count stays in device memory and is read by the next kernel).
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <tuple>
+#include <utility>
+#include <vector>
+
+#include "../../include/genga.h"
+#include "kernels.cuh"
+
+using namespace genga;
+
+static thread_local char g_cuda_err[256] = "";
+
+#define CK(call)                                                                             \
+    do {                                                                                     \
+        cudaError_t e_ = (call);                                                             \
+        if (e_ != cudaSuccess) {                                                             \
+            snprintf(g_cuda_err, sizeof g_cuda_err, "%s:%d %s: %s", __FILE__, __LINE__, #call, \
+                     cudaGetErrorString(e_));                                                \
+            return GENGA_ECUDA;                                                              \
+        }                                                                                    \
+    } while (0)
+
+struct GraphKey {
+    double dt; int order; int nsteps;
+    bool operator<(const GraphKey &o) const { return std::tie(dt, order, nsteps) < std::tie(o.dt, o.order, o.nsteps); }
+};
+
+struct genga_ctx {
+    genga_config cfg;
+    DevState d;
+    cudaStream_t st;
+    int sms;
+    int *exp_labels;            // device [np]
+    double *eout;               // device [4*nsys]
+    struct GraphEntry { cudaGraphExec_t exec; long long launches; };
+    std::map<GraphKey, GraphEntry> graphs;
+    long long steps, force_evals, interactions, launches;
+    long long acc;              // launches enqueued (or captured) since last reset
+};
+
+static inline size_t up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+static bool valid_cfg(const genga_config *c)
+{
+    if (!c) return false;
+    if (c->mode == GENGA_MODE_MASSIVE) { if (c->n_massive < 1 || c->n_massive > 2048 || c->n_test != 0) return false; }
+    else if (c->mode == GENGA_MODE_TEST_PARTICLE) { if (c->n_massive < 1 || c->n_massive > 32 || c->n_test < 0 || c->n_test > 1000000) return false; }
+    else if (c->mode == GENGA_MODE_MULTI_SYSTEM) { if (c->n_massive < 1 || c->n_massive > 16 || c->n_systems < 1 || c->n_systems > 100000 || c->n_test != 0) return false; }
+    else return false;
+    if (!(c->G > 0.0) || c->n1 < 0.0 || c->n2 < 0.0 || !(c->bs_eps > 0.0) || c->max_pairs < 1) return false;
+    return true;
+}
+
+// Lay the workspace out.  base == nullptr: only compute the size.
+static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_labels, double **eout, int sms)
+{
+    size_t off = 0;
+    auto take = [&](size_t bytes) { char *p = base ? base + off : nullptr; off += up(bytes, 256); return p; };
+    const int nsys = c->mode == GENGA_MODE_MULTI_SYSTEM ? c->n_systems : 1;
+    const long long ntot = c->mode == GENGA_MODE_MULTI_SYSTEM ? (long long)nsys * c->n_massive : c->n_massive + c->n_test;
+    const int np = (int)up((size_t)ntot, 128), nm = c->n_massive;
+    const int npm = (int)up((size_t)nm, 128);
+    DevState t;
+    memset(&t, 0, sizeof t);
+    t.mode = c->mode; t.nm = nm; t.ntot = (int)ntot; t.nsys = nsys; t.np = np; t.npm = npm;
+    t.nmtot = c->mode == GENGA_MODE_MULTI_SYSTEM ? (int)ntot : nm;
+    t.G = c->G; t.n1 = c->n1; t.n2 = c->n2; t.eps = c->bs_eps; t.cap = c->max_pairs;
+    double **arrs[] = {&t.x, &t.y, &t.z, &t.vx, &t.vy, &t.vz, &t.m, &t.radius, &t.rc, &t.c9,
+                       &t.x0, &t.y0, &t.z0, &t.vx0, &t.vy0, &t.vz0};
+    for (auto a : arrs) *a = (double *)take(sizeof(double) * np);
+    t.m0 = (double *)take(sizeof(double) * nsys);
+    t.psum = (double *)take(sizeof(double) * 4 * nsys);
+    *eout = (double *)take(sizeof(double) * 4 * nsys);
+    if (c->mode != GENGA_MODE_MULTI_SYSTEM) {
+        int ib = (nm + KP_THREADS * KP_TI - 1) / (KP_THREADS * KP_TI);
+        int smin = (nm + KP_MAXJ - 1) / KP_MAXJ;
+        int s = std::min(std::max(1, sms / ib), (nm + 7) / 8);
+        t.nslice = std::max(smin, s);
+        t.apart = (double *)take(sizeof(double) * (size_t)t.nslice * 3 * npm);
+        t.gstart = (int *)take(sizeof(int) * npm);
+        t.gsize = (int *)take(sizeof(int) * npm);
+        t.gmem = (int *)take(sizeof(int) * npm);
+        t.gmask = (unsigned *)take(sizeof(unsigned) * 32);
+    }
+    if (c->mode == GENGA_MODE_MASSIVE && nm > 32) {
+        t.bss.stride = npm;
+        t.bss.base = (double *)take(sizeof(double) * (size_t)BSA_COUNT * npm);
+    }
+    if (c->mode == GENGA_MODE_TEST_PARTICLE) {
+        size_t nt = (size_t)std::max<long long>(c->n_test, 1);
+        t.tpmask = (unsigned *)take(sizeof(unsigned) * nt);
+        t.tplist = (int *)take(sizeof(int) * nt);
+    }
+    t.cand = (int2 *)take(sizeof(int2) * (size_t)c->max_pairs);
+    t.enc = (int2 *)take(sizeof(int2) * (size_t)c->max_pairs);
+    t.cnt = (int *)take(sizeof(int) * CI_COUNT);
+    t.stat = (long long *)take(sizeof(long long) * CNT_N);
+    t.label = (int *)take(sizeof(int) * np);
+    *exp_labels = (int *)take(sizeof(int) * np);
+    if (d) *d = t;
+    return off;
+}
+
+extern "C" __attribute__((visibility("default"))) size_t genga_workspace_bytes(const genga_config *cfg)
+{
+    if (!valid_cfg(cfg)) return 0;
+    int *l; double *e;
+    return carve(cfg, nullptr, nullptr, &l, &e, 148);   // the layout for 148 SMs is the largest we use
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_create(const genga_config *cfg, genga_ctx **out)
+{
+    if (!out) return GENGA_EINVAL;
+    *out = nullptr;
+    if (!valid_cfg(cfg) || !cfg->workspace) return GENGA_EINVAL;
+    if (((uintptr_t)cfg->workspace & 255) != 0) return GENGA_EINVAL;
+    int dev;
+    CK(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major < 10) {
+        snprintf(g_cuda_err, sizeof g_cuda_err, "device is sm_%d%d; this library is built for sm_100a only", prop.major, prop.minor);
+        return GENGA_ECUDA;
+    }
+    genga_ctx *c = new (std::nothrow) genga_ctx();
+    if (!c) return GENGA_EINVAL;
+    c->cfg = *cfg;
+    c->st = (cudaStream_t)cfg->stream;
+    c->sms = std::min(prop.multiProcessorCount, 148);
+    c->steps = c->force_evals = c->interactions = c->launches = 0;
+    c->acc = 0;
+    size_t need = carve(cfg, (char *)cfg->workspace, &c->d, &c->exp_labels, &c->eout, c->sms);
+    if (need > cfg->workspace_bytes) { delete c; return GENGA_EINVAL; }
+    cudaError_t e = cudaMemsetAsync(cfg->workspace, 0, need, c->st);
+    if (e != cudaSuccess) { delete c; snprintf(g_cuda_err, sizeof g_cuda_err, "memset: %s", cudaGetErrorString(e)); return GENGA_ECUDA; }
+    *out = c;
+    return GENGA_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_destroy(genga_ctx *c)
+{
+    if (!c) return GENGA_EINVAL;
+    for (auto &kv : c->graphs) cudaGraphExecDestroy(kv.second.exec);
+    delete c;
+    return GENGA_OK;
+}
+
+static inline int nblk(long long n, int b) { return (int)std::max<long long>(1, (n + b - 1) / b); }
+#define LAUNCH(c) ((c)->acc += 1)
+
+static int red_threads(int nm) { return std::min(1024, std::max(32, (int)up((size_t)nm, 32))); }
+
+// heliocentric v (in vx0..) -> democratic V, or back (L69)
+static void enqueue_helio_to_demo(genga_ctx *c)
+{
+    DevState &d = c->d;
+    k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx0, d.vy0, d.vz0);
+    k_shift_out<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx0, d.vy0, d.vz0, d.vx, d.vy, d.vz, -1.0, 1);
+    c->launches += 2;
+}
+
+static int set_state_impl(genga_ctx *c, const double *m0, const double *m, const double *radius,
+                          const double *x, const double *v, cudaMemcpyKind kind)
+{
+    if (!c || !m0 || !m || !x || !v) return GENGA_EINVAL;
+    DevState &d = c->d;
+    const size_t n = (size_t)d.ntot, B = sizeof(double);
+    CK(cudaMemcpyAsync(d.m0, m0, B * d.nsys, kind, c->st));
+    CK(cudaMemcpyAsync(d.m, m, B * n, kind, c->st));
+    if (radius) CK(cudaMemcpyAsync(d.radius, radius, B * n, kind, c->st));
+    double *dst[6] = {d.x, d.y, d.z, d.vx0, d.vy0, d.vz0};
+    for (int k = 0; k < 3; ++k) {
+        CK(cudaMemcpyAsync(dst[k], x + k * n, B * n, kind, c->st));
+        CK(cudaMemcpyAsync(dst[3 + k], v + k * n, B * n, kind, c->st));
+    }
+    enqueue_helio_to_demo(c);
+    CK(cudaGetLastError());
+    return GENGA_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_set_state(genga_ctx *c, const double *m0, const double *m, const double *radius,
+                               const double *x, const double *v)
+{
+    return set_state_impl(c, m0, m, radius, x, v, cudaMemcpyDeviceToDevice);
+}
+extern "C" __attribute__((visibility("default"))) int genga_set_state_host(genga_ctx *c, const double *m0, const double *m, const double *radius,
+                                    const double *x, const double *v)
+{
+    int r = set_state_impl(c, m0, m, radius, x, v, cudaMemcpyHostToDevice);
+    if (r) return r;
+    CK(cudaStreamSynchronize(c->st));
+    return GENGA_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+static void enqueue_kick(genga_ctx *c, double h, int record, double *aout)
+{
+    DevState &d = c->d;
+    if (d.mode == GENGA_MODE_MULTI_SYSTEM) {
+        k_kick_multi<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, h, record, aout);
+        LAUNCH(c);
+        return;
+    }
+    dim3 grid((d.nm + KP_THREADS * KP_TI - 1) / (KP_THREADS * KP_TI), d.nslice);
+    k_kick_pairs<<<grid, KP_THREADS, 0, c->st>>>(d, record);
+    k_kick_apply<<<nblk(d.nm, 128), 128, 0, c->st>>>(d, h, aout);
+    LAUNCH(c); LAUNCH(c);
+    if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {
+        k_tp_kick<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, h, record, aout);
+        LAUNCH(c);
+    }
+}
+
+static void enqueue_sun(genga_ctx *c, double h)
+{
+    DevState &d = c->d;
+    k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx, d.vy, d.vz);
+    k_shift<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.x, d.y, d.z, h, 0);
+    LAUNCH(c); LAUNCH(c);
+}
+
+// One second-order map S2(h), Eq. 7 (L100), in the order of the bullet list L153-166.
+static void enqueue_map(genga_ctx *c, double h)
+{
+    DevState &d = c->d;
+    cudaStream_t st = c->st;
+    if (d.mode == GENGA_MODE_TEST_PARTICLE) { k_begin_map<<<c->sms, 256, 0, st>>>(d); LAUNCH(c); }
+    k_reset_counters<<<1, 32, 0, st>>>(d); LAUNCH(c);
+    enqueue_kick(c, 0.5 * h, 1, nullptr);
+    enqueue_sun(c, 0.5 * h);
+    k_drift<<<nblk(d.ntot, 128), 128, 0, st>>>(d, h); LAUNCH(c);
+    const int pair_blocks = (int)std::min<long long>((d.cap + 127) / 128, 4LL * c->sms);
+    k_confirm<<<pair_blocks, 128, 0, st>>>(d, h); LAUNCH(c);
+    k_label_init<<<nblk(d.nmtot, 256), 256, 0, st>>>(d); LAUNCH(c);
+    k_union<<<pair_blocks, 128, 0, st>>>(d); LAUNCH(c);
+    k_flatten<<<nblk(d.nmtot, 256), 256, 0, st>>>(d); LAUNCH(c);
+    if (d.mode == GENGA_MODE_MULTI_SYSTEM) {
+        k_bs_multi<<<nblk(d.nsys, 8), 128, 0, st>>>(d, h); LAUNCH(c);
+    } else {
+        k_build_groups<<<1, 1024, 0, st>>>(d); LAUNCH(c);
+        k_bs_warp<<<c->sms, 128, 0, st>>>(d, h); LAUNCH(c);
+        if (d.bss.base) { k_bs_block<<<16, 256, 0, st>>>(d, h); LAUNCH(c); }
+        if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {
+            k_tp_bs<4><<<4 * c->sms, 128, 0, st>>>(d, h, 0);
+            k_tp_bs<32><<<2 * c->sms, 128, 0, st>>>(d, h, 4);
+            LAUNCH(c); LAUNCH(c);
+        }
+    }
+    enqueue_sun(c, 0.5 * h);
+    enqueue_kick(c, 0.5 * h, 0, nullptr);
+}
+
+static int maps_per_step(int order) { return order == 2 ? 1 : order == 4 ? 3 : 7; }
+
+static void enqueue_step(genga_ctx *c, double dt, int order)
+{
+    DevState &d = c->d;
+    double w[7];
+    int nw = yoshida_weights(order, w);
+    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt); LAUNCH(c);
+    for (int k = 0; k < nw; ++k) enqueue_map(c, w[k] * dt);
+}
+
+static long long interactions_per_eval(const DevState &d)
+{
+    long long nm = d.nm;
+    if (d.mode == GENGA_MODE_MULTI_SYSTEM) return (long long)d.nsys * nm * (nm - 1);
+    return nm * (nm - 1) + (long long)(d.ntot - d.nm) * nm;
+}
+
+static int get_graph(genga_ctx *c, double dt, int order, int nsteps, genga_ctx::GraphEntry *out)
+{
+    GraphKey key{dt, order, nsteps};
+    auto it = c->graphs.find(key);
+    if (it == c->graphs.end()) {
+        cudaGraph_t g;
+        CK(cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal));
+        c->acc = 0;
+        for (int s = 0; s < nsteps; ++s) enqueue_step(c, dt, order);
+        long long n = c->acc;
+        c->acc = 0;
+        CK(cudaStreamEndCapture(c->st, &g));
+        cudaGraphExec_t ge;
+        CK(cudaGraphInstantiate(&ge, g, 0));
+        cudaGraphDestroy(g);
+        if (c->graphs.size() > 16) {          // bound the cache
+            for (auto &kv : c->graphs) cudaGraphExecDestroy(kv.second.exec);
+            c->graphs.clear();
+        }
+        it = c->graphs.emplace(key, genga_ctx::GraphEntry{ge, n}).first;
+    }
+    *out = it->second;
+    return GENGA_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_step(genga_ctx *c, int64_t n_steps, double dt, int order)
+{
+    if (!c || n_steps < 0 || dt == 0.0 || !(dt == dt) || (order != 2 && order != 4 && order != 6)) return GENGA_EINVAL;
+    if (n_steps == 0) return GENGA_OK;
+    if (c->st == nullptr) {                       // legacy stream cannot be captured: plain launches
+        c->acc = 0;
+        for (int64_t s = 0; s < n_steps; ++s) enqueue_step(c, dt, order);
+        c->launches += c->acc; c->acc = 0;
+    } else {
+        const int chunk = 16;
+        int64_t left = n_steps;
+        while (left > 0) {
+            int n = left >= chunk ? chunk : 1;
+            genga_ctx::GraphEntry ge;
+            int r = get_graph(c, dt, order, n, &ge);
+            if (r) return r;
+            CK(cudaGraphLaunch(ge.exec, c->st));
+            c->launches += ge.launches;
+            left -= n;
+        }
+    }
+    CK(cudaGetLastError());
+    c->steps += n_steps;
+    long long evals = 2LL * maps_per_step(order) * n_steps;
+    c->force_evals += evals;
+    c->interactions += evals * interactions_per_eval(c->d);
+    return GENGA_OK;
+}
+
+static int latch(genga_ctx *c)
+{
+    int st = 0;
+    CK(cudaMemcpyAsync(&st, c->d.cnt + CI_STATUS, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    if (st) {
+        CK(cudaMemsetAsync(c->d.cnt + CI_STATUS, 0, sizeof(int), c->st));
+        if (st & ERRBIT_KEPLER) return GENGA_EKEPLER;
+        if (st & ERRBIT_BS) return GENGA_EBS;
+        if (st & ERRBIT_CAPACITY) return GENGA_ECAPACITY;
+    }
+    return GENGA_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_status(genga_ctx *c)
+{
+    if (!c) return GENGA_EINVAL;
+    return latch(c);
+}
+
+static int get_state_impl(genga_ctx *c, double *x, double *v, cudaMemcpyKind kind)
+{
+    if (!c || !x || !v) return GENGA_EINVAL;
+    DevState &d = c->d;
+    const size_t n = (size_t)d.ntot, B = sizeof(double);
+    k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx, d.vy, d.vz);
+    k_shift_out<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0);
+    c->launches += 2;
+    const double *src[6] = {d.x, d.y, d.z, d.vx0, d.vy0, d.vz0};
+    for (int k = 0; k < 3; ++k) {
+        CK(cudaMemcpyAsync(x + k * n, src[k], B * n, kind, c->st));
+        CK(cudaMemcpyAsync(v + k * n, src[3 + k], B * n, kind, c->st));
+    }
+    CK(cudaGetLastError());
+    return GENGA_OK;
+}
+extern "C" __attribute__((visibility("default"))) int genga_get_state(genga_ctx *c, double *x, double *v)
+{
+    return get_state_impl(c, x, v, cudaMemcpyDeviceToDevice);
+}
+extern "C" __attribute__((visibility("default"))) int genga_get_state_host(genga_ctx *c, double *x, double *v)
+{
+    int r = get_state_impl(c, x, v, cudaMemcpyDeviceToHost);
+    if (r) return r;
+    return latch(c);
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_energy(genga_ctx *c, double *E, double *L)
+{
+    if (!c || !E) return GENGA_EINVAL;
+    DevState &d = c->d;
+    k_energy<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, c->eout);
+    c->launches += 1;
+    std::vector<double> h(4 * (size_t)d.nsys);
+    CK(cudaMemcpyAsync(h.data(), c->eout, sizeof(double) * h.size(), cudaMemcpyDeviceToHost, c->st));
+    int r = latch(c);
+    for (int s = 0; s < d.nsys; ++s) {
+        E[s] = h[4 * s];
+        if (L) { L[3 * s] = h[4 * s + 1]; L[3 * s + 1] = h[4 * s + 2]; L[3 * s + 2] = h[4 * s + 3]; }
+    }
+    return r;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_encounters(genga_ctx *c, int32_t *pairs, int64_t cap, int64_t *n_pairs,
+                                int64_t *n_candidates, int32_t *group_label)
+{
+    if (!c || (cap > 0 && !pairs) || cap < 0) return GENGA_EINVAL;
+    DevState &d = c->d;
+    int cnt[CI_COUNT];
+    CK(cudaMemcpyAsync(cnt, d.cnt, sizeof cnt, cudaMemcpyDeviceToHost, c->st));
+    if (group_label) {
+        k_export_labels<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, c->exp_labels);
+        c->launches += 1;
+        CK(cudaMemcpyAsync(group_label, c->exp_labels, sizeof(int) * (size_t)d.ntot, cudaMemcpyDeviceToHost, c->st));
+    }
+    CK(cudaStreamSynchronize(c->st));
+    long long ne = std::min<long long>(cnt[CI_NENC], d.cap);
+    std::vector<int2> h((size_t)ne);
+    if (ne) CK(cudaMemcpyAsync(h.data(), d.enc, sizeof(int2) * (size_t)ne, cudaMemcpyDeviceToHost, c->st));
+    int r = latch(c);
+    std::sort(h.begin(), h.end(), [](const int2 &a, const int2 &b) { return a.x != b.x ? a.x < b.x : a.y < b.y; });
+    for (long long k = 0; k < ne && k < cap; ++k) { pairs[2 * k] = h[k].x; pairs[2 * k + 1] = h[k].y; }
+    if (n_pairs) *n_pairs = cnt[CI_NENC];
+    if (n_candidates) *n_candidates = cnt[CI_NCAND];
+    return r;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_accelerations(genga_ctx *c, double dt, double *a, double *rcrit)
+{
+    if (!c || !a || dt == 0.0) return GENGA_EINVAL;
+    DevState &d = c->d;
+    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt);
+    if (d.mode == GENGA_MODE_TEST_PARTICLE) { k_begin_map<<<c->sms, 256, 0, c->st>>>(d); c->launches += 1; }
+    k_reset_counters<<<1, 32, 0, c->st>>>(d);
+    c->launches += 2;
+    c->acc = 0;
+    enqueue_kick(c, 0.0, 1, a);
+    c->launches += c->acc; c->acc = 0;
+    if (rcrit) CK(cudaMemcpyAsync(rcrit, d.rc, sizeof(double) * (size_t)d.ntot, cudaMemcpyDeviceToDevice, c->st));
+    CK(cudaGetLastError());
+    c->force_evals += 1;
+    c->interactions += interactions_per_eval(d);
+    return GENGA_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_kepler_drift(genga_ctx *c, int64_t n, double mu, double h, double *x, double *v)
+{
+    if (!c || n < 0 || !x || !v || !(mu > 0.0)) return GENGA_EINVAL;
+    if (n == 0) return GENGA_OK;
+    k_drift_arrays<<<nblk(n, 128), 128, 0, c->st>>>(n, mu, h, x, v, c->d.cnt + CI_STATUS);
+    c->launches += 1;
+    CK(cudaGetLastError());
+    return GENGA_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_counters(genga_ctx *c, int64_t *out)
+{
+    if (!c || !out) return GENGA_EINVAL;
+    long long st[CNT_N];
+    CK(cudaMemcpyAsync(st, c->d.stat, sizeof st, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    out[0] = c->steps; out[1] = c->force_evals; out[2] = c->interactions; out[3] = c->launches;
+    out[4] = st[CNT_GROUPS]; out[5] = st[CNT_MAXGROUP]; out[6] = st[CNT_BSSTEPS]; out[7] = st[CNT_CAND];
+    return GENGA_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) const char *genga_strerror(int code)
+{
+    switch (code) {
+    case GENGA_OK: return "ok";
+    case GENGA_EINVAL: return "invalid argument";
+    case GENGA_ECAPACITY: return "pair list capacity (max_pairs) exceeded";
+    case GENGA_EKEPLER: return "Kepler solver did not converge";
+    case GENGA_EBS: return "Bulirsch-Stoer step size underflow";
+    case GENGA_ECUDA: return "CUDA runtime error";
+    default: return "unknown error";
+    }
+}
+extern "C" __attribute__((visibility("default"))) const char *genga_last_cuda_error(void) { return g_cuda_err; }

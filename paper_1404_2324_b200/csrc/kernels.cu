@@ -1,0 +1,680 @@
+// Kernels of the hybrid symplectic step, sm_100a.
+// Each kernel states the operator it implements and the passage that defines it.
+#include "kernels.cuh"
+
+namespace genga {
+
+// =====================================================================================
+// Start of a map S2: forget the previous substep's lists.  Mode 1: clear the per-particle
+// encounter masks of the particles listed last time.
+__global__ void k_begin_map(DevState d)
+{
+    int nprev = d.cnt[CI_NTP];
+    if (d.mode == 1) {
+        for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nprev; k += gridDim.x * blockDim.x)
+            d.tpmask[d.tplist[k] - d.nm] = 0u;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) d.cnt[CI_NTP_PREV] = nprev;
+}
+__global__ void k_reset_counters(DevState d)
+{
+    if (threadIdx.x == 0) {
+        d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
+    }
+}
+
+// =====================================================================================
+// Critical radius, Eq. 6 (L94-96): rc_i = max(n1 R_H,i , n2 |tau| v_i), v_i = |V_i| the body's
+// own velocity (L96), R_H,i = a_i (m_i / 3 m0)^(1/3) with a_i from the vis-viva relation
+// (r_i if unbound); test particles have R_H = 0.  Also stores 9 rc^2, the squared precheck
+// distance (L142: "increasing the critical radius by a factor of three").
+__global__ void k_rcrit(DevState d, double tau)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.ntot) return;
+    double x = d.x[i], y = d.y[i], z = d.z[i], vx = d.vx[i], vy = d.vy[i], vz = d.vz[i], m = d.m[i];
+    double m0 = d.m0[system_of(d, i)];
+    double r = sqrt(x * x + y * y + z * z);
+    double v2 = vx * vx + vy * vy + vz * vz;
+    double ainv = 2.0 / r - v2 / (d.G * m0);
+    double a = ainv > 0.0 ? 1.0 / ainv : r;
+    double rh = m > 0.0 ? a * cbrt(m / (3.0 * m0)) : 0.0;
+    double rv = d.n2 * fabs(tau) * sqrt(v2);
+    double rc = fmax(d.n1 * rh, rv);
+    d.rc[i] = rc;
+    d.c9[i] = 9.0 * rc * rc;
+}
+
+// =====================================================================================
+// Kick, operator B (Eq. 2; L197, L238-264): a_i = sum_j G m_j (q_j - q_i)/r^3 W(r, rc_ij)
+// and the prechecker (L142).  Massive bodies of one system, N <= 2048.
+//
+// Decomposition: grid (i-blocks of 512 bodies, j-slices).  Each thread keeps KP_TI bodies i
+// in registers and walks its j-slice, staged in shared memory and read as warp broadcasts.
+// Pairs inside the precheck sphere (r^2 < 9 rc_ij^2, which contains the whole changeover
+// zone r < rc_ij) are taken OUT of the fast loop: their (i, j) goes to a shared-memory list,
+// the weight W is evaluated for the list in parallel afterwards and added by the owning
+// thread in list order, so the sum is deterministic.  Partial sums per slice go to
+// apart[slice][c][i]; k_kick_apply adds the slices in fixed order.
+__global__ void __launch_bounds__(KP_THREADS) k_kick_pairs(DevState d, int record)
+{
+    __shared__ double sx[KP_MAXJ], sy[KP_MAXJ], sz[KP_MAXJ], sgm[KP_MAXJ], sc9[KP_MAXJ];
+    __shared__ int hits[KP_HCAP];
+    __shared__ double hcx[KP_HCAP], hcy[KP_HCAP], hcz[KP_HCAP];
+    __shared__ int nh;
+
+    const int N = d.nm, tid = threadIdx.x;
+    const int S = gridDim.y, s = blockIdx.y;
+    const int j0 = (int)((long long)s * N / S), j1 = (int)((long long)(s + 1) * N / S), jl = j1 - j0;
+    if (tid == 0) nh = 0;
+    for (int t = tid; t < jl; t += KP_THREADS) {
+        sx[t] = d.x[j0 + t]; sy[t] = d.y[j0 + t]; sz[t] = d.z[j0 + t];
+        sgm[t] = d.G * d.m[j0 + t]; sc9[t] = d.c9[j0 + t];
+    }
+    int ii[KP_TI];
+    double xi[KP_TI], yi[KP_TI], zi[KP_TI], ci[KP_TI], ax[KP_TI], ay[KP_TI], az[KP_TI];
+#pragma unroll
+    for (int t = 0; t < KP_TI; ++t) {
+        ii[t] = blockIdx.x * (KP_THREADS * KP_TI) + t * KP_THREADS + tid;
+        bool valid = ii[t] < N;
+        xi[t] = valid ? d.x[ii[t]] : 1e100; yi[t] = valid ? d.y[ii[t]] : 1e100; zi[t] = valid ? d.z[ii[t]] : 1e100;
+        ci[t] = valid ? d.c9[ii[t]] : -1.0;
+        ax[t] = ay[t] = az[t] = 0.0;
+    }
+    __syncthreads();
+
+#pragma unroll 2
+    for (int jj = 0; jj < jl; ++jj) {
+        const double xj = sx[jj], yj = sy[jj], zj = sz[jj], gm = sgm[jj], cj = sc9[jj];
+#pragma unroll
+        for (int t = 0; t < KP_TI; ++t) {
+            double dx = xj - xi[t], dy = yj - yi[t], dz = zj - zi[t];
+            double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            bool hit = r2 < fmax(ci[t], cj);
+            double rinv = rsqrt(r2);
+            double s3 = gm * rinv * (rinv * rinv);
+            if (hit) {
+                s3 = 0.0;
+                if (j0 + jj != ii[t]) {
+                    int slot = atomicAdd(&nh, 1);
+                    if (slot < KP_HCAP) hits[slot] = ((t * KP_THREADS + tid) << 16) | jj;
+                    else {
+                        // list full (pathologically dense encounters): finish the pair here
+                        double r = sqrt(r2);
+                        double rcij = fmax(d.rc[ii[t]], d.rc[j0 + jj]);
+                        s3 = gm / (r2 * r) * kick_weight(r, rcij);
+                        if (record && ii[t] < j0 + jj) {
+                            int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
+                            if (idx < d.cap) d.cand[idx] = make_int2(ii[t], j0 + jj);
+                            else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+                        }
+                    }
+                }
+            }
+            ax[t] = fma(s3, dx, ax[t]); ay[t] = fma(s3, dy, ay[t]); az[t] = fma(s3, dz, az[t]);
+        }
+    }
+    __syncthreads();
+    const int nhc = min(nh, KP_HCAP);
+    // weights of the listed pairs, one pair per thread
+    for (int e = tid; e < nhc; e += KP_THREADS) {
+        int h = hits[e], jj = h & 0xffff, slot = h >> 16;
+        int i = blockIdx.x * (KP_THREADS * KP_TI) + slot, j = j0 + jj;
+        double dx = sx[jj] - d.x[i], dy = sy[jj] - d.y[i], dz = sz[jj] - d.z[i];
+        double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+        double r = sqrt(r2);
+        double rcij = fmax(d.rc[i], d.rc[j]);
+        double s3 = sgm[jj] / (r2 * r) * kick_weight(r, rcij);
+        hcx[e] = s3 * dx; hcy[e] = s3 * dy; hcz[e] = s3 * dz;
+        if (record && i < j) {
+            int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
+            if (idx < d.cap) d.cand[idx] = make_int2(i, j);
+            else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+        }
+    }
+    __syncthreads();
+    if (nhc > 0) {
+        for (int e = 0; e < nhc; ++e) {
+            int slot = hits[e] >> 16;
+#pragma unroll
+            for (int t = 0; t < KP_TI; ++t)
+                if (slot == t * KP_THREADS + tid) { ax[t] += hcx[e]; ay[t] += hcy[e]; az[t] += hcz[e]; }
+        }
+    }
+#pragma unroll
+    for (int t = 0; t < KP_TI; ++t)
+        if (ii[t] < N) {
+            double *p = d.apart + (size_t)s * 3 * d.npm;
+            p[ii[t]] = ax[t]; p[d.npm + ii[t]] = ay[t]; p[2 * d.npm + ii[t]] = az[t];
+        }
+}
+
+// V_i += h a_i with a_i = sum over slices in fixed order.  aout (optional): store a.
+__global__ void k_kick_apply(DevState d, double h, double *aout)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.nm) return;
+    double ax = 0, ay = 0, az = 0;
+    for (int s = 0; s < d.nslice; ++s) {
+        const double *p = d.apart + (size_t)s * 3 * d.npm;
+        ax += p[i]; ay += p[d.npm + i]; az += p[2 * d.npm + i];
+    }
+    if (aout) { aout[i] = ax; aout[d.ntot + i] = ay; aout[2 * (size_t)d.ntot + i] = az; }
+    d.vx[i] = fma(h, ax, d.vx[i]); d.vy[i] = fma(h, ay, d.vy[i]); d.vz[i] = fma(h, az, d.vz[i]);
+}
+
+// Kick of the test particles (L334-340): one thread per particle looping over the <= 32
+// massive bodies, which sit in shared memory (broadcast reads).  Precheck against every
+// massive body; candidate pairs are (massive j, particle i).
+__global__ void __launch_bounds__(128) k_tp_kick(DevState d, double h, int record, double *aout)
+{
+    __shared__ double sx[32], sy[32], sz[32], sgm[32], src[32];
+    const int nm = d.nm;
+    if (threadIdx.x < nm) {
+        int j = threadIdx.x;
+        sx[j] = d.x[j]; sy[j] = d.y[j]; sz[j] = d.z[j]; sgm[j] = d.G * d.m[j]; src[j] = d.rc[j];
+    }
+    __syncthreads();
+    int i = nm + blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.ntot) return;
+    double xi = d.x[i], yi = d.y[i], zi = d.z[i], rci = d.rc[i];
+    double ax = 0, ay = 0, az = 0;
+    for (int j = 0; j < nm; ++j) {
+        double dx = sx[j] - xi, dy = sy[j] - yi, dz = sz[j] - zi;
+        double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+        double rcij = fmax(rci, src[j]);
+        double rinv = rsqrt(r2);
+        double s3 = sgm[j] * rinv * (rinv * rinv);
+        if (r2 < 9.0 * rcij * rcij) {
+            double r = sqrt(r2);
+            s3 = sgm[j] / (r2 * r) * kick_weight(r, rcij);
+            if (record) {
+                int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
+                if (idx < d.cap) d.cand[idx] = make_int2(j, i);
+                else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+            }
+        }
+        ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
+    }
+    if (aout) { aout[i] = ax; aout[d.ntot + i] = ay; aout[2 * (size_t)d.ntot + i] = az; }
+    d.vx[i] = fma(h, ax, d.vx[i]); d.vy[i] = fma(h, ay, d.vy[i]); d.vz[i] = fma(h, az, d.vz[i]);
+}
+
+// Kick in multi-system mode (L368-370): one thread per body, partners = the bodies of its
+// own system (contiguous, body = system * nm + k).
+__global__ void __launch_bounds__(128) k_kick_multi(DevState d, double h, int record, double *aout)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.ntot) return;
+    const int nm = d.nm, base = (i / nm) * nm;
+    double xi = d.x[i], yi = d.y[i], zi = d.z[i], rci = d.rc[i];
+    double ax = 0, ay = 0, az = 0;
+    for (int k = 0; k < nm; ++k) {
+        int j = base + k;
+        if (j == i) continue;
+        double dx = d.x[j] - xi, dy = d.y[j] - yi, dz = d.z[j] - zi;
+        double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+        double rcij = fmax(rci, d.rc[j]);
+        double gm = d.G * d.m[j];
+        double rinv = rsqrt(r2);
+        double s3 = gm * rinv * (rinv * rinv);
+        if (r2 < 9.0 * rcij * rcij) {
+            double r = sqrt(r2);
+            s3 = gm / (r2 * r) * kick_weight(r, rcij);
+            if (record && i < j) {
+                int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
+                if (idx < d.cap) d.cand[idx] = make_int2(i, j);
+                else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+            }
+        }
+        ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
+    }
+    if (aout) { aout[i] = ax; aout[d.ntot + i] = ay; aout[2 * (size_t)d.ntot + i] = az; }
+    d.vx[i] = fma(h, ax, d.vx[i]); d.vy[i] = fma(h, ay, d.vy[i]); d.vz[i] = fma(h, az, d.vz[i]);
+}
+
+// =====================================================================================
+// Sun kick, operator C (Eq. 3; L196, L232-236, L338, L360-366): s = sum over massive
+// bodies of m V (one block per system, fixed-order tree), then q_i += h s / m0 for every
+// body of the system, test particles included.
+// which: 0 = democratic V as stored; used also for the coordinate maps (with other arrays).
+__global__ void k_momentum(DevState d, const double *vx, const double *vy, const double *vz)
+{
+    __shared__ double red[4][32];
+    const int sys = blockIdx.x, base = sys * d.nm * (d.mode == 2 ? 1 : 0);
+    double s[4] = {0, 0, 0, 0};
+    for (int k = threadIdx.x; k < d.nm; k += blockDim.x) {
+        double m = d.m[base + k];
+        s[0] = fma(m, vx[base + k], s[0]); s[1] = fma(m, vy[base + k], s[1]); s[2] = fma(m, vz[base + k], s[2]);
+        s[3] += m;
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+        for (int o = 16; o > 0; o >>= 1) s[c] += __shfl_xor_sync(0xffffffffu, s[c], o);
+    int w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if ((threadIdx.x & 31) == 0)
+        for (int c = 0; c < 4; ++c) red[c][w] = s[c];
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double t = 0;
+        for (int k = 0; k < nw; ++k) t += red[threadIdx.x][k];
+        d.psum[4 * sys + threadIdx.x] = t;
+    }
+}
+// q += f * psum / m0   (f = h for the Sun kick)
+__global__ void k_shift(DevState d, double *ax, double *ay, double *az, double f, int divide_by_total)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.ntot) return;
+    int sys = system_of(d, i);
+    double den = divide_by_total ? d.m0[sys] + d.psum[4 * sys + 3] : d.m0[sys];
+    double g = f / den;
+    ax[i] = fma(g, d.psum[4 * sys], ax[i]); ay[i] = fma(g, d.psum[4 * sys + 1], ay[i]); az[i] = fma(g, d.psum[4 * sys + 2], az[i]);
+}
+// out = in + f * psum / den  (coordinate maps at the ABI, L69)
+__global__ void k_shift_out(DevState d, const double *ix, const double *iy, const double *iz,
+                            double *ox, double *oy, double *oz, double f, int divide_by_total)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.ntot) return;
+    int sys = system_of(d, i);
+    double den = divide_by_total ? d.m0[sys] + d.psum[4 * sys + 3] : d.m0[sys];
+    double g = f / den;
+    ox[i] = fma(g, d.psum[4 * sys], ix[i]); oy[i] = fma(g, d.psum[4 * sys + 1], iy[i]); oz[i] = fma(g, d.psum[4 * sys + 2], iz[i]);
+}
+
+// =====================================================================================
+// Kepler drift, the analytic part of operator A (Eq. 9; L195, L208-230): one thread per
+// body, state kept before the drift for the encounter search and for BS.
+__global__ void __launch_bounds__(128) k_drift(DevState d, double h)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.ntot) return;
+    double x = d.x[i], y = d.y[i], z = d.z[i], vx = d.vx[i], vy = d.vy[i], vz = d.vz[i];
+    d.x0[i] = x; d.y0[i] = y; d.z0[i] = z; d.vx0[i] = vx; d.vy0[i] = vy; d.vz0[i] = vz;
+    double mu = d.G * d.m0[system_of(d, i)];
+    if (!kepler_drift(mu, h, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
+    d.x[i] = x; d.y[i] = y; d.z[i] = z; d.vx[i] = vx; d.vy[i] = vy; d.vz[i] = vz;
+}
+// stand-alone drift on caller arrays (genga_kepler_drift)
+__global__ void __launch_bounds__(128) k_drift_arrays(long long n, double mu, double h, double *x, double *v, int *status)
+{
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double a = x[i], b = x[n + i], c = x[2 * n + i], va = v[i], vb = v[n + i], vc = v[2 * n + i];
+    if (!kepler_drift(mu, h, a, b, c, va, vb, vc)) atomicOr(status, ERRBIT_KEPLER);
+    x[i] = a; x[n + i] = b; x[2 * n + i] = c; v[i] = va; v[n + i] = vb; v[2 * n + i] = vc;
+}
+
+// =====================================================================================
+// Encounter search (Eq. 10-12; L200, L276-278): one thread per candidate, confirmed
+// pairs appended to the encounter list (warp-aggregated atomic).  Mode 1: a pair with a test
+// particle also sets the massive body's bit in the particle's mask and lists the particle once.
+__global__ void __launch_bounds__(128) k_confirm(DevState d, double h)
+{
+    const int nc = min(d.cnt[CI_NCAND], (int)d.cap);
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < nc; e += gridDim.x * blockDim.x) {
+        int2 p = d.cand[e];
+        int i = p.x, j = p.y;
+        double dx = d.x0[j] - d.x0[i], dy = d.y0[j] - d.y0[i], dz = d.z0[j] - d.z0[i];
+        double dvx = d.vx0[j] - d.vx0[i], dvy = d.vy0[j] - d.vy0[i], dvz = d.vz0[j] - d.vz0[i];
+        double P0 = dx * dx + dy * dy + dz * dz, Pd0 = 2.0 * (dx * dvx + dy * dvy + dz * dvz);
+        dx = d.x[j] - d.x[i]; dy = d.y[j] - d.y[i]; dz = d.z[j] - d.z[i];
+        dvx = d.vx[j] - d.vx[i]; dvy = d.vy[j] - d.vy[i]; dvz = d.vz[j] - d.vz[i];
+        double P1 = dx * dx + dy * dy + dz * dz, Pd1 = 2.0 * (dx * dvx + dy * dvy + dz * dvz);
+        double rcij = fmax(d.rc[i], d.rc[j]);
+        double D = hermite_min(P0, P1, Pd0, Pd1, h);
+        if (D < rcij * rcij) {
+            int idx = atomicAdd(&d.cnt[CI_NENC], 1);
+            if (idx < d.cap) d.enc[idx] = p;
+            else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+            if (d.mode == 1 && j >= d.nm) {
+                unsigned old = atomicOr(&d.tpmask[j - d.nm], 1u << i);
+                if (old == 0u) {
+                    int k = atomicAdd(&d.cnt[CI_NTP], 1);
+                    d.tplist[k] = j;     // at most n_test entries: never overflows
+                }
+            }
+        }
+    }
+}
+
+// =====================================================================================
+// Grouping (L280-284, Appendix): equivalence classes of the encounter graph,
+// label = lowest member index.  Union-find with atomicMin hooks (larger root under smaller
+// root), then pointer jumping to the root -- the LINK iteration of the Appendix without the
+// repeat-until-unchanged sweep.
+__global__ void k_label_init(DevState d)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < d.nmtot) d.label[i] = i;
+}
+__device__ __forceinline__ int uf_find(const int *L, int i)
+{
+    int p = L[i];
+    while (p != i) { i = p; p = L[i]; }
+    return i;
+}
+__global__ void k_union(DevState d)
+{
+    const int ne = min(d.cnt[CI_NENC], (int)d.cap);
+    int *L = d.label;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < ne; e += gridDim.x * blockDim.x) {
+        int2 p = d.enc[e];
+        if (d.mode == 1 && p.y >= d.nm) continue;       // particle pairs do not link massive bodies
+        int a = p.x, b = p.y;
+        while (true) {
+            a = uf_find(L, a); b = uf_find(L, b);
+            if (a == b) break;
+            int hi = max(a, b), lo = min(a, b);
+            int old = atomicMin(&L[hi], lo);
+            if (old == hi) break;
+            a = old; b = lo;
+        }
+    }
+}
+__global__ void k_flatten(DevState d)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < d.nmtot) d.label[i] = uf_find(d.label, i);
+}
+
+// exclusive scan of two ints per thread over a 1024-thread block
+__device__ __forceinline__ void block_scan2(int v0, int v1, int &e0, int &e1, int &total, int *wsum)
+{
+    int t = v0 + v1, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int inc = t;
+    for (int o = 1; o < 32; o <<= 1) { int n = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += n; }
+    __syncthreads();
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        int s = wsum[lane], si = s;
+        for (int o = 1; o < 32; o <<= 1) { int n = __shfl_up_sync(0xffffffffu, si, o); if (lane >= o) si += n; }
+        wsum[lane] = si - s;
+        if (lane == 31) wsum[32] = si;
+    }
+    __syncthreads();
+    int base = wsum[w] + inc - t;
+    e0 = base; e1 = base + v0; total = wsum[32];
+}
+
+// Member lists of the groups of massive bodies (modes 0 and 1; N <= 2048): groups ordered by
+// root index, members sorted by body index ("write the members of the groups line by line
+// into a matrix", L565 -- here a CSR list).  One block of 1024 threads.
+__global__ void __launch_bounds__(1024) k_build_groups(DevState d)
+{
+    __shared__ int lab[2048], sz[2048], E[2048], gst[2048];
+    __shared__ int wsum[33];
+    const int N = d.nm, tid = threadIdx.x, i0 = 2 * tid, i1 = 2 * tid + 1;
+    lab[i0] = i0 < N ? d.label[i0] : i0; lab[i1] = i1 < N ? d.label[i1] : i1;
+    sz[i0] = 0; sz[i1] = 0;
+    __syncthreads();
+    if (i0 < N) atomicAdd(&sz[lab[i0]], 1);
+    if (i1 < N) atomicAdd(&sz[lab[i1]], 1);
+    __syncthreads();
+    int f0 = i0 < N && sz[lab[i0]] >= 2, f1 = i1 < N && sz[lab[i1]] >= 2;
+    int e0, e1, ne, g0, g1, ng, s0, s1, ns;
+    block_scan2(f0, f1, e0, e1, ne, wsum);
+    if (f0) E[e0] = i0;
+    if (f1) E[e1] = i1;
+    int r0 = f0 && lab[i0] == i0, r1 = f1 && lab[i1] == i1;
+    block_scan2(r0, r1, g0, g1, ng, wsum);
+    block_scan2(r0 ? sz[i0] : 0, r1 ? sz[i1] : 0, s0, s1, ns, wsum);
+    if (r0) { gst[i0] = s0; d.gstart[g0] = s0; d.gsize[g0] = sz[i0]; }
+    if (r1) { gst[i1] = s1; d.gstart[g1] = s1; d.gsize[g1] = sz[i1]; }
+    __syncthreads();
+    for (int k = tid; k < ne; k += blockDim.x) {
+        int i = E[k], r = lab[i], rank = 0;
+        for (int kk = 0; kk < k; ++kk) rank += (lab[E[kk]] == r);
+        d.gmem[gst[r] + rank] = i;
+    }
+    if (d.mode == 1 && tid < N) {
+        unsigned mask = 0u;
+        for (int j = 0; j < N; ++j) if (lab[j] == lab[tid]) mask |= 1u << j;
+        d.gmask[tid] = mask;
+    }
+    if (tid == 0) {
+        d.cnt[CI_NGROUPS] = ng;
+        d.stat[CNT_GROUPS] += ng;
+        d.stat[CNT_CAND] += d.cnt[CI_NCAND];
+    }
+    int big = (r0 ? sz[i0] : 0) > (r1 ? sz[i1] : 0) ? (r0 ? sz[i0] : 0) : (r1 ? sz[i1] : 0);
+    for (int o = 16; o > 0; o >>= 1) big = max(big, __shfl_xor_sync(0xffffffffu, big, o));
+    if ((tid & 31) == 0 && big > 0) {
+        atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)big);
+        if (big > 32) atomicAdd(&d.cnt[CI_NBIG], 1);
+    }
+}
+
+// =====================================================================================
+// Bulirsch-Stoer on the groups of massive bodies (modes 0, 1): one warp per group of 2..32
+// bodies; all members start from the state before the drift and overwrite the drift result
+// (L163, L301-314).
+__global__ void __launch_bounds__(128) k_bs_warp(DevState d, double h)
+{
+    __shared__ TeamSmem<32> sm[4];
+    const int ng = d.cnt[CI_NGROUPS];
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    WarpTeam<32> t{0xffffffffu, lane};
+    for (int g = blockIdx.x * 4 + wib; g < ng; g += gridDim.x * 4) {
+        const int nb = d.gsize[g];
+        if (nb > 32) continue;
+        const bool active = lane < nb;
+        const int i = active ? d.gmem[d.gstart[g] + lane] : 0;
+        double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0}, rc = 0.0;
+        __syncwarp();
+        sm[wib].m[lane] = 0.0; sm[wib].rc[lane] = 0.0;
+        if (active) {
+            q[0] = d.x0[i]; q[1] = d.y0[i]; q[2] = d.z0[i]; V[0] = d.vx0[i]; V[1] = d.vy0[i]; V[2] = d.vz0[i];
+            rc = d.rc[i];
+            sm[wib].m[lane] = d.m[i]; sm[wib].rc[lane] = rc;
+        }
+        __syncwarp();
+        int nsteps = 0;
+        unsigned srcmask = nb >= 32 ? 0xffffffffu : ((1u << nb) - 1u);
+        bool ok = bs_team<32>(t, sm[wib], nb, active, srcmask, d.G, d.m0[0], rc, q, V, h, d.eps, &nsteps);
+        if (active) { d.x[i] = q[0]; d.y[i] = q[1]; d.z[i] = q[2]; d.vx[i] = V[0]; d.vy[i] = V[1]; d.vz[i] = V[2]; }
+        if (lane == 0) {
+            if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
+        }
+    }
+}
+
+// Groups larger than a warp: one block per group, tableau in global scratch.
+__global__ void __launch_bounds__(256) k_bs_block(DevState d, double h)
+{
+    __shared__ double red[32];
+    __shared__ int nsteps;
+    if (d.cnt[CI_NBIG] == 0) return;
+    const int ng = d.cnt[CI_NGROUPS];
+    for (int g = blockIdx.x; g < ng; g += gridDim.x) {
+        const int nb = d.gsize[g];
+        if (nb <= 32) continue;
+        const int off = d.gstart[g];
+        if (threadIdx.x == 0) nsteps = 0;
+        for (int b = threadIdx.x; b < nb; b += blockDim.x) {
+            int i = d.gmem[off + b];
+            d.bss.arr(BSA_Y + 0)[off + b] = d.x0[i]; d.bss.arr(BSA_Y + 1)[off + b] = d.y0[i]; d.bss.arr(BSA_Y + 2)[off + b] = d.z0[i];
+            d.bss.arr(BSA_Y + 3)[off + b] = d.vx0[i]; d.bss.arr(BSA_Y + 4)[off + b] = d.vy0[i]; d.bss.arr(BSA_Y + 5)[off + b] = d.vz0[i];
+            d.bss.arr(BSA_M)[off + b] = d.m[i]; d.bss.arr(BSA_RC)[off + b] = d.rc[i];
+        }
+        bool ok = bs_block(d.bss, off, nb, d.G, d.m0[0], h, d.eps, red, &nsteps);
+        __syncthreads();
+        for (int b = threadIdx.x; b < nb; b += blockDim.x) {
+            int i = d.gmem[off + b];
+            d.x[i] = d.bss.arr(BSA_Y + 0)[off + b]; d.y[i] = d.bss.arr(BSA_Y + 1)[off + b]; d.z[i] = d.bss.arr(BSA_Y + 2)[off + b];
+            d.vx[i] = d.bss.arr(BSA_Y + 3)[off + b]; d.vy[i] = d.bss.arr(BSA_Y + 4)[off + b]; d.vz[i] = d.bss.arr(BSA_Y + 5)[off + b];
+        }
+        if (threadIdx.x == 0) {
+            if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
+        }
+        __syncthreads();
+    }
+}
+
+// Test-particle groups (L342): {particle} + the massive bodies it meets + their massive
+// groups; everything integrated from the state before the drift, only the particle is
+// written back.  One team of TW lanes per listed particle; teams whose group does not fit
+// TW (or fits the next smaller instantiation, `lo`) skip.
+template <int TW>
+__global__ void __launch_bounds__(128) k_tp_bs(DevState d, double h, int lo)
+{
+    constexpr int TPB = 128 / TW;                       // teams per block
+    __shared__ TeamSmem<TW> sm[TPB];
+    const int ntp = d.cnt[CI_NTP];
+    const int team = threadIdx.x / TW, lane = threadIdx.x % TW;
+    const int lane32 = threadIdx.x & 31;
+    const unsigned tmask = TW == 32 ? 0xffffffffu : (((1u << TW) - 1u) << (lane32 - lane));
+    WarpTeam<TW> t{tmask, lane};
+    for (int k = blockIdx.x * TPB + team; k < ntp; k += gridDim.x * TPB) {
+        const int p = d.tplist[k];
+        unsigned mask = d.tpmask[p - d.nm], full = 0u;
+        int lab = p;
+        for (unsigned mm = mask; mm; mm &= mm - 1) {
+            int j = __ffs(mm) - 1;
+            full |= d.gmask[j];
+            lab = min(lab, d.label[j]);
+        }
+        const int nb = __popc(full) + 1;
+        if (nb > TW || nb <= lo) {
+            if (nb > 32 && TW == 32 && lane == 0) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);  // 32 massive + particle
+            continue;
+        }
+        const bool active = lane < nb;
+        int i = p;
+        if (lane < nb - 1) {                         // lane-th set bit of full
+            unsigned mm = full;
+            for (int c = 0; c < lane; ++c) mm &= mm - 1;
+            i = __ffs(mm) - 1;
+        }
+        double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0}, rc = 0.0;
+        t.sync();
+        sm[team].m[lane] = 0.0; sm[team].rc[lane] = 0.0;
+        if (active) {
+            q[0] = d.x0[i]; q[1] = d.y0[i]; q[2] = d.z0[i]; V[0] = d.vx0[i]; V[1] = d.vy0[i]; V[2] = d.vz0[i];
+            rc = d.rc[i];
+            sm[team].m[lane] = d.m[i]; sm[team].rc[lane] = rc;
+        }
+        t.sync();
+        int nsteps = 0;
+        unsigned srcmask = nb >= 32 ? 0xffffffffu : ((1u << nb) - 1u);
+        bool ok = bs_team<TW>(t, sm[team], nb, active, srcmask, d.G, d.m0[0], rc, q, V, h, d.eps, &nsteps);
+        if (lane == nb - 1) {
+            d.x[p] = q[0]; d.y[p] = q[1]; d.z[p] = q[2]; d.vx[p] = V[0]; d.vy[p] = V[1]; d.vz[p] = V[2];
+            d.label[p] = lab;
+            if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
+            atomicAdd((unsigned long long *)&d.stat[CNT_GROUPS], 1ull);
+            atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)nb);
+        }
+    }
+}
+template __global__ void k_tp_bs<4>(DevState, double, int);
+template __global__ void k_tp_bs<32>(DevState, double, int);
+
+// Multi-system mode (L372-376): 16 lanes per system; the groups of a system are the sets of
+// equal labels among its bodies, integrated one after the other by the system's lanes.
+__global__ void __launch_bounds__(128) k_bs_multi(DevState d, double h)
+{
+    constexpr int TW = 16, TPB = 128 / TW;
+    __shared__ TeamSmem<TW> sm[TPB];
+    if (d.cnt[CI_NENC] == 0) return;
+    const int team = threadIdx.x / TW, lane = threadIdx.x % TW, lane32 = threadIdx.x & 31;
+    const unsigned tmask = 0xffffu << (lane32 - lane);
+    WarpTeam<TW> t{tmask, lane};
+    const int sys = blockIdx.x * TPB + team;
+    if (sys >= d.nsys) return;
+    const int nm = d.nm, base = sys * nm;
+    const bool have = lane < nm;
+    const int i = base + lane;
+    int lab = have ? d.label[i] - base : -1 - lane;
+    // lanes of my group
+    unsigned grp = 0u;
+    for (int j = 0; j < TW; ++j) {
+        int lj = __shfl_sync(tmask, lab, j, TW);
+        if (lj == lab) grp |= 1u << j;
+    }
+    unsigned todo = __ballot_sync(tmask, have && __popc(grp) >= 2 && lab == lane) >> (lane32 - lane) & 0xffffu;  // roots
+    if (todo == 0u) return;
+    double rc = have ? d.rc[i] : 0.0;
+    sm[team].m[lane] = have ? d.m[i] : 0.0; sm[team].rc[lane] = rc;
+    t.sync();
+    int ngroups = 0, nsteps_tot = 0, big = 0;
+    bool ok = true;
+    while (todo) {
+        int root = __ffs(todo) - 1;
+        todo &= todo - 1;
+        unsigned gm = __shfl_sync(tmask, grp, root, TW);
+        bool active = (gm >> lane) & 1u;
+        double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0};
+        if (active) { q[0] = d.x0[i]; q[1] = d.y0[i]; q[2] = d.z0[i]; V[0] = d.vx0[i]; V[1] = d.vy0[i]; V[2] = d.vz0[i]; }
+        int nsteps = 0;
+        ok = bs_team<TW>(t, sm[team], TW, active, gm, d.G, d.m0[sys], rc, q, V, h, d.eps, &nsteps) && ok;
+        if (active) { d.x[i] = q[0]; d.y[i] = q[1]; d.z[i] = q[2]; d.vx[i] = V[0]; d.vy[i] = V[1]; d.vz[i] = V[2]; }
+        ++ngroups; nsteps_tot += nsteps; big = max(big, __popc(gm));
+    }
+    if (lane == 0) {
+        if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
+        atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps_tot);
+        atomicAdd((unsigned long long *)&d.stat[CNT_GROUPS], (unsigned long long)ngroups);
+        atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)big);
+    }
+}
+
+// =====================================================================================
+// Energy and angular momentum (Eq. 1-3 summed, L73-80; L225): one block per system.
+// out[sys][0] = E, out[sys][1..3] = L.
+__global__ void __launch_bounds__(1024) k_energy(DevState d, double *out)
+{
+    __shared__ double red[8][32];
+    const int sys = blockIdx.x, nm = d.nm, base = d.mode == 2 ? sys * nm : 0;
+    const double m0 = d.m0[sys];
+    double s[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // kin, pot0, pair, px, py, pz | Lx.. in second pass
+    double lx = 0, ly = 0, lz = 0;
+    for (int k = threadIdx.x; k < nm; k += blockDim.x) {
+        int i = base + k;
+        double m = d.m[i], x = d.x[i], y = d.y[i], z = d.z[i], vx = d.vx[i], vy = d.vy[i], vz = d.vz[i];
+        s[0] += 0.5 * m * (vx * vx + vy * vy + vz * vz);
+        s[1] -= d.G * m0 * m / sqrt(x * x + y * y + z * z);
+        s[3] += m * vx; s[4] += m * vy; s[5] += m * vz;
+        lx += m * (y * vz - z * vy); ly += m * (z * vx - x * vz); lz += m * (x * vy - y * vx);
+        double pp = 0.0;
+        for (int kk = k + 1; kk < nm; ++kk) {
+            int j = base + kk;
+            double dx = d.x[j] - x, dy = d.y[j] - y, dz = d.z[j] - z;
+            pp += d.m[j] / sqrt(dx * dx + dy * dy + dz * dz);
+        }
+        s[2] -= d.G * m * pp;
+    }
+    s[6] = lx; s[7] = ly;
+    double extra = lz;
+    for (int c = 0; c < 8; ++c)
+        for (int o = 16; o > 0; o >>= 1) s[c] += __shfl_xor_sync(0xffffffffu, s[c], o);
+    for (int o = 16; o > 0; o >>= 1) extra += __shfl_xor_sync(0xffffffffu, extra, o);
+    __shared__ double red2[32];
+    int w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if ((threadIdx.x & 31) == 0) { for (int c = 0; c < 8; ++c) red[c][w] = s[c]; red2[w] = extra; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+        for (int k = 0; k < nw; ++k) { for (int c = 0; c < 8; ++c) t[c] += red[c][k]; t[8] += red2[k]; }
+        out[4 * sys] = t[0] + (t[3] * t[3] + t[4] * t[4] + t[5] * t[5]) / (2.0 * m0) + t[1] + t[2];
+        out[4 * sys + 1] = t[6]; out[4 * sys + 2] = t[7]; out[4 * sys + 3] = t[8];
+    }
+}
+
+// labels for genga_encounters: body's own index unless it is in a group
+__global__ void k_export_labels(DevState d, int *out)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.ntot) return;
+    int l = i;
+    if (d.mode != 1 || i < d.nm) l = d.label[i];
+    else if (d.tpmask[i - d.nm] != 0u) l = d.label[i];
+    out[i] = l;
+}
+
+}  // namespace genga

@@ -1,0 +1,42 @@
+// Device-side view of one context's workspace (passed by value to every kernel).
+#pragma once
+#include "bs.cuh"
+#include "common.cuh"
+
+namespace genga {
+
+struct DevState {
+    int mode;        // 0 massive, 1 test particles, 2 multi system
+    int nm;          // massive bodies per system
+    int ntot;        // all bodies
+    int nsys;        // systems
+    int np;          // padded array stride (>= ntot)
+    int nmtot;       // massive bodies in total (nm, or nsys*nm in mode 2)
+    double G, n1, n2, eps;
+    double *m0;      // [nsys]
+    // democratic state, SoA [np]
+    double *x, *y, *z, *vx, *vy, *vz, *m, *radius;
+    double *rc, *c9;             // critical radius, 9 rc^2 (precheck threshold squared, L142)
+    double *x0, *y0, *z0, *vx0, *vy0, *vz0;   // state before the drift (Eq. 10 needs both ends)
+    double *apart;   // kick partial sums [nslice][3][npm]
+    int nslice, npm;
+    double *psum;    // [nsys][4]: sum m V (x,y,z) of the massive bodies, and sum m
+    int2 *cand, *enc;
+    long long cap;
+    int *cnt;        // device ints: see CI_* below
+    int *label;      // [np] group label of massive bodies
+    int *gstart, *gsize, *gmem;  // groups of massive bodies (mode 0/1): [npm]
+    unsigned *gmask;             // mode 1: bit mask of the massive group of body i
+    unsigned *tpmask;            // mode 1: per particle, massive bodies it meets
+    int *tplist;                 // mode 1: particles with encounters in this substep
+    long long *stat;             // CNT_* accumulators
+    BsScratch bss;
+};
+
+// indices into DevState::cnt
+enum : int { CI_NCAND = 0, CI_NENC = 1, CI_NGROUPS = 2, CI_NTP = 3, CI_STATUS = 4, CI_NTP_PREV = 5,
+             CI_NBIG = 6, CI_COUNT = 16 };
+
+__device__ __forceinline__ int system_of(const DevState &d, int i) { return d.mode == 2 ? i / d.nm : 0; }
+
+}  // namespace genga
