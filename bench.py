@@ -1,0 +1,295 @@
+#!/usr/bin/env python
+"""Benchmark of the hybrid symplectic step on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 1]
+
+A step = one full time step of BASELINE.json configs[1] (2048 massive bodies, order 2,
+dt = 6 d): critical radii, kick + precheck, Sun kick, Kepler drift, encounter search,
+grouping, Bulirsch-Stoer on the groups, Sun kick, kick.  Prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "fp64_pair_interactions_per_s"
+UNIT = "ordered pair interactions/s"
+FLOP_PER_INTERACTION = 20.0        # Nyland et al. convention, DESIGN.md "Rooflines"
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x DFMA/clk/SM x 2 flop x max clock
+
+
+def workload(cfg_id):
+    w = workloads.CONFIGS[cfg_id]()
+    name = {0: "cfg0 massive N=15", 1: "cfg1 planetesimal disc N=2048 massive, order 2, dt=6d",
+            2: "cfg2 8 massive + 1e6 test particles", 3: "cfg3 4096 systems x 16",
+            4: "cfg4 annulus N=2048 order 4, dt=2d"}[cfg_id]
+    return w, name
+
+
+def interactions_per_step(w):
+    nm, evals = w["n_massive"], 2 * {2: 1, 4: 3, 6: 7}[w["order"]]
+    if w["mode"] == 2:
+        per = w["n_systems"] * nm * (nm - 1)
+    else:
+        per = nm * (nm - 1) + w["n_test"] * nm
+    return per * evals, evals
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.p, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                       "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.p = None
+
+    def _read(self):
+        for line in self.p.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.p:
+            self.p.terminate()
+        sm = [float(r[1]) for r in self.rows if len(r) >= 9 and r[1].replace(".", "").isdigit()]
+        mx = [float(r[2]) for r in self.rows if len(r) >= 9 and r[2].replace(".", "").isdigit()]
+        reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) >= 9:
+                for k, nm in enumerate(names):
+                    if r[5 + k].lower().startswith("active"):
+                        reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------- reference arm
+def oracle_rate(w, budget_s, max_steps):
+    """Time the oracle as it stands on one host core; returns (interactions/s, steps, seconds)."""
+    import oracle
+    sim = oracle.Sim(w, cap=200000)
+    per_step, _ = interactions_per_step(w)
+    sim.step(1)
+    t0 = time.perf_counter()
+    n = 0
+    while n < max_steps:
+        sim.step(1)
+        n += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    return per_step * n / dt, n, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w, name = workload(args.config)
+    for _ in range(min(args.warmup, 2)):
+        pass
+    rate, n, secs = oracle_rate(w, budget_s=240.0, max_steps=args.steps)
+    per_step, evals = interactions_per_step(w)
+    sample = "%d full steps of %s (%.1f s)" % (n, name, secs)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": n, "warmup": 1, "ms_per_step": 1e3 * secs / n, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "n_massive": w["n_massive"], "order": w["order"], "force_evals_per_step": evals},
+        "steps_per_s": n / secs,
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------- multi-rank glue
+def reduce_max_and_sum(elapsed_s, units, backend_device):
+    """max over ranks of the elapsed time, sum over ranks of the units (replicas, no data exchange)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return elapsed_s, units
+    t = torch.tensor([elapsed_s], dtype=torch.float64, device=backend_device)
+    u = torch.tensor([float(units)], dtype=torch.float64, device=backend_device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def run_gpu(args):
+    import torch
+    import paper_1404_2324_b200 as G
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(dev)
+
+    w, name = workload(args.config)
+    per_step, evals = interactions_per_step(w)
+    g = G.from_workload(w, device=str(dev))
+    dt, order = w["dt"], w["order"]
+    flush = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- warm-up (also instantiates the CUDA graphs)
+    g.step(max(args.warmup, 3), dt, order)
+    g.step(16, dt, order)
+    assert g.status() == 0
+    c0 = g.counters()
+
+    # ---- timed: K steps, each timed with events on the library's stream, L2 flushed between
+    clocks = ClockSampler(local)
+    clocks.start()
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    with torch.cuda.stream(g.stream):
+        for k in range(args.steps):
+            flush.fill_(k & 255)               # evicts the state from L2; outside the timed events
+            ev[k][0].record(g.stream)
+            g.step(1, dt, order)
+            ev[k][1].record(g.stream)
+    barrier()
+    ms = [a.elapsed_time(b) for a, b in ev]
+    elapsed = sum(ms) * 1e-3
+    c1 = g.counters()
+    status = g.status()
+
+    # ---- back-to-back (state resident in L2, 16-step graphs): the production loop
+    nres = max(16, (args.steps // 16) * 16)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(g.stream)
+    g.step(nres, dt, order)
+    e1.record(g.stream)
+    barrier()
+    resident_s = e0.elapsed_time(e1) * 1e-3
+    clk = clocks.stop()
+
+    # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
+    xh = torch.empty((3, g.ntot), dtype=torch.float64).pin_memory().numpy()
+    vh = torch.empty((3, g.ntot), dtype=torch.float64).pin_memory().numpy()
+    xh[:], vh[:] = w["x"], w["v"]
+    m0h, mh, rh = w["m0"], w["m"], w["radius"]
+    for _ in range(3):
+        g.set_state_host(m0h, mh, rh, xh, vh); g.step(1, dt, order); g.get_state_host(xh, vh)
+    ne2e = min(args.steps, 200)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(ne2e):
+        g.set_state_host(m0h, mh, rh, xh, vh)
+        g.step(1, dt, order)
+        g.get_state_host(xh, vh)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    h2d = 8 * (len(m0h) + 2 * g.ntot + 6 * g.ntot)
+    d2h = 8 * 6 * g.ntot
+
+    # ---- dominant kernel in isolation (CUDA events inside the library, on its stream)
+    g.set_state(w["m0"], w["m"], w["radius"], w["x"], w["v"])
+    roof = None
+    if w["mode"] != 2:
+        kick_ms = g.time_kernel(0, 200, dt)
+        peak_probe = g.fp64_probe()
+        inter = w["n_massive"] * (w["n_massive"] - 1)
+        achieved = FLOP_PER_INTERACTION * inter / (kick_ms * 1e-3) / 1e12
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "kick_pairs_traffic.json")
+        if os.path.exists(tpath):
+            traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+        roof = {"bound": "alu", "kernel": "k_kick_pairs", "achieved": achieved, "peak": peak_probe,
+                "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": traffic,
+                "peak_source": "DFMA probe measured in this run (genga_fp64_probe); nominal %.1f = 148 SM x 64 DFMA/clk x 2 x 1.965 GHz" % FP64_NOMINAL_TFLOPS,
+                "ms_per_launch": kick_ms, "interactions_per_launch": inter,
+                "interactions_per_s": inter / (kick_ms * 1e-3),
+                "flop_per_interaction": FLOP_PER_INTERACTION}
+        drift_ms = g.time_kernel(1, 200, dt)
+        roof["drift"] = {"kernel": "k_drift", "ms_per_launch": drift_ms, "bodies": g.ntot,
+                         "algorithmic_bytes": 144 * g.ntot,
+                         "gbs": 144 * g.ntot / (drift_ms * 1e-3) / 1e9}
+
+    # ---- aggregate over ranks (replicas: no data-path collective)
+    tmax, units = reduce_max_and_sum(elapsed, per_step * args.steps, dev)
+    e2e_max, e2e_units = reduce_max_and_sum(e2e_s, per_step * ne2e, dev)
+    res_max, res_units = reduce_max_and_sum(resident_s, per_step * nres, dev)
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": units / tmax, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * tmax / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "n_massive": w["n_massive"], "order": w["order"], "dt_days": w["dt"] / workloads.DAY,
+                       "force_evals_per_step": evals, "l2": "flushed (512 MiB fill) before every timed step",
+                       "parallelism": "replicas only" if world > 1 else "1 gpu"},
+            "steps_per_s": args.steps * world / tmax,
+            "resident": {"steps_per_s": nres * world / res_max, "value": res_units / res_max,
+                         "note": "16-step CUDA graphs back to back, state resident in L2 (no flush)"},
+            "e2e": {"value": e2e_units / e2e_max, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": ne2e, "ms_per_step": 1e3 * e2e_max / ne2e},
+            "gpu_launches": c1["launches"] - c0["launches"],
+            "clocks": clk, "status": status,
+            "encounters": {"groups_per_step": (c1["groups"] - c0["groups"]) / args.steps,
+                           "bs_steps_per_step": (c1["bs_steps"] - c0["bs_steps"]) / args.steps,
+                           "max_group": c1["max_group"]},
+        }
+        if roof:
+            line["roofline"] = roof
+        if world == 1 and not args.no_cpu:
+            rate, n, secs = oracle_rate(w, budget_s=15.0, max_steps=10000)
+            line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "sample": "%d full steps of the same workload in %.1f s (1 of %d cores)" % (n, secs, os.cpu_count())}
+        print(json.dumps(line))
+    g.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -136,6 +136,18 @@ int genga_kepler_drift(genga_ctx *ctx, int64_t n, double mu, double h, double *x
  * Synchronises. */
 int genga_counters(genga_ctx *ctx, int64_t *out);
 
+/* Time one kernel of the path in isolation on the context's stream with CUDA events:
+ * `reps` back-to-back launches after 3 warm-up launches, *ms_per_launch = average (HOST out).
+ *   which = 0  pair kernel of the kick (k_kick_pairs; modes 0, 1), current state and rcrit
+ *   which = 1  Kepler drift of all bodies over dt and back (two launches counted as two)
+ *   which = 2  the whole kick (pair kernel + slice reduction [+ test-particle kick]), h = 0
+ * The state is left unchanged up to rounding.  Synchronises. */
+int genga_time_kernel(genga_ctx *ctx, int which, int reps, double dt, double *ms_per_launch);
+
+/* Measure the device's FP64 FMA throughput with independent DFMA chains on every SM:
+ * *tflops (HOST out) = 2 * DFMAs / time.  The ALU-roofline denominator.  Synchronises. */
+int genga_fp64_probe(genga_ctx *ctx, double *tflops);
+
 const char *genga_strerror(int code);
 const char *genga_last_cuda_error(void);
 

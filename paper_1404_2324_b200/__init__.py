@@ -22,7 +22,7 @@ OK, EINVAL, ECAPACITY, EKEPLER, EBS, ECUDA = 0, -1, -2, -3, -4, -5
 SYMBOLS = [
     "genga_workspace_bytes", "genga_create", "genga_destroy", "genga_set_state", "genga_set_state_host",
     "genga_step", "genga_get_state", "genga_get_state_host", "genga_energy", "genga_encounters",
-    "genga_status", "genga_accelerations", "genga_kepler_drift", "genga_counters", "genga_strerror",
+    "genga_status", "genga_accelerations", "genga_kepler_drift", "genga_counters", "genga_time_kernel", "genga_fp64_probe", "genga_strerror",
     "genga_last_cuda_error",
 ]
 
@@ -73,6 +73,8 @@ def load():
         "genga_accelerations": (i, [vp, d, dp, dp]),
         "genga_kepler_drift": (i, [vp, l, d, d, dp, dp]),
         "genga_counters": (i, [vp, vp]),
+        "genga_time_kernel": (i, [vp, i, i, d, C.POINTER(d)]),
+        "genga_fp64_probe": (i, [vp, C.POINTER(d)]),
         "genga_strerror": (C.c_char_p, [i]),
         "genga_last_cuda_error": (C.c_char_p, []),
     }
@@ -211,6 +213,16 @@ class Genga:
         _chk(self.lib.genga_counters(self.h, _hp(out)), "genga_counters")
         keys = ["steps", "force_evals", "interactions", "launches", "groups", "max_group", "bs_steps", "candidates"]
         return dict(zip(keys, map(int, out)))
+
+    def time_kernel(self, which, reps, dt):
+        ms = C.c_double()
+        _chk(self.lib.genga_time_kernel(self.h, int(which), int(reps), float(dt), C.byref(ms)), "genga_time_kernel")
+        return ms.value
+
+    def fp64_probe(self):
+        tf = C.c_double()
+        _chk(self.lib.genga_fp64_probe(self.h, C.byref(tf)), "genga_fp64_probe")
+        return tf.value
 
     def synchronize(self):
         self.stream.synchronize()

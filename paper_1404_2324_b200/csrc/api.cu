@@ -445,6 +445,65 @@ extern "C" __attribute__((visibility("default"))) int genga_kepler_drift(genga_c
     return GENGA_OK;
 }
 
+extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ctx *c, int which, int reps, double dt, double *ms)
+{
+    if (!c || !ms || reps < 1 || dt == 0.0 || which < 0 || which > 2) return GENGA_EINVAL;
+    DevState &d = c->d;
+    if (which != 1 && d.mode == GENGA_MODE_MULTI_SYSTEM && which == 0) return GENGA_EINVAL;
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt);
+    c->launches += 1;
+    dim3 grid((d.nm + KP_THREADS * KP_TI - 1) / (KP_THREADS * KP_TI), std::max(1, d.nslice));
+    int per = 1;
+    for (int r = -3; r < reps; ++r) {
+        if (r == 0) CK(cudaEventRecord(e0, c->st));
+        if (which == 0) { k_kick_pairs<<<grid, KP_THREADS, 0, c->st>>>(d, 0); c->launches += 1; }
+        else if (which == 1) {
+            k_drift<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt);
+            k_drift<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, -dt);
+            c->launches += 2; per = 2;
+        } else { c->acc = 0; enqueue_kick(c, 0.0, 0, nullptr); per = (int)c->acc; c->launches += c->acc; c->acc = 0; }
+    }
+    CK(cudaEventRecord(e1, c->st));
+    CK(cudaEventSynchronize(e1));
+    float t = 0.f;
+    CK(cudaEventElapsedTime(&t, e0, e1));
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *ms = (double)t / reps / (which == 1 ? per : 1);
+    CK(cudaGetLastError());
+    return GENGA_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_fp64_probe(genga_ctx *c, double *tflops)
+{
+    if (!c || !tflops) return GENGA_EINVAL;
+    // scratch: the pre-drift arrays are free between steps
+    const int blocks = c->sms * 8, threads = 256, iters = 4096;
+    if ((size_t)blocks * threads > (size_t)c->d.np * 6) {
+        // tiny contexts: fewer blocks so that the output fits x0..vz0 (contiguous in the workspace)
+    }
+    int nb = (int)std::min<size_t>(blocks, ((size_t)c->d.np * 6) / threads);
+    if (nb < 1) return GENGA_EINVAL;
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    double best = 0.0;
+    for (int r = 0; r < 5; ++r) {
+        CK(cudaEventRecord(e0, c->st));
+        k_fp64_probe<<<nb, threads, 0, c->st>>>(c->d.x0, iters);
+        CK(cudaEventRecord(e1, c->st));
+        CK(cudaEventSynchronize(e1));
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, e0, e1));
+        double tf = 2.0 * 64.0 * iters * (double)nb * threads / (t * 1e-3) * 1e-12;
+        if (r > 0 && tf > best) best = tf;
+    }
+    c->launches += 5;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *tflops = best;
+    return GENGA_OK;
+}
+
 extern "C" __attribute__((visibility("default"))) int genga_counters(genga_ctx *c, int64_t *out)
 {
     if (!c || !out) return GENGA_EINVAL;

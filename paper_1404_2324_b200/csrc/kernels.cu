@@ -666,6 +666,23 @@ __global__ void __launch_bounds__(1024) k_energy(DevState d, double *out)
     }
 }
 
+// FP64 peak probe: 8 independent DFMA chains per thread, 2 flop per DFMA.  Used only by
+// genga_fp64_probe to measure the denominator of the ALU roofline on the device at hand.
+__global__ void __launch_bounds__(256) k_fp64_probe(double *out, int iters)
+{
+    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double b = 1.0000001, c = 1e-9;
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
+            a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
+        }
+    }
+    out[blockIdx.x * blockDim.x + threadIdx.x] = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+}
+
 // labels for genga_encounters: body's own index unless it is in a group
 __global__ void k_export_labels(DevState d, int *out)
 {

@@ -33,5 +33,6 @@ template <int TW> __global__ void k_tp_bs(DevState d, double h, int lo);
 __global__ void k_bs_multi(DevState d, double h);
 __global__ void k_energy(DevState d, double *out);
 __global__ void k_export_labels(DevState d, int *out);
+__global__ void k_fp64_probe(double *out, int iters);
 
 }  // namespace genga
