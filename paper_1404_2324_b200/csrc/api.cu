@@ -37,6 +37,8 @@ struct genga_ctx {
     genga_config cfg;
     DevState d;
     cudaStream_t st;
+    cudaStream_t aux[2];        // helper streams: the Bulirsch-Stoer layouts run side by side
+    cudaEvent_t ev_fork, ev_join[2];
     int sms;
     int *exp_labels;            // device [np]
     double *eout;               // device [4*nsys]
@@ -80,17 +82,12 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
     t.psum = (double *)take(sizeof(double) * 4 * nsys);
     *eout = (double *)take(sizeof(double) * 4 * nsys);
     if (c->mode != GENGA_MODE_MULTI_SYSTEM) {
-        int ib = (nm + KP_THREADS * KP_TI - 1) / (KP_THREADS * KP_TI);
-        int smin = (nm + KP_MAXJ - 1) / KP_MAXJ;
-        int s = std::min(std::max(1, sms / ib), (nm + 7) / 8);
-        t.nslice = std::max(smin, s);
-        t.apart = (double *)take(sizeof(double) * (size_t)t.nslice * 3 * npm);
         t.gstart = (int *)take(sizeof(int) * npm);
         t.gsize = (int *)take(sizeof(int) * npm);
         t.gmem = (int *)take(sizeof(int) * npm);
         t.gmask = (unsigned *)take(sizeof(unsigned) * 32);
     }
-    if (c->mode == GENGA_MODE_MASSIVE && nm > 32) {
+    if (c->mode == GENGA_MODE_MASSIVE && nm > BSS_MAXN) {
         t.bss.stride = npm;
         t.bss.base = (double *)take(sizeof(double) * (size_t)BSA_COUNT * npm);
     }
@@ -140,7 +137,13 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     size_t need = carve(cfg, (char *)cfg->workspace, &c->d, &c->exp_labels, &c->eout, c->sms);
     if (need > cfg->workspace_bytes) { delete c; return GENGA_EINVAL; }
     cudaError_t e = cudaMemsetAsync(cfg->workspace, 0, need, c->st);
-    if (e != cudaSuccess) { delete c; snprintf(g_cuda_err, sizeof g_cuda_err, "memset: %s", cudaGetErrorString(e)); return GENGA_ECUDA; }
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bs_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BssSmem));
+    for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+        e = cudaStreamCreateWithFlags(&c->aux[k], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
+    if (e != cudaSuccess) { delete c; snprintf(g_cuda_err, sizeof g_cuda_err, "create: %s", cudaGetErrorString(e)); return GENGA_ECUDA; }
     *out = c;
     return GENGA_OK;
 }
@@ -149,6 +152,8 @@ extern "C" __attribute__((visibility("default"))) int genga_destroy(genga_ctx *c
 {
     if (!c) return GENGA_EINVAL;
     for (auto &kv : c->graphs) cudaGraphExecDestroy(kv.second.exec);
+    for (int k = 0; k < 2; ++k) { cudaStreamDestroy(c->aux[k]); cudaEventDestroy(c->ev_join[k]); }
+    cudaEventDestroy(c->ev_fork);
     delete c;
     return GENGA_OK;
 }
@@ -201,6 +206,19 @@ extern "C" __attribute__((visibility("default"))) int genga_set_state_host(genga
 }
 
 // ---------------------------------------------------------------------------------------
+// kick of the massive bodies: one block per SM owning ni bodies i, TJ bodies j per thread
+static void launch_kick(genga_ctx *c, double h, int record, double *aout)
+{
+    DevState &d = c->d;
+    const int ni = std::min(KK_NI, (d.nm + c->sms - 1) / c->sms);
+    const int grid = (d.nm + ni - 1) / ni;
+    const int tj = (d.nm + KK_THREADS - 1) / KK_THREADS;
+    if (tj <= 1) k_kick<1><<<grid, KK_THREADS, 0, c->st>>>(d, h, record, ni, aout);
+    else if (tj <= 2) k_kick<2><<<grid, KK_THREADS, 0, c->st>>>(d, h, record, ni, aout);
+    else if (tj <= 4) k_kick<4><<<grid, KK_THREADS, 0, c->st>>>(d, h, record, ni, aout);
+    else k_kick<8><<<grid, KK_THREADS, 0, c->st>>>(d, h, record, ni, aout);
+}
+
 static void enqueue_kick(genga_ctx *c, double h, int record, double *aout)
 {
     DevState &d = c->d;
@@ -209,10 +227,8 @@ static void enqueue_kick(genga_ctx *c, double h, int record, double *aout)
         LAUNCH(c);
         return;
     }
-    dim3 grid((d.nm + KP_THREADS * KP_TI - 1) / (KP_THREADS * KP_TI), d.nslice);
-    k_kick_pairs<<<grid, KP_THREADS, 0, c->st>>>(d, record);
-    k_kick_apply<<<nblk(d.nm, 128), 128, 0, c->st>>>(d, h, aout);
-    LAUNCH(c); LAUNCH(c);
+    launch_kick(c, h, record, aout);
+    LAUNCH(c);
     if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {
         k_tp_kick<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, h, record, aout);
         LAUNCH(c);
@@ -246,8 +262,24 @@ static void enqueue_map(genga_ctx *c, double h)
         k_bs_multi<<<nblk(d.nsys, 8), 128, 0, st>>>(d, h); LAUNCH(c);
     } else {
         k_build_groups<<<1, 1024, 0, st>>>(d); LAUNCH(c);
+        // the three Bulirsch-Stoer layouts work on disjoint groups: run them side by side
+        const bool mid = d.nm > BSW_MAXN;
+        if (mid) {
+            cudaEventRecord(c->ev_fork, st);
+            cudaStreamWaitEvent(c->aux[0], c->ev_fork, 0);
+            k_bs_smem<<<c->sms, BSS_THREADS, sizeof(BssSmem), c->aux[0]>>>(d, h); LAUNCH(c);
+            cudaEventRecord(c->ev_join[0], c->aux[0]);
+            if (d.bss.base) {
+                cudaStreamWaitEvent(c->aux[1], c->ev_fork, 0);
+                k_bs_block<<<16, 256, 0, c->aux[1]>>>(d, h); LAUNCH(c);
+                cudaEventRecord(c->ev_join[1], c->aux[1]);
+            }
+        }
         k_bs_warp<<<c->sms, 128, 0, st>>>(d, h); LAUNCH(c);
-        if (d.bss.base) { k_bs_block<<<16, 256, 0, st>>>(d, h); LAUNCH(c); }
+        if (mid) {
+            cudaStreamWaitEvent(st, c->ev_join[0], 0);
+            if (d.bss.base) cudaStreamWaitEvent(st, c->ev_join[1], 0);
+        }
         if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {
             k_tp_bs<4><<<4 * c->sms, 128, 0, st>>>(d, h, 0);
             k_tp_bs<32><<<2 * c->sms, 128, 0, st>>>(d, h, 4);
@@ -449,16 +481,15 @@ extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ct
 {
     if (!c || !ms || reps < 1 || dt == 0.0 || which < 0 || which > 2) return GENGA_EINVAL;
     DevState &d = c->d;
-    if (which != 1 && d.mode == GENGA_MODE_MULTI_SYSTEM && which == 0) return GENGA_EINVAL;
+    if (d.mode == GENGA_MODE_MULTI_SYSTEM && which == 0) return GENGA_EINVAL;
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
     k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt);
     c->launches += 1;
-    dim3 grid((d.nm + KP_THREADS * KP_TI - 1) / (KP_THREADS * KP_TI), std::max(1, d.nslice));
     int per = 1;
     for (int r = -3; r < reps; ++r) {
         if (r == 0) CK(cudaEventRecord(e0, c->st));
-        if (which == 0) { k_kick_pairs<<<grid, KP_THREADS, 0, c->st>>>(d, 0); c->launches += 1; }
+        if (which == 0) { launch_kick(c, 0.0, 0, nullptr); c->launches += 1; }
         else if (which == 1) {
             k_drift<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt);
             k_drift<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, -dt);

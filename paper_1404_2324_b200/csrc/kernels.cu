@@ -19,7 +19,7 @@ __global__ void k_begin_map(DevState d)
 __global__ void k_reset_counters(DevState d)
 {
     if (threadIdx.x == 0) {
-        d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
+        d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0; d.cnt[CI_NMID] = 0;
     }
 }
 
@@ -46,122 +46,161 @@ __global__ void k_rcrit(DevState d, double tau)
 }
 
 // =====================================================================================
-// Kick, operator B (Eq. 2; L197, L238-264): a_i = sum_j G m_j (q_j - q_i)/r^3 W(r, rc_ij)
-// and the prechecker (L142).  Massive bodies of one system, N <= 2048.
+// Kick, operator B (Eq. 2; L197, L238-264): V_i += h a_i, a_i = sum_j G m_j (q_j - q_i)/r^3
+// W(r, rc_ij), and the prechecker (L142).  Massive bodies of one system, N <= 2048.
 //
-// Decomposition: grid (i-blocks of 512 bodies, j-slices).  Each thread keeps KP_TI bodies i
-// in registers and walks its j-slice, staged in shared memory and read as warp broadcasts.
-// Pairs inside the precheck sphere (r^2 < 9 rc_ij^2, which contains the whole changeover
-// zone r < rc_ij) are taken OUT of the fast loop: their (i, j) goes to a shared-memory list,
-// the weight W is evaluated for the list in parallel afterwards and added by the owning
-// thread in list order, so the sum is deterministic.  Partial sums per slice go to
-// apart[slice][c][i]; k_kick_apply adds the slices in fixed order.
-__global__ void __launch_bounds__(KP_THREADS) k_kick_pairs(DevState d, int record)
+// Layout.  The paper gives every body i a thread block whose threads split the j loop and
+// reduce (Table 2).  Here one block per SM owns ni = ceil(N / #SM) <= 14 bodies i;
+// each of its 256 threads keeps TJ = ceil(N / 256) bodies j in REGISTERS for the whole kernel
+// and meets the block's bodies i as shared-memory broadcasts, so a body j is loaded once per
+// block and the inner loop has no memory traffic.  The 3 ni partial sums per thread are
+// reduced by a halving butterfly inside each warp (48 shuffle+add steps for 42 values, fixed
+// order) and across the 8 warps through shared memory; the block then applies the kick to its
+// own bodies, so the whole operator is one launch with no partial sums in global memory.
+//
+// Per pair the fast path costs 16 FP64 issue slots: 3 subtractions, 3 for r^2, 7 for
+// G m_j r^-3 from the MUFU.RSQ64H seed (rinv3_fast), 3 accumulating FMAs.  The precheck
+// r^2 < 9 max(rc_i, rc_j)^2 is done on the HIGH WORDS of the doubles with integer compares
+// (a superset of the exact test, off the FP64 pipe); pairs that pass -- the whole changeover
+// zone r < rc_ij lies inside the precheck sphere -- get weight 0 in the fast path and set a
+// bit in a shared bitmap [ni][N], and are afterwards evaluated exactly (sqrt, W = K - r dK/dr,
+// candidate list) by the warp that owns the row, in ascending j per lane and a fixed
+// butterfly over lanes, so the sum is deterministic.
+template <int TJ>
+__global__ void __launch_bounds__(KK_THREADS) k_kick(DevState d, double h, int record, int ni, double *aout)
 {
-    __shared__ double sx[KP_MAXJ], sy[KP_MAXJ], sz[KP_MAXJ], sgm[KP_MAXJ], sc9[KP_MAXJ];
-    __shared__ int hits[KP_HCAP];
-    __shared__ double hcx[KP_HCAP], hcy[KP_HCAP], hcz[KP_HCAP];
-    __shared__ int nh;
+    __shared__ double sxi[KK_NI], syi[KK_NI], szi[KK_NI];
+    __shared__ int shc[KK_NI];
+    __shared__ unsigned bitmap[KK_NI][KK_WORDS];
+    __shared__ double red[KK_THREADS / 32][KK_NV];
+    __shared__ double acc_s[KK_NV];
+    __shared__ int anyhit;
 
-    const int N = d.nm, tid = threadIdx.x;
-    const int S = gridDim.y, s = blockIdx.y;
-    const int j0 = (int)((long long)s * N / S), j1 = (int)((long long)(s + 1) * N / S), jl = j1 - j0;
-    if (tid == 0) nh = 0;
-    for (int t = tid; t < jl; t += KP_THREADS) {
-        sx[t] = d.x[j0 + t]; sy[t] = d.y[j0 + t]; sz[t] = d.z[j0 + t];
-        sgm[t] = d.G * d.m[j0 + t]; sc9[t] = d.c9[j0 + t];
+    const int N = d.nm, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int i0 = blockIdx.x * ni;
+    const int nib = min(ni, N - i0);
+    if (tid < KK_NI) {
+        bool v = tid < nib;
+        sxi[tid] = v ? d.x[i0 + tid] : 0.0; syi[tid] = v ? d.y[i0 + tid] : 0.0; szi[tid] = v ? d.z[i0 + tid] : 0.0;
+        shc[tid] = v ? __double2hiint(d.c9[i0 + tid]) : -1;
     }
-    int ii[KP_TI];
-    double xi[KP_TI], yi[KP_TI], zi[KP_TI], ci[KP_TI], ax[KP_TI], ay[KP_TI], az[KP_TI];
+    for (int w = tid; w < KK_NI * KK_WORDS; w += KK_THREADS) (&bitmap[0][0])[w] = 0u;
+    if (tid == 0) anyhit = 0;
+
+    double xj[TJ], yj[TJ], zj[TJ], gm[TJ];
+    int hcj[TJ];
 #pragma unroll
-    for (int t = 0; t < KP_TI; ++t) {
-        ii[t] = blockIdx.x * (KP_THREADS * KP_TI) + t * KP_THREADS + tid;
-        bool valid = ii[t] < N;
-        xi[t] = valid ? d.x[ii[t]] : 1e100; yi[t] = valid ? d.y[ii[t]] : 1e100; zi[t] = valid ? d.z[ii[t]] : 1e100;
-        ci[t] = valid ? d.c9[ii[t]] : -1.0;
-        ax[t] = ay[t] = az[t] = 0.0;
+    for (int k = 0; k < TJ; ++k) {
+        int j = k * KK_THREADS + tid;
+        bool v = j < N;
+        xj[k] = v ? d.x[j] : 1e100; yj[k] = v ? d.y[j] : 1e100; zj[k] = v ? d.z[j] : 1e100;
+        gm[k] = v ? d.G * d.m[j] : 0.0;
+        hcj[k] = v ? __double2hiint(d.c9[j]) : -1;
+    }
+    double acc[KK_NV];
+#pragma unroll
+    for (int v = 0; v < KK_NV; ++v) acc[v] = 0.0;
+    __syncthreads();
+
+#pragma unroll
+    for (int ii = 0; ii < KK_NI; ++ii) {
+        if (ii < nib) {
+            const double xi = sxi[ii], yi = syi[ii], zi = szi[ii];
+            const int hci = shc[ii];
+#pragma unroll
+            for (int k = 0; k < TJ; ++k) {
+                double dx = xj[k] - xi, dy = yj[k] - yi, dz = zj[k] - zi;
+                double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                bool hit = __double2hiint(r2) <= max(hci, hcj[k]);
+                double s3 = gm[k] * rinv3_fast(r2);
+                if (hit) {
+                    int j = k * KK_THREADS + tid;
+                    atomicOr(&bitmap[ii][j >> 5], 1u << (j & 31));
+                    anyhit = 1;
+                    s3 = 0.0;                                   // counted exactly below (and r2 == 0 is the body itself)
+                }
+                acc[3 * ii] = fma(s3, dx, acc[3 * ii]);
+                acc[3 * ii + 1] = fma(s3, dy, acc[3 * ii + 1]);
+                acc[3 * ii + 2] = fma(s3, dz, acc[3 * ii + 2]);
+            }
+        }
+    }
+
+    // ---- warp reduction: halving butterfly 48 -> 24 -> 12 -> 6 -> 3, then the lane pair
+#pragma unroll
+    for (int half = KK_NV / 2, o = 16; o >= 2; half >>= 1, o >>= 1) {
+        const bool up = (lane & o) != 0;
+#pragma unroll
+        for (int v = 0; v < half; ++v) {
+            double send = up ? acc[v] : acc[v + half];
+            double keep = up ? acc[v + half] : acc[v];
+            acc[v] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+        }
+    }
+#pragma unroll
+    for (int v = 0; v < 3; ++v) acc[v] += __shfl_xor_sync(0xffffffffu, acc[v], 1);
+    if ((lane & 1) == 0) {
+        int base = ((lane >> 4) & 1) * 24 + ((lane >> 3) & 1) * 12 + ((lane >> 2) & 1) * 6 + ((lane >> 1) & 1) * 3;
+#pragma unroll
+        for (int v = 0; v < 3; ++v) red[warp][base + v] = acc[v];
+    }
+    __syncthreads();
+    if (tid < KK_NV) {
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < KK_THREADS / 32; ++w) t += red[w][tid];
+        acc_s[tid] = t;
     }
     __syncthreads();
 
-#pragma unroll 2
-    for (int jj = 0; jj < jl; ++jj) {
-        const double xj = sx[jj], yj = sy[jj], zj = sz[jj], gm = sgm[jj], cj = sc9[jj];
-#pragma unroll
-        for (int t = 0; t < KP_TI; ++t) {
-            double dx = xj - xi[t], dy = yj - yi[t], dz = zj - zi[t];
-            double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-            bool hit = r2 < fmax(ci[t], cj);
-            double rinv = rsqrt(r2);
-            double s3 = gm * rinv * (rinv * rinv);
-            if (hit) {
-                s3 = 0.0;
-                if (j0 + jj != ii[t]) {
-                    int slot = atomicAdd(&nh, 1);
-                    if (slot < KP_HCAP) hits[slot] = ((t * KP_THREADS + tid) << 16) | jj;
-                    else {
-                        // list full (pathologically dense encounters): finish the pair here
-                        double r = sqrt(r2);
-                        double rcij = fmax(d.rc[ii[t]], d.rc[j0 + jj]);
-                        s3 = gm / (r2 * r) * kick_weight(r, rcij);
-                        if (record && ii[t] < j0 + jj) {
-                            int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
-                            if (idx < d.cap) d.cand[idx] = make_int2(ii[t], j0 + jj);
-                            else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
-                        }
+    // ---- pairs inside the precheck sphere: exact weight, candidate list
+    if (anyhit) {
+        const int words = (N + 31) >> 5;
+        for (int ii = warp; ii < nib; ii += KK_THREADS / 32) {
+            const int i = i0 + ii;
+            const double xi = sxi[ii], yi = syi[ii], zi = szi[ii], rci = d.rc[i], c9i = d.c9[i];
+            double ax = 0.0, ay = 0.0, az = 0.0;
+            for (int w = lane; w < words; w += 32) {
+                unsigned bits = bitmap[ii][w];
+                while (bits) {
+                    int j = (w << 5) + __ffs(bits) - 1;
+                    bits &= bits - 1;
+                    if (j == i) continue;
+                    double dx = d.x[j] - xi, dy = d.y[j] - yi, dz = d.z[j] - zi;
+                    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                    double r = sqrt(r2);
+                    double rcij = fmax(rci, d.rc[j]);
+                    double s3 = d.G * d.m[j] / (r2 * r) * kick_weight(r, rcij);
+                    ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
+                    if (record && i < j && r2 < fmax(c9i, d.c9[j])) {
+                        int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
+                        if (idx < d.cap) d.cand[idx] = make_int2(i, j);
+                        else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
                     }
                 }
             }
-            ax[t] = fma(s3, dx, ax[t]); ay[t] = fma(s3, dy, ay[t]); az[t] = fma(s3, dz, az[t]);
-        }
-    }
-    __syncthreads();
-    const int nhc = min(nh, KP_HCAP);
-    // weights of the listed pairs, one pair per thread
-    for (int e = tid; e < nhc; e += KP_THREADS) {
-        int h = hits[e], jj = h & 0xffff, slot = h >> 16;
-        int i = blockIdx.x * (KP_THREADS * KP_TI) + slot, j = j0 + jj;
-        double dx = sx[jj] - d.x[i], dy = sy[jj] - d.y[i], dz = sz[jj] - d.z[i];
-        double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-        double r = sqrt(r2);
-        double rcij = fmax(d.rc[i], d.rc[j]);
-        double s3 = sgm[jj] / (r2 * r) * kick_weight(r, rcij);
-        hcx[e] = s3 * dx; hcy[e] = s3 * dy; hcz[e] = s3 * dz;
-        if (record && i < j) {
-            int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
-            if (idx < d.cap) d.cand[idx] = make_int2(i, j);
-            else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
-        }
-    }
-    __syncthreads();
-    if (nhc > 0) {
-        for (int e = 0; e < nhc; ++e) {
-            int slot = hits[e] >> 16;
 #pragma unroll
-            for (int t = 0; t < KP_TI; ++t)
-                if (slot == t * KP_THREADS + tid) { ax[t] += hcx[e]; ay[t] += hcy[e]; az[t] += hcz[e]; }
+            for (int o = 16; o > 0; o >>= 1) {
+                ax += __shfl_xor_sync(0xffffffffu, ax, o);
+                ay += __shfl_xor_sync(0xffffffffu, ay, o);
+                az += __shfl_xor_sync(0xffffffffu, az, o);
+            }
+            if (lane == 0) { acc_s[3 * ii] += ax; acc_s[3 * ii + 1] += ay; acc_s[3 * ii + 2] += az; }
         }
+        __syncthreads();
     }
-#pragma unroll
-    for (int t = 0; t < KP_TI; ++t)
-        if (ii[t] < N) {
-            double *p = d.apart + (size_t)s * 3 * d.npm;
-            p[ii[t]] = ax[t]; p[d.npm + ii[t]] = ay[t]; p[2 * d.npm + ii[t]] = az[t];
-        }
-}
-
-// V_i += h a_i with a_i = sum over slices in fixed order.  aout (optional): store a.
-__global__ void k_kick_apply(DevState d, double h, double *aout)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= d.nm) return;
-    double ax = 0, ay = 0, az = 0;
-    for (int s = 0; s < d.nslice; ++s) {
-        const double *p = d.apart + (size_t)s * 3 * d.npm;
-        ax += p[i]; ay += p[d.npm + i]; az += p[2 * d.npm + i];
+    if (tid < 3 * nib) {
+        const int ii = tid / 3, c = tid - 3 * ii, i = i0 + ii;
+        const double a = acc_s[tid];
+        double *v = c == 0 ? d.vx : c == 1 ? d.vy : d.vz;
+        v[i] = fma(h, a, v[i]);
+        if (aout) aout[(size_t)c * d.ntot + i] = a;
     }
-    if (aout) { aout[i] = ax; aout[d.ntot + i] = ay; aout[2 * (size_t)d.ntot + i] = az; }
-    d.vx[i] = fma(h, ax, d.vx[i]); d.vy[i] = fma(h, ay, d.vy[i]); d.vz[i] = fma(h, az, d.vz[i]);
 }
+template __global__ void k_kick<1>(DevState, double, int, int, double *);
+template __global__ void k_kick<2>(DevState, double, int, int, double *);
+template __global__ void k_kick<4>(DevState, double, int, int, double *);
+template __global__ void k_kick<8>(DevState, double, int, int, double *);
 
 // Kick of the test particles (L334-340): one thread per particle looping over the <= 32
 // massive bodies, which sit in shared memory (broadcast reads).  Precheck against every
@@ -183,8 +222,7 @@ __global__ void __launch_bounds__(128) k_tp_kick(DevState d, double h, int recor
         double dx = sx[j] - xi, dy = sy[j] - yi, dz = sz[j] - zi;
         double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
         double rcij = fmax(rci, src[j]);
-        double rinv = rsqrt(r2);
-        double s3 = sgm[j] * rinv * (rinv * rinv);
+        double s3 = sgm[j] * rinv3_fast(r2);
         if (r2 < 9.0 * rcij * rcij) {
             double r = sqrt(r2);
             s3 = sgm[j] / (r2 * r) * kick_weight(r, rcij);
@@ -216,8 +254,7 @@ __global__ void __launch_bounds__(128) k_kick_multi(DevState d, double h, int re
         double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
         double rcij = fmax(rci, d.rc[j]);
         double gm = d.G * d.m[j];
-        double rinv = rsqrt(r2);
-        double s3 = gm * rinv * (rinv * rinv);
+        double s3 = gm * rinv3_fast(r2);
         if (r2 < 9.0 * rcij * rcij) {
             double r = sqrt(r2);
             s3 = gm / (r2 * r) * kick_weight(r, rcij);
@@ -443,8 +480,10 @@ __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
     for (int o = 16; o > 0; o >>= 1) big = max(big, __shfl_xor_sync(0xffffffffu, big, o));
     if ((tid & 31) == 0 && big > 0) {
         atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)big);
-        if (big > 32) atomicAdd(&d.cnt[CI_NBIG], 1);
+        if (big > BSS_MAXN) atomicAdd(&d.cnt[CI_NBIG], 1);
     }
+    int mid = ((r0 && sz[i0] > BSW_MAXN && sz[i0] <= BSS_MAXN) || (r1 && sz[i1] > BSW_MAXN && sz[i1] <= BSS_MAXN)) ? 1 : 0;
+    if (__any_sync(0xffffffffu, mid) && (tid & 31) == 0) atomicAdd(&d.cnt[CI_NMID], 1);
 }
 
 // =====================================================================================
@@ -459,16 +498,16 @@ __global__ void __launch_bounds__(128) k_bs_warp(DevState d, double h)
     WarpTeam<32> t{0xffffffffu, lane};
     for (int g = blockIdx.x * 4 + wib; g < ng; g += gridDim.x * 4) {
         const int nb = d.gsize[g];
-        if (nb > 32) continue;
+        if (nb > BSW_MAXN) continue;
         const bool active = lane < nb;
         const int i = active ? d.gmem[d.gstart[g] + lane] : 0;
         double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0}, rc = 0.0;
         __syncwarp();
-        sm[wib].m[lane] = 0.0; sm[wib].rc[lane] = 0.0;
+        sm[wib].m[lane] = 0.0; sm[wib].rc[lane] = 0.0; sm[wib].irc[lane] = 0.0;
         if (active) {
             q[0] = d.x0[i]; q[1] = d.y0[i]; q[2] = d.z0[i]; V[0] = d.vx0[i]; V[1] = d.vy0[i]; V[2] = d.vz0[i];
             rc = d.rc[i];
-            sm[wib].m[lane] = d.m[i]; sm[wib].rc[lane] = rc;
+            sm[wib].m[lane] = d.m[i]; sm[wib].rc[lane] = rc; sm[wib].irc[lane] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
         }
         __syncwarp();
         int nsteps = 0;
@@ -476,6 +515,46 @@ __global__ void __launch_bounds__(128) k_bs_warp(DevState d, double h)
         bool ok = bs_team<32>(t, sm[wib], nb, active, srcmask, d.G, d.m0[0], rc, q, V, h, d.eps, &nsteps);
         if (active) { d.x[i] = q[0]; d.y[i] = q[1]; d.z[i] = q[2]; d.vx[i] = V[0]; d.vy[i] = V[1]; d.vz[i] = V[2]; }
         if (lane == 0) {
+            if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
+        }
+    }
+}
+
+// Groups of BSW_MAXN < n <= BSS_MAXN bodies: one block per group, everything in shared memory
+// (bs.cuh "Shared-memory block layout").
+__global__ void __launch_bounds__(BSS_THREADS) k_bs_smem(DevState d, double h)
+{
+    extern __shared__ __align__(16) unsigned char bss_raw[];
+    BssSmem &S = *reinterpret_cast<BssSmem *>(bss_raw);
+    __shared__ int nsteps;
+    if (d.cnt[CI_NMID] == 0) return;
+    const int ng = d.cnt[CI_NGROUPS];
+    for (int g = blockIdx.x; g < ng; g += gridDim.x) {
+        const int n = d.gsize[g];
+        if (n <= BSW_MAXN || n > BSS_MAXN) continue;
+        const int off = d.gstart[g];
+        int P = 32;
+        while (P < n) P <<= 1;
+        BssLane t;
+        t.n = n; t.L = BSS_THREADS / P; t.i = threadIdx.x / t.L; t.s = threadIdx.x % t.L;
+        t.owner = t.s == 0 && t.i < n;
+        __syncthreads();
+        if (threadIdx.x == 0) nsteps = 0;
+        for (int b = threadIdx.x; b < n; b += BSS_THREADS) {
+            int i = d.gmem[off + b];
+            S.Y[0][b] = d.x0[i]; S.Y[1][b] = d.y0[i]; S.Y[2][b] = d.z0[i];
+            S.Y[3][b] = d.vx0[i]; S.Y[4][b] = d.vy0[i]; S.Y[5][b] = d.vz0[i];
+            double rc = d.rc[i];
+            S.m[b] = d.m[i]; S.rc[b] = rc; S.irc[b] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
+        }
+        bool ok = bss_integrate(S, t, d.G, d.m0[0], h, d.eps, &nsteps);
+        for (int b = threadIdx.x; b < n; b += BSS_THREADS) {
+            int i = d.gmem[off + b];
+            d.x[i] = S.Y[0][b]; d.y[i] = S.Y[1][b]; d.z[i] = S.Y[2][b];
+            d.vx[i] = S.Y[3][b]; d.vy[i] = S.Y[4][b]; d.vz[i] = S.Y[5][b];
+        }
+        if (threadIdx.x == 0) {
             if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
             atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
         }
@@ -491,7 +570,7 @@ __global__ void __launch_bounds__(256) k_bs_block(DevState d, double h)
     const int ng = d.cnt[CI_NGROUPS];
     for (int g = blockIdx.x; g < ng; g += gridDim.x) {
         const int nb = d.gsize[g];
-        if (nb <= 32) continue;
+        if (nb <= BSS_MAXN) continue;
         const int off = d.gstart[g];
         if (threadIdx.x == 0) nsteps = 0;
         for (int b = threadIdx.x; b < nb; b += blockDim.x) {
@@ -552,11 +631,11 @@ __global__ void __launch_bounds__(128) k_tp_bs(DevState d, double h, int lo)
         }
         double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0}, rc = 0.0;
         t.sync();
-        sm[team].m[lane] = 0.0; sm[team].rc[lane] = 0.0;
+        sm[team].m[lane] = 0.0; sm[team].rc[lane] = 0.0; sm[team].irc[lane] = 0.0;
         if (active) {
             q[0] = d.x0[i]; q[1] = d.y0[i]; q[2] = d.z0[i]; V[0] = d.vx0[i]; V[1] = d.vy0[i]; V[2] = d.vz0[i];
             rc = d.rc[i];
-            sm[team].m[lane] = d.m[i]; sm[team].rc[lane] = rc;
+            sm[team].m[lane] = d.m[i]; sm[team].rc[lane] = rc; sm[team].irc[lane] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
         }
         t.sync();
         int nsteps = 0;
@@ -600,7 +679,7 @@ __global__ void __launch_bounds__(128) k_bs_multi(DevState d, double h)
     unsigned todo = __ballot_sync(tmask, have && __popc(grp) >= 2 && lab == lane) >> (lane32 - lane) & 0xffffu;  // roots
     if (todo == 0u) return;
     double rc = have ? d.rc[i] : 0.0;
-    sm[team].m[lane] = have ? d.m[i] : 0.0; sm[team].rc[lane] = rc;
+    sm[team].m[lane] = have ? d.m[i] : 0.0; sm[team].rc[lane] = rc; sm[team].irc[lane] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
     t.sync();
     int ngroups = 0, nsteps_tot = 0, big = 0;
     bool ok = true;

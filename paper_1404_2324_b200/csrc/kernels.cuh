@@ -4,16 +4,15 @@
 
 namespace genga {
 
-constexpr int KP_THREADS = 256;   // threads per block of the pair kernel
-constexpr int KP_TI = 2;          // bodies i per thread (register tile)
-constexpr int KP_MAXJ = 256;      // longest j-slice staged in shared memory
-constexpr int KP_HCAP = 1024;     // per-block list of pairs inside the precheck sphere
+constexpr int KK_THREADS = 256;   // threads per block of the kick kernel
+constexpr int KK_NI = 14;         // bodies i a block owns at most: ceil(2048 / 148)
+constexpr int KK_NV = 48;         // 3 KK_NI accumulators padded to 3 * 16 for the halving butterfly
+constexpr int KK_WORDS = 64;      // 2048 / 32 bitmap words per body i
 
 __global__ void k_begin_map(DevState d);
 __global__ void k_reset_counters(DevState d);
 __global__ void k_rcrit(DevState d, double tau);
-__global__ void k_kick_pairs(DevState d, int record);
-__global__ void k_kick_apply(DevState d, double h, double *aout);
+template <int TJ> __global__ void k_kick(DevState d, double h, int record, int ni, double *aout);
 __global__ void k_tp_kick(DevState d, double h, int record, double *aout);
 __global__ void k_kick_multi(DevState d, double h, int record, double *aout);
 __global__ void k_momentum(DevState d, const double *vx, const double *vy, const double *vz);
@@ -28,6 +27,7 @@ __global__ void k_union(DevState d);
 __global__ void k_flatten(DevState d);
 __global__ void k_build_groups(DevState d);
 __global__ void k_bs_warp(DevState d, double h);
+__global__ void k_bs_smem(DevState d, double h);
 __global__ void k_bs_block(DevState d, double h);
 template <int TW> __global__ void k_tp_bs(DevState d, double h, int lo);
 __global__ void k_bs_multi(DevState d, double h);

@@ -18,8 +18,7 @@ struct DevState {
     double *x, *y, *z, *vx, *vy, *vz, *m, *radius;
     double *rc, *c9;             // critical radius, 9 rc^2 (precheck threshold squared, L142)
     double *x0, *y0, *z0, *vx0, *vy0, *vz0;   // state before the drift (Eq. 10 needs both ends)
-    double *apart;   // kick partial sums [nslice][3][npm]
-    int nslice, npm;
+    int npm;         // nm padded to 128
     double *psum;    // [nsys][4]: sum m V (x,y,z) of the massive bodies, and sum m
     int2 *cand, *enc;
     long long cap;
@@ -35,7 +34,7 @@ struct DevState {
 
 // indices into DevState::cnt
 enum : int { CI_NCAND = 0, CI_NENC = 1, CI_NGROUPS = 2, CI_NTP = 3, CI_STATUS = 4, CI_NTP_PREV = 5,
-             CI_NBIG = 6, CI_COUNT = 16 };
+             CI_NBIG = 6, CI_NMID = 7, CI_COUNT = 16 };
 
 __device__ __forceinline__ int system_of(const DevState &d, int i) { return d.mode == 2 ? i / d.nm : 0; }
 

@@ -144,19 +144,21 @@ def test_encounter_heavy_small_case_with_groups(G):
         g.close()
 
 
-def test_large_group_block_path(G):
-    """n2 = 1.5 chains the inner disc into one big group (Fig. 15): the block-per-group
-    Bulirsch-Stoer layout must agree with the oracle."""
-    w = workloads.config1(n=300)
-    w["n2"] = 1.5
-    g = G.from_workload(w)
+@pytest.mark.parametrize("n,n2,min_group", [(300, 1.5, 17), (700, 8.0, 257)])
+def test_large_group_block_paths(G, n, n2, min_group):
+    """A large n2 chains the inner disc into big groups (Fig. 15): the shared-memory
+    block layout (17..256 bodies) and the global-scratch layout (> 256 bodies) of Bulirsch-Stoer must
+    agree with the oracle."""
+    w = workloads.config1(n=n)
+    w["n2"] = n2
+    g = G.from_workload(w, max_pairs=n * (n - 1) // 2)      # every pair may be a candidate here
     o = oracle.Sim(w, cap=g.max_pairs)
     g.step(2, w["dt"], 2)
     o.step(2, w["dt"], 2)
     x, v = g.get_state_host()
     assert g.status() == 0
     xo, vo = o.state()
-    assert g.counters()["max_group"] > 32
+    assert g.counters()["max_group"] >= min_group
     assert o.sys[0].stats()["max_group"] == g.counters()["max_group"]
     assert relerr(x, xo).max() < STATE_TOL and relerr(v, vo).max() < STATE_TOL
     pairs, _, labels = g.encounters()
@@ -172,7 +174,7 @@ def test_test_particle_groups(G):
     V = oracle.helio_to_demo(1.0, w["m"], v, 3)
     rc1 = oracle.rcrit(1.0, 1.0, 3.0, 0.4, w["dt"], w["m"], x, V)[1]
     for k in range(200):
-        f = 0.01 * (k + 1) * rc1 / np.linalg.norm(x[:, 1])
+        f = (0.05 + 0.01 * (k + 1)) * rc1 / np.linalg.norm(x[:, 1])
         x[:, 3 + k] = x[:, 1] * (1 + f); v[:, 3 + k] = v[:, 1] * (1 - 0.5 * f)
     w["x"], w["v"] = x, v
     g = G.from_workload(w)
@@ -187,6 +189,27 @@ def test_test_particle_groups(G):
     assert len(eo) > 50 and ncand == len(co)
     assert np.array_equal(pairs, eo) and np.array_equal(labels, lo)
     assert relerr(xs, xo).max() < STATE_TOL and relerr(vs, vo).max() < STATE_TOL
+    g.close()
+
+
+def test_point_mass_near_collision_reports_bs_underflow(G):
+    """Bodies are point masses on this path (collisions are not on it): a particle dropped
+    almost onto a planet makes Bulirsch-Stoer shrink its step below the guard; both sides must report
+    that as an error instead of hanging or returning garbage."""
+    w = workloads.config2(n_massive=3, n_test=8)
+    x, v = w["x"].copy(), w["v"].copy()
+    V = oracle.helio_to_demo(1.0, w["m"], v, 3)
+    rc1 = oracle.rcrit(1.0, 1.0, 3.0, 0.4, w["dt"], w["m"], x, V)[1]
+    for k in range(8):
+        f = 0.01 * (k + 1) * rc1 / np.linalg.norm(x[:, 1])
+        x[:, 3 + k] = x[:, 1] * (1 + f); v[:, 3 + k] = v[:, 1] * (1 - 0.5 * f)
+    w["x"], w["v"] = x, v
+    g = G.from_workload(w)
+    o = oracle.Sim(w)
+    g.step(6, w["dt"], 2)
+    assert g.status() == G.EBS
+    with pytest.raises(oracle.OracleError, match="Bulirsch"):
+        o.step(6, w["dt"], 2)
     g.close()
 
 
