@@ -40,6 +40,7 @@ struct genga_ctx {
     cudaStream_t aux[2];        // helper streams: the Bulirsch-Stoer layouts run side by side
     cudaEvent_t ev_fork, ev_join[2];
     int sms;
+    int bs_big_clusters, bs_small_clusters;   // grid sizes of the Bulirsch-Stoer cluster kernels
     int *exp_labels;            // device [np]
     double *eout;               // device [4*nsys]
     struct GraphEntry { cudaGraphExec_t exec; long long launches; };
@@ -85,9 +86,10 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
         t.gstart = (int *)take(sizeof(int) * npm);
         t.gsize = (int *)take(sizeof(int) * npm);
         t.gmem = (int *)take(sizeof(int) * npm);
+        t.gorder = (int *)take(sizeof(int) * npm);
         t.gmask = (unsigned *)take(sizeof(unsigned) * 32);
     }
-    if (c->mode == GENGA_MODE_MASSIVE && nm > BSS_MAXN) {
+    if (c->mode == GENGA_MODE_MASSIVE && nm > BCB_MAXN) {
         t.bss.stride = npm;
         t.bss.base = (double *)take(sizeof(double) * (size_t)BSA_COUNT * npm);
     }
@@ -132,12 +134,17 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     c->cfg = *cfg;
     c->st = (cudaStream_t)cfg->stream;
     c->sms = std::min(prop.multiProcessorCount, 148);
+    c->bs_big_clusters = std::max(1, c->sms / BCB_CS);
+    c->bs_small_clusters = 8 * c->sms / BCS_CS;
     c->steps = c->force_evals = c->interactions = c->launches = 0;
     c->acc = 0;
     size_t need = carve(cfg, (char *)cfg->workspace, &c->d, &c->exp_labels, &c->eout, c->sms);
     if (need > cfg->workspace_bytes) { delete c; return GENGA_EINVAL; }
     cudaError_t e = cudaMemsetAsync(cfg->workspace, 0, need, c->st);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bs_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BssSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                   (int)sizeof(BcSmem<BCB_MAXN, BCB_THREADS>));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bs_cluster<BCS_MAXN, BCS_THREADS, BCS_CS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                   (int)sizeof(BcSmem<BCS_MAXN, BCS_THREADS>));
     for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
         e = cudaStreamCreateWithFlags(&c->aux[k], cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming);
@@ -243,6 +250,22 @@ static void enqueue_sun(genga_ctx *c, double h)
     LAUNCH(c); LAUNCH(c);
 }
 
+template <int MAXN, int THREADS, int CS>
+static cudaError_t launch_bs_cluster(cudaStream_t st, int clusters, const DevState &d, double h, int qslot, int endslot)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(clusters * CS);
+    cfg.blockDim = dim3(THREADS);
+    cfg.dynamicSmemBytes = sizeof(BcSmem<MAXN, THREADS>);
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = CS > 1 ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, k_bs_cluster<MAXN, THREADS, CS>, d, h, qslot, endslot);
+}
+
 // One second-order map S2(h), Eq. 7 (L100), in the order of the bullet list L153-166.
 static void enqueue_map(genga_ctx *c, double h)
 {
@@ -262,12 +285,12 @@ static void enqueue_map(genga_ctx *c, double h)
         k_bs_multi<<<nblk(d.nsys, 8), 128, 0, st>>>(d, h); LAUNCH(c);
     } else {
         k_build_groups<<<1, 1024, 0, st>>>(d); LAUNCH(c);
-        // the three Bulirsch-Stoer layouts work on disjoint groups: run them side by side
-        const bool mid = d.nm > BSW_MAXN;
+        // the Bulirsch-Stoer layouts work on disjoint parts of the size-ordered group queue: side by side
+        const bool mid = d.nm > BCS_MAXN;
         if (mid) {
             cudaEventRecord(c->ev_fork, st);
             cudaStreamWaitEvent(c->aux[0], c->ev_fork, 0);
-            k_bs_smem<<<c->sms, BSS_THREADS, sizeof(BssSmem), c->aux[0]>>>(d, h); LAUNCH(c);
+            launch_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>(c->aux[0], c->bs_big_clusters, d, h, CI_QBIG, CI_NMIDEND); LAUNCH(c);
             cudaEventRecord(c->ev_join[0], c->aux[0]);
             if (d.bss.base) {
                 cudaStreamWaitEvent(c->aux[1], c->ev_fork, 0);
@@ -275,7 +298,7 @@ static void enqueue_map(genga_ctx *c, double h)
                 cudaEventRecord(c->ev_join[1], c->aux[1]);
             }
         }
-        k_bs_warp<<<c->sms, 128, 0, st>>>(d, h); LAUNCH(c);
+        launch_bs_cluster<BCS_MAXN, BCS_THREADS, BCS_CS>(st, c->bs_small_clusters, d, h, CI_QSMALL, CI_NGROUPS); LAUNCH(c);
         if (mid) {
             cudaStreamWaitEvent(st, c->ev_join[0], 0);
             if (d.bss.base) cudaStreamWaitEvent(st, c->ev_join[1], 0);
@@ -509,13 +532,7 @@ extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ct
 extern "C" __attribute__((visibility("default"))) int genga_fp64_probe(genga_ctx *c, double *tflops)
 {
     if (!c || !tflops) return GENGA_EINVAL;
-    // scratch: the pre-drift arrays are free between steps
-    const int blocks = c->sms * 8, threads = 256, iters = 4096;
-    if ((size_t)blocks * threads > (size_t)c->d.np * 6) {
-        // tiny contexts: fewer blocks so that the output fits x0..vz0 (contiguous in the workspace)
-    }
-    int nb = (int)std::min<size_t>(blocks, ((size_t)c->d.np * 6) / threads);
-    if (nb < 1) return GENGA_EINVAL;
+    const int nb = c->sms * 8, threads = 256, iters = 4096;
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
     double best = 0.0;

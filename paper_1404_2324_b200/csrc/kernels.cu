@@ -1,6 +1,7 @@
 // Kernels of the hybrid symplectic step, sm_100a.
 // Each kernel states the operator it implements and the passage that defines it.
 #include "kernels.cuh"
+#include "bs_cluster.cuh"
 
 namespace genga {
 
@@ -19,7 +20,7 @@ __global__ void k_begin_map(DevState d)
 __global__ void k_reset_counters(DevState d)
 {
     if (threadIdx.x == 0) {
-        d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0; d.cnt[CI_NMID] = 0;
+        d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
     }
 }
 
@@ -436,16 +437,18 @@ __device__ __forceinline__ void block_scan2(int v0, int v1, int &e0, int &e1, in
     e0 = base; e1 = base + v0; total = wsum[32];
 }
 
-// Member lists of the groups of massive bodies (modes 0 and 1; N <= 2048): groups ordered by
+// Member lists of the groups of massive bodies (modes 0 and 1; N <= 2048): groups numbered by
 // root index, members sorted by body index ("write the members of the groups line by line
-// into a matrix", L565 -- here a CSR list).  One block of 1024 threads.
+// into a matrix", L565 -- here a CSR list), plus `gorder`: the group numbers by DECREASING size
+// (counting sort), the order in which the Bulirsch-Stoer kernels take them from their queue so
+// that the longest integrations start first.  One block of 1024 threads.
 __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
 {
-    __shared__ int lab[2048], sz[2048], E[2048], gst[2048];
+    __shared__ int lab[2048], sz[2048], E[2048], gst[2048], hist[2048];
     __shared__ int wsum[33];
     const int N = d.nm, tid = threadIdx.x, i0 = 2 * tid, i1 = 2 * tid + 1;
     lab[i0] = i0 < N ? d.label[i0] : i0; lab[i1] = i1 < N ? d.label[i1] : i1;
-    sz[i0] = 0; sz[i1] = 0;
+    sz[i0] = 0; sz[i1] = 0; hist[i0] = 0; hist[i1] = 0;
     __syncthreads();
     if (i0 < N) atomicAdd(&sz[lab[i0]], 1);
     if (i1 < N) atomicAdd(&sz[lab[i1]], 1);
@@ -458,9 +461,17 @@ __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
     int r0 = f0 && lab[i0] == i0, r1 = f1 && lab[i1] == i1;
     block_scan2(r0, r1, g0, g1, ng, wsum);
     block_scan2(r0 ? sz[i0] : 0, r1 ? sz[i1] : 0, s0, s1, ns, wsum);
-    if (r0) { gst[i0] = s0; d.gstart[g0] = s0; d.gsize[g0] = sz[i0]; }
-    if (r1) { gst[i1] = s1; d.gstart[g1] = s1; d.gsize[g1] = sz[i1]; }
+    if (r0) { gst[i0] = s0; d.gstart[g0] = s0; d.gsize[g0] = sz[i0]; atomicAdd(&hist[2048 - sz[i0]], 1); }
+    if (r1) { gst[i1] = s1; d.gstart[g1] = s1; d.gsize[g1] = sz[i1]; atomicAdd(&hist[2048 - sz[i1]], 1); }
     __syncthreads();
+    // hist[b] = number of groups of 2048 - b bodies -> start of that size class in gorder
+    int h0, h1, nh;
+    block_scan2(hist[i0], hist[i1], h0, h1, nh, wsum);
+    __syncthreads();
+    hist[i0] = h0; hist[i1] = h1;
+    __syncthreads();
+    if (r0) d.gorder[atomicAdd(&hist[2048 - sz[i0]], 1)] = g0;
+    if (r1) d.gorder[atomicAdd(&hist[2048 - sz[i1]], 1)] = g1;
     for (int k = tid; k < ne; k += blockDim.x) {
         int i = E[k], r = lab[i], rank = 0;
         for (int kk = 0; kk < k; ++kk) rank += (lab[E[kk]] == r);
@@ -471,6 +482,19 @@ __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
         for (int j = 0; j < N; ++j) if (lab[j] == lab[tid]) mask |= 1u << j;
         d.gmask[tid] = mask;
     }
+    // groups too large for the cluster layout come first in gorder: their count is the start of
+    // the cluster kernels' queues.  The exclusive scan value at the class "S bodies" counts the groups larger than S.
+    const int bbig = 2048 - BCB_MAXN, bmid = 2048 - BCS_MAXN;
+    if (i0 == bbig || i1 == bbig) {
+        int nbig = i0 == bbig ? h0 : h1;
+        d.cnt[CI_NBIG] = nbig;
+        d.cnt[CI_QBIG] = nbig;
+    }
+    if (i0 == bmid || i1 == bmid) {
+        int nmid = i0 == bmid ? h0 : h1;            // groups too large for the small-cluster layout
+        d.cnt[CI_NMIDEND] = nmid;
+        d.cnt[CI_QSMALL] = nmid;
+    }
     if (tid == 0) {
         d.cnt[CI_NGROUPS] = ng;
         d.stat[CNT_GROUPS] += ng;
@@ -478,88 +502,63 @@ __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
     }
     int big = (r0 ? sz[i0] : 0) > (r1 ? sz[i1] : 0) ? (r0 ? sz[i0] : 0) : (r1 ? sz[i1] : 0);
     for (int o = 16; o > 0; o >>= 1) big = max(big, __shfl_xor_sync(0xffffffffu, big, o));
-    if ((tid & 31) == 0 && big > 0) {
-        atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)big);
-        if (big > BSS_MAXN) atomicAdd(&d.cnt[CI_NBIG], 1);
-    }
-    int mid = ((r0 && sz[i0] > BSW_MAXN && sz[i0] <= BSS_MAXN) || (r1 && sz[i1] > BSW_MAXN && sz[i1] <= BSS_MAXN)) ? 1 : 0;
-    if (__any_sync(0xffffffffu, mid) && (tid & 31) == 0) atomicAdd(&d.cnt[CI_NMID], 1);
+    if ((tid & 31) == 0 && big > 0) atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)big);
 }
 
 // =====================================================================================
-// Bulirsch-Stoer on the groups of massive bodies (modes 0, 1): one warp per group of 2..32
-// bodies; all members start from the state before the drift and overwrite the drift result
-// (L163, L301-314).
-__global__ void __launch_bounds__(128) k_bs_warp(DevState d, double h)
+// Bulirsch-Stoer on the groups of massive bodies (modes 0, 1) of 2..MAXN bodies: one CLUSTER
+// of CS CTAs per group, each CTA integrating 8 / CS extrapolation columns (bs_cluster.cuh).  All
+// members start from the state before the drift and overwrite the drift result (L163, L301-314).
+// Clusters take groups from a queue in order of decreasing size: entries [cnt[qslot], cnt[endslot])
+// of gorder (two instantiations run side by side on the two halves of the queue).
+template <int MAXN, int THREADS, int CS>
+__global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, int qslot, int endslot)
 {
-    __shared__ TeamSmem<32> sm[4];
-    const int ng = d.cnt[CI_NGROUPS];
-    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    WarpTeam<32> t{0xffffffffu, lane};
-    for (int g = blockIdx.x * 4 + wib; g < ng; g += gridDim.x * 4) {
-        const int nb = d.gsize[g];
-        if (nb > BSW_MAXN) continue;
-        const bool active = lane < nb;
-        const int i = active ? d.gmem[d.gstart[g] + lane] : 0;
-        double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0}, rc = 0.0;
-        __syncwarp();
-        sm[wib].m[lane] = 0.0; sm[wib].rc[lane] = 0.0; sm[wib].irc[lane] = 0.0;
-        if (active) {
-            q[0] = d.x0[i]; q[1] = d.y0[i]; q[2] = d.z0[i]; V[0] = d.vx0[i]; V[1] = d.vy0[i]; V[2] = d.vz0[i];
-            rc = d.rc[i];
-            sm[wib].m[lane] = d.m[i]; sm[wib].rc[lane] = rc; sm[wib].irc[lane] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
-        }
-        __syncwarp();
-        int nsteps = 0;
-        unsigned srcmask = nb >= 32 ? 0xffffffffu : ((1u << nb) - 1u);
-        bool ok = bs_team<32>(t, sm[wib], nb, active, srcmask, d.G, d.m0[0], rc, q, V, h, d.eps, &nsteps);
-        if (active) { d.x[i] = q[0]; d.y[i] = q[1]; d.z[i] = q[2]; d.vx[i] = V[0]; d.vy[i] = V[1]; d.vz[i] = V[2]; }
-        if (lane == 0) {
-            if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
-            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
-        }
+    extern __shared__ __align__(16) unsigned char bc_raw[];
+    using Smem = BcSmem<MAXN, THREADS>;
+    Smem &S = *reinterpret_cast<Smem *>(bc_raw);
+    int rank = 0;
+    Smem *S0 = &S;
+    if constexpr (CS > 1) {
+        cg::cluster_group cluster = cg::this_cluster();
+        rank = (int)cluster.block_rank();
+        S0 = cluster.map_shared_rank(&S, 0);
     }
-}
-
-// Groups of BSW_MAXN < n <= BSS_MAXN bodies: one block per group, everything in shared memory
-// (bs.cuh "Shared-memory block layout").
-__global__ void __launch_bounds__(BSS_THREADS) k_bs_smem(DevState d, double h)
-{
-    extern __shared__ __align__(16) unsigned char bss_raw[];
-    BssSmem &S = *reinterpret_cast<BssSmem *>(bss_raw);
-    __shared__ int nsteps;
-    if (d.cnt[CI_NMID] == 0) return;
-    const int ng = d.cnt[CI_NGROUPS];
-    for (int g = blockIdx.x; g < ng; g += gridDim.x) {
-        const int n = d.gsize[g];
-        if (n <= BSW_MAXN || n > BSS_MAXN) continue;
-        const int off = d.gstart[g];
-        int P = 32;
-        while (P < n) P <<= 1;
-        BssLane t;
-        t.n = n; t.L = BSS_THREADS / P; t.i = threadIdx.x / t.L; t.s = threadIdx.x % t.L;
-        t.owner = t.s == 0 && t.i < n;
-        __syncthreads();
-        if (threadIdx.x == 0) nsteps = 0;
-        for (int b = threadIdx.x; b < n; b += BSS_THREADS) {
+    const int qend = d.cnt[endslot];
+    while (true) {
+        if (rank == 0 && threadIdx.x == 0) S.cur = atomicAdd(&d.cnt[qslot], 1);
+        bc_sync<CS>();
+        const int qi = S0->cur;
+        if (qi >= qend) break;
+        const int g = d.gorder[qi];
+        const int n = d.gsize[g], off = d.gstart[g];
+        const BcLane t = bc_lanes<THREADS>(n);
+        for (int b = threadIdx.x; b < n; b += THREADS) {
             int i = d.gmem[off + b];
             S.Y[0][b] = d.x0[i]; S.Y[1][b] = d.y0[i]; S.Y[2][b] = d.z0[i];
             S.Y[3][b] = d.vx0[i]; S.Y[4][b] = d.vy0[i]; S.Y[5][b] = d.vz0[i];
             double rc = d.rc[i];
             S.m[b] = d.m[i]; S.rc[b] = rc; S.irc[b] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
         }
-        bool ok = bss_integrate(S, t, d.G, d.m0[0], h, d.eps, &nsteps);
-        for (int b = threadIdx.x; b < n; b += BSS_THREADS) {
-            int i = d.gmem[off + b];
-            d.x[i] = S.Y[0][b]; d.y[i] = S.Y[1][b]; d.z[i] = S.Y[2][b];
-            d.vx[i] = S.Y[3][b]; d.vy[i] = S.Y[4][b]; d.vz[i] = S.Y[5][b];
-        }
-        if (threadIdx.x == 0) {
-            if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
-            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
+        int nsteps = 0;
+        bool ok = bc_integrate<MAXN, THREADS, CS>(S, S0, rank, t, d.G, d.m0[0], h, d.eps, &nsteps);
+        if (rank == 0) {
+            __syncthreads();
+            for (int b = threadIdx.x; b < n; b += THREADS) {
+                int i = d.gmem[off + b];
+                d.x[i] = S.Y[0][b]; d.y[i] = S.Y[1][b]; d.z[i] = S.Y[2][b];
+                d.vx[i] = S.Y[3][b]; d.vy[i] = S.Y[4][b]; d.vz[i] = S.Y[5][b];
+            }
+            if (threadIdx.x == 0) {
+                if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
+                atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
+            }
         }
     }
+    bc_sync<CS>();      // nobody leaves while its shared memory may still be read
 }
+template __global__ void k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>(DevState, double, int, int);
+template __global__ void k_bs_cluster<BCS_MAXN, BCS_THREADS, BCS_CS>(DevState, double, int, int);
 
 // Groups larger than a warp: one block per group, tableau in global scratch.
 __global__ void __launch_bounds__(256) k_bs_block(DevState d, double h)
@@ -570,7 +569,7 @@ __global__ void __launch_bounds__(256) k_bs_block(DevState d, double h)
     const int ng = d.cnt[CI_NGROUPS];
     for (int g = blockIdx.x; g < ng; g += gridDim.x) {
         const int nb = d.gsize[g];
-        if (nb <= BSS_MAXN) continue;
+        if (nb <= BCB_MAXN) continue;
         const int off = d.gstart[g];
         if (threadIdx.x == 0) nsteps = 0;
         for (int b = threadIdx.x; b < nb; b += blockDim.x) {
@@ -759,7 +758,8 @@ __global__ void __launch_bounds__(256) k_fp64_probe(double *out, int iters)
             a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
         }
     }
-    out[blockIdx.x * blockDim.x + threadIdx.x] = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    double r = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (r == 0.12345) out[threadIdx.x] = r;      // never true: keeps the chains alive without a per-thread output array
 }
 
 // labels for genga_encounters: body's own index unless it is in a group

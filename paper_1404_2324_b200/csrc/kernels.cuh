@@ -1,6 +1,7 @@
 // Kernel declarations (definitions in kernels.cu); see each definition for the operator it implements.
 #pragma once
 #include "state.cuh"
+#include "bs_cluster.cuh"
 
 namespace genga {
 
@@ -8,6 +9,10 @@ constexpr int KK_THREADS = 256;   // threads per block of the kick kernel
 constexpr int KK_NI = 14;         // bodies i a block owns at most: ceil(2048 / 148)
 constexpr int KK_NV = 48;         // 3 KK_NI accumulators padded to 3 * 16 for the halving butterfly
 constexpr int KK_WORDS = 64;      // 2048 / 32 bitmap words per body i
+
+// Bulirsch-Stoer cluster layouts (bs_cluster.cuh): groups of 17..256 bodies and of 2..16 bodies
+constexpr int BCB_MAXN = 256, BCB_THREADS = 256, BCB_CS = 8;
+constexpr int BCS_MAXN = 16, BCS_THREADS = 64, BCS_CS = 8;
 
 __global__ void k_begin_map(DevState d);
 __global__ void k_reset_counters(DevState d);
@@ -26,8 +31,7 @@ __global__ void k_label_init(DevState d);
 __global__ void k_union(DevState d);
 __global__ void k_flatten(DevState d);
 __global__ void k_build_groups(DevState d);
-__global__ void k_bs_warp(DevState d, double h);
-__global__ void k_bs_smem(DevState d, double h);
+template <int MAXN, int THREADS, int CS> __global__ void k_bs_cluster(DevState d, double h, int qslot, int endslot);
 __global__ void k_bs_block(DevState d, double h);
 template <int TW> __global__ void k_tp_bs(DevState d, double h, int lo);
 __global__ void k_bs_multi(DevState d, double h);
