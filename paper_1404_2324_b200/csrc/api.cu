@@ -40,7 +40,7 @@ struct genga_ctx {
     cudaStream_t aux[2];        // helper streams: the Bulirsch-Stoer layouts run side by side
     cudaEvent_t ev_fork, ev_join[2];
     int sms;
-    int bs_big_clusters, bs_small_clusters;   // grid sizes of the Bulirsch-Stoer cluster kernels
+    int bs_big_clusters;        // grid size (in clusters) of the Bulirsch-Stoer cluster kernel
     int *exp_labels;            // device [np]
     double *eout;               // device [4*nsys]
     struct GraphEntry { cudaGraphExec_t exec; long long launches; };
@@ -88,6 +88,8 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
         t.gmem = (int *)take(sizeof(int) * npm);
         t.gorder = (int *)take(sizeof(int) * npm);
         t.gmask = (unsigned *)take(sizeof(unsigned) * 32);
+    } else {
+        t.gorder = (int *)take(sizeof(int) * np);          // (system, member mask) per group, at most ntot / 2 groups
     }
     if (c->mode == GENGA_MODE_MASSIVE && nm > BCB_MAXN) {
         t.bss.stride = npm;
@@ -135,7 +137,6 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     c->st = (cudaStream_t)cfg->stream;
     c->sms = std::min(prop.multiProcessorCount, 148);
     c->bs_big_clusters = std::max(1, c->sms / BCB_CS);
-    c->bs_small_clusters = 8 * c->sms / BCS_CS;
     c->steps = c->force_evals = c->interactions = c->launches = 0;
     c->acc = 0;
     size_t need = carve(cfg, (char *)cfg->workspace, &c->d, &c->exp_labels, &c->eout, c->sms);
@@ -143,8 +144,6 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     cudaError_t e = cudaMemsetAsync(cfg->workspace, 0, need, c->st);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                    (int)sizeof(BcSmem<BCB_MAXN, BCB_THREADS>));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bs_cluster<BCS_MAXN, BCS_THREADS, BCS_CS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                   (int)sizeof(BcSmem<BCS_MAXN, BCS_THREADS>));
     for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
         e = cudaStreamCreateWithFlags(&c->aux[k], cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming);
@@ -281,12 +280,15 @@ static void enqueue_map(genga_ctx *c, double h)
     k_label_init<<<nblk(d.nmtot, 256), 256, 0, st>>>(d); LAUNCH(c);
     k_union<<<pair_blocks, 128, 0, st>>>(d); LAUNCH(c);
     k_flatten<<<nblk(d.nmtot, 256), 256, 0, st>>>(d); LAUNCH(c);
+    const int warp_blocks = 2 * c->sms;                       // 4 warps each; warps take groups from a queue
     if (d.mode == GENGA_MODE_MULTI_SYSTEM) {
-        k_bs_multi<<<nblk(d.nsys, 8), 128, 0, st>>>(d, h); LAUNCH(c);
+        k_list_groups_multi<<<nblk(d.ntot, 256), 256, 0, st>>>(d); LAUNCH(c);
+        k_bs_warp<<<warp_blocks, 32 * BW_WARPS, 0, st>>>(d, h, 0); LAUNCH(c);
+        if (d.nm > BW_MAXN) { k_bs_multi<<<nblk(d.nsys, 8), 128, 0, st>>>(d, h); LAUNCH(c); }
     } else {
         k_build_groups<<<1, 1024, 0, st>>>(d); LAUNCH(c);
         // the Bulirsch-Stoer layouts work on disjoint parts of the size-ordered group queue: side by side
-        const bool mid = d.nm > BCS_MAXN;
+        const bool mid = d.nm > BW_MAXN;
         if (mid) {
             cudaEventRecord(c->ev_fork, st);
             cudaStreamWaitEvent(c->aux[0], c->ev_fork, 0);
@@ -298,15 +300,14 @@ static void enqueue_map(genga_ctx *c, double h)
                 cudaEventRecord(c->ev_join[1], c->aux[1]);
             }
         }
-        launch_bs_cluster<BCS_MAXN, BCS_THREADS, BCS_CS>(st, c->bs_small_clusters, d, h, CI_QSMALL, CI_NGROUPS); LAUNCH(c);
+        k_bs_warp<<<warp_blocks, 32 * BW_WARPS, 0, st>>>(d, h, 0); LAUNCH(c);
         if (mid) {
             cudaStreamWaitEvent(st, c->ev_join[0], 0);
             if (d.bss.base) cudaStreamWaitEvent(st, c->ev_join[1], 0);
         }
         if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {
-            k_tp_bs<4><<<4 * c->sms, 128, 0, st>>>(d, h, 0);
-            k_tp_bs<32><<<2 * c->sms, 128, 0, st>>>(d, h, 4);
-            LAUNCH(c); LAUNCH(c);
+            k_bs_warp<<<warp_blocks, 32 * BW_WARPS, 0, st>>>(d, h, 1); LAUNCH(c);
+            if (d.nm + 1 > BW_MAXN) { k_tp_bs<32><<<2 * c->sms, 128, 0, st>>>(d, h, BW_MAXN); LAUNCH(c); }
         }
     }
     enqueue_sun(c, 0.5 * h);

@@ -2,6 +2,7 @@
 // Each kernel states the operator it implements and the passage that defines it.
 #include "kernels.cuh"
 #include "bs_cluster.cuh"
+#include "bs_warp.cuh"
 
 namespace genga {
 
@@ -21,6 +22,7 @@ __global__ void k_reset_counters(DevState d)
 {
     if (threadIdx.x == 0) {
         d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
+        d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0;
     }
 }
 
@@ -484,14 +486,14 @@ __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
     }
     // groups too large for the cluster layout come first in gorder: their count is the start of
     // the cluster kernels' queues.  The exclusive scan value at the class "S bodies" counts the groups larger than S.
-    const int bbig = 2048 - BCB_MAXN, bmid = 2048 - BCS_MAXN;
+    const int bbig = 2048 - BCB_MAXN, bmid = 2048 - BW_MAXN;
     if (i0 == bbig || i1 == bbig) {
         int nbig = i0 == bbig ? h0 : h1;
         d.cnt[CI_NBIG] = nbig;
         d.cnt[CI_QBIG] = nbig;
     }
     if (i0 == bmid || i1 == bmid) {
-        int nmid = i0 == bmid ? h0 : h1;            // groups too large for the small-cluster layout
+        int nmid = i0 == bmid ? h0 : h1;            // groups too large for the warp layout
         d.cnt[CI_NMIDEND] = nmid;
         d.cnt[CI_QSMALL] = nmid;
     }
@@ -558,7 +560,107 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
     bc_sync<CS>();      // nobody leaves while its shared memory may still be read
 }
 template __global__ void k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>(DevState, double, int, int);
-template __global__ void k_bs_cluster<BCS_MAXN, BCS_THREADS, BCS_CS>(DevState, double, int, int);
+
+// Bulirsch-Stoer on the SMALL groups (2..BW_MAXN bodies) of every mode: one warp per group, the
+// extrapolation columns side by side in its lanes (bs_warp.cuh).  Warps take groups from a queue:
+//   mode 0/1: entries [cnt[CI_QSMALL], cnt[CI_NGROUPS]) of gorder (groups by decreasing size);
+//   mode 2  : entries [0, cnt[CI_NGROUPS]) of gorder, each (system, 16-bit member mask);
+//   particles (tp = 1, mode 1): entries [0, cnt[CI_NTP]) of tplist; group = {particle} + the massive
+//             bodies it meets + their massive groups (L342), only the particle is written back.
+__global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h, int tp)
+{
+    __shared__ BwSmem sm[BW_WARPS];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    BwSmem &W = sm[warp];
+    const int qslot = tp ? CI_QTP : CI_QWARP;
+    const int qend = tp ? d.cnt[CI_NTP] : d.cnt[CI_NGROUPS];
+    if (!tp && d.mode != 2 && d.cnt[CI_QSMALL] >= qend) return;
+    while (true) {
+        int qi = 0;
+        if (lane == 0) qi = atomicAdd(&d.cnt[qslot], 1);
+        qi = __shfl_sync(0xffffffffu, qi, 0);
+        if (!tp && d.mode != 2) qi += d.cnt[CI_QSMALL];
+        if (qi >= qend) break;
+        // ---- members of the group: body index of slot b = lane % 8
+        const int b8 = lane & 7;
+        int n, i = -1, sys = 0, plabel = 0;
+        bool writeback;
+        if (tp) {
+            const int p = d.tplist[qi];
+            unsigned mask = d.tpmask[p - d.nm], fullm = 0u;
+            plabel = p;
+            for (unsigned mm = mask; mm; mm &= mm - 1) {
+                int j = __ffs(mm) - 1;
+                fullm |= d.gmask[j];
+                plabel = min(plabel, d.label[j]);
+            }
+            n = __popc(fullm) + 1;
+            if (n > BW_MAXN) continue;                     // k_tp_bs<32> takes it
+            if (b8 < n - 1) i = __fns(fullm, 0, b8 + 1); else if (b8 == n - 1) i = p;
+            writeback = b8 == n - 1;
+        } else if (d.mode == 2) {
+            sys = d.gorder[2 * qi];
+            const unsigned mask = (unsigned)d.gorder[2 * qi + 1];
+            n = __popc(mask);
+            if (n > BW_MAXN) continue;                     // k_bs_multi takes it
+            if (b8 < n) i = sys * d.nm + __fns(mask, 0, b8 + 1);
+            writeback = b8 < n;
+        } else {
+            const int g = d.gorder[qi];
+            n = d.gsize[g];
+            if (b8 < n) i = d.gmem[d.gstart[g] + b8];
+            writeback = b8 < n;
+        }
+        double Y[6] = {1.0, 0.0, 0.0, 0.0, 1.0, 0.0}, rc = 0.0, m = 0.0;
+        if (i >= 0) {
+            Y[0] = d.x0[i]; Y[1] = d.y0[i]; Y[2] = d.z0[i]; Y[3] = d.vx0[i]; Y[4] = d.vy0[i]; Y[5] = d.vz0[i];
+            rc = d.rc[i]; m = d.m[i];
+        }
+        const double Gm0 = d.G * d.m0[sys];
+        int nsteps = 0;
+        bool ok;
+        if (n <= 4) {
+            // segments of 2 or 4 lanes: slot b = lane % S takes body b from lane b of the 8-slot layout
+            const int src = n == 2 ? (lane & 1) : (lane & 3);
+#pragma unroll
+            for (int c = 0; c < 6; ++c) Y[c] = __shfl_sync(0xffffffffu, Y[c], src);
+            rc = __shfl_sync(0xffffffffu, rc, src); m = __shfl_sync(0xffffffffu, m, src);
+            if (n == 2) ok = bw_integrate<2>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, &nsteps);
+            else ok = bw_integrate<4>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, &nsteps);
+        } else {
+            ok = bw_integrate<8>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, &nsteps);
+        }
+        if (lane < 8 && writeback) {
+            d.x[i] = Y[0]; d.y[i] = Y[1]; d.z[i] = Y[2]; d.vx[i] = Y[3]; d.vy[i] = Y[4]; d.vz[i] = Y[5];
+            if (tp) d.label[i] = plabel;
+        }
+        if (lane == 0) {
+            if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
+            if (tp || d.mode == 2) {
+                atomicAdd((unsigned long long *)&d.stat[CNT_GROUPS], 1ull);
+                atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)n);
+            }
+        }
+        __syncwarp();
+    }
+}
+
+// Multi-system mode: the groups of every system as one queue for k_bs_warp.  One thread per body; a
+// root (label = own index) with at least one other member appends (system, member mask).
+__global__ void k_list_groups_multi(DevState d)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (d.cnt[CI_NENC] == 0 || i >= d.ntot) return;
+    if (d.label[i] != i) return;
+    const int nm = d.nm, sys = i / nm, base = sys * nm;
+    unsigned mask = 0u;
+    for (int k = 0; k < nm; ++k) if (d.label[base + k] == i) mask |= 1u << k;
+    if (__popc(mask) < 2) return;
+    int slot = atomicAdd(&d.cnt[CI_NGROUPS], 1);
+    d.gorder[2 * slot] = sys; d.gorder[2 * slot + 1] = (int)mask;
+    if (__popc(mask) > BW_MAXN) atomicAdd(&d.cnt[CI_NBIG], 1);
+}
 
 // Groups larger than a warp: one block per group, tableau in global scratch.
 __global__ void __launch_bounds__(256) k_bs_block(DevState d, double h)
@@ -650,16 +752,15 @@ __global__ void __launch_bounds__(128) k_tp_bs(DevState d, double h, int lo)
         }
     }
 }
-template __global__ void k_tp_bs<4>(DevState, double, int);
 template __global__ void k_tp_bs<32>(DevState, double, int);
 
-// Multi-system mode (L372-376): 16 lanes per system; the groups of a system are the sets of
-// equal labels among its bodies, integrated one after the other by the system's lanes.
+// Multi-system mode (L372-376), groups of more than BW_MAXN bodies (the others: k_bs_warp): 16 lanes
+// per system; the groups of a system are the sets of equal labels among its bodies.
 __global__ void __launch_bounds__(128) k_bs_multi(DevState d, double h)
 {
     constexpr int TW = 16, TPB = 128 / TW;
     __shared__ TeamSmem<TW> sm[TPB];
-    if (d.cnt[CI_NENC] == 0) return;
+    if (d.cnt[CI_NBIG] == 0) return;
     const int team = threadIdx.x / TW, lane = threadIdx.x % TW, lane32 = threadIdx.x & 31;
     const unsigned tmask = 0xffffu << (lane32 - lane);
     WarpTeam<TW> t{tmask, lane};
@@ -675,7 +776,7 @@ __global__ void __launch_bounds__(128) k_bs_multi(DevState d, double h)
         int lj = __shfl_sync(tmask, lab, j, TW);
         if (lj == lab) grp |= 1u << j;
     }
-    unsigned todo = __ballot_sync(tmask, have && __popc(grp) >= 2 && lab == lane) >> (lane32 - lane) & 0xffffu;  // roots
+    unsigned todo = __ballot_sync(tmask, have && __popc(grp) > BW_MAXN && lab == lane) >> (lane32 - lane) & 0xffffu;  // roots of groups too large for k_bs_warp
     if (todo == 0u) return;
     double rc = have ? d.rc[i] : 0.0;
     sm[team].m[lane] = have ? d.m[i] : 0.0; sm[team].rc[lane] = rc; sm[team].irc[lane] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;

@@ -2,6 +2,7 @@
 #pragma once
 #include "state.cuh"
 #include "bs_cluster.cuh"
+#include "bs_warp.cuh"
 
 namespace genga {
 
@@ -10,9 +11,9 @@ constexpr int KK_NI = 14;         // bodies i a block owns at most: ceil(2048 / 
 constexpr int KK_NV = 48;         // 3 KK_NI accumulators padded to 3 * 16 for the halving butterfly
 constexpr int KK_WORDS = 64;      // 2048 / 32 bitmap words per body i
 
-// Bulirsch-Stoer cluster layouts (bs_cluster.cuh): groups of 17..256 bodies and of 2..16 bodies
+// Bulirsch-Stoer layouts: groups of 2..8 bodies on one warp (bs_warp.cuh), of 9..256 bodies on a
+// cluster of 8 CTAs (bs_cluster.cuh), larger ones on one block with a global-memory tableau (bs.cuh)
 constexpr int BCB_MAXN = 256, BCB_THREADS = 256, BCB_CS = 8;
-constexpr int BCS_MAXN = 16, BCS_THREADS = 64, BCS_CS = 8;
 
 __global__ void k_begin_map(DevState d);
 __global__ void k_reset_counters(DevState d);
@@ -32,6 +33,8 @@ __global__ void k_union(DevState d);
 __global__ void k_flatten(DevState d);
 __global__ void k_build_groups(DevState d);
 template <int MAXN, int THREADS, int CS> __global__ void k_bs_cluster(DevState d, double h, int qslot, int endslot);
+__global__ void k_bs_warp(DevState d, double h, int tp);
+__global__ void k_list_groups_multi(DevState d);
 __global__ void k_bs_block(DevState d, double h);
 template <int TW> __global__ void k_tp_bs(DevState d, double h, int lo);
 __global__ void k_bs_multi(DevState d, double h);

@@ -25,7 +25,7 @@ struct DevState {
     int *cnt;        // device ints: see CI_* below
     int *label;      // [np] group label of massive bodies
     int *gstart, *gsize, *gmem;  // groups of massive bodies (mode 0/1): [npm]
-    int *gorder;                 // group numbers by decreasing size: the Bulirsch-Stoer queue
+    int *gorder;                 // group numbers by decreasing size: the Bulirsch-Stoer queue (mode 2: (system, member mask) per group)
     unsigned *gmask;             // mode 1: bit mask of the massive group of body i
     unsigned *tpmask;            // mode 1: per particle, massive bodies it meets
     int *tplist;                 // mode 1: particles with encounters in this substep
@@ -35,7 +35,7 @@ struct DevState {
 
 // indices into DevState::cnt
 enum : int { CI_NCAND = 0, CI_NENC = 1, CI_NGROUPS = 2, CI_NTP = 3, CI_STATUS = 4, CI_NTP_PREV = 5,
-             CI_NBIG = 6, CI_QBIG = 7, CI_NMIDEND = 8, CI_QSMALL = 9, CI_COUNT = 16 };
+             CI_NBIG = 6, CI_QBIG = 7, CI_NMIDEND = 8, CI_QSMALL = 9, CI_QWARP = 10, CI_QTP = 11, CI_COUNT = 16 };
 
 __device__ __forceinline__ int system_of(const DevState &d, int i) { return d.mode == 2 ? i / d.nm : 0; }
 
