@@ -144,6 +144,7 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     cudaError_t e = cudaMemsetAsync(cfg->workspace, 0, need, c->st);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                    (int)sizeof(BcSmem<BCB_MAXN, BCB_THREADS>));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_kick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kick_smem_bytes());
     for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
         e = cudaStreamCreateWithFlags(&c->aux[k], cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming);
@@ -218,11 +219,7 @@ static void launch_kick(genga_ctx *c, double h, int record, double *aout)
     DevState &d = c->d;
     const int ni = std::min(KK_NI, (d.nm + c->sms - 1) / c->sms);
     const int grid = (d.nm + ni - 1) / ni;
-    const int tj = (d.nm + KK_THREADS - 1) / KK_THREADS;
-    if (tj <= 1) k_kick<1><<<grid, KK_THREADS, 0, c->st>>>(d, h, record, ni, aout);
-    else if (tj <= 2) k_kick<2><<<grid, KK_THREADS, 0, c->st>>>(d, h, record, ni, aout);
-    else if (tj <= 4) k_kick<4><<<grid, KK_THREADS, 0, c->st>>>(d, h, record, ni, aout);
-    else k_kick<8><<<grid, KK_THREADS, 0, c->st>>>(d, h, record, ni, aout);
+    k_kick<<<grid, KK_THREADS, kick_smem_bytes(), c->st>>>(d, h, record, ni, aout);
 }
 
 static void enqueue_kick(genga_ctx *c, double h, int record, double *aout)

@@ -53,157 +53,244 @@ __global__ void k_rcrit(DevState d, double tau)
 // W(r, rc_ij), and the prechecker (L142).  Massive bodies of one system, N <= 2048.
 //
 // Layout.  The paper gives every body i a thread block whose threads split the j loop and
-// reduce (Table 2).  Here one block per SM owns ni = ceil(N / #SM) <= 14 bodies i;
-// each of its 256 threads keeps TJ = ceil(N / 256) bodies j in REGISTERS for the whole kernel
-// and meets the block's bodies i as shared-memory broadcasts, so a body j is loaded once per
-// block and the inner loop has no memory traffic.  The 3 ni partial sums per thread are
-// reduced by a halving butterfly inside each warp (48 shuffle+add steps for 42 values, fixed
-// order) and across the 8 warps through shared memory; the block then applies the kick to its
-// own bodies, so the whole operator is one launch with no partial sums in global memory.
+// reduce in shared memory (Table 2).  Here one block per SM owns ni = ceil(N / #SM)
+// <= 14 bodies i ("rows") and stages all bodies j once in shared memory (a 32-byte record
+// x, y, z, G m_j per body, the high word of its precheck distance, its critical radius).
+// A LANE owns two rows: their positions sit in registers and their sums never leave the lane,
+// so the pair loop ends without any reduction over the 2048 partners, and every body j read
+// from shared memory serves two pairs.  The 32 lanes of a warp are R row pairs x P phases;
+// the lanes of one phase read the same body j (a multicast) and the P phases read P
+// consecutive bodies.  14 rows = 8 + 4 + 2: warps 0-15 take rows 0-7 with P = 8, warps 16-23
+// rows 8-11 with P = 16, warps 24-27 rows 12-13 with P = 32, and every warp covers 1/16, 1/8,
+// 1/4 of the bodies j: all 28 warps (7 per SM sub-partition) run exactly ceil(N / 128) <= 16
+// iterations of two pairs with all lanes busy.
 //
 // Per pair the fast path costs 16 FP64 issue slots: 3 subtractions, 3 for r^2, 7 for
-// G m_j r^-3 from the MUFU.RSQ64H seed (rinv3_fast), 3 accumulating FMAs.  The precheck
-// r^2 < 9 max(rc_i, rc_j)^2 is done on the HIGH WORDS of the doubles with integer compares
-// (a superset of the exact test, off the FP64 pipe); pairs that pass -- the whole changeover
-// zone r < rc_ij lies inside the precheck sphere -- get weight 0 in the fast path and set a
-// bit in a shared bitmap [ni][N], and are afterwards evaluated exactly (sqrt, W = K - r dK/dr,
-// candidate list) by the warp that owns the row, in ascending j per lane and a fixed
-// butterfly over lanes, so the sum is deterministic.
-template <int TJ>
-__global__ void __launch_bounds__(KK_THREADS) k_kick(DevState d, double h, int record, int ni, double *aout)
+// G m_j r^-3 from the MUFU.RSQ64H seed (rinv3_fast), 3 accumulating FMAs, and no branch.
+// The precheck r^2 < 9 max(rc_i, rc_j)^2 is done on the HIGH WORDS of the doubles with
+// integer compares (a superset of the exact test, off the FP64 pipe).  A pair that passes --
+// the whole changeover zone r < rc_ij lies inside the precheck sphere, and so does the body
+// itself -- gets weight 0 by clearing the seed, and the warp's ballot of the test is stored
+// as a hit word.  After its pair loop each warp lists its hits in a fixed order, evaluates
+// them one per lane with the exact weight W = K - r dK/dr and the exact candidate test, and
+// the row pair's first lane adds them in list order: no atomics on the sums, deterministic.  The row sums of the warps meet in shared memory and the block applies the
+// kick to its own bodies: one launch, no partial sums in global memory.
+__device__ __forceinline__ double kick_scale_exact(double r2, double rcij, double Gmj)
 {
-    __shared__ double sxi[KK_NI], syi[KK_NI], szi[KK_NI];
-    __shared__ int shc[KK_NI];
-    __shared__ unsigned bitmap[KK_NI][KK_WORDS];
-    __shared__ double red[KK_THREADS / 32][KK_NV];
-    __shared__ double acc_s[KK_NV];
-    __shared__ int anyhit;
+    // G m_j W(r, rc_ij) / r^3 with W of kick_weight(), arranged on the reciprocal seeds (a few ulp)
+    double rinv = rsqrt_fast(r2);
+    double r = r2 * rinv;
+    double s3 = Gmj * (rinv * rinv) * rinv;
+    double irc = rcp_fast(0.9 * rcij);
+    double y = (r - 0.1 * rcij) * irc;
+    if (!(y > 0.0)) return 0.0;
+    if (y >= 1.0) return s3;
+    double D = fma(2.0 * y, y - 1.0, 1.0);
+    double iD = rcp_fast(D);
+    double yD = y * iD;                                           // K = y yD
+    double rdK = 2.0 * (1.0 - y) * (yD * iD) * (r * irc);
+    return s3 * fma(y, yD, -rdK);
+}
 
+struct __align__(32) KickBody { double x, y, z, gm; };
+struct KickHit { int code; int pad; double cx, cy, cz; };      // code = lane bit << 8 | iteration
+
+struct KickSmem {
+    KickBody body[KK_MAXN];                 // all bodies j, padded to a multiple of 64
+    int hc[KK_MAXN];                        // high word of 9 rc_j^2 (-1 for padding)
+    double rc[KK_MAXN];                     // critical radius (exact pass)
+    unsigned hitw[KK_WARPS][32];            // per warp: ballot of the precheck, one word per iteration
+    KickHit list[KK_WARPS][32];             // per warp: hits of the current window of the exact pass
+    double wsum[KK_WARPS][8][3];            // per warp: sums of its rows
+};
+
+__global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, int record, int ni, double *aout)
+{
+    extern __shared__ __align__(32) unsigned char kk_raw[];
+    KickSmem &S = *reinterpret_cast<KickSmem *>(kk_raw);
     const int N = d.nm, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int i0 = blockIdx.x * ni;
     const int nib = min(ni, N - i0);
-    if (tid < KK_NI) {
-        bool v = tid < nib;
-        sxi[tid] = v ? d.x[i0 + tid] : 0.0; syi[tid] = v ? d.y[i0 + tid] : 0.0; szi[tid] = v ? d.z[i0 + tid] : 0.0;
-        shc[tid] = v ? __double2hiint(d.c9[i0 + tid]) : -1;
-    }
-    for (int w = tid; w < KK_NI * KK_WORDS; w += KK_THREADS) (&bitmap[0][0])[w] = 0u;
-    if (tid == 0) anyhit = 0;
+    const int iters = (N + 127) >> 7;                  // iterations of every warp
+    const int npad = iters << 7;
 
-    double xj[TJ], yj[TJ], zj[TJ], gm[TJ];
-    int hcj[TJ];
-#pragma unroll
-    for (int k = 0; k < TJ; ++k) {
-        int j = k * KK_THREADS + tid;
-        bool v = j < N;
-        xj[k] = v ? d.x[j] : 1e100; yj[k] = v ? d.y[j] : 1e100; zj[k] = v ? d.z[j] : 1e100;
-        gm[k] = v ? d.G * d.m[j] : 0.0;
-        hcj[k] = v ? __double2hiint(d.c9[j]) : -1;
-    }
-    double acc[KK_NV];
-#pragma unroll
-    for (int v = 0; v < KK_NV; ++v) acc[v] = 0.0;
-    __syncthreads();
+    // geometry of this warp: R row pairs x P phases, warp wi of its group, covering bodies [wi L, (wi + 1) L)
+    const int logP = warp < 16 ? 3 : warp < 24 ? 4 : 5;
+    const int wi = warp < 16 ? warp : warp < 24 ? warp - 16 : warp - 24;
+    const int rowbase = warp < 16 ? 0 : warp < 24 ? 8 : 12;
+    const int P = 1 << logP, phase = lane & (P - 1), rp = lane >> logP;
+    const int ii = rowbase + 2 * rp, i = i0 + ii;
+    const bool ok0 = ii < nib, ok1 = ii + 1 < nib;
 
+    // stage the bodies j: all loads of the (at most 3) rounds in flight together; 9 rc^2 as k_rcrit forms it
+    {
+        constexpr int ROUNDS = (KK_MAXN + KK_THREADS - 1) / KK_THREADS;
+        double lx[ROUNDS], ly[ROUNDS], lz[ROUNDS], lm[ROUNDS], lr[ROUNDS];
 #pragma unroll
-    for (int ii = 0; ii < KK_NI; ++ii) {
-        if (ii < nib) {
-            const double xi = sxi[ii], yi = syi[ii], zi = szi[ii];
-            const int hci = shc[ii];
+        for (int q = 0; q < ROUNDS; ++q) {
+            const int j = tid + q * KK_THREADS;
+            const bool v = j < N;
+            lx[q] = v ? d.x[j] : 1e100; ly[q] = v ? d.y[j] : 1e100; lz[q] = v ? d.z[j] : 1e100;
+            lm[q] = v ? d.m[j] : 0.0; lr[q] = v ? d.rc[j] : -1.0;
+        }
 #pragma unroll
-            for (int k = 0; k < TJ; ++k) {
-                double dx = xj[k] - xi, dy = yj[k] - yi, dz = zj[k] - zi;
-                double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                bool hit = __double2hiint(r2) <= max(hci, hcj[k]);
-                double s3 = gm[k] * rinv3_fast(r2);
-                if (hit) {
-                    int j = k * KK_THREADS + tid;
-                    atomicOr(&bitmap[ii][j >> 5], 1u << (j & 31));
-                    anyhit = 1;
-                    s3 = 0.0;                                   // counted exactly below (and r2 == 0 is the body itself)
-                }
-                acc[3 * ii] = fma(s3, dx, acc[3 * ii]);
-                acc[3 * ii + 1] = fma(s3, dy, acc[3 * ii + 1]);
-                acc[3 * ii + 2] = fma(s3, dz, acc[3 * ii + 2]);
+        for (int q = 0; q < ROUNDS; ++q) {
+            const int j = tid + q * KK_THREADS;
+            if (j < npad) {
+                KickBody b;
+                b.x = lx[q]; b.y = ly[q]; b.z = lz[q]; b.gm = d.G * lm[q];
+                S.body[j] = b;
+                S.rc[j] = lr[q];
+                S.hc[j] = lr[q] >= 0.0 ? __double2hiint(9.0 * lr[q] * lr[q]) : -1;
             }
         }
     }
-
-    // ---- warp reduction: halving butterfly 48 -> 24 -> 12 -> 6 -> 3, then the lane pair
-#pragma unroll
-    for (int half = KK_NV / 2, o = 16; o >= 2; half >>= 1, o >>= 1) {
-        const bool up = (lane & o) != 0;
-#pragma unroll
-        for (int v = 0; v < half; ++v) {
-            double send = up ? acc[v] : acc[v + half];
-            double keep = up ? acc[v + half] : acc[v];
-            acc[v] = keep + __shfl_xor_sync(0xffffffffu, send, o);
-        }
-    }
-#pragma unroll
-    for (int v = 0; v < 3; ++v) acc[v] += __shfl_xor_sync(0xffffffffu, acc[v], 1);
-    if ((lane & 1) == 0) {
-        int base = ((lane >> 4) & 1) * 24 + ((lane >> 3) & 1) * 12 + ((lane >> 2) & 1) * 6 + ((lane >> 1) & 1) * 3;
-#pragma unroll
-        for (int v = 0; v < 3; ++v) red[warp][base + v] = acc[v];
-    }
-    __syncthreads();
-    if (tid < KK_NV) {
-        double t = 0.0;
-#pragma unroll
-        for (int w = 0; w < KK_THREADS / 32; ++w) t += red[w][tid];
-        acc_s[tid] = t;
+    // a row that does not exist sits far away: it never passes the precheck and its sums are never read
+    const double xi0 = ok0 ? d.x[i] : 1e150, yi0 = ok0 ? d.y[i] : 1e150, zi0 = ok0 ? d.z[i] : 1e150;
+    const double xi1 = ok1 ? d.x[i + 1] : 1e150, yi1 = ok1 ? d.y[i + 1] : 1e150, zi1 = ok1 ? d.z[i + 1] : 1e150;
+    const double rci0 = ok0 ? d.rc[i] : 0.0, rci1 = ok1 ? d.rc[i + 1] : 0.0;
+    const int hci0 = ok0 ? __double2hiint(9.0 * rci0 * rci0) : -1, hci1 = ok1 ? __double2hiint(9.0 * rci1 * rci1) : -1;
+    // the velocity component this thread will kick at the end: loaded now, off the critical path
+    double vel0 = 0.0;
+    if (tid < 3 * nib) {
+        const int r = tid / 3, c = tid - 3 * r;
+        vel0 = (c == 0 ? d.vx : c == 1 ? d.vy : d.vz)[i0 + r];
     }
     __syncthreads();
 
-    // ---- pairs inside the precheck sphere: exact weight, candidate list
-    if (anyhit) {
-        const int words = (N + 31) >> 5;
-        for (int ii = warp; ii < nib; ii += KK_THREADS / 32) {
-            const int i = i0 + ii;
-            const double xi = sxi[ii], yi = syi[ii], zi = szi[ii], rci = d.rc[i], c9i = d.c9[i];
-            double ax = 0.0, ay = 0.0, az = 0.0;
-            for (int w = lane; w < words; w += 32) {
-                unsigned bits = bitmap[ii][w];
-                while (bits) {
-                    int j = (w << 5) + __ffs(bits) - 1;
-                    bits &= bits - 1;
-                    if (j == i) continue;
-                    double dx = d.x[j] - xi, dy = d.y[j] - yi, dz = d.z[j] - zi;
+    double ax0 = 0.0, ay0 = 0.0, az0 = 0.0, ax1 = 0.0, ay1 = 0.0, az1 = 0.0;
+    if (rowbase < nib) {                                // warp-uniform: the group has rows in this block
+        const int L = iters << logP;
+        {
+            const KickBody *pb = &S.body[wi * L + phase];
+            const int *ph = &S.hc[wi * L + phase];
+            unsigned *pw = S.hitw[warp];
+            const bool lane0 = lane == 0;
+#pragma unroll 2
+            for (int t = 0; t < iters; ++t) {
+                const KickBody bj = *pb;
+                const int hcj = *ph;
+                pb += P; ph += P;
+                {
+                    double dx = bj.x - xi0, dy = bj.y - yi0, dz = bj.z - zi0;
                     double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                    double r = sqrt(r2);
-                    double rcij = fmax(rci, d.rc[j]);
-                    double s3 = d.G * d.m[j] / (r2 * r) * kick_weight(r, rcij);
-                    ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
-                    if (record && i < j && r2 < fmax(c9i, d.c9[j])) {
-                        int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
-                        if (idx < d.cap) d.cand[idx] = make_int2(i, j);
-                        else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+                    bool hit = __double2hiint(r2) <= max(hci0, hcj);
+                    int yh = __double2hiint(rsqrt_seed(r2));
+                    double y0 = __hiloint2double(hit ? 0 : yh, 0);  // weight 0 for hits (and r2 == 0: the body itself)
+                    double u = y0 * y0;
+                    double e = fma(-r2, u, 1.0);
+                    double w = y0 * u;
+                    double p = fma(1.875, e, 1.5);
+                    double s3 = bj.gm * fma(p * e, w, w);           // G m_j y0^3 (1 + 3e/2 + 15 e^2/8)
+                    ax0 = fma(s3, dx, ax0); ay0 = fma(s3, dy, ay0); az0 = fma(s3, dz, az0);
+                    unsigned hm = __ballot_sync(0xffffffffu, hit);
+                    if (lane0) pw[0] = hm;
+                }
+                {
+                    double dx = bj.x - xi1, dy = bj.y - yi1, dz = bj.z - zi1;
+                    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                    bool hit = __double2hiint(r2) <= max(hci1, hcj);
+                    int yh = __double2hiint(rsqrt_seed(r2));
+                    double y0 = __hiloint2double(hit ? 0 : yh, 0);
+                    double u = y0 * y0;
+                    double e = fma(-r2, u, 1.0);
+                    double w = y0 * u;
+                    double p = fma(1.875, e, 1.5);
+                    double s3 = bj.gm * fma(p * e, w, w);
+                    ax1 = fma(s3, dx, ax1); ay1 = fma(s3, dy, ay1); az1 = fma(s3, dz, az1);
+                    unsigned hm = __ballot_sync(0xffffffffu, hit);
+                    if (lane0) pw[1] = hm;
+                }
+                pw += 2;
+            }
+        }
+        // the P phases of a row pair: every lane of the pair gets the sums of its two rows
+        for (int o = 1; o < P; o <<= 1) {
+            ax0 += __shfl_xor_sync(0xffffffffu, ax0, o); ay0 += __shfl_xor_sync(0xffffffffu, ay0, o); az0 += __shfl_xor_sync(0xffffffffu, az0, o);
+            ax1 += __shfl_xor_sync(0xffffffffu, ax1, o); ay1 += __shfl_xor_sync(0xffffffffu, ay1, o); az1 += __shfl_xor_sync(0xffffffffu, az1, o);
+        }
+        __syncwarp();
+
+        // ---- this warp's pairs inside the precheck sphere: exact weight, candidate list.
+        // Hit word 2 t + s, bit b: row rowbase + 2 (b >> logP) + s, body j = wi L + t P + (b & (P - 1)).  The hits are listed
+        // in (word, b) order, 32 at a time; lane e evaluates entry e; the row pair's first lane adds its entries in list order.
+        const unsigned word = lane < 2 * iters ? S.hitw[warp][lane] : 0u;
+        const int cnt = __popc(word);
+        int inc = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int n = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += n; }
+        const int total = __shfl_sync(0xffffffffu, inc, 31), off = inc - cnt;
+        for (int base = 0; base < total; base += 32) {
+            {
+                unsigned wb = word;
+                int e = off - base;
+                while (wb) {
+                    int b = __ffs(wb) - 1;
+                    wb &= wb - 1;
+                    if (e >= 0 && e < 32) S.list[warp][e].code = (b << 8) | lane;
+                    ++e;
+                }
+            }
+            __syncwarp();
+            const int nwin = min(32, total - base);
+            bool cand = false;
+            int ci = 0, cj = 0;
+            if (lane < nwin) {
+                const int code = S.list[warp][lane].code, b = code >> 8, wd = code & 255;
+                ci = i0 + rowbase + 2 * (b >> logP) + (wd & 1); cj = wi * L + ((wd >> 1) << logP) + (b & (P - 1));
+                double cx = 0.0, cy = 0.0, cz = 0.0;
+                if (cj != ci) {
+                    const KickBody bj = S.body[cj], bi = S.body[ci];
+                    double dx = bj.x - bi.x, dy = bj.y - bi.y, dz = bj.z - bi.z;
+                    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                    const double rcij = fmax(S.rc[ci], S.rc[cj]);
+                    double s3 = kick_scale_exact(r2, rcij, bj.gm);
+                    cand = record && ci < cj && r2 < 9.0 * rcij * rcij;      // = max(9 rc_i^2, 9 rc_j^2) as k_rcrit rounds it
+                    cx = s3 * dx; cy = s3 * dy; cz = s3 * dz;
+                }
+                S.list[warp][lane].cx = cx; S.list[warp][lane].cy = cy; S.list[warp][lane].cz = cz;
+            }
+            const unsigned cm = __ballot_sync(0xffffffffu, cand);
+            if (cm) {
+                int cb = 0;
+                if (lane == 0) cb = atomicAdd(&d.cnt[CI_NCAND], __popc(cm));
+                cb = __shfl_sync(0xffffffffu, cb, 0);
+                if (cand) {
+                    int idx = cb + __popc(cm & ((1u << lane) - 1u));
+                    if (idx < d.cap) d.cand[idx] = make_int2(ci, cj);
+                    else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+                }
+            }
+            __syncwarp();
+            if (phase == 0) {
+                for (int e = 0; e < nwin; ++e) {
+                    const int code = S.list[warp][e].code;
+                    if (((code >> 8) >> logP) == rp) {
+                        const double cx = S.list[warp][e].cx, cy = S.list[warp][e].cy, cz = S.list[warp][e].cz;
+                        if (code & 1) { ax1 += cx; ay1 += cy; az1 += cz; } else { ax0 += cx; ay0 += cy; az0 += cz; }
                     }
                 }
             }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                ax += __shfl_xor_sync(0xffffffffu, ax, o);
-                ay += __shfl_xor_sync(0xffffffffu, ay, o);
-                az += __shfl_xor_sync(0xffffffffu, az, o);
-            }
-            if (lane == 0) { acc_s[3 * ii] += ax; acc_s[3 * ii + 1] += ay; acc_s[3 * ii + 2] += az; }
+            __syncwarp();
         }
-        __syncthreads();
+        if (phase == 0) {
+            S.wsum[warp][2 * rp][0] = ax0; S.wsum[warp][2 * rp][1] = ay0; S.wsum[warp][2 * rp][2] = az0;
+            S.wsum[warp][2 * rp + 1][0] = ax1; S.wsum[warp][2 * rp + 1][1] = ay1; S.wsum[warp][2 * rp + 1][2] = az1;
+        }
     }
+    __syncthreads();
     if (tid < 3 * nib) {
-        const int ii = tid / 3, c = tid - 3 * ii, i = i0 + ii;
-        const double a = acc_s[tid];
-        double *v = c == 0 ? d.vx : c == 1 ? d.vy : d.vz;
-        v[i] = fma(h, a, v[i]);
-        if (aout) aout[(size_t)c * d.ntot + i] = a;
+        const int r = tid / 3, c = tid - 3 * r;
+        const int w0 = r < 8 ? 0 : r < 12 ? 16 : 24, nw = r < 8 ? 16 : r < 12 ? 8 : 4, rr = r < 8 ? r : r < 12 ? r - 8 : r - 12;
+        double a = 0.0;
+        for (int w = 0; w < nw; ++w) a += S.wsum[w0 + w][rr][c];
+        double *vel = c == 0 ? d.vx : c == 1 ? d.vy : d.vz;
+        vel[i0 + r] = fma(h, a, vel0);
+        if (aout) aout[(size_t)c * d.ntot + i0 + r] = a;
     }
 }
-template __global__ void k_kick<1>(DevState, double, int, int, double *);
-template __global__ void k_kick<2>(DevState, double, int, int, double *);
-template __global__ void k_kick<4>(DevState, double, int, int, double *);
-template __global__ void k_kick<8>(DevState, double, int, int, double *);
+
+size_t kick_smem_bytes() { return sizeof(KickSmem); }
 
 // Kick of the test particles (L334-340): one thread per particle looping over the <= 32
 // massive bodies, which sit in shared memory (broadcast reads).  Precheck against every

@@ -6,10 +6,10 @@
 
 namespace genga {
 
-constexpr int KK_THREADS = 256;   // threads per block of the kick kernel
+constexpr int KK_THREADS = 896;   // threads per block of the kick kernel: 28 warps, 7 per SM sub-partition
+constexpr int KK_WARPS = KK_THREADS / 32;
 constexpr int KK_NI = 14;         // bodies i a block owns at most: ceil(2048 / 148)
-constexpr int KK_NV = 48;         // 3 KK_NI accumulators padded to 3 * 16 for the halving butterfly
-constexpr int KK_WORDS = 64;      // 2048 / 32 bitmap words per body i
+constexpr int KK_MAXN = 2048;     // massive bodies of one system (L188)
 
 // Bulirsch-Stoer layouts: groups of 2..8 bodies on one warp (bs_warp.cuh), of 9..256 bodies on a
 // cluster of 8 CTAs (bs_cluster.cuh), larger ones on one block with a global-memory tableau (bs.cuh)
@@ -18,7 +18,8 @@ constexpr int BCB_MAXN = 256, BCB_THREADS = 256, BCB_CS = 8;
 __global__ void k_begin_map(DevState d);
 __global__ void k_reset_counters(DevState d);
 __global__ void k_rcrit(DevState d, double tau);
-template <int TJ> __global__ void k_kick(DevState d, double h, int record, int ni, double *aout);
+__global__ void k_kick(DevState d, double h, int record, int ni, double *aout);
+size_t kick_smem_bytes();
 __global__ void k_tp_kick(DevState d, double h, int record, double *aout);
 __global__ void k_kick_multi(DevState d, double h, int record, double *aout);
 __global__ void k_momentum(DevState d, const double *vx, const double *vy, const double *vz);
