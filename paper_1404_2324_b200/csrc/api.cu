@@ -263,15 +263,27 @@ static cudaError_t launch_bs_cluster(cudaStream_t st, int clusters, const DevSta
 }
 
 // One second-order map S2(h), Eq. 7 (L100), in the order of the bullet list L153-166.
-static void enqueue_map(genga_ctx *c, double h)
+static void enqueue_map(genga_ctx *c, double h, double tau, int first)
 {
     DevState &d = c->d;
     cudaStream_t st = c->st;
+    const bool tp = d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm;
+    DevState dm = d;                                          // the massive bodies alone (mode 1)
+    dm.ntot = d.nm;
     if (d.mode == GENGA_MODE_TEST_PARTICLE) { k_begin_map<<<c->sms, 256, 0, st>>>(d); LAUNCH(c); }
     k_reset_counters<<<1, 32, 0, st>>>(d); LAUNCH(c);
-    enqueue_kick(c, 0.5 * h, 1, nullptr);
-    enqueue_sun(c, 0.5 * h);
-    k_drift<<<nblk(d.ntot, 128), 128, 0, st>>>(d, h); LAUNCH(c);
+    if (tp) {
+        // particles: kick, Sun kick and drift in one pass (k_tp_front); the massive bodies as in mode 0
+        launch_kick(c, 0.5 * h, 1, nullptr); LAUNCH(c);
+        k_momentum<<<1, red_threads(d.nm), 0, st>>>(d, d.vx, d.vy, d.vz); LAUNCH(c);
+        k_tp_front<<<nblk(d.ntot - d.nm, 128), 128, 0, st>>>(d, h, tau, first); LAUNCH(c);
+        k_shift<<<nblk(d.nm, 256), 256, 0, st>>>(dm, d.x, d.y, d.z, 0.5 * h, 0); LAUNCH(c);
+        k_drift<<<nblk(d.nm, 128), 128, 0, st>>>(dm, h); LAUNCH(c);
+    } else {
+        enqueue_kick(c, 0.5 * h, 1, nullptr);
+        enqueue_sun(c, 0.5 * h);
+        k_drift<<<nblk(d.ntot, 128), 128, 0, st>>>(d, h); LAUNCH(c);
+    }
     const int pair_blocks = (int)std::min<long long>((d.cap + 127) / 128, 4LL * c->sms);
     k_confirm<<<pair_blocks, 128, 0, st>>>(d, h); LAUNCH(c);
     k_label_init<<<nblk(d.nmtot, 256), 256, 0, st>>>(d); LAUNCH(c);
@@ -307,8 +319,15 @@ static void enqueue_map(genga_ctx *c, double h)
             if (d.nm + 1 > BW_MAXN) { k_tp_bs<32><<<2 * c->sms, 128, 0, st>>>(d, h, BW_MAXN); LAUNCH(c); }
         }
     }
-    enqueue_sun(c, 0.5 * h);
-    enqueue_kick(c, 0.5 * h, 0, nullptr);
+    if (tp) {
+        k_momentum<<<1, red_threads(d.nm), 0, st>>>(d, d.vx, d.vy, d.vz); LAUNCH(c);
+        k_shift<<<nblk(d.nm, 256), 256, 0, st>>>(dm, d.x, d.y, d.z, 0.5 * h, 0); LAUNCH(c);
+        k_tp_back<<<nblk(d.ntot - d.nm, 128), 128, 0, st>>>(d, h); LAUNCH(c);
+        launch_kick(c, 0.5 * h, 0, nullptr); LAUNCH(c);
+    } else {
+        enqueue_sun(c, 0.5 * h);
+        enqueue_kick(c, 0.5 * h, 0, nullptr);
+    }
 }
 
 static int maps_per_step(int order) { return order == 2 ? 1 : order == 4 ? 3 : 7; }
@@ -318,8 +337,14 @@ static void enqueue_step(genga_ctx *c, double dt, int order)
     DevState &d = c->d;
     double w[7];
     int nw = yoshida_weights(order, w);
-    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt); LAUNCH(c);
-    for (int k = 0; k < nw; ++k) enqueue_map(c, w[k] * dt);
+    if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {    // the particles' rc: k_tp_front of the first map
+        DevState dm = d;
+        dm.ntot = d.nm;
+        k_rcrit<<<nblk(d.nm, 128), 128, 0, c->st>>>(dm, dt); LAUNCH(c);
+    } else {
+        k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt); LAUNCH(c);
+    }
+    for (int k = 0; k < nw; ++k) enqueue_map(c, w[k] * dt, dt, k == 0);
 }
 
 static long long interactions_per_eval(const DevState &d)

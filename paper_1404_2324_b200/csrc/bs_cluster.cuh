@@ -58,6 +58,14 @@ __device__ __forceinline__ BcLane bc_lanes(int n)
     return t;
 }
 
+#ifdef GENGA_TRACE
+__device__ long long g_bc_prof[1024][8];     // per CTA: cycles in rhs, cluster syncs, tableau, attempts
+#define BC_T0() long long tq_ = clock64()
+#define BC_ACC(k) do { long long tn_ = clock64(); if (threadIdx.x == 0) g_bc_prof[blockIdx.x][k] += tn_ - tq_; tq_ = tn_; } while (0)
+#else
+#define BC_T0()
+#define BC_ACC(k)
+#endif
 // Force on body t.i at the positions q of the owners (Eq. 1 L73-74 through Eq. 8; star fixed
 // at the origin, L314; every pair of the group is examined at every evaluation, L505).  The n^2
 // examinations are done first in FP32 against a threshold widened by more than the FP32 rounding,
@@ -67,6 +75,7 @@ __device__ __forceinline__ void bc_rhs(BcSmem<MAXN, THREADS> &S, const BcLane &t
                                        const double q[3], double a[3])
 {
     GENGA_BS_RHS_HOOK();
+    BC_T0();
     double(*p)[MAXN] = S.pos[buf];
     float(*pf)[MAXN] = S.pf[buf];
     if (t.owner) {
@@ -74,6 +83,7 @@ __device__ __forceinline__ void bc_rhs(BcSmem<MAXN, THREADS> &S, const BcLane &t
         pf[0][t.i] = (float)q[0]; pf[1][t.i] = (float)q[1]; pf[2][t.i] = (float)q[2];
     }
     __syncthreads();
+    BC_ACC(4);
     buf ^= 1;
     double ax = 0.0, ay = 0.0, az = 0.0;
     if (t.i < t.n) {
@@ -93,6 +103,7 @@ __device__ __forceinline__ void bc_rhs(BcSmem<MAXN, THREADS> &S, const BcLane &t
                 bool in = (d2 < fmaxf(ft, S.thr2[jc]) && j != i) || j == n;
                 mask |= (in ? 1u : 0u) << kk;
             }
+            BC_ACC(5);
             while (mask) {
                 int j = j0 + (__ffs(mask) - 1) * L;
                 mask &= mask - 1;
@@ -113,12 +124,14 @@ __device__ __forceinline__ void bc_rhs(BcSmem<MAXN, THREADS> &S, const BcLane &t
             }
         }
     }
+    BC_ACC(6);
     for (int o = t.L >> 1; o > 0; o >>= 1) {
         ax += __shfl_xor_sync(0xffffffffu, ax, o);
         ay += __shfl_xor_sync(0xffffffffu, ay, o);
         az += __shfl_xor_sync(0xffffffffu, az, o);
     }
     a[0] = ax; a[1] = ay; a[2] = az;
+    BC_ACC(7);
 }
 
 template <int MAXN, int THREADS>
@@ -183,6 +196,7 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
             bc_rhs(S, t, buf, G, m0, q, acc0);
             fresh = false;
         }
+        BC_T0();
         // ---- my columns: Gragg's modified midpoint rule with nk substeps
 #pragma unroll 1
         for (int pass = 0; pass < BS_KMAX / CS; ++pass) {
@@ -214,7 +228,9 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
                 }
             }
         }
+        BC_ACC(0);
         bc_sync<CS>();
+        BC_ACC(1);
         // ---- CTA 0: Aitken-Neville tableau in (H/n_k)^2, first row whose error passes
         if (rank == 0) {
             double e[BS_KMAX];
@@ -271,7 +287,12 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
             }
             if (threadIdx.x == 0) S.kstar = kstar;
         }
+        BC_ACC(2);
         bc_sync<CS>();
+        BC_ACC(1);
+#ifdef GENGA_TRACE
+        if (threadIdx.x == 0) g_bc_prof[blockIdx.x][3] += 1;
+#endif
         const int kstar = S0->kstar;
         if (kstar >= 0) {
             if (CS > 1 && rank != 0) {

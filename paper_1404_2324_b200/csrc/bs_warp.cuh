@@ -44,38 +44,79 @@ __device__ __forceinline__ double direct_scale_nb(double d2, double rcij, double
     return Gmj * (rinv * rinv) * rinv * w1;
 }
 
-// Force on this lane's body at position q; the partners are the other lanes of its S-lane segment
-// (same column): partner t = 0..n-2 sits in segment lane src[t] = (b + 1 + t) mod n and carries
-// rcij[t] = max(rc_b, rc_j) (0 for a massless or missing partner, so that it never passes the test),
-// irc[t] = 1 / (0.9 rcij), gm[t] = G m_j.  n is uniform over the warp.
-// Star fixed at the origin (L314); every pair of the group is examined at every evaluation (L505).
+// Forces on this lane's body at TWO positions qA, qB at once; the partners are the other lanes of its
+// S-lane segment (same column): partner t = 0..n-2 sits in segment lane src[t] = (b + 1 + t) mod n and
+// carries rcij[t] = max(rc_b, rc_j) (0 for a massless or missing partner, so that it never passes the
+// test), irc[t] = 1 / (0.9 rcij), gm[t] = G m_j.  Star fixed at the origin (L314); every pair of the group
+// is examined at every evaluation (L505).
+// Why two: in Gragg's rule q_{k+1} = q_{k-1} + 2 eta V_k and V_{k+1} = V_{k-1} + 2 eta a(q_k), so a(q_k)
+// and a(q_{k+1}) do not depend on each other; evaluated in one straight-line block their two dependent
+// chains (~300 cycles each: shuffle, distance, changeover weight) overlap.  For S <= 4 there is no branch
+// at all (a partner outside rc_ij is computed and discarded); for S = 8 a partner nobody in the warp is
+// close to is skipped.
 template <int S>
-__device__ __forceinline__ void bw_rhs(const double q[3], const int n, double Gm0, const int (&src)[S], const double (&rcij)[S],
-                                       const double (&irc)[S], const double (&gm)[S], double a[3])
+__device__ __forceinline__ void bw_rhs2(const double (&qA)[3], const double (&qB)[3], double Gm0, const int (&src)[S],
+                                        const double (&rcij)[S], const double (&irc)[S], const double (&gm)[S],
+                                        double (&aA)[3], double (&aB)[3])
 {
     GENGA_BS_RHS_HOOK();
     const unsigned full = 0xffffffffu;
-    double r2 = fma(q[2], q[2], fma(q[1], q[1], q[0] * q[0]));
-    double s0 = -Gm0 * rinv3_fast(r2);
-    double ax = s0 * q[0], ay = s0 * q[1], az = s0 * q[2];
+    double rA = fma(qA[2], qA[2], fma(qA[1], qA[1], qA[0] * qA[0]));
+    double rB = fma(qB[2], qB[2], fma(qB[1], qB[1], qB[0] * qB[0]));
+    double sA = -Gm0 * rinv3_fast(rA), sB = -Gm0 * rinv3_fast(rB);
+    double ax = sA * qA[0], ay = sA * qA[1], az = sA * qA[2];
+    double bx = sB * qB[0], by = sB * qB[1], bz = sB * qB[2];
 #pragma unroll
     for (int t = 0; t < S - 1; ++t) {
-        if (t < n - 1) {                                      // warp-uniform
-            double dx = __shfl_sync(full, q[0], src[t], S) - q[0];
-            double dy = __shfl_sync(full, q[1], src[t], S) - q[1];
-            double dz = __shfl_sync(full, q[2], src[t], S) - q[2];
-            double d2 = fma(dz, dz, fma(dy, dy, dx * dx));
-            bool in = d2 < rcij[t] * rcij[t];
-            if (__any_sync(full, in)) {                       // warp-uniform: no divergence
-                double sc = direct_scale_nb(in ? d2 : 1.0, rcij[t], irc[t], gm[t]);
-                sc = in ? sc : 0.0;
-                ax = fma(sc, dx, ax); ay = fma(sc, dy, ay); az = fma(sc, dz, az);
-            }
+        double dxA = __shfl_sync(full, qA[0], src[t], S) - qA[0];
+        double dyA = __shfl_sync(full, qA[1], src[t], S) - qA[1];
+        double dzA = __shfl_sync(full, qA[2], src[t], S) - qA[2];
+        double dxB = __shfl_sync(full, qB[0], src[t], S) - qB[0];
+        double dyB = __shfl_sync(full, qB[1], src[t], S) - qB[1];
+        double dzB = __shfl_sync(full, qB[2], src[t], S) - qB[2];
+        double dA = fma(dzA, dzA, fma(dyA, dyA, dxA * dxA)), dB = fma(dzB, dzB, fma(dyB, dyB, dxB * dxB));
+        const double rc2 = rcij[t] * rcij[t];
+        bool inA = dA < rc2, inB = dB < rc2;
+        if (S <= 4 || __any_sync(full, inA || inB)) {             // S = 8: warp-uniform skip
+            double scA = direct_scale_nb(inA ? dA : 1.0, rcij[t], irc[t], gm[t]);
+            double scB = direct_scale_nb(inB ? dB : 1.0, rcij[t], irc[t], gm[t]);
+            scA = inA ? scA : 0.0; scB = inB ? scB : 0.0;
+            ax = fma(scA, dxA, ax); ay = fma(scA, dyA, ay); az = fma(scA, dzA, az);
+            bx = fma(scB, dxB, bx); by = fma(scB, dyB, by); bz = fma(scB, dzB, bz);
         }
     }
-    a[0] = ax; a[1] = ay; a[2] = az;
+    aA[0] = ax; aA[1] = ay; aA[2] = az;
+    aB[0] = bx; aB[1] = by; aB[2] = bz;
 }
 
+// One entry of the Aitken-Neville tableau in (H/n_k)^2: component c of body b.  Reads the column results
+// T[k][0], writes the diagonal T[k][k] back and returns the squared last corrections (T[k][k] - T[k][k-1])^2.
+__device__ __forceinline__ void bw_neville(BwSmem &W, int c, int b, double (&d2)[BS_KMAX])
+{
+    double row[BS_KMAX] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int k = 0; k < BS_KMAX; ++k) {
+        double cur = W.tab[k][c][b], prev = row[0], diff = 0.0;
+        row[0] = cur;
+#pragma unroll
+        for (int j = 1; j <= k; ++j) {
+            const double ratio = double(k + 1) / double(k - j + 1);
+            const double iden = 1.0 / (ratio * ratio - 1.0);
+            double tmp = row[j];
+            double nxt = cur + (cur - prev) * iden;
+            diff = nxt - cur;
+            cur = nxt;
+            row[j] = cur;
+            prev = tmp;
+        }
+        W.tab[k][c][b] = cur;                                     // T[k][k]
+        d2[k] = diff * diff;
+    }
+}
+
+#ifdef GENGA_TRACE
+__device__ unsigned long long g_bw_prof[4];
+#endif
 // Integrate one group over h.  Lane = S * g + b; Y = state of body b (same in every segment; any
 // finite dummy for b >= n).  On return Y holds the result.  Returns false on step-size underflow
 // (uniform over the warp).
@@ -86,7 +127,8 @@ __device__ __forceinline__ bool bw_integrate(BwSmem &W, const int lane, const in
 {
     constexpr int NCG = 32 / S;                // segments: 16 (8 of them idle), 8 or 4
     constexpr int CPL = NCG >= BS_KMAX ? 1 : BS_KMAX / NCG;          // columns per lane: 1 or 2
-    constexpr int NIT = CPL == 1 ? 2 * BS_KMAX : 2 * BS_KMAX + 2;   // force evaluations per attempt after the first
+    constexpr int NIT = CPL == 1 ? BS_KMAX : BS_KMAX + 1;            // double force evaluations per attempt
+    constexpr int NROUND = (6 * S + 31) / 32;                         // tableau entries (c, b) per lane
     const unsigned full = 0xffffffffu;
     const int cg = lane / S, b = lane % S;
     const bool body = b < n && cg < BS_KMAX;
@@ -102,7 +144,7 @@ __device__ __forceinline__ bool bw_integrate(BwSmem &W, const int lane, const in
         double rcj = __shfl_sync(full, my_rc, j, S);
         double mj = __shfl_sync(full, my_m, j, S);
         double r = fmax(my_rc, rcj);
-        bool valid = body && j != b && mj != 0.0 && r > 0.0;
+        bool valid = body && j != b && mj != 0.0 && r > 0.0 && t < n - 1;
         rcij[t] = valid ? r : 0.0;
         irc[t] = valid ? 1.0 / (0.9 * r) : 0.0;
         gm[t] = valid ? G * mj : 0.0;
@@ -120,14 +162,18 @@ __device__ __forceinline__ bool bw_integrate(BwSmem &W, const int lane, const in
             for (int c = 0; c < 3; ++c) { q[c] = Y[c]; V[c] = Y[3 + c]; }
             isq = body ? 1.0 / (q[0] * q[0] + q[1] * q[1] + q[2] * q[2]) : 0.0;
             isv = body ? 1.0 / (V[0] * V[0] + V[1] * V[1] + V[2] * V[2]) : 0.0;
-            bw_rhs<S>(q, n, Gm0, src, rcij, irc, gm, acc0);
+            double dummy[3];
+            bw_rhs2<S>(q, q, Gm0, src, rcij, irc, gm, acc0, dummy);
             fresh = false;
         }
-        // ---- my column(s): Gragg's modified midpoint rule, all lanes in step
-        int pass = 0, col = cg, nk = 2 * (col + 1), ms = 1;
-        bool act = true;
-        double eta = H / nk;
-        double qa[3], Va[3], qb[3], Vb[3], acc[3];
+        // ---- my column(s): Gragg's modified midpoint rule, two substeps per iteration, all lanes in step.
+        // Column col (n_k = 2 (col + 1) substeps) ends in its iteration number col.
+#ifdef GENGA_TRACE
+        long long tp0 = clock64();
+#endif
+        int col = cg, left = col + 1, pass = 0;
+        double eta = H / (2 * (col + 1));
+        double qa[3], Va[3], qb[3], Vb[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             qa[c] = q[c]; Va[c] = V[c];
@@ -135,83 +181,68 @@ __device__ __forceinline__ bool bw_integrate(BwSmem &W, const int lane, const in
         }
 #pragma unroll 1
         for (int it = 0; it < NIT; ++it) {
-            bw_rhs<S>(qb, n, Gm0, src, rcij, irc, gm, acc);
-            if (act) {
-                if (ms < nk) {
+            double qc[3], A[3], C[3];
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        double qn = qa[c] + 2.0 * eta * Vb[c];
-                        double vn = Va[c] + 2.0 * eta * acc[c];
-                        qa[c] = qb[c]; Va[c] = Vb[c]; qb[c] = qn; Vb[c] = vn;
-                    }
-                    ++ms;
-                } else {
-                    if (body) {
+            for (int c = 0; c < 3; ++c) qc[c] = qa[c] + 2.0 * eta * Vb[c];
+            bw_rhs2<S>(qb, qc, Gm0, src, rcij, irc, gm, A, C);
+            const bool fin = --left == 0;
 #pragma unroll
-                        for (int c = 0; c < 3; ++c) {
-                            W.tab[col][c][b] = 0.5 * (qb[c] + qa[c] + eta * Vb[c]);
-                            W.tab[col][3 + c][b] = 0.5 * (Vb[c] + Va[c] + eta * acc[c]);
-                        }
-                    }
-                    if (++pass < CPL) {
-                        col = BS_KMAX - 1 - cg; nk = 2 * (col + 1); ms = 1; eta = H / nk;
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) {
-                            qa[c] = q[c]; Va[c] = V[c];
-                            qb[c] = q[c] + eta * V[c]; Vb[c] = V[c] + eta * acc0[c];
-                        }
-                    } else {
-                        act = false;
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) qb[c] = q[c];      // idle lanes: keep evaluating a harmless point
-                    }
+            for (int c = 0; c < 3; ++c) {
+                double vc = Va[c] + 2.0 * eta * A[c];
+                if (fin && body) {
+                    W.tab[col][c][b] = 0.5 * (qc[c] + qb[c] + eta * vc);
+                    W.tab[col][3 + c][b] = 0.5 * (vc + Vb[c] + eta * C[c]);
                 }
+                double qd = qb[c] + 2.0 * eta * vc, vd = Vb[c] + 2.0 * eta * C[c];
+                qa[c] = qc[c]; Va[c] = vc; qb[c] = qd; Vb[c] = vd;
+            }
+            if (CPL == 2 && fin && pass == 0) {                       // second column of this lane
+                pass = 1; col = BS_KMAX - 1 - cg; left = col + 1; eta = H / (2 * (col + 1));
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    qa[c] = q[c]; Va[c] = V[c];
+                    qb[c] = q[c] + eta * V[c]; Vb[c] = V[c] + eta * acc0[c];
+                }
+            } else if (left < 0) {                                    // finished lanes: stay at a harmless point
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { qa[c] = q[c]; qb[c] = q[c]; Va[c] = 0.0; Vb[c] = 0.0; }
+                eta = 0.0;
             }
         }
         __syncwarp();
-        // ---- Aitken-Neville tableau in (H/n_k)^2 by the first segment; first row whose error passes
-        double e[BS_KMAX];
+#ifdef GENGA_TRACE
+        long long tp1 = clock64();
+#endif
+        // ---- Aitken-Neville tableau in (H/n_k)^2, one (component, body) entry per lane; first row whose error passes
+        double d2[NROUND][BS_KMAX];
 #pragma unroll
-        for (int k = 0; k < BS_KMAX; ++k) e[k] = 0.0;
-        if (lane < S && body) {
-            double dq2[BS_KMAX], dv2[BS_KMAX];
+        for (int r = 0; r < NROUND; ++r) {
+            const int item = lane + 32 * r, c = item / S, bb = item % S;
 #pragma unroll
-            for (int k = 0; k < BS_KMAX; ++k) { dq2[k] = 0.0; dv2[k] = 0.0; }
-#pragma unroll
-            for (int c = 0; c < 6; ++c) {
-                double row[BS_KMAX] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-                for (int k = 0; k < BS_KMAX; ++k) {
-                    double cur = W.tab[k][c][b], prev = row[0], diff = 0.0;
-                    row[0] = cur;
-#pragma unroll
-                    for (int j = 1; j <= k; ++j) {
-                        const double ratio = double(k + 1) / double(k - j + 1);
-                        const double iden = 1.0 / (ratio * ratio - 1.0);
-                        double tmp = row[j];
-                        double nxt = cur + (cur - prev) * iden;
-                        diff = nxt - cur;
-                        cur = nxt;
-                        row[j] = cur;
-                        prev = tmp;
-                    }
-                    W.tab[k][c][b] = cur;                       // T[k][k]
-                    if (c < 3) dq2[k] += diff * diff; else dv2[k] += diff * diff;
-                }
-            }
-#pragma unroll
-            for (int k = 1; k < BS_KMAX; ++k) e[k] = fmax(dq2[k] * isq, dv2[k] * isv);
+            for (int k = 0; k < BS_KMAX; ++k) d2[r][k] = 0.0;
+            if (item < 6 * S && bb < n) bw_neville(W, c, bb, d2[r]);
         }
         int kstar = -1;
 #pragma unroll
         for (int k = BS_KMAX - 1; k >= 1; --k) {
-            double r = e[k];
+            // body b (lanes < S): sum over the components, entry (c, b) sits in lane (c S + b) % 32 of round (c S + b) / 32
+            double dq = 0.0, dv = 0.0;
+#pragma unroll
+            for (int c = 0; c < 6; ++c) {
+                const int item = c * S + (lane % S);
+                double v = __shfl_sync(full, d2[(c * S) / 32][k], item & 31);
+                if (c < 3) dq += v; else dv += v;
+            }
+            double r = (lane < S && body) ? fmax(dq * isq, dv * isv) : 0.0;
 #pragma unroll
             for (int o = S / 2; o > 0; o >>= 1) r = fmax(r, __shfl_xor_sync(full, r, o, S));
             if (r <= eps2) kstar = k;
         }
         kstar = __shfl_sync(full, kstar, 0);
         __syncwarp();
+#ifdef GENGA_TRACE
+        if (lane == 0 && S == 2) { atomicAdd(&g_bw_prof[0], (unsigned long long)(tp1 - tp0)); atomicAdd(&g_bw_prof[1], (unsigned long long)(clock64() - tp1)); atomicAdd(&g_bw_prof[2], 1ull); }
+#endif
         if (kstar >= 0) {
             if (body) {
 #pragma unroll

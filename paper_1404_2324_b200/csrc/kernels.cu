@@ -1,5 +1,12 @@
 // Kernels of the hybrid symplectic step, sm_100a.
 // Each kernel states the operator it implements and the passage that defines it.
+#ifdef GENGA_TRACE
+#include <cuda_runtime.h>
+__device__ int g_rhs[1024];
+__device__ long long g_bs_trace[8192][4];
+__device__ int g_bs_ntrace;
+
+#endif
 #include "kernels.cuh"
 #include "bs_cluster.cuh"
 #include "bs_warp.cuh"
@@ -328,6 +335,94 @@ __global__ void __launch_bounds__(128) k_tp_kick(DevState d, double h, int recor
     d.vx[i] = fma(h, ax, d.vx[i]); d.vy[i] = fma(h, ay, d.vy[i]); d.vz[i] = fma(h, az, d.vz[i]);
 }
 
+// Test particles, fused (L334-342): a particle meets only the <= 32 massive bodies and the star, so its
+// whole half map is one pass over its 48 bytes of state instead of four kernels.
+//   k_tp_front: [rc_i = n2 |tau| |V_i| at the start of a step (Eq. 6 with R_H = 0)]  B(h/2): kick by the
+//               massive bodies + precheck, C(h/2): Sun kick, A(h): Kepler drift.  A particle that recorded a
+//               candidate keeps its state before the drift (Eq. 10 and Bulirsch-Stoer need it).
+//   k_tp_back : C(h/2), B(h/2) at the end of the map (no precheck).
+// psum must hold sum m V of the massive bodies after their own kick (front) / after Bulirsch-Stoer (back);
+// the massive bodies must not have been shifted yet (front) / must have been shifted (back): B only sees
+// differences of positions, which a common shift leaves alone.
+struct TpMassive { double x[32], y[32], z[32], gm[32], rc[32]; };
+__device__ __forceinline__ void tp_load_massive(const DevState &d, TpMassive &M)
+{
+    if (threadIdx.x < d.nm) {
+        int j = threadIdx.x;
+        M.x[j] = d.x[j]; M.y[j] = d.y[j]; M.z[j] = d.z[j]; M.gm[j] = d.G * d.m[j]; M.rc[j] = d.rc[j];
+    }
+    __syncthreads();
+}
+// acceleration of a particle at (xi, yi, zi) by the massive bodies; returns the number of candidates recorded
+template <bool RECORD>
+__device__ __forceinline__ int tp_accel(const DevState &d, const TpMassive &M, int i, double xi, double yi, double zi, double rci,
+                                        double &ax, double &ay, double &az)
+{
+    int ncand = 0;
+    ax = ay = az = 0.0;
+    const int nm = d.nm;
+    for (int j = 0; j < nm; ++j) {
+        double dx = M.x[j] - xi, dy = M.y[j] - yi, dz = M.z[j] - zi;
+        double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+        double rcij = fmax(rci, M.rc[j]);
+        double s3 = M.gm[j] * rinv3_fast(r2);
+        if (r2 < 9.0 * rcij * rcij) {
+            double r = sqrt(r2);
+            s3 = M.gm[j] / (r2 * r) * kick_weight(r, rcij);
+            if (RECORD) {
+                int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
+                if (idx < d.cap) d.cand[idx] = make_int2(j, i);
+                else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+                ++ncand;
+            }
+        }
+        ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
+    }
+    return ncand;
+}
+__global__ void __launch_bounds__(128) k_tp_front(DevState d, double h, double tau, int first)
+{
+    __shared__ TpMassive M;
+    const int i = d.nm + blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = i < d.ntot;
+    // the particle's own loads go out before the block waits for the massive bodies: one memory round trip
+    double x = 0.0, y = 0.0, z = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, rci = 0.0;
+    if (live) {
+        x = d.x[i]; y = d.y[i]; z = d.z[i]; vx = d.vx[i]; vy = d.vy[i]; vz = d.vz[i];
+        if (!first) rci = d.rc[i];
+    }
+    tp_load_massive(d, M);
+    if (!live) return;
+    if (first) {
+        rci = fmax(d.n1 * 0.0, d.n2 * fabs(tau) * sqrt(vx * vx + vy * vy + vz * vz));
+        d.rc[i] = rci;
+    }
+    double ax, ay, az;
+    const int ncand = tp_accel<true>(d, M, i, x, y, z, rci, ax, ay, az);
+    const double hh = 0.5 * h, g = hh / d.m0[0];
+    vx = fma(hh, ax, vx); vy = fma(hh, ay, vy); vz = fma(hh, az, vz);
+    x = fma(g, d.psum[0], x); y = fma(g, d.psum[1], y); z = fma(g, d.psum[2], z);
+    if (ncand) { d.x0[i] = x; d.y0[i] = y; d.z0[i] = z; d.vx0[i] = vx; d.vy0[i] = vy; d.vz0[i] = vz; }
+    if (!kepler_drift(d.G * d.m0[0], h, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
+    d.x[i] = x; d.y[i] = y; d.z[i] = z; d.vx[i] = vx; d.vy[i] = vy; d.vz[i] = vz;
+}
+__global__ void __launch_bounds__(128) k_tp_back(DevState d, double h)
+{
+    __shared__ TpMassive M;
+    const int i = d.nm + blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = i < d.ntot;
+    double x = 0.0, y = 0.0, z = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, rci = 0.0;
+    if (live) { x = d.x[i]; y = d.y[i]; z = d.z[i]; vx = d.vx[i]; vy = d.vy[i]; vz = d.vz[i]; rci = d.rc[i]; }
+    tp_load_massive(d, M);
+    if (!live) return;
+    const double hh = 0.5 * h, g = hh / d.m0[0];
+    x = fma(g, d.psum[0], x); y = fma(g, d.psum[1], y); z = fma(g, d.psum[2], z);
+    double ax, ay, az;
+    tp_accel<false>(d, M, i, x, y, z, rci, ax, ay, az);
+    d.x[i] = x; d.y[i] = y; d.z[i] = z;
+    d.vx[i] = fma(hh, ax, vx); d.vy[i] = fma(hh, ay, vy); d.vz[i] = fma(hh, az, vz);
+}
+
 // Kick in multi-system mode (L368-370): one thread per body, partners = the bodies of its
 // own system (contiguous, body = system * nm + k).
 __global__ void __launch_bounds__(128) k_kick_multi(DevState d, double h, int record, double *aout)
@@ -630,7 +725,16 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
             S.m[b] = d.m[i]; S.rc[b] = rc; S.irc[b] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
         }
         int nsteps = 0;
+#ifdef GENGA_TRACE
+        long long tc0 = clock64(); int r0 = g_rhs[blockIdx.x];
+#endif
         bool ok = bc_integrate<MAXN, THREADS, CS>(S, S0, rank, t, d.G, d.m0[0], h, d.eps, &nsteps);
+#ifdef GENGA_TRACE
+        if (rank == 0 && threadIdx.x == 0) {
+            int k = atomicAdd(&g_bs_ntrace, 1) & 8191;
+            g_bs_trace[k][0] = n; g_bs_trace[k][1] = nsteps; g_bs_trace[k][2] = g_rhs[blockIdx.x] - r0; g_bs_trace[k][3] = clock64() - tc0;
+        }
+#endif
         if (rank == 0) {
             __syncthreads();
             for (int b = threadIdx.x; b < n; b += THREADS) {
@@ -706,6 +810,9 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
         const double Gm0 = d.G * d.m0[sys];
         int nsteps = 0;
         bool ok;
+#ifdef GENGA_TRACE
+        long long tw0 = clock64();
+#endif
         if (n <= 4) {
             // segments of 2 or 4 lanes: slot b = lane % S takes body b from lane b of the 8-slot layout
             const int src = n == 2 ? (lane & 1) : (lane & 3);
@@ -717,6 +824,12 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
         } else {
             ok = bw_integrate<8>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, &nsteps);
         }
+#ifdef GENGA_TRACE
+        if (lane == 0) {
+            int k = atomicAdd(&g_bs_ntrace, 1) & 8191;
+            g_bs_trace[k][0] = n; g_bs_trace[k][1] = nsteps; g_bs_trace[k][2] = -1; g_bs_trace[k][3] = clock64() - tw0;
+        }
+#endif
         if (lane < 8 && writeback) {
             d.x[i] = Y[0]; d.y[i] = Y[1]; d.z[i] = Y[2]; d.vx[i] = Y[3]; d.vy[i] = Y[4]; d.vz[i] = Y[5];
             if (tp) d.label[i] = plabel;
@@ -962,3 +1075,18 @@ __global__ void k_export_labels(DevState d, int *out)
 }
 
 }  // namespace genga
+
+#ifdef GENGA_TRACE
+extern "C" __attribute__((visibility("default"))) int genga_debug_bs_trace(long long *out, int *n, int reset)
+{
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(n, g_bs_ntrace, sizeof(int));
+    cudaMemcpyFromSymbol(out, g_bs_trace, sizeof(long long) * 8192 * 4);
+    if (reset) { int z = 0; cudaMemcpyToSymbol(g_bs_ntrace, &z, sizeof(int)); }
+    cudaMemcpyFromSymbol(out + 8192 * 4 + 1024 * 8, genga::g_bw_prof, sizeof(unsigned long long) * 4);
+    if (reset) { static long long z4[4]; cudaMemcpyToSymbol(genga::g_bw_prof, z4, sizeof z4); }
+    cudaMemcpyFromSymbol(out + 8192 * 4, genga::g_bc_prof, sizeof(long long) * 1024 * 8);
+    if (reset) { static long long zz[1024 * 8]; cudaMemcpyToSymbol(genga::g_bc_prof, zz, sizeof zz); }
+    return 0;
+}
+#endif

@@ -13,7 +13,7 @@ constexpr int KK_MAXN = 2048;     // massive bodies of one system (L188)
 
 // Bulirsch-Stoer layouts: groups of 2..8 bodies on one warp (bs_warp.cuh), of 9..256 bodies on a
 // cluster of 8 CTAs (bs_cluster.cuh), larger ones on one block with a global-memory tableau (bs.cuh)
-constexpr int BCB_MAXN = 256, BCB_THREADS = 256, BCB_CS = 8;
+constexpr int BCB_MAXN = 256, BCB_THREADS = 512, BCB_CS = 8;
 
 __global__ void k_begin_map(DevState d);
 __global__ void k_reset_counters(DevState d);
@@ -21,6 +21,8 @@ __global__ void k_rcrit(DevState d, double tau);
 __global__ void k_kick(DevState d, double h, int record, int ni, double *aout);
 size_t kick_smem_bytes();
 __global__ void k_tp_kick(DevState d, double h, int record, double *aout);
+__global__ void k_tp_front(DevState d, double h, double tau, int first);
+__global__ void k_tp_back(DevState d, double h);
 __global__ void k_kick_multi(DevState d, double h, int record, double *aout);
 __global__ void k_momentum(DevState d, const double *vx, const double *vy, const double *vz);
 __global__ void k_shift(DevState d, double *ax, double *ay, double *az, double f, int divide_by_total);
