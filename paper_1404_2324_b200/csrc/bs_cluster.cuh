@@ -29,8 +29,9 @@ namespace cg = cooperative_groups;
 
 template <int MAXN, int THREADS>
 struct BcSmem {
-    double pos[2][3][MAXN];
-    float pf[2][3][MAXN];           // positions rounded to FP32 for the conservative pretest
+    double pos[2][2][3][MAXN];      // [buffer][point A / B][component][body]
+    float pf[2][2][3][MAXN];        // positions rounded to FP32 for the conservative pretest
+    double isq[MAXN], isv[MAXN];    // 1 / |q|^2, 1 / |V|^2 at the start of the attempted step (error norm)
     float thr2[MAXN];               // (rc_i + margin)^2 rounded up
     double m[MAXN], rc[MAXN], irc[MAXN];
     double Y[6][MAXN];              // state at the start of the attempted step
@@ -66,30 +67,35 @@ __device__ long long g_bc_prof[1024][8];     // per CTA: cycles in rhs, cluster 
 #define BC_T0()
 #define BC_ACC(k)
 #endif
-// Force on body t.i at the positions q of the owners (Eq. 1 L73-74 through Eq. 8; star fixed
-// at the origin, L314; every pair of the group is examined at every evaluation, L505).  The n^2
-// examinations are done first in FP32 against a threshold widened by more than the FP32 rounding,
-// so the test can only err towards "inside"; pairs that pass take the exact FP64 test and weight.
+// Forces on body t.i at TWO sets of positions (qA, qB of the owners) at once (Eq. 1 L73-74 through Eq. 8
+// L104; star fixed at the origin, L314; every pair of the group is examined at every evaluation, L505).
+// Two at once because a(q_k) and a(q_{k+1}) of Gragg's rule are independent (bs_warp.cuh): one barrier and
+// one segment reduction serve both, and their dependent chains overlap.  The n^2 examinations are done
+// first in FP32 against a threshold widened by more than the FP32 rounding, so the test can only err
+// towards "inside"; pairs that pass take the exact FP64 test and weight.
 template <int MAXN, int THREADS>
-__device__ __forceinline__ void bc_rhs(BcSmem<MAXN, THREADS> &S, const BcLane &t, int &buf, double G, double m0,
-                                       const double q[3], double a[3])
+__device__ __forceinline__ void bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t, int &buf, double G, double m0,
+                                        const double qA[3], const double qB[3], double aA[3], double aB[3])
 {
     GENGA_BS_RHS_HOOK();
-    BC_T0();
-    double(*p)[MAXN] = S.pos[buf];
-    float(*pf)[MAXN] = S.pf[buf];
+    double(*pA)[MAXN] = S.pos[buf][0];
+    double(*pB)[MAXN] = S.pos[buf][1];
+    float(*fA)[MAXN] = S.pf[buf][0];
+    float(*fB)[MAXN] = S.pf[buf][1];
     if (t.owner) {
-        p[0][t.i] = q[0]; p[1][t.i] = q[1]; p[2][t.i] = q[2];
-        pf[0][t.i] = (float)q[0]; pf[1][t.i] = (float)q[1]; pf[2][t.i] = (float)q[2];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            pA[c][t.i] = qA[c]; pB[c][t.i] = qB[c];
+            fA[c][t.i] = (float)qA[c]; fB[c][t.i] = (float)qB[c];
+        }
     }
     __syncthreads();
-    BC_ACC(4);
     buf ^= 1;
-    double ax = 0.0, ay = 0.0, az = 0.0;
+    double ax = 0.0, ay = 0.0, az = 0.0, bx = 0.0, by = 0.0, bz = 0.0;
     if (t.i < t.n) {
         const int n = t.n, L = t.L, i = t.i;
-        const float fx = pf[0][i], fy = pf[1][i], fz = pf[2][i], ft = S.thr2[i];
-        const double qx = p[0][i], qy = p[1][i], qz = p[2][i];
+        const float fxA = fA[0][i], fyA = fA[1][i], fzA = fA[2][i], fxB = fB[0][i], fyB = fB[1][i], fzB = fB[2][i], ft = S.thr2[i];
+        const double xA = pA[0][i], yA = pA[1][i], zA = pA[2][i], xB = pB[0][i], yB = pB[1][i], zB = pB[2][i];
         const double my_rc = S.rc[i], my_irc = S.irc[i];
         for (int j0 = t.s; j0 <= n; j0 += 32 * L) {              // partner j = n is the star
             unsigned mask = 0u;
@@ -98,40 +104,45 @@ __device__ __forceinline__ void bc_rhs(BcSmem<MAXN, THREADS> &S, const BcLane &t
                 int j = j0 + kk * L;
                 if (j > n) break;
                 int jc = j < n ? j : i;                           // star / self: computed, not used
-                float dx = pf[0][jc] - fx, dy = pf[1][jc] - fy, dz = pf[2][jc] - fz;
-                float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                float dx = fA[0][jc] - fxA, dy = fA[1][jc] - fyA, dz = fA[2][jc] - fzA;
+                float ex = fB[0][jc] - fxB, ey = fB[1][jc] - fyB, ez = fB[2][jc] - fzB;
+                float d2 = fminf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), fmaf(ez, ez, fmaf(ey, ey, ex * ex)));
                 bool in = (d2 < fmaxf(ft, S.thr2[jc]) && j != i) || j == n;
                 mask |= (in ? 1u : 0u) << kk;
             }
-            BC_ACC(5);
             while (mask) {
                 int j = j0 + (__ffs(mask) - 1) * L;
                 mask &= mask - 1;
                 if (j == n) {
-                    double r2 = qx * qx + qy * qy + qz * qz;
-                    double s0 = -G * m0 * rinv3_fast(r2);
-                    ax += s0 * qx; ay += s0 * qy; az += s0 * qz;
+                    double rA = xA * xA + yA * yA + zA * zA, rB = xB * xB + yB * yB + zB * zB;
+                    double sA = -G * m0 * rinv3_fast(rA), sB = -G * m0 * rinv3_fast(rB);
+                    ax += sA * xA; ay += sA * yA; az += sA * zA;
+                    bx += sB * xB; by += sB * yB; bz += sB * zB;
                 } else {
                     double rcj = S.rc[j];
-                    double rcij = fmax(my_rc, rcj);
-                    double dx = p[0][j] - qx, dy = p[1][j] - qy, dz = p[2][j] - qz;
-                    double d2 = dx * dx + dy * dy + dz * dz;
-                    if (d2 < rcij * rcij) {
-                        double sc = direct_scale(d2, rcij, my_rc >= rcj ? my_irc : S.irc[j], G * S.m[j]);
-                        ax += sc * dx; ay += sc * dy; az += sc * dz;
+                    double rcij = fmax(my_rc, rcj), rc2 = rcij * rcij;
+                    double dx = pA[0][j] - xA, dy = pA[1][j] - yA, dz = pA[2][j] - zA;
+                    double ex = pB[0][j] - xB, ey = pB[1][j] - yB, ez = pB[2][j] - zB;
+                    double dA = dx * dx + dy * dy + dz * dz, dB = ex * ex + ey * ey + ez * ez;
+                    const bool inA = dA < rc2, inB = dB < rc2;
+                    if (inA || inB) {
+                        const double ir = my_rc >= rcj ? my_irc : S.irc[j], gmj = G * S.m[j];
+                        double scA = direct_scale(inA ? dA : rc2, rcij, ir, gmj);
+                        double scB = direct_scale(inB ? dB : rc2, rcij, ir, gmj);
+                        scA = inA ? scA : 0.0; scB = inB ? scB : 0.0;
+                        ax += scA * dx; ay += scA * dy; az += scA * dz;
+                        bx += scB * ex; by += scB * ey; bz += scB * ez;
                     }
                 }
             }
         }
     }
-    BC_ACC(6);
     for (int o = t.L >> 1; o > 0; o >>= 1) {
-        ax += __shfl_xor_sync(0xffffffffu, ax, o);
-        ay += __shfl_xor_sync(0xffffffffu, ay, o);
-        az += __shfl_xor_sync(0xffffffffu, az, o);
+        ax += __shfl_xor_sync(0xffffffffu, ax, o); ay += __shfl_xor_sync(0xffffffffu, ay, o); az += __shfl_xor_sync(0xffffffffu, az, o);
+        bx += __shfl_xor_sync(0xffffffffu, bx, o); by += __shfl_xor_sync(0xffffffffu, by, o); bz += __shfl_xor_sync(0xffffffffu, bz, o);
     }
-    a[0] = ax; a[1] = ay; a[2] = az;
-    BC_ACC(7);
+    aA[0] = ax; aA[1] = ay; aA[2] = az;
+    aB[0] = bx; aB[1] = by; aB[2] = bz;
 }
 
 template <int MAXN, int THREADS>
@@ -182,7 +193,7 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
         }
         __syncthreads();
     }
-    double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0}, isq = 0.0, isv = 0.0, acc0[3] = {0.0, 0.0, 0.0};
+    double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0}, acc0[3] = {0.0, 0.0, 0.0};
     while (!last) {
         double rem = h - done;
         if (fabs(H) >= fabs(rem)) { H = rem; last = true; }
@@ -190,10 +201,13 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
             if (t.owner) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) { q[c] = S.Y[c][i]; V[c] = S.Y[3 + c][i]; }
-                isq = 1.0 / (q[0] * q[0] + q[1] * q[1] + q[2] * q[2]);
-                isv = 1.0 / (V[0] * V[0] + V[1] * V[1] + V[2] * V[2]);
+                if (rank == 0) {
+                    S.isq[i] = 1.0 / (q[0] * q[0] + q[1] * q[1] + q[2] * q[2]);
+                    S.isv[i] = 1.0 / (V[0] * V[0] + V[1] * V[1] + V[2] * V[2]);
+                }
             }
-            bc_rhs(S, t, buf, G, m0, q, acc0);
+            double dummy[3];
+            bc_rhs2(S, t, buf, G, m0, q, q, acc0, dummy);
             fresh = false;
         }
         BC_T0();
@@ -203,28 +217,28 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
             const int col = (pass & 1) ? pass * CS + CS - 1 - rank : pass * CS + rank;
             const int nk = 2 * (col + 1);
             const double eta = H / nk;
-            double qa[3], Va[3], qb[3], Vb[3], acc[3];
+            double qa[3], Va[3], qb[3], Vb[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 qa[c] = q[c]; Va[c] = V[c];
                 qb[c] = q[c] + eta * V[c]; Vb[c] = V[c] + eta * acc0[c];
             }
+            // two substeps per iteration (bc_rhs2): q_{k+1} = q_{k-1} + 2 eta V_k does not need a(q_k)
 #pragma unroll 1
-            for (int ms = 1; ms < nk; ++ms) {
-                bc_rhs(S, t, buf, G, m0, qb, acc);
+            for (int it = 0; it <= col; ++it) {
+                double qc[3], A[3], C[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) qc[c] = qa[c] + 2.0 * eta * Vb[c];
+                bc_rhs2(S, t, buf, G, m0, qb, qc, A, C);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    double qn = qa[c] + 2.0 * eta * Vb[c];
-                    double vn = Va[c] + 2.0 * eta * acc[c];
-                    qa[c] = qb[c]; Va[c] = Vb[c]; qb[c] = qn; Vb[c] = vn;
-                }
-            }
-            bc_rhs(S, t, buf, G, m0, qb, acc);
-            if (t.owner) {
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    S0->tab[col][c][i] = 0.5 * (qb[c] + qa[c] + eta * Vb[c]);
-                    S0->tab[col][3 + c][i] = 0.5 * (Vb[c] + Va[c] + eta * acc[c]);
+                    double vc = Va[c] + 2.0 * eta * A[c];
+                    if (it == col && t.owner) {
+                        S0->tab[col][c][i] = 0.5 * (qc[c] + qb[c] + eta * vc);
+                        S0->tab[col][3 + c][i] = 0.5 * (vc + Vb[c] + eta * C[c]);
+                    }
+                    double qd = qb[c] + 2.0 * eta * vc, vd = Vb[c] + 2.0 * eta * C[c];
+                    qa[c] = qc[c]; Va[c] = vc; qb[c] = qd; Vb[c] = vd;
                 }
             }
         }
@@ -236,16 +250,17 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
             double e[BS_KMAX];
 #pragma unroll
             for (int k = 0; k < BS_KMAX; ++k) e[k] = 0.0;
-            if (t.owner) {
-                double dq2[BS_KMAX], dv2[BS_KMAX];
+            // eight lanes per body, six of them take one component each
+            for (int i8 = threadIdx.x >> 3; i8 < ((t.n + 3) & ~3); i8 += THREADS / 8) {
+                const int c = threadIdx.x & 7;
+                double d2[BS_KMAX];
 #pragma unroll
-                for (int k = 0; k < BS_KMAX; ++k) { dq2[k] = 0.0; dv2[k] = 0.0; }
-#pragma unroll
-                for (int c = 0; c < 6; ++c) {
+                for (int k = 0; k < BS_KMAX; ++k) d2[k] = 0.0;
+                if (c < 6 && i8 < t.n) {
                     double row[BS_KMAX] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
 #pragma unroll
                     for (int k = 0; k < BS_KMAX; ++k) {
-                        double cur = S.tab[k][c][i], prev = row[0], diff = 0.0;
+                        double cur = S.tab[k][c][i8], prev = row[0], diff = 0.0;
                         row[0] = cur;
 #pragma unroll
                         for (int j = 1; j <= k; ++j) {
@@ -258,12 +273,18 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
                             row[j] = cur;
                             prev = tmp;
                         }
-                        S.tab[k][c][i] = cur;                       // T[k][k]
-                        if (c < 3) dq2[k] += diff * diff; else dv2[k] += diff * diff;
+                        S.tab[k][c][i8] = cur;                      // T[k][k]
+                        d2[k] = diff * diff;
                     }
                 }
+                const int base = (threadIdx.x & 31) & ~7;
+                const double isq = i8 < t.n ? S.isq[i8] : 0.0, isv = i8 < t.n ? S.isv[i8] : 0.0;
 #pragma unroll
-                for (int k = 1; k < BS_KMAX; ++k) e[k] = fmax(dq2[k] * isq, dv2[k] * isv);
+                for (int k = 1; k < BS_KMAX; ++k) {
+                    double dq = __shfl_sync(0xffffffffu, d2[k], base) + __shfl_sync(0xffffffffu, d2[k], base + 1) + __shfl_sync(0xffffffffu, d2[k], base + 2);
+                    double dv = __shfl_sync(0xffffffffu, d2[k], base + 3) + __shfl_sync(0xffffffffu, d2[k], base + 4) + __shfl_sync(0xffffffffu, d2[k], base + 5);
+                    e[k] = fmax(e[k], fmax(dq * isq, dv * isv));
+                }
             }
 #pragma unroll
             for (int k = 1; k < BS_KMAX; ++k)
