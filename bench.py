@@ -220,25 +220,51 @@ def run_gpu(args):
     # ---- dominant kernel in isolation (CUDA events inside the library, on its stream)
     g.set_state(w["m0"], w["m"], w["radius"], w["x"], w["v"])
     roof = None
-    if w["mode"] != 2:
+    peak_probe = g.fp64_probe()
+    hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs") if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs (measured copy bandwidth)" if hbm_peak else "fallback of B200_PROFILING.md"
+    hbm_peak = hbm_peak or 6650.0
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    traffic_tab = json.load(open(tpath)) if os.path.exists(tpath) else {}
+    if w["mode"] == 0:
         kick_ms = g.time_kernel(0, 200, dt)
-        peak_probe = g.fp64_probe()
         inter = w["n_massive"] * (w["n_massive"] - 1)
         achieved = FLOP_PER_INTERACTION * inter / (kick_ms * 1e-3) / 1e12
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "kick_pairs_traffic.json")
-        if os.path.exists(tpath):
-            traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
-        roof = {"bound": "alu", "kernel": "k_kick_pairs", "achieved": achieved, "peak": peak_probe,
-                "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": traffic,
+        roof = {"bound": "alu", "kernel": "k_kick", "achieved": achieved, "peak": peak_probe,
+                "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": traffic_tab.get("k_kick"),
                 "peak_source": "DFMA probe measured in this run (genga_fp64_probe); nominal %.1f = 148 SM x 64 DFMA/clk x 2 x 1.965 GHz" % FP64_NOMINAL_TFLOPS,
                 "ms_per_launch": kick_ms, "interactions_per_launch": inter,
                 "interactions_per_s": inter / (kick_ms * 1e-3),
-                "flop_per_interaction": FLOP_PER_INTERACTION}
+                "flop_per_interaction": FLOP_PER_INTERACTION,
+                # the kernel issues 16 FP64 instructions per interaction: share of the DFMA issue rate
+                "fp64_issue_frac": 16.0 * 2.0 * inter / (kick_ms * 1e-3) / 1e12 / peak_probe}
         drift_ms = g.time_kernel(1, 200, dt)
         roof["drift"] = {"kernel": "k_drift", "ms_per_launch": drift_ms, "bodies": g.ntot,
                          "algorithmic_bytes": 144 * g.ntot,
-                         "gbs": 144 * g.ntot / (drift_ms * 1e-3) / 1e9}
+                         "gbs": 144 * g.ntot / (drift_ms * 1e-3) / 1e9,
+                         "note": "launch-latency bound at N = 2048 (295 KB)"}
+    elif w["mode"] == 1:
+        # dominant kernels: the fused particle passes; algorithmic bytes per particle: 48 read + 48 written + 8 (rc)
+        nt = w["n_test"]
+        front_ms = g.time_kernel(3, 100, dt)
+        back_ms = g.time_kernel(4, 100, dt)
+        fb = 104.0 * nt
+        roof = {"bound": "hbm", "kernel": "k_tp_back", "achieved": fb / (back_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "frac": fb / (back_ms * 1e-3) / 1e9 / hbm_peak, "traffic": traffic_tab.get("k_tp_back"),
+                "peak_source": hbm_src, "ms_per_launch": back_ms, "algorithmic_bytes_per_launch": fb,
+                "front": {"kernel": "k_tp_front", "ms_per_launch": front_ms, "algorithmic_bytes_per_launch": fb,
+                          "gbs": fb / (front_ms * 1e-3) / 1e9, "frac_hbm": fb / (front_ms * 1e-3) / 1e9 / hbm_peak,
+                          "traffic": traffic_tab.get("k_tp_front"),
+                          "note": "kick by %d massive bodies + Kepler solve: ~510 FP64 issue slots per particle, FP64-bound (DESIGN.md section 6)" % w["n_massive"],
+                          "fp64_peak_tflops": peak_probe}}
+    else:
+        kick_ms = g.time_kernel(2, 200, dt)
+        inter = w["n_systems"] * w["n_massive"] * (w["n_massive"] - 1)
+        achieved = FLOP_PER_INTERACTION * inter / (kick_ms * 1e-3) / 1e12
+        roof = {"bound": "alu", "kernel": "k_kick_multi", "achieved": achieved, "peak": peak_probe, "unit": "TFLOP/s",
+                "frac": achieved / peak_probe, "traffic": traffic_tab.get("k_kick_multi"), "ms_per_launch": kick_ms,
+                "interactions_per_launch": inter, "flop_per_interaction": FLOP_PER_INTERACTION,
+                "peak_source": "DFMA probe measured in this run (genga_fp64_probe)"}
 
     # ---- aggregate over ranks (replicas: no data-path collective)
     tmax, units = reduce_max_and_sum(elapsed, per_step * args.steps, dev)

@@ -138,10 +138,13 @@ int genga_counters(genga_ctx *ctx, int64_t *out);
 
 /* Time one kernel of the path in isolation on the context's stream with CUDA events:
  * `reps` back-to-back launches after 3 warm-up launches, *ms_per_launch = average (HOST out).
- *   which = 0  pair kernel of the kick (k_kick_pairs; modes 0, 1), current state and rcrit
+ *   which = 0  pair kernel of the kick (k_kick; modes 0, 1), current state and rcrit
  *   which = 1  Kepler drift of all bodies over dt and back (two launches counted as two)
- *   which = 2  the whole kick (pair kernel + slice reduction [+ test-particle kick]), h = 0
- * The state is left unchanged up to rounding.  Synchronises. */
+ *   which = 2  the whole kick (k_kick [+ k_tp_kick of the test particles]), h = 0
+ *   which = 3  mode 1: fused particle pass kick + Sun kick + drift (k_tp_front) over dt and back
+ *   which = 4  mode 1: fused particle pass Sun kick + kick (k_tp_back) over dt and back
+ * The state is left unchanged up to rounding (3, 4: up to the integration error of the
+ * pass and its inverse).  Synchronises. */
 int genga_time_kernel(genga_ctx *ctx, int which, int reps, double dt, double *ms_per_launch);
 
 /* Measure the device's FP64 FMA throughput with independent DFMA chains on every SM:

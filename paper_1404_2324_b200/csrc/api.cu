@@ -525,9 +525,10 @@ extern "C" __attribute__((visibility("default"))) int genga_kepler_drift(genga_c
 
 extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ctx *c, int which, int reps, double dt, double *ms)
 {
-    if (!c || !ms || reps < 1 || dt == 0.0 || which < 0 || which > 2) return GENGA_EINVAL;
+    if (!c || !ms || reps < 1 || dt == 0.0 || which < 0 || which > 4) return GENGA_EINVAL;
     DevState &d = c->d;
     if (d.mode == GENGA_MODE_MULTI_SYSTEM && which == 0) return GENGA_EINVAL;
+    if (which >= 3 && !(d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm)) return GENGA_EINVAL;
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
     k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt);
@@ -540,14 +541,23 @@ extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ct
             k_drift<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt);
             k_drift<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, -dt);
             c->launches += 2; per = 2;
-        } else { c->acc = 0; enqueue_kick(c, 0.0, 0, nullptr); per = (int)c->acc; c->launches += c->acc; c->acc = 0; }
+        } else if (which == 2) { c->acc = 0; enqueue_kick(c, 0.0, 0, nullptr); per = (int)c->acc; c->launches += c->acc; c->acc = 0; }
+        else if (which == 3) {                       // fused particle pass, forwards then backwards
+            k_tp_front<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, dt, dt, 1);
+            k_tp_front<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, -dt, dt, 0);
+            c->launches += 2; per = 2;
+        } else {
+            k_tp_back<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, dt);
+            k_tp_back<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, -dt);
+            c->launches += 2; per = 2;
+        }
     }
     CK(cudaEventRecord(e1, c->st));
     CK(cudaEventSynchronize(e1));
     float t = 0.f;
     CK(cudaEventElapsedTime(&t, e0, e1));
     cudaEventDestroy(e0); cudaEventDestroy(e1);
-    *ms = (double)t / reps / (which == 1 ? per : 1);
+    *ms = (double)t / reps / (which == 1 || which >= 3 ? per : 1);
     CK(cudaGetLastError());
     return GENGA_OK;
 }

@@ -59,14 +59,6 @@ __device__ __forceinline__ BcLane bc_lanes(int n)
     return t;
 }
 
-#ifdef GENGA_TRACE
-__device__ long long g_bc_prof[1024][8];     // per CTA: cycles in rhs, cluster syncs, tableau, attempts
-#define BC_T0() long long tq_ = clock64()
-#define BC_ACC(k) do { long long tn_ = clock64(); if (threadIdx.x == 0) g_bc_prof[blockIdx.x][k] += tn_ - tq_; tq_ = tn_; } while (0)
-#else
-#define BC_T0()
-#define BC_ACC(k)
-#endif
 // Forces on body t.i at TWO sets of positions (qA, qB of the owners) at once (Eq. 1 L73-74 through Eq. 8
 // L104; star fixed at the origin, L314; every pair of the group is examined at every evaluation, L505).
 // Two at once because a(q_k) and a(q_{k+1}) of Gragg's rule are independent (bs_warp.cuh): one barrier and
@@ -210,7 +202,6 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
             bc_rhs2(S, t, buf, G, m0, q, q, acc0, dummy);
             fresh = false;
         }
-        BC_T0();
         // ---- my columns: Gragg's modified midpoint rule with nk substeps
 #pragma unroll 1
         for (int pass = 0; pass < BS_KMAX / CS; ++pass) {
@@ -242,9 +233,7 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
                 }
             }
         }
-        BC_ACC(0);
         bc_sync<CS>();
-        BC_ACC(1);
         // ---- CTA 0: Aitken-Neville tableau in (H/n_k)^2, first row whose error passes
         if (rank == 0) {
             double e[BS_KMAX];
@@ -308,12 +297,7 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
             }
             if (threadIdx.x == 0) S.kstar = kstar;
         }
-        BC_ACC(2);
         bc_sync<CS>();
-        BC_ACC(1);
-#ifdef GENGA_TRACE
-        if (threadIdx.x == 0) g_bc_prof[blockIdx.x][3] += 1;
-#endif
         const int kstar = S0->kstar;
         if (kstar >= 0) {
             if (CS > 1 && rank != 0) {

@@ -114,9 +114,6 @@ __device__ __forceinline__ void bw_neville(BwSmem &W, int c, int b, double (&d2)
     }
 }
 
-#ifdef GENGA_TRACE
-__device__ unsigned long long g_bw_prof[4];
-#endif
 // Integrate one group over h.  Lane = S * g + b; Y = state of body b (same in every segment; any
 // finite dummy for b >= n).  On return Y holds the result.  Returns false on step-size underflow
 // (uniform over the warp).
@@ -168,9 +165,6 @@ __device__ __forceinline__ bool bw_integrate(BwSmem &W, const int lane, const in
         }
         // ---- my column(s): Gragg's modified midpoint rule, two substeps per iteration, all lanes in step.
         // Column col (n_k = 2 (col + 1) substeps) ends in its iteration number col.
-#ifdef GENGA_TRACE
-        long long tp0 = clock64();
-#endif
         int col = cg, left = col + 1, pass = 0;
         double eta = H / (2 * (col + 1));
         double qa[3], Va[3], qb[3], Vb[3];
@@ -210,9 +204,6 @@ __device__ __forceinline__ bool bw_integrate(BwSmem &W, const int lane, const in
             }
         }
         __syncwarp();
-#ifdef GENGA_TRACE
-        long long tp1 = clock64();
-#endif
         // ---- Aitken-Neville tableau in (H/n_k)^2, one (component, body) entry per lane; first row whose error passes
         double d2[NROUND][BS_KMAX];
 #pragma unroll
@@ -240,9 +231,6 @@ __device__ __forceinline__ bool bw_integrate(BwSmem &W, const int lane, const in
         }
         kstar = __shfl_sync(full, kstar, 0);
         __syncwarp();
-#ifdef GENGA_TRACE
-        if (lane == 0 && S == 2) { atomicAdd(&g_bw_prof[0], (unsigned long long)(tp1 - tp0)); atomicAdd(&g_bw_prof[1], (unsigned long long)(clock64() - tp1)); atomicAdd(&g_bw_prof[2], 1ull); }
-#endif
         if (kstar >= 0) {
             if (body) {
 #pragma unroll

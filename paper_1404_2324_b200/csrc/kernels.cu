@@ -1,12 +1,5 @@
 // Kernels of the hybrid symplectic step, sm_100a.
 // Each kernel states the operator it implements and the passage that defines it.
-#ifdef GENGA_TRACE
-#include <cuda_runtime.h>
-__device__ int g_rhs[1024];
-__device__ long long g_bs_trace[8192][4];
-__device__ int g_bs_ntrace;
-
-#endif
 #include "kernels.cuh"
 #include "bs_cluster.cuh"
 #include "bs_warp.cuh"
@@ -178,36 +171,23 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
                 const KickBody bj = *pb;
                 const int hcj = *ph;
                 pb += P; ph += P;
-                {
-                    double dx = bj.x - xi0, dy = bj.y - yi0, dz = bj.z - zi0;
-                    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                    bool hit = __double2hiint(r2) <= max(hci0, hcj);
-                    int yh = __double2hiint(rsqrt_seed(r2));
-                    double y0 = __hiloint2double(hit ? 0 : yh, 0);  // weight 0 for hits (and r2 == 0: the body itself)
-                    double u = y0 * y0;
-                    double e = fma(-r2, u, 1.0);
-                    double w = y0 * u;
-                    double p = fma(1.875, e, 1.5);
-                    double s3 = bj.gm * fma(p * e, w, w);           // G m_j y0^3 (1 + 3e/2 + 15 e^2/8)
-                    ax0 = fma(s3, dx, ax0); ay0 = fma(s3, dy, ay0); az0 = fma(s3, dz, az0);
-                    unsigned hm = __ballot_sync(0xffffffffu, hit);
-                    if (lane0) pw[0] = hm;
-                }
-                {
-                    double dx = bj.x - xi1, dy = bj.y - yi1, dz = bj.z - zi1;
-                    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                    bool hit = __double2hiint(r2) <= max(hci1, hcj);
-                    int yh = __double2hiint(rsqrt_seed(r2));
-                    double y0 = __hiloint2double(hit ? 0 : yh, 0);
-                    double u = y0 * y0;
-                    double e = fma(-r2, u, 1.0);
-                    double w = y0 * u;
-                    double p = fma(1.875, e, 1.5);
-                    double s3 = bj.gm * fma(p * e, w, w);
-                    ax1 = fma(s3, dx, ax1); ay1 = fma(s3, dy, ay1); az1 = fma(s3, dz, az1);
-                    unsigned hm = __ballot_sync(0xffffffffu, hit);
-                    if (lane0) pw[1] = hm;
-                }
+                // both pairs' arithmetic first, the two ballots after it: a ballot is a scheduling barrier
+                const double dx0 = bj.x - xi0, dy0 = bj.y - yi0, dz0 = bj.z - zi0;
+                const double dx1 = bj.x - xi1, dy1 = bj.y - yi1, dz1 = bj.z - zi1;
+                const double r20 = fma(dz0, dz0, fma(dy0, dy0, dx0 * dx0)), r21 = fma(dz1, dz1, fma(dy1, dy1, dx1 * dx1));
+                const bool hit0 = __double2hiint(r20) <= max(hci0, hcj), hit1 = __double2hiint(r21) <= max(hci1, hcj);
+                const int yh0 = __double2hiint(rsqrt_seed(r20)), yh1 = __double2hiint(rsqrt_seed(r21));
+                // weight 0 for hits (and r2 == 0: the body itself): clear the seed
+                const double y00 = __hiloint2double(hit0 ? 0 : yh0, 0), y01 = __hiloint2double(hit1 ? 0 : yh1, 0);
+                const double u0 = y00 * y00, u1 = y01 * y01;
+                const double e0 = fma(-r20, u0, 1.0), e1 = fma(-r21, u1, 1.0);
+                const double w0 = y00 * u0, w1 = y01 * u1;
+                const double p0 = fma(1.875, e0, 1.5), p1 = fma(1.875, e1, 1.5);
+                const double s30 = bj.gm * fma(p0 * e0, w0, w0), s31 = bj.gm * fma(p1 * e1, w1, w1);   // G m_j y0^3 (1 + 3e/2 + 15 e^2/8)
+                ax0 = fma(s30, dx0, ax0); ay0 = fma(s30, dy0, ay0); az0 = fma(s30, dz0, az0);
+                ax1 = fma(s31, dx1, ax1); ay1 = fma(s31, dy1, ay1); az1 = fma(s31, dz1, az1);
+                const unsigned hm0 = __ballot_sync(0xffffffffu, hit0), hm1 = __ballot_sync(0xffffffffu, hit1);
+                if (lane0) { pw[0] = hm0; pw[1] = hm1; }
                 pw += 2;
             }
         }
@@ -725,16 +705,7 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
             S.m[b] = d.m[i]; S.rc[b] = rc; S.irc[b] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
         }
         int nsteps = 0;
-#ifdef GENGA_TRACE
-        long long tc0 = clock64(); int r0 = g_rhs[blockIdx.x];
-#endif
         bool ok = bc_integrate<MAXN, THREADS, CS>(S, S0, rank, t, d.G, d.m0[0], h, d.eps, &nsteps);
-#ifdef GENGA_TRACE
-        if (rank == 0 && threadIdx.x == 0) {
-            int k = atomicAdd(&g_bs_ntrace, 1) & 8191;
-            g_bs_trace[k][0] = n; g_bs_trace[k][1] = nsteps; g_bs_trace[k][2] = g_rhs[blockIdx.x] - r0; g_bs_trace[k][3] = clock64() - tc0;
-        }
-#endif
         if (rank == 0) {
             __syncthreads();
             for (int b = threadIdx.x; b < n; b += THREADS) {
@@ -810,9 +781,6 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
         const double Gm0 = d.G * d.m0[sys];
         int nsteps = 0;
         bool ok;
-#ifdef GENGA_TRACE
-        long long tw0 = clock64();
-#endif
         if (n <= 4) {
             // segments of 2 or 4 lanes: slot b = lane % S takes body b from lane b of the 8-slot layout
             const int src = n == 2 ? (lane & 1) : (lane & 3);
@@ -824,12 +792,6 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
         } else {
             ok = bw_integrate<8>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, &nsteps);
         }
-#ifdef GENGA_TRACE
-        if (lane == 0) {
-            int k = atomicAdd(&g_bs_ntrace, 1) & 8191;
-            g_bs_trace[k][0] = n; g_bs_trace[k][1] = nsteps; g_bs_trace[k][2] = -1; g_bs_trace[k][3] = clock64() - tw0;
-        }
-#endif
         if (lane < 8 && writeback) {
             d.x[i] = Y[0]; d.y[i] = Y[1]; d.z[i] = Y[2]; d.vx[i] = Y[3]; d.vy[i] = Y[4]; d.vz[i] = Y[5];
             if (tp) d.label[i] = plabel;
@@ -1076,17 +1038,3 @@ __global__ void k_export_labels(DevState d, int *out)
 
 }  // namespace genga
 
-#ifdef GENGA_TRACE
-extern "C" __attribute__((visibility("default"))) int genga_debug_bs_trace(long long *out, int *n, int reset)
-{
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(n, g_bs_ntrace, sizeof(int));
-    cudaMemcpyFromSymbol(out, g_bs_trace, sizeof(long long) * 8192 * 4);
-    if (reset) { int z = 0; cudaMemcpyToSymbol(g_bs_ntrace, &z, sizeof(int)); }
-    cudaMemcpyFromSymbol(out + 8192 * 4 + 1024 * 8, genga::g_bw_prof, sizeof(unsigned long long) * 4);
-    if (reset) { static long long z4[4]; cudaMemcpyToSymbol(genga::g_bw_prof, z4, sizeof z4); }
-    cudaMemcpyFromSymbol(out + 8192 * 4, genga::g_bc_prof, sizeof(long long) * 1024 * 8);
-    if (reset) { static long long zz[1024 * 8]; cudaMemcpyToSymbol(genga::g_bc_prof, zz, sizeof zz); }
-    return 0;
-}
-#endif
