@@ -151,12 +151,16 @@ static __device__ __noinline__ bool kepler_solve_slow(double mu, double h, doubl
 __device__ __forceinline__ bool kepler_drift(double mu, double h, double &x, double &y, double &z,
                                              double &vx, double &vy, double &vz)
 {
-    double r0 = sqrt(x * x + y * y + z * z);
+    // reciprocals by rcp_fast / rsqrt_fast (0.5 / 1.25 ulp, above): an IEEE divide or square root costs
+    // 14-20 FP64 issue slots and the particle pass is bound by them
+    double r02 = x * x + y * y + z * z;
+    double ir0 = rsqrt_fast(r02);
+    double r0 = r02 * ir0;
     double v2 = vx * vx + vy * vy + vz * vz;
     double u = x * vx + y * vy + z * vz;
-    double alpha = 2.0 * mu / r0 - v2;
+    double alpha = 2.0 * mu * ir0 - v2;
     double k3 = mu - alpha * r0;
-    double s = h / r0;
+    double s = h * ir0;
     double c0, c1, c2, c3, r;
     bool ok = false;
 #pragma unroll 1
@@ -167,9 +171,9 @@ __device__ __forceinline__ bool kepler_drift(double mu, double h, double &x, dou
         r = r0 * c0 + u * sc1 + mu * s2c2;                    // F'
         double F2 = k3 * sc1 + u * c0;                        // F''
         double F3 = k3 * c0 - alpha * u * sc1;                // F'''
-        double d = -F / r;
-        d = -F / (r + 0.5 * d * F2);
-        d = -F / (r + 0.5 * d * F2 + d * d * F3 * (1.0 / 6.0));
+        double d = -F * rcp_fast(r);
+        d = -F * rcp_fast(r + 0.5 * d * F2);
+        d = -F * rcp_fast(r + 0.5 * d * F2 + d * d * F3 * (1.0 / 6.0));
         if (fabs(d) <= 1e-14 * fabs(s)) { ok = true; break; }
         s += d;
     }
@@ -178,11 +182,12 @@ __device__ __forceinline__ bool kepler_drift(double mu, double h, double &x, dou
         stumpff(alpha * s * s, c0, c1, c2, c3);
         r = r0 * c0 + u * s * c1 + mu * s * s * c2;
     }
+    double ir = rcp_fast(r);
     double ms2c2 = mu * s * s * c2;
-    double f = 1.0 - ms2c2 / r0;
+    double f = 1.0 - ms2c2 * ir0;
     double g = h - mu * s * s * s * c3;
-    double fd = -mu * s * c1 / (r * r0);
-    double gd = 1.0 - ms2c2 / r;
+    double fd = -mu * s * c1 * (ir * ir0);
+    double gd = 1.0 - ms2c2 * ir;
     double nx = f * x + g * vx, ny = f * y + g * vy, nz = f * z + g * vz;
     double nvx = fd * x + gd * vx, nvy = fd * y + gd * vy, nvz = fd * z + gd * vz;
     x = nx; y = ny; z = nz; vx = nvx; vy = nvy; vz = nvz;
