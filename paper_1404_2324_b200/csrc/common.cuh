@@ -161,33 +161,47 @@ __device__ __forceinline__ bool kepler_drift(double mu, double h, double &x, dou
     double alpha = 2.0 * mu * ir0 - v2;
     double k3 = mu - alpha * r0;
     double s = h * ir0;
-    double c0, c1, c2, c3, r;
+    double G0, G1, G2, G3, r;                                 // G_k = s^k c_k(alpha s^2)
     bool ok = false;
 #pragma unroll 1
     for (int it = 0; it < KEPLER_MAXIT; ++it) {
-        stumpff(alpha * s * s, c0, c1, c2, c3);
-        double sc1 = s * c1, s2c2 = s * s * c2;
-        double F = r0 * sc1 + u * s2c2 + mu * s * s * s * c3 - h;
-        r = r0 * c0 + u * sc1 + mu * s2c2;                    // F'
-        double F2 = k3 * sc1 + u * c0;                        // F''
-        double F3 = k3 * c0 - alpha * u * sc1;                // F'''
+        double c1, c2, c3;
+        stumpff(alpha * s * s, G0, c1, c2, c3);
+        G1 = s * c1; G2 = s * s * c2; G3 = s * s * s * c3;
+        double F = r0 * G1 + u * G2 + mu * G3 - h;
+        r = r0 * G0 + u * G1 + mu * G2;                       // dF/ds
+        double F2 = k3 * G1 + u * G0;                         // second derivative
+        double F3 = k3 * G0 - alpha * u * G1;                 // third derivative
         double d = -F * rcp_fast(r);
         d = -F * rcp_fast(r + 0.5 * d * F2);
         d = -F * rcp_fast(r + 0.5 * d * F2 + d * d * F3 * (1.0 / 6.0));
-        if (fabs(d) <= 1e-14 * fabs(s)) { ok = true; break; }
+        if (fabs(d) <= 1e-6 * fabs(s) && fabs(F) <= 1e-5 * fabs(h)) {   // in the basin: quartic convergence
+            // the last correction: carried into the G functions by their Taylor series (dG0 = -alpha G1,
+            // dG1 = G0, dG2 = G1, dG3 = G2), truncation O(d^3) < 1e-18 relative: saves the confirming pass
+            const double hd2 = 0.5 * d * d;
+            const double n0 = G0 - alpha * (G1 * d + G0 * hd2);
+            const double n1 = G1 + G0 * d - alpha * G1 * hd2;
+            const double n2 = G2 + G1 * d + G0 * hd2;
+            const double n3 = G3 + G2 * d + G1 * hd2;
+            G0 = n0; G1 = n1; G2 = n2; G3 = n3;
+            r = r0 * G0 + u * G1 + mu * G2;
+            ok = true;
+            break;
+        }
         s += d;
     }
     if (!ok) {
         if (!kepler_solve_slow(mu, h, r0, u, alpha, s)) return false;
-        stumpff(alpha * s * s, c0, c1, c2, c3);
-        r = r0 * c0 + u * s * c1 + mu * s * s * c2;
+        double c1, c2, c3;
+        stumpff(alpha * s * s, G0, c1, c2, c3);
+        G1 = s * c1; G2 = s * s * c2; G3 = s * s * s * c3;
+        r = r0 * G0 + u * G1 + mu * G2;
     }
     double ir = rcp_fast(r);
-    double ms2c2 = mu * s * s * c2;
-    double f = 1.0 - ms2c2 * ir0;
-    double g = h - mu * s * s * s * c3;
-    double fd = -mu * s * c1 * (ir * ir0);
-    double gd = 1.0 - ms2c2 * ir;
+    double f = 1.0 - mu * G2 * ir0;
+    double g = h - mu * G3;
+    double fd = -mu * G1 * (ir * ir0);
+    double gd = 1.0 - mu * G2 * ir;
     double nx = f * x + g * vx, ny = f * y + g * vy, nz = f * z + g * vz;
     double nvx = fd * x + gd * vx, nvy = fd * y + gd * vy, nvz = fd * z + gd * vz;
     x = nx; y = ny; z = nz; vx = nvx; vy = nvy; vz = nvz;
