@@ -30,7 +30,7 @@ namespace cg = cooperative_groups;
 template <int MAXN, int THREADS>
 struct BcSmem {
     double pos[2][2][3][MAXN];      // [buffer][point A / B][component][body]
-    float pf[2][2][3][MAXN];        // positions rounded to FP32 for the conservative pretest
+    float4 pf[2][2][MAXN];          // positions rounded to FP32 for the conservative pretest, .w = thr2: one LDS.128 per partner
     double isq[MAXN], isv[MAXN];    // 1 / |q|^2, 1 / |V|^2 at the start of the attempted step (error norm)
     float thr2[MAXN];               // (rc_i + margin)^2 rounded up
     double m[MAXN], rc[MAXN], irc[MAXN];
@@ -72,21 +72,24 @@ __device__ __forceinline__ void bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &
     GENGA_BS_RHS_HOOK();
     double(*pA)[MAXN] = S.pos[buf][0];
     double(*pB)[MAXN] = S.pos[buf][1];
-    float(*fA)[MAXN] = S.pf[buf][0];
-    float(*fB)[MAXN] = S.pf[buf][1];
+    float4 *fA = S.pf[buf][0];
+    float4 *fB = S.pf[buf][1];
     if (t.owner) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             pA[c][t.i] = qA[c]; pB[c][t.i] = qB[c];
-            fA[c][t.i] = (float)qA[c]; fB[c][t.i] = (float)qB[c];
         }
+        const float th = S.thr2[t.i];
+        fA[t.i] = make_float4((float)qA[0], (float)qA[1], (float)qA[2], th);
+        fB[t.i] = make_float4((float)qB[0], (float)qB[1], (float)qB[2], th);
     }
     __syncthreads();
     buf ^= 1;
     double ax = 0.0, ay = 0.0, az = 0.0, bx = 0.0, by = 0.0, bz = 0.0;
     if (t.i < t.n) {
         const int n = t.n, L = t.L, i = t.i;
-        const float fxA = fA[0][i], fyA = fA[1][i], fzA = fA[2][i], fxB = fB[0][i], fyB = fB[1][i], fzB = fB[2][i], ft = S.thr2[i];
+        const float4 mA = fA[i], mB = fB[i];
+        const float ft = mA.w;
         const double xA = pA[0][i], yA = pA[1][i], zA = pA[2][i], xB = pB[0][i], yB = pB[1][i], zB = pB[2][i];
         const double my_rc = S.rc[i], my_irc = S.irc[i];
         for (int j0 = t.s; j0 <= n; j0 += 32 * L) {              // partner j = n is the star
@@ -96,10 +99,11 @@ __device__ __forceinline__ void bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &
                 int j = j0 + kk * L;
                 if (j > n) break;
                 int jc = j < n ? j : i;                           // star / self: computed, not used
-                float dx = fA[0][jc] - fxA, dy = fA[1][jc] - fyA, dz = fA[2][jc] - fzA;
-                float ex = fB[0][jc] - fxB, ey = fB[1][jc] - fyB, ez = fB[2][jc] - fzB;
+                const float4 pa = fA[jc], pb = fB[jc];
+                float dx = pa.x - mA.x, dy = pa.y - mA.y, dz = pa.z - mA.z;
+                float ex = pb.x - mB.x, ey = pb.y - mB.y, ez = pb.z - mB.z;
                 float d2 = fminf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), fmaf(ez, ez, fmaf(ey, ey, ex * ex)));
-                bool in = (d2 < fmaxf(ft, S.thr2[jc]) && j != i) || j == n;
+                bool in = (d2 < fmaxf(ft, pa.w) && j != i) || j == n;
                 mask |= (in ? 1u : 0u) << kk;
             }
             while (mask) {
