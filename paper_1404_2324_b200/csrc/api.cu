@@ -238,9 +238,14 @@ static void enqueue_kick(genga_ctx *c, double h, int record, double *aout)
     }
 }
 
-static void enqueue_sun(genga_ctx *c, double h)
+static void enqueue_sun(genga_ctx *c, double h, int reset = 0)
 {
     DevState &d = c->d;
+    if (d.mode != GENGA_MODE_TEST_PARTICLE) {                 // one launch: every block forms the momentum itself
+        k_sun<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, h, reset);
+        LAUNCH(c);
+        return;
+    }
     k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx, d.vy, d.vz);
     k_shift<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.x, d.y, d.z, h, 0);
     LAUNCH(c); LAUNCH(c);
@@ -263,7 +268,7 @@ static cudaError_t launch_bs_cluster(cudaStream_t st, int clusters, const DevSta
 }
 
 // One second-order map S2(h), Eq. 7 (L100), in the order of the bullet list L153-166.
-static void enqueue_map(genga_ctx *c, double h, double tau, int first)
+static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last)
 {
     DevState &d = c->d;
     cudaStream_t st = c->st;
@@ -271,7 +276,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first)
     DevState dm = d;                                          // the massive bodies alone (mode 1)
     dm.ntot = d.nm;
     if (d.mode == GENGA_MODE_TEST_PARTICLE) { k_begin_map<<<c->sms, 256, 0, st>>>(d); LAUNCH(c); }
-    k_reset_counters<<<1, 32, 0, st>>>(d); LAUNCH(c);
+    if (d.mode == GENGA_MODE_TEST_PARTICLE || first) { k_reset_counters<<<1, 32, 0, st>>>(d); LAUNCH(c); }   // later maps: closing k_sun
     if (tp) {
         // particles: kick, Sun kick and drift in one pass (k_tp_front); the massive bodies as in mode 0
         launch_kick(c, 0.5 * h, 1, nullptr); LAUNCH(c);
@@ -286,9 +291,11 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first)
     }
     const int pair_blocks = (int)std::min<long long>((d.cap + 127) / 128, 4LL * c->sms);
     k_confirm<<<pair_blocks, 128, 0, st>>>(d, h); LAUNCH(c);
-    k_label_init<<<nblk(d.nmtot, 256), 256, 0, st>>>(d); LAUNCH(c);
-    k_union<<<pair_blocks, 128, 0, st>>>(d); LAUNCH(c);
-    k_flatten<<<nblk(d.nmtot, 256), 256, 0, st>>>(d); LAUNCH(c);
+    if (d.mode == GENGA_MODE_MULTI_SYSTEM) {                  // modes 0, 1: labelling inside k_build_groups
+        k_label_init<<<nblk(d.nmtot, 256), 256, 0, st>>>(d); LAUNCH(c);
+        k_union<<<pair_blocks, 128, 0, st>>>(d); LAUNCH(c);
+        k_flatten<<<nblk(d.nmtot, 256), 256, 0, st>>>(d); LAUNCH(c);
+    }
     const int warp_blocks = 2 * c->sms;                       // 4 warps each; warps take groups from a queue
     if (d.mode == GENGA_MODE_MULTI_SYSTEM) {
         k_list_groups_multi<<<nblk(d.ntot, 256), 256, 0, st>>>(d); LAUNCH(c);
@@ -325,7 +332,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first)
         k_tp_back<<<nblk(d.ntot - d.nm, 128), 128, 0, st>>>(d, h); LAUNCH(c);
         launch_kick(c, 0.5 * h, 0, nullptr); LAUNCH(c);
     } else {
-        enqueue_sun(c, 0.5 * h);
+        enqueue_sun(c, 0.5 * h, last ? 0 : 1);
         enqueue_kick(c, 0.5 * h, 0, nullptr);
     }
 }
@@ -344,7 +351,7 @@ static void enqueue_step(genga_ctx *c, double dt, int order)
     } else {
         k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt); LAUNCH(c);
     }
-    for (int k = 0; k < nw; ++k) enqueue_map(c, w[k] * dt, dt, k == 0);
+    for (int k = 0; k < nw; ++k) enqueue_map(c, w[k] * dt, dt, k == 0, k == nw - 1);
 }
 
 static long long interactions_per_eval(const DevState &d)

@@ -473,6 +473,46 @@ __global__ void k_shift(DevState d, double *ax, double *ay, double *az, double f
     double g = f / den;
     ax[i] = fma(g, d.psum[4 * sys], ax[i]); ay[i] = fma(g, d.psum[4 * sys + 1], ay[i]); az[i] = fma(g, d.psum[4 * sys + 2], az[i]);
 }
+// Sun kick in one launch (modes 0 and 2): every block forms s = sum m V itself -- mode 0: the block sums the
+// massive bodies in a fixed order (at most 8 per thread, then a tree); mode 2: a thread sums the <= 16 bodies of
+// its own system -- and shifts its bodies.  reset != 0: thread 0 also zeroes the per-map counters (the map is over).
+__global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset)
+{
+    __shared__ double red[3][8];
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    if (reset && i == 0) {
+        d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
+        d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0;
+    }
+    double sx = 0.0, sy = 0.0, sz = 0.0, m0;
+    if (d.mode == 2) {
+        if (i >= d.ntot) return;
+        const int sys = i / d.nm, base = sys * d.nm;
+        for (int k = 0; k < d.nm; ++k) {
+            double m = d.m[base + k];
+            sx = fma(m, d.vx[base + k], sx); sy = fma(m, d.vy[base + k], sy); sz = fma(m, d.vz[base + k], sz);
+        }
+        m0 = d.m0[sys];
+    } else {
+        for (int k = threadIdx.x; k < d.nm; k += 256) {
+            double m = d.m[k];
+            sx = fma(m, d.vx[k], sx); sy = fma(m, d.vy[k], sy); sz = fma(m, d.vz[k], sz);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            sx += __shfl_xor_sync(0xffffffffu, sx, o); sy += __shfl_xor_sync(0xffffffffu, sy, o); sz += __shfl_xor_sync(0xffffffffu, sz, o);
+        }
+        if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = sx; red[1][threadIdx.x >> 5] = sy; red[2][threadIdx.x >> 5] = sz; }
+        __syncthreads();
+        sx = sy = sz = 0.0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) { sx += red[0][w]; sy += red[1][w]; sz += red[2][w]; }
+        m0 = d.m0[0];
+        if (i >= d.ntot) return;
+    }
+    const double g = h / m0;
+    d.x[i] = fma(g, sx, d.x[i]); d.y[i] = fma(g, sy, d.y[i]); d.z[i] = fma(g, sz, d.z[i]);
+}
 // out = in + f * psum / den  (coordinate maps at the ABI, L69)
 __global__ void k_shift_out(DevState d, const double *ix, const double *iy, const double *iz,
                             double *ox, double *oy, double *oz, double f, int divide_by_total)
@@ -606,13 +646,37 @@ __device__ __forceinline__ void block_scan2(int v0, int v1, int &e0, int &e1, in
 // into a matrix", L565 -- here a CSR list), plus `gorder`: the group numbers by DECREASING size
 // (counting sort), the order in which the Bulirsch-Stoer kernels take them from their queue so
 // that the longest integrations start first.  One block of 1024 threads.
+// The labelling itself (k_label_init, k_union, k_flatten: same union-find, in shared memory) runs first in the same block.
 __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
 {
     __shared__ int lab[2048], sz[2048], E[2048], gst[2048], hist[2048];
     __shared__ int wsum[33];
     const int N = d.nm, tid = threadIdx.x, i0 = 2 * tid, i1 = 2 * tid + 1;
-    lab[i0] = i0 < N ? d.label[i0] : i0; lab[i1] = i1 < N ? d.label[i1] : i1;
+    lab[i0] = i0; lab[i1] = i1;
     sz[i0] = 0; sz[i1] = 0; hist[i0] = 0; hist[i1] = 0;
+    __syncthreads();
+    {
+        const int nenc = min(d.cnt[CI_NENC], (int)d.cap);
+        for (int e = tid; e < nenc; e += 1024) {
+            int2 p = d.enc[e];
+            if (d.mode == 1 && p.y >= d.nm) continue;       // particle pairs do not link massive bodies
+            int a = p.x, b = p.y;
+            while (true) {
+                a = uf_find(lab, a); b = uf_find(lab, b);
+                if (a == b) break;
+                int hi = max(a, b), lo = min(a, b);
+                int old = atomicMin(&lab[hi], lo);
+                if (old == hi) break;
+                a = old; b = lo;
+            }
+        }
+        __syncthreads();
+        int r0 = uf_find(lab, i0), r1 = uf_find(lab, i1);   // roots do not change any more: concurrent shortening is safe
+        __syncthreads();
+        lab[i0] = r0; lab[i1] = r1;
+        if (i0 < N) d.label[i0] = r0;
+        if (i1 < N) d.label[i1] = r1;
+    }
     __syncthreads();
     if (i0 < N) atomicAdd(&sz[lab[i0]], 1);
     if (i1 < N) atomicAdd(&sz[lab[i1]], 1);
