@@ -89,6 +89,58 @@ __device__ __forceinline__ void bw_rhs2(const double (&qA)[3], const double (&qB
     aB[0] = bx; aB[1] = by; aB[2] = bz;
 }
 
+// The same for the 8-lane segments (groups of 5..8 bodies), in two phases so that the expensive changeover
+// weight is evaluated once per close pair instead of once per partner slot: (1) squared distances to the
+// n - 1 partners at both points, one bit per partner that is inside rc_ij at either point; (2) while any
+// lane has a bit left, every lane takes ITS next close partner (a shuffle with a per-lane source), evaluates
+// both weights and accumulates.  Rounds = the largest number of close partners of any body (typically 1 or 2).
+__device__ __forceinline__ void bw_rhs2_seg8(const double (&qA)[3], const double (&qB)[3], const int n, const int b,
+                                             double Gm0, double G, double my_rc, double my_m, const double (&rcij)[8],
+                                             double (&aA)[3], double (&aB)[3])
+{
+    GENGA_BS_RHS_HOOK();
+    const unsigned full = 0xffffffffu;
+    double rA = fma(qA[2], qA[2], fma(qA[1], qA[1], qA[0] * qA[0]));
+    double rB = fma(qB[2], qB[2], fma(qB[1], qB[1], qB[0] * qB[0]));
+    double sA = -Gm0 * rinv3_fast(rA), sB = -Gm0 * rinv3_fast(rB);
+    double ax = sA * qA[0], ay = sA * qA[1], az = sA * qA[2];
+    double bx = sB * qB[0], by = sB * qB[1], bz = sB * qB[2];
+    unsigned close = 0u;
+#pragma unroll
+    for (int t = 0; t < 7; ++t) {
+        if (t < n - 1) {                                          // warp-uniform
+            int j = b + 1 + t;
+            j = j >= n ? j - n : j;
+            double dxA = __shfl_sync(full, qA[0], j, 8) - qA[0], dyA = __shfl_sync(full, qA[1], j, 8) - qA[1], dzA = __shfl_sync(full, qA[2], j, 8) - qA[2];
+            double dxB = __shfl_sync(full, qB[0], j, 8) - qB[0], dyB = __shfl_sync(full, qB[1], j, 8) - qB[1], dzB = __shfl_sync(full, qB[2], j, 8) - qB[2];
+            double dA = fma(dzA, dzA, fma(dyA, dyA, dxA * dxA)), dB = fma(dzB, dzB, fma(dyB, dyB, dxB * dxB));
+            const double rc2 = rcij[t] * rcij[t];
+            if (fmin(dA, dB) < rc2) close |= 1u << t;
+        }
+    }
+    while (__any_sync(full, close != 0u)) {
+        const bool act = close != 0u;
+        const int t = act ? __ffs(close) - 1 : 0;
+        close &= close - 1;
+        int j = b + 1 + t;
+        j = j >= n ? j - n : j;
+        j = act ? j : b;
+        double dxA = __shfl_sync(full, qA[0], j, 8) - qA[0], dyA = __shfl_sync(full, qA[1], j, 8) - qA[1], dzA = __shfl_sync(full, qA[2], j, 8) - qA[2];
+        double dxB = __shfl_sync(full, qB[0], j, 8) - qB[0], dyB = __shfl_sync(full, qB[1], j, 8) - qB[1], dzB = __shfl_sync(full, qB[2], j, 8) - qB[2];
+        const double rcj = __shfl_sync(full, my_rc, j, 8), mj = __shfl_sync(full, my_m, j, 8);
+        const double r = fmax(my_rc, rcj), rc2 = r * r;
+        double dA = fma(dzA, dzA, fma(dyA, dyA, dxA * dxA)), dB = fma(dzB, dzB, fma(dyB, dyB, dxB * dxB));
+        const bool inA = act && dA < rc2, inB = act && dB < rc2;
+        const double ir = rcp_fast(0.9 * (act ? r : 1.0)), gmj = G * mj;
+        double scA = direct_scale_nb(inA ? dA : 1.0, r, ir, gmj), scB = direct_scale_nb(inB ? dB : 1.0, r, ir, gmj);
+        scA = inA ? scA : 0.0; scB = inB ? scB : 0.0;
+        ax = fma(scA, dxA, ax); ay = fma(scA, dyA, ay); az = fma(scA, dzA, az);
+        bx = fma(scB, dxB, bx); by = fma(scB, dyB, by); bz = fma(scB, dzB, bz);
+    }
+    aA[0] = ax; aA[1] = ay; aA[2] = az;
+    aB[0] = bx; aB[1] = by; aB[2] = bz;
+}
+
 // One entry of the Aitken-Neville tableau in (H/n_k)^2: component c of body b.  Reads the column results
 // T[k][0], writes the diagonal T[k][k] back and returns the squared last corrections (T[k][k] - T[k][k-1])^2.
 __device__ __forceinline__ void bw_neville(BwSmem &W, int c, int b, double (&d2)[BS_KMAX])
@@ -160,7 +212,8 @@ __device__ __forceinline__ bool bw_integrate(BwSmem &W, const int lane, const in
             isq = body ? 1.0 / (q[0] * q[0] + q[1] * q[1] + q[2] * q[2]) : 0.0;
             isv = body ? 1.0 / (V[0] * V[0] + V[1] * V[1] + V[2] * V[2]) : 0.0;
             double dummy[3];
-            bw_rhs2<S>(q, q, Gm0, src, rcij, irc, gm, acc0, dummy);
+            if constexpr (S == 8) bw_rhs2_seg8(q, q, n, b, Gm0, G, my_rc, my_m, rcij, acc0, dummy);
+            else bw_rhs2<S>(q, q, Gm0, src, rcij, irc, gm, acc0, dummy);
             fresh = false;
         }
         // ---- my column(s): Gragg's modified midpoint rule, two substeps per iteration, all lanes in step.
@@ -178,7 +231,8 @@ __device__ __forceinline__ bool bw_integrate(BwSmem &W, const int lane, const in
             double qc[3], A[3], C[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) qc[c] = qa[c] + 2.0 * eta * Vb[c];
-            bw_rhs2<S>(qb, qc, Gm0, src, rcij, irc, gm, A, C);
+            if constexpr (S == 8) bw_rhs2_seg8(qb, qc, n, b, Gm0, G, my_rc, my_m, rcij, A, C);
+            else bw_rhs2<S>(qb, qc, Gm0, src, rcij, irc, gm, A, C);
             const bool fin = --left == 0;
 #pragma unroll
             for (int c = 0; c < 3; ++c) {

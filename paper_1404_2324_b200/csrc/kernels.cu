@@ -1101,4 +1101,3 @@ __global__ void k_export_labels(DevState d, int *out)
 }
 
 }  // namespace genga
-
