@@ -324,12 +324,13 @@ __global__ void __launch_bounds__(128) k_tp_kick(DevState d, double h, int recor
 // psum must hold sum m V of the massive bodies after their own kick (front) / after Bulirsch-Stoer (back);
 // the massive bodies must not have been shifted yet (front) / must have been shifted (back): B only sees
 // differences of positions, which a common shift leaves alone.
-struct TpMassive { double x[32], y[32], z[32], gm[32], rc[32]; };
+struct TpMassive { double x[32], y[32], z[32], gm[32], rc[32]; int hc[32]; };
 __device__ __forceinline__ void tp_load_massive(const DevState &d, TpMassive &M)
 {
     if (threadIdx.x < d.nm) {
         int j = threadIdx.x;
         M.x[j] = d.x[j]; M.y[j] = d.y[j]; M.z[j] = d.z[j]; M.gm[j] = d.G * d.m[j]; M.rc[j] = d.rc[j];
+        M.hc[j] = __double2hiint(9.0 * M.rc[j] * M.rc[j]);
     }
     __syncthreads();
 }
@@ -341,12 +342,13 @@ __device__ __forceinline__ int tp_accel(const DevState &d, const TpMassive &M, i
     int ncand = 0;
     ax = ay = az = 0.0;
     const int nm = d.nm;
+    const int hci = __double2hiint(9.0 * rci * rci);            // precheck on the high words first (a superset, off the FP64 pipe)
     for (int j = 0; j < nm; ++j) {
         double dx = M.x[j] - xi, dy = M.y[j] - yi, dz = M.z[j] - zi;
         double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-        double rcij = fmax(rci, M.rc[j]);
         double s3 = M.gm[j] * rinv3_fast(r2);
-        if (r2 < 9.0 * rcij * rcij) {
+        const double rcij = fmax(rci, M.rc[j]);
+        if (__double2hiint(r2) <= max(hci, M.hc[j]) && r2 < 9.0 * rcij * rcij) {
             double r = sqrt(r2);
             s3 = M.gm[j] / (r2 * r) * kick_weight(r, rcij);
             if (RECORD) {
@@ -649,7 +651,8 @@ __device__ __forceinline__ void block_scan2(int v0, int v1, int &e0, int &e1, in
 // The labelling itself (k_label_init, k_union, k_flatten: same union-find, in shared memory) runs first in the same block.
 __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
 {
-    __shared__ int lab[2048], sz[2048], E[2048], gst[2048], hist[2048];
+    __shared__ int lab[2048], sz[2048], E[2048], gst[2048];
+    __shared__ __align__(16) int hist[2048];
     __shared__ int wsum[33];
     const int N = d.nm, tid = threadIdx.x, i0 = 2 * tid, i1 = 2 * tid + 1;
     lab[i0] = i0; lab[i1] = i1;
@@ -700,10 +703,21 @@ __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
     __syncthreads();
     if (r0) d.gorder[atomicAdd(&hist[2048 - sz[i0]], 1)] = g0;
     if (r1) d.gorder[atomicAdd(&hist[2048 - sz[i1]], 1)] = g1;
+    // rank of a member inside its group = members of the same group before it in the (index-ordered) list E;
+    // the roots of the listed bodies go to a compact array first (hist is free now) and are scanned 8 at a time
+    __syncthreads();
+    for (int k = tid; k < ne; k += blockDim.x) hist[k] = lab[E[k]];
+    __syncthreads();
     for (int k = tid; k < ne; k += blockDim.x) {
-        int i = E[k], r = lab[i], rank = 0;
-        for (int kk = 0; kk < k; ++kk) rank += (lab[E[kk]] == r);
-        d.gmem[gst[r] + rank] = i;
+        const int r = hist[k];
+        int rank = 0, kk = 0;
+        const int4 *h4 = reinterpret_cast<const int4 *>(hist);
+        for (; kk + 8 <= k; kk += 8) {
+            const int4 a = h4[kk >> 2], b = h4[(kk >> 2) + 1];
+            rank += (a.x == r) + (a.y == r) + (a.z == r) + (a.w == r) + (b.x == r) + (b.y == r) + (b.z == r) + (b.w == r);
+        }
+        for (; kk < k; ++kk) rank += (hist[kk] == r);
+        d.gmem[gst[r] + rank] = E[k];
     }
     if (d.mode == 1 && tid < N) {
         unsigned mask = 0u;
