@@ -189,9 +189,14 @@ static int set_state_impl(genga_ctx *c, const double *m0, const double *m, const
     CK(cudaMemcpyAsync(d.m, m, B * n, kind, c->st));
     if (radius) CK(cudaMemcpyAsync(d.radius, radius, B * n, kind, c->st));
     double *dst[6] = {d.x, d.y, d.z, d.vx0, d.vy0, d.vz0};
-    for (int k = 0; k < 3; ++k) {
-        CK(cudaMemcpyAsync(dst[k], x + k * n, B * n, kind, c->st));
-        CK(cudaMemcpyAsync(dst[3 + k], v + k * n, B * n, kind, c->st));
+    if ((size_t)d.np == n) {                      // no padding between the component arrays: one copy each for x and v
+        CK(cudaMemcpyAsync(d.x, x, 3 * B * n, kind, c->st));
+        CK(cudaMemcpyAsync(d.vx0, v, 3 * B * n, kind, c->st));
+    } else {
+        for (int k = 0; k < 3; ++k) {
+            CK(cudaMemcpyAsync(dst[k], x + k * n, B * n, kind, c->st));
+            CK(cudaMemcpyAsync(dst[3 + k], v + k * n, B * n, kind, c->st));
+        }
     }
     enqueue_helio_to_demo(c);
     CK(cudaGetLastError());
@@ -444,9 +449,14 @@ static int get_state_impl(genga_ctx *c, double *x, double *v, cudaMemcpyKind kin
     k_shift_out<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0);
     c->launches += 2;
     const double *src[6] = {d.x, d.y, d.z, d.vx0, d.vy0, d.vz0};
-    for (int k = 0; k < 3; ++k) {
-        CK(cudaMemcpyAsync(x + k * n, src[k], B * n, kind, c->st));
-        CK(cudaMemcpyAsync(v + k * n, src[3 + k], B * n, kind, c->st));
+    if ((size_t)d.np == n) {
+        CK(cudaMemcpyAsync(x, d.x, 3 * B * n, kind, c->st));
+        CK(cudaMemcpyAsync(v, d.vx0, 3 * B * n, kind, c->st));
+    } else {
+        for (int k = 0; k < 3; ++k) {
+            CK(cudaMemcpyAsync(x + k * n, src[k], B * n, kind, c->st));
+            CK(cudaMemcpyAsync(v + k * n, src[3 + k], B * n, kind, c->st));
+        }
     }
     CK(cudaGetLastError());
     return GENGA_OK;
