@@ -4,6 +4,7 @@
 // every count stays in device memory and is read by the next kernel).
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <new>
@@ -40,6 +41,7 @@ struct genga_ctx {
     cudaStream_t aux[2];        // helper streams: the Bulirsch-Stoer layouts run side by side
     cudaEvent_t ev_fork, ev_join[2];
     int sms;
+    bool pdl;                   // programmatic dependent launch on the main stream (GENGA_NO_PDL=1 switches it off)
     int bs_big_clusters;        // grid size (in clusters) of the Bulirsch-Stoer cluster kernel
     int *exp_labels;            // device [np]
     double *eout;               // device [4*nsys]
@@ -136,6 +138,7 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     c->cfg = *cfg;
     c->st = (cudaStream_t)cfg->stream;
     c->sms = std::min(prop.multiProcessorCount, 148);
+    { const char *e = getenv("GENGA_NO_PDL"); c->pdl = !(e && e[0] == '1'); }
     c->bs_big_clusters = std::max(1, c->sms / BCB_CS);
     c->steps = c->force_evals = c->interactions = c->launches = 0;
     c->acc = 0;
@@ -166,6 +169,22 @@ extern "C" __attribute__((visibility("default"))) int genga_destroy(genga_ctx *c
 }
 
 static inline int nblk(long long n, int b) { return (int)std::max<long long>(1, (n + b - 1) / b); }
+
+// Launch on the main stream with programmatic dependent launch (PDL): the next kernel of the stream may be
+// scheduled while this one runs; every kernel starts with griddepcontrol.wait (pdl_sync() in kernels.cu), so it
+// touches memory only after its predecessor has completed.  What is overlapped is the launch latency, which is
+// most of a step at small N (the paper's N = 32 case, L427-433).
+template <typename... KArgs, typename... Args>
+static void launch_k(bool pdl, void (*kern)(KArgs...), int grid, int block, size_t smem, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
 #define LAUNCH(c) ((c)->acc += 1)
 
 static int red_threads(int nm) { return std::min(1024, std::max(32, (int)up((size_t)nm, 32))); }
@@ -224,35 +243,37 @@ static void launch_kick(genga_ctx *c, double h, int record, double *aout)
     DevState &d = c->d;
     const int ni = std::min(KK_NI, (d.nm + c->sms - 1) / c->sms);
     const int grid = (d.nm + ni - 1) / ni;
-    k_kick<<<grid, KK_THREADS, kick_smem_bytes(), c->st>>>(d, h, record, ni, aout);
+    launch_k(c->pdl, k_kick, grid, KK_THREADS, kick_smem_bytes(), c->st, d, h, record, ni, aout);
 }
 
 static void enqueue_kick(genga_ctx *c, double h, int record, double *aout)
 {
     DevState &d = c->d;
     if (d.mode == GENGA_MODE_MULTI_SYSTEM) {
-        k_kick_multi<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, h, record, aout);
+        launch_k(c->pdl, k_kick_multi, nblk(d.ntot, 128), 128, 0, c->st, d, h, record, aout);
         LAUNCH(c);
         return;
     }
     launch_kick(c, h, record, aout);
     LAUNCH(c);
     if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {
-        k_tp_kick<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, h, record, aout);
+        launch_k(c->pdl, k_tp_kick, nblk(d.ntot - d.nm, 128), 128, 0, c->st, d, h, record, aout);
         LAUNCH(c);
     }
 }
 
-static void enqueue_sun(genga_ctx *c, double h, int reset = 0)
+static void enqueue_sun(genga_ctx *c, double h, int reset = 0, bool after_bs = false)
 {
     DevState &d = c->d;
+    // after Bulirsch-Stoer: a plain launch, so that the kernels behind it are not scheduled (and their blocks do not
+    // sit on the SMs) while the groups are still being integrated
     if (d.mode != GENGA_MODE_TEST_PARTICLE) {                 // one launch: every block forms the momentum itself
-        k_sun<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, h, reset);
+        launch_k(c->pdl && !after_bs, k_sun, nblk(d.ntot, 256), 256, 0, c->st, d, h, reset);
         LAUNCH(c);
         return;
     }
-    k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx, d.vy, d.vz);
-    k_shift<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.x, d.y, d.z, h, 0);
+    launch_k(c->pdl, k_momentum, d.nsys, red_threads(d.nm), 0, c->st, d, d.vx, d.vy, d.vz);
+    launch_k(c->pdl, k_shift, nblk(d.ntot, 256), 256, 0, c->st, d, d.x, d.y, d.z, h, 0);
     LAUNCH(c); LAUNCH(c);
 }
 
@@ -280,34 +301,34 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last)
     const bool tp = d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm;
     DevState dm = d;                                          // the massive bodies alone (mode 1)
     dm.ntot = d.nm;
-    if (d.mode == GENGA_MODE_TEST_PARTICLE) { k_begin_map<<<c->sms, 256, 0, st>>>(d); LAUNCH(c); }
-    if (d.mode == GENGA_MODE_TEST_PARTICLE || first) { k_reset_counters<<<1, 32, 0, st>>>(d); LAUNCH(c); }   // later maps: closing k_sun
+    if (d.mode == GENGA_MODE_TEST_PARTICLE) { launch_k(c->pdl, k_begin_map, c->sms, 256, 0, st, d); LAUNCH(c); }
+    if (d.mode == GENGA_MODE_TEST_PARTICLE || first) { launch_k(c->pdl, k_reset_counters, 1, 32, 0, st, d); LAUNCH(c); }   // later maps: closing k_sun
     if (tp) {
         // particles: kick, Sun kick and drift in one pass (k_tp_front); the massive bodies as in mode 0
         launch_kick(c, 0.5 * h, 1, nullptr); LAUNCH(c);
-        k_momentum<<<1, red_threads(d.nm), 0, st>>>(d, d.vx, d.vy, d.vz); LAUNCH(c);
-        k_tp_front<<<nblk(d.ntot - d.nm, 128), 128, 0, st>>>(d, h, tau, first); LAUNCH(c);
-        k_shift<<<nblk(d.nm, 256), 256, 0, st>>>(dm, d.x, d.y, d.z, 0.5 * h, 0); LAUNCH(c);
-        k_drift<<<nblk(d.nm, 128), 128, 0, st>>>(dm, h); LAUNCH(c);
+        launch_k(c->pdl, k_momentum, 1, red_threads(d.nm), 0, st, d, d.vx, d.vy, d.vz); LAUNCH(c);
+        launch_k(c->pdl, k_tp_front, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h, tau, first); LAUNCH(c);
+        launch_k(c->pdl, k_shift, nblk(d.nm, 256), 256, 0, st, dm, d.x, d.y, d.z, 0.5 * h, 0); LAUNCH(c);
+        launch_k(c->pdl, k_drift, nblk(d.nm, 128), 128, 0, st, dm, h); LAUNCH(c);
     } else {
         enqueue_kick(c, 0.5 * h, 1, nullptr);
         enqueue_sun(c, 0.5 * h);
-        k_drift<<<nblk(d.ntot, 128), 128, 0, st>>>(d, h); LAUNCH(c);
+        launch_k(c->pdl, k_drift, nblk(d.ntot, 128), 128, 0, st, d, h); LAUNCH(c);
     }
     const int pair_blocks = (int)std::min<long long>((d.cap + 127) / 128, 4LL * c->sms);
-    k_confirm<<<pair_blocks, 128, 0, st>>>(d, h); LAUNCH(c);
+    launch_k(c->pdl, k_confirm, pair_blocks, 128, 0, st, d, h); LAUNCH(c);
     if (d.mode == GENGA_MODE_MULTI_SYSTEM) {                  // modes 0, 1: labelling inside k_build_groups
-        k_label_init<<<nblk(d.nmtot, 256), 256, 0, st>>>(d); LAUNCH(c);
-        k_union<<<pair_blocks, 128, 0, st>>>(d); LAUNCH(c);
-        k_flatten<<<nblk(d.nmtot, 256), 256, 0, st>>>(d); LAUNCH(c);
+        launch_k(c->pdl, k_label_init, nblk(d.nmtot, 256), 256, 0, st, d); LAUNCH(c);
+        launch_k(c->pdl, k_union, pair_blocks, 128, 0, st, d); LAUNCH(c);
+        launch_k(c->pdl, k_flatten, nblk(d.nmtot, 256), 256, 0, st, d); LAUNCH(c);
     }
     const int warp_blocks = 2 * c->sms;                       // 4 warps each; warps take groups from a queue
     if (d.mode == GENGA_MODE_MULTI_SYSTEM) {
-        k_list_groups_multi<<<nblk(d.ntot, 256), 256, 0, st>>>(d); LAUNCH(c);
-        k_bs_warp<<<warp_blocks, 32 * BW_WARPS, 0, st>>>(d, h, 0); LAUNCH(c);
-        if (d.nm > BW_MAXN) { k_bs_multi<<<nblk(d.nsys, 8), 128, 0, st>>>(d, h); LAUNCH(c); }
+        launch_k(c->pdl, k_list_groups_multi, nblk(d.ntot, 256), 256, 0, st, d); LAUNCH(c);
+        launch_k(c->pdl, k_bs_warp, warp_blocks, 32 * BW_WARPS, 0, st, d, h, 0); LAUNCH(c);
+        if (d.nm > BW_MAXN) { launch_k(c->pdl, k_bs_multi, nblk(d.nsys, 8), 128, 0, st, d, h); LAUNCH(c); }
     } else {
-        k_build_groups<<<1, 1024, 0, st>>>(d); LAUNCH(c);
+        launch_k(c->pdl, k_build_groups, 1, 1024, 0, st, d); LAUNCH(c);
         // the Bulirsch-Stoer layouts work on disjoint parts of the size-ordered group queue: side by side
         const bool mid = d.nm > BW_MAXN;
         if (mid) {
@@ -321,23 +342,23 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last)
                 cudaEventRecord(c->ev_join[1], c->aux[1]);
             }
         }
-        k_bs_warp<<<warp_blocks, 32 * BW_WARPS, 0, st>>>(d, h, 0); LAUNCH(c);
+        launch_k(c->pdl, k_bs_warp, warp_blocks, 32 * BW_WARPS, 0, st, d, h, 0); LAUNCH(c);
         if (mid) {
             cudaStreamWaitEvent(st, c->ev_join[0], 0);
             if (d.bss.base) cudaStreamWaitEvent(st, c->ev_join[1], 0);
         }
         if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {
-            k_bs_warp<<<warp_blocks, 32 * BW_WARPS, 0, st>>>(d, h, 1); LAUNCH(c);
+            launch_k(c->pdl, k_bs_warp, warp_blocks, 32 * BW_WARPS, 0, st, d, h, 1); LAUNCH(c);
             if (d.nm + 1 > BW_MAXN) { k_tp_bs<32><<<2 * c->sms, 128, 0, st>>>(d, h, BW_MAXN); LAUNCH(c); }
         }
     }
     if (tp) {
-        k_momentum<<<1, red_threads(d.nm), 0, st>>>(d, d.vx, d.vy, d.vz); LAUNCH(c);
-        k_shift<<<nblk(d.nm, 256), 256, 0, st>>>(dm, d.x, d.y, d.z, 0.5 * h, 0); LAUNCH(c);
-        k_tp_back<<<nblk(d.ntot - d.nm, 128), 128, 0, st>>>(d, h); LAUNCH(c);
+        launch_k(false, k_momentum, 1, red_threads(d.nm), 0, st, d, d.vx, d.vy, d.vz); LAUNCH(c);     // plain: see enqueue_sun
+        launch_k(c->pdl, k_shift, nblk(d.nm, 256), 256, 0, st, dm, d.x, d.y, d.z, 0.5 * h, 0); LAUNCH(c);
+        launch_k(c->pdl, k_tp_back, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h); LAUNCH(c);
         launch_kick(c, 0.5 * h, 0, nullptr); LAUNCH(c);
     } else {
-        enqueue_sun(c, 0.5 * h, last ? 0 : 1);
+        enqueue_sun(c, 0.5 * h, last ? 0 : 1, true);
         enqueue_kick(c, 0.5 * h, 0, nullptr);
     }
 }
@@ -352,9 +373,9 @@ static void enqueue_step(genga_ctx *c, double dt, int order)
     if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {    // the particles' rc: k_tp_front of the first map
         DevState dm = d;
         dm.ntot = d.nm;
-        k_rcrit<<<nblk(d.nm, 128), 128, 0, c->st>>>(dm, dt); LAUNCH(c);
+        launch_k(c->pdl, k_rcrit, nblk(d.nm, 128), 128, 0, c->st, dm, dt); LAUNCH(c);
     } else {
-        k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt); LAUNCH(c);
+        launch_k(c->pdl, k_rcrit, nblk(d.ntot, 128), 128, 0, c->st, d, dt); LAUNCH(c);
     }
     for (int k = 0; k < nw; ++k) enqueue_map(c, w[k] * dt, dt, k == 0, k == nw - 1);
 }

@@ -6,11 +6,20 @@
 
 namespace genga {
 
+// First statement of every kernel: let the next kernel of the stream be scheduled, then wait until the previous one has
+// completed and its memory is visible (no-ops unless launched with programmatic stream serialization, api.cu launch_k).
+__device__ __forceinline__ void pdl_sync()
+{
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 // =====================================================================================
 // Start of a map S2: forget the previous substep's lists.  Mode 1: clear the per-particle
 // encounter masks of the particles listed last time.
 __global__ void k_begin_map(DevState d)
 {
+    pdl_sync();
     int nprev = d.cnt[CI_NTP];
     if (d.mode == 1) {
         for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nprev; k += gridDim.x * blockDim.x)
@@ -20,6 +29,7 @@ __global__ void k_begin_map(DevState d)
 }
 __global__ void k_reset_counters(DevState d)
 {
+    pdl_sync();
     if (threadIdx.x == 0) {
         d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
         d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0;
@@ -33,6 +43,7 @@ __global__ void k_reset_counters(DevState d)
 // distance (L142: "increasing the critical radius by a factor of three").
 __global__ void k_rcrit(DevState d, double tau)
 {
+    pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= d.ntot) return;
     double x = d.x[i], y = d.y[i], z = d.z[i], vx = d.vx[i], vy = d.vy[i], vz = d.vz[i], m = d.m[i];
@@ -106,6 +117,7 @@ struct KickSmem {
 
 __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, int record, int ni, double *aout)
 {
+    pdl_sync();
     extern __shared__ __align__(32) unsigned char kk_raw[];
     KickSmem &S = *reinterpret_cast<KickSmem *>(kk_raw);
     const int N = d.nm, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -284,6 +296,7 @@ size_t kick_smem_bytes() { return sizeof(KickSmem); }
 // massive body; candidate pairs are (massive j, particle i).
 __global__ void __launch_bounds__(128) k_tp_kick(DevState d, double h, int record, double *aout)
 {
+    pdl_sync();
     __shared__ double sx[32], sy[32], sz[32], sgm[32], src[32];
     const int nm = d.nm;
     if (threadIdx.x < nm) {
@@ -362,6 +375,7 @@ __device__ __forceinline__ int tp_accel(const DevState &d, const TpMassive &M, i
 }
 __global__ void __launch_bounds__(128) k_tp_front(DevState d, double h, double tau, int first)
 {
+    pdl_sync();
     __shared__ TpMassive M;
     const int i = d.nm + blockIdx.x * blockDim.x + threadIdx.x;
     const bool live = i < d.ntot;
@@ -388,6 +402,7 @@ __global__ void __launch_bounds__(128) k_tp_front(DevState d, double h, double t
 }
 __global__ void __launch_bounds__(128) k_tp_back(DevState d, double h)
 {
+    pdl_sync();
     __shared__ TpMassive M;
     const int i = d.nm + blockIdx.x * blockDim.x + threadIdx.x;
     const bool live = i < d.ntot;
@@ -407,6 +422,7 @@ __global__ void __launch_bounds__(128) k_tp_back(DevState d, double h)
 // own system (contiguous, body = system * nm + k).
 __global__ void __launch_bounds__(128) k_kick_multi(DevState d, double h, int record, double *aout)
 {
+    pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= d.ntot) return;
     const int nm = d.nm, base = (i / nm) * nm;
@@ -442,6 +458,7 @@ __global__ void __launch_bounds__(128) k_kick_multi(DevState d, double h, int re
 // which: 0 = democratic V as stored; used also for the coordinate maps (with other arrays).
 __global__ void k_momentum(DevState d, const double *vx, const double *vy, const double *vz)
 {
+    pdl_sync();
     __shared__ double red[4][32];
     const int sys = blockIdx.x, base = sys * d.nm * (d.mode == 2 ? 1 : 0);
     double s[4] = {0, 0, 0, 0};
@@ -466,6 +483,7 @@ __global__ void k_momentum(DevState d, const double *vx, const double *vy, const
 // q += f * psum / m0   (f = h for the Sun kick)
 __global__ void k_shift(DevState d, double *ax, double *ay, double *az, double f, int divide_by_total)
 {
+    pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= d.ntot) return;
     int sys = system_of(d, i);
@@ -478,6 +496,7 @@ __global__ void k_shift(DevState d, double *ax, double *ay, double *az, double f
 // its own system -- and shifts its bodies.  reset != 0: thread 0 also zeroes the per-map counters (the map is over).
 __global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset)
 {
+    pdl_sync();
     __shared__ double red[3][8];
     const int i = blockIdx.x * 256 + threadIdx.x;
     if (reset && i == 0) {
@@ -517,6 +536,7 @@ __global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset)
 __global__ void k_shift_out(DevState d, const double *ix, const double *iy, const double *iz,
                             double *ox, double *oy, double *oz, double f, int divide_by_total)
 {
+    pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= d.ntot) return;
     int sys = system_of(d, i);
@@ -530,6 +550,7 @@ __global__ void k_shift_out(DevState d, const double *ix, const double *iy, cons
 // body, state kept before the drift for the encounter search and for BS.
 __global__ void __launch_bounds__(128) k_drift(DevState d, double h)
 {
+    pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= d.ntot) return;
     double x = d.x[i], y = d.y[i], z = d.z[i], vx = d.vx[i], vy = d.vy[i], vz = d.vz[i];
@@ -541,6 +562,7 @@ __global__ void __launch_bounds__(128) k_drift(DevState d, double h)
 // stand-alone drift on caller arrays (genga_kepler_drift)
 __global__ void __launch_bounds__(128) k_drift_arrays(long long n, double mu, double h, double *x, double *v, int *status)
 {
+    pdl_sync();
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     double a = x[i], b = x[n + i], c = x[2 * n + i], va = v[i], vb = v[n + i], vc = v[2 * n + i];
@@ -554,6 +576,7 @@ __global__ void __launch_bounds__(128) k_drift_arrays(long long n, double mu, do
 // particle also sets the massive body's bit in the particle's mask and lists the particle once.
 __global__ void __launch_bounds__(128) k_confirm(DevState d, double h)
 {
+    pdl_sync();
     const int nc = min(d.cnt[CI_NCAND], (int)d.cap);
     for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < nc; e += gridDim.x * blockDim.x) {
         int2 p = d.cand[e];
@@ -588,6 +611,7 @@ __global__ void __launch_bounds__(128) k_confirm(DevState d, double h)
 // repeat-until-unchanged sweep.
 __global__ void k_label_init(DevState d)
 {
+    pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < d.nmtot) d.label[i] = i;
 }
@@ -599,6 +623,7 @@ __device__ __forceinline__ int uf_find(const int *L, int i)
 }
 __global__ void k_union(DevState d)
 {
+    pdl_sync();
     const int ne = min(d.cnt[CI_NENC], (int)d.cap);
     int *L = d.label;
     for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < ne; e += gridDim.x * blockDim.x) {
@@ -617,6 +642,7 @@ __global__ void k_union(DevState d)
 }
 __global__ void k_flatten(DevState d)
 {
+    pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < d.nmtot) d.label[i] = uf_find(d.label, i);
 }
@@ -649,6 +675,7 @@ __device__ __forceinline__ void block_scan2(int v0, int v1, int &e0, int &e1, in
 // The labelling itself (k_label_init, k_union, k_flatten: same union-find, in shared memory) runs first in the same block.
 __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
 {
+    pdl_sync();
     __shared__ int lab[2048], sz[2048], E[2048], gst[2048];
     __shared__ __align__(16) int hist[2048];
     __shared__ int wsum[33];
@@ -754,6 +781,7 @@ __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
 template <int MAXN, int THREADS, int CS>
 __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, int qslot, int endslot)
 {
+    pdl_sync();
     extern __shared__ __align__(16) unsigned char bc_raw[];
     using Smem = BcSmem<MAXN, THREADS>;
     Smem &S = *reinterpret_cast<Smem *>(bc_raw);
@@ -807,6 +835,7 @@ template __global__ void k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>(DevState, d
 //             bodies it meets + their massive groups (L342), only the particle is written back.
 __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h, int tp)
 {
+    pdl_sync();
     __shared__ BwSmem sm[BW_WARPS];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     BwSmem &W = sm[warp];
@@ -888,6 +917,7 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
 // root (label = own index) with at least one other member appends (system, member mask).
 __global__ void k_list_groups_multi(DevState d)
 {
+    pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (d.cnt[CI_NENC] == 0 || i >= d.ntot) return;
     if (d.label[i] != i) return;
@@ -903,6 +933,7 @@ __global__ void k_list_groups_multi(DevState d)
 // Groups larger than a warp: one block per group, tableau in global scratch.
 __global__ void __launch_bounds__(256) k_bs_block(DevState d, double h)
 {
+    pdl_sync();
     __shared__ double red[32];
     __shared__ int nsteps;
     if (d.cnt[CI_NBIG] == 0) return;
@@ -940,6 +971,7 @@ __global__ void __launch_bounds__(256) k_bs_block(DevState d, double h)
 template <int TW>
 __global__ void __launch_bounds__(128) k_tp_bs(DevState d, double h, int lo)
 {
+    pdl_sync();
     constexpr int TPB = 128 / TW;                       // teams per block
     __shared__ TeamSmem<TW> sm[TPB];
     const int ntp = d.cnt[CI_NTP];
@@ -996,6 +1028,7 @@ template __global__ void k_tp_bs<32>(DevState, double, int);
 // per system; the groups of a system are the sets of equal labels among its bodies.
 __global__ void __launch_bounds__(128) k_bs_multi(DevState d, double h)
 {
+    pdl_sync();
     constexpr int TW = 16, TPB = 128 / TW;
     __shared__ TeamSmem<TW> sm[TPB];
     if (d.cnt[CI_NBIG] == 0) return;
@@ -1046,6 +1079,7 @@ __global__ void __launch_bounds__(128) k_bs_multi(DevState d, double h)
 // out[sys][0] = E, out[sys][1..3] = L.
 __global__ void __launch_bounds__(1024) k_energy(DevState d, double *out)
 {
+    pdl_sync();
     __shared__ double red[8][32];
     const int sys = blockIdx.x, nm = d.nm, base = d.mode == 2 ? sys * nm : 0;
     const double m0 = d.m0[sys];
@@ -1087,6 +1121,7 @@ __global__ void __launch_bounds__(1024) k_energy(DevState d, double *out)
 // genga_fp64_probe to measure the denominator of the ALU roofline on the device at hand.
 __global__ void __launch_bounds__(256) k_fp64_probe(double *out, int iters)
 {
+    pdl_sync();
     double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
     const double b = 1.0000001, c = 1e-9;
 #pragma unroll 1
@@ -1104,6 +1139,7 @@ __global__ void __launch_bounds__(256) k_fp64_probe(double *out, int iters)
 // labels for genga_encounters: body's own index unless it is in a group
 __global__ void k_export_labels(DevState d, int *out)
 {
+    pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= d.ntot) return;
     int l = i;
