@@ -123,6 +123,25 @@ def test_config0_1000_steps_energy_and_state(G):
     g.close()
 
 
+def test_config0_1e4_steps_energy_within_2x_of_the_oracle(G):
+    """north_star: |dE/E| after 10^4 steps within 2x of the oracle's (config 0, order 2 and order 4)."""
+    w = workloads.config0()
+    for order in (2, 4):
+        g = G.from_workload(w)
+        o = oracle.Sim(w)
+        E0, L0 = g.energy()
+        Eo0, _ = o.energy()
+        g.step(10000, w["dt"], order)
+        o.step(10000, w["dt"], order)
+        E1, L1 = g.energy()
+        Eo1, _ = o.energy()
+        assert g.status() == 0
+        dg, do = abs((E1 - E0) / E0)[0], abs((Eo1 - Eo0) / Eo0)[0]
+        assert dg <= 2 * do + 1e-13, (order, dg, do)
+        assert np.abs(L1 - L0).max() <= 1e-11 * np.abs(L0).max()
+        g.close()
+
+
 def test_encounter_heavy_small_case_with_groups(G):
     """16 bodies with inflated masses: many encounters, groups of 3+, exercised at orders 2, 4, 6 and
     backwards in time."""
