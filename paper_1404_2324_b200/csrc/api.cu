@@ -250,7 +250,7 @@ static void enqueue_kick(genga_ctx *c, double h, int record, double *aout)
 {
     DevState &d = c->d;
     if (d.mode == GENGA_MODE_MULTI_SYSTEM) {
-        launch_k(c->pdl, k_kick_multi, nblk(d.ntot, 128), 128, 0, c->st, d, h, record, aout);
+        launch_k(c->pdl, k_kick_multi, nblk(d.nsys, 128 / d.nm), 128, 0, c->st, d, h, record, aout);
         LAUNCH(c);
         return;
     }

@@ -418,27 +418,38 @@ __global__ void __launch_bounds__(128) k_tp_back(DevState d, double h)
     d.vx[i] = fma(hh, ax, vx); d.vy[i] = fma(hh, ay, vy); d.vz[i] = fma(hh, az, vz);
 }
 
-// Kick in multi-system mode (L368-370): one thread per body, partners = the bodies of its
-// own system (contiguous, body = system * nm + k).
+// Kick in multi-system mode (L368-370): one thread per body, partners = the bodies of its own system
+// (contiguous, body = system * nm + k).  A block takes 128 / nm whole systems and stages their bodies in shared
+// memory once (coalesced), so the partner loop reads shared memory (the lanes of a system read the same address).
 __global__ void __launch_bounds__(128) k_kick_multi(DevState d, double h, int record, double *aout)
 {
     pdl_sync();
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= d.ntot) return;
-    const int nm = d.nm, base = (i / nm) * nm;
-    double xi = d.x[i], yi = d.y[i], zi = d.z[i], rci = d.rc[i];
+    __shared__ double sx[128], sy[128], sz[128], sgm[128], src[128];
+    const int nm = d.nm, spb = 128 / nm, t = threadIdx.x;
+    const int i = blockIdx.x * spb * nm + t;
+    const bool live = t < spb * nm && i < d.ntot;
+    double xi = 0.0, yi = 0.0, zi = 0.0, rci = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
+    if (live) {
+        xi = d.x[i]; yi = d.y[i]; zi = d.z[i]; rci = d.rc[i];
+        vx = d.vx[i]; vy = d.vy[i]; vz = d.vz[i];
+        sx[t] = xi; sy[t] = yi; sz[t] = zi; src[t] = rci; sgm[t] = d.G * d.m[i];
+    }
+    __syncthreads();
+    if (!live) return;
+    const int sb = (t / nm) * nm;
     double ax = 0, ay = 0, az = 0;
     for (int k = 0; k < nm; ++k) {
-        int j = base + k;
-        if (j == i) continue;
-        double dx = d.x[j] - xi, dy = d.y[j] - yi, dz = d.z[j] - zi;
+        const int jt = sb + k;
+        if (jt == t) continue;
+        double dx = sx[jt] - xi, dy = sy[jt] - yi, dz = sz[jt] - zi;
         double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-        double rcij = fmax(rci, d.rc[j]);
-        double gm = d.G * d.m[j];
+        double rcij = fmax(rci, src[jt]);
+        double gm = sgm[jt];
         double s3 = gm * rinv3_fast(r2);
         if (r2 < 9.0 * rcij * rcij) {
             double r = sqrt(r2);
             s3 = gm / (r2 * r) * kick_weight(r, rcij);
+            const int j = i - t + jt;
             if (record && i < j) {
                 int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
                 if (idx < d.cap) d.cand[idx] = make_int2(i, j);
@@ -448,7 +459,7 @@ __global__ void __launch_bounds__(128) k_kick_multi(DevState d, double h, int re
         ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
     }
     if (aout) { aout[i] = ax; aout[d.ntot + i] = ay; aout[2 * (size_t)d.ntot + i] = az; }
-    d.vx[i] = fma(h, ax, d.vx[i]); d.vy[i] = fma(h, ay, d.vy[i]); d.vz[i] = fma(h, az, d.vz[i]);
+    d.vx[i] = fma(h, ax, vx); d.vy[i] = fma(h, ay, vy); d.vz[i] = fma(h, az, vz);
 }
 
 // =====================================================================================
