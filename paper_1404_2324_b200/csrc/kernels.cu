@@ -164,8 +164,8 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
     const int hci0 = ok0 ? __double2hiint(9.0 * rci0 * rci0) : -1, hci1 = ok1 ? __double2hiint(9.0 * rci1 * rci1) : -1;
     // the velocity component this thread will kick at the end: loaded now, off the critical path
     double vel0 = 0.0;
-    if (tid < 3 * nib) {
-        const int r = tid / 3, c = tid - 3 * r;
+    if ((tid & 3) == 0 && (tid >> 2) < 3 * nib) {
+        const int r = (tid >> 2) / 3, c = (tid >> 2) - 3 * r;
         vel0 = (c == 0 ? d.vx : c == 1 ? d.vy : d.vz)[i0 + r];
     }
     __syncthreads();
@@ -278,14 +278,25 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
         }
     }
     __syncthreads();
-    if (tid < 3 * nib) {
-        const int r = tid / 3, c = tid - 3 * r;
+    // four lanes per sum (value v = 3 row + component): each adds a quarter of the row's warps, two shuffle levels join them
+    if (tid < 4 * 3 * KK_NI + (32 - (4 * 3 * KK_NI) % 32) % 32) {
+        const int v = tid >> 2, part = tid & 3;
+        const bool live = v < 3 * nib;
+        const int r = live ? v / 3 : 0, c = live ? v - 3 * r : 0;
         const int w0 = r < 8 ? 0 : r < 12 ? 16 : 24, nw = r < 8 ? 16 : r < 12 ? 8 : 4, rr = r < 8 ? r : r < 12 ? r - 8 : r - 12;
         double a = 0.0;
-        for (int w = 0; w < nw; ++w) a += S.wsum[w0 + w][rr][c];
-        double *vel = c == 0 ? d.vx : c == 1 ? d.vy : d.vz;
-        vel[i0 + r] = fma(h, a, vel0);
-        if (aout) aout[(size_t)c * d.ntot + i0 + r] = a;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int w = part + 4 * k;
+            if (live && w < nw) a += S.wsum[w0 + w][rr][c];
+        }
+        a += __shfl_xor_sync(0xffffffffu, a, 1);
+        a += __shfl_xor_sync(0xffffffffu, a, 2);
+        if (live && part == 0) {
+            double *vel = c == 0 ? d.vx : c == 1 ? d.vy : d.vz;
+            vel[i0 + r] = fma(h, a, vel0);
+            if (aout) aout[(size_t)c * d.ntot + i0 + r] = a;
+        }
     }
 }
 
