@@ -81,8 +81,8 @@ __global__ void k_rcrit(DevState d, double tau)
 // The precheck r^2 < 9 max(rc_i, rc_j)^2 is done on the HIGH WORDS of the doubles with
 // integer compares (a superset of the exact test, off the FP64 pipe).  A pair that passes --
 // the whole changeover zone r < rc_ij lies inside the precheck sphere, and so does the body
-// itself -- gets weight 0 by clearing the seed, and the warp's ballot of the test is stored
-// as a hit word.  After its pair loop each warp lists its hits in a fixed order, evaluates
+// itself -- gets weight 0 by clearing the seed and sets a bit in the lane's hit mask (two bits
+// per iteration).  After its pair loop each warp lists its hits in a fixed order, evaluates
 // them one per lane with the exact weight W = K - r dK/dr and the exact candidate test, and
 // the row pair's first lane adds them in list order: no atomics on the sums, deterministic.  The row sums of the warps meet in shared memory and the block applies the
 // kick to its own bodies: one launch, no partial sums in global memory.
@@ -104,13 +104,12 @@ __device__ __forceinline__ double kick_scale_exact(double r2, double rcij, doubl
 }
 
 struct __align__(32) KickBody { double x, y, z, gm; };
-struct KickHit { int code; int pad; double cx, cy, cz; };      // code = lane bit << 8 | iteration
+struct KickHit { int code; int pad; double cx, cy, cz; };      // code = bit of the lane's hit mask << 8 | lane
 
 struct KickSmem {
     KickBody body[KK_MAXN];                 // all bodies j, padded to a multiple of 64
     int hc[KK_MAXN];                        // high word of 9 rc_j^2 (-1 for padding)
     double rc[KK_MAXN];                     // critical radius (exact pass)
-    unsigned hitw[KK_WARPS][32];            // per warp: ballot of the precheck, one word per iteration
     KickHit list[KK_WARPS][32];             // per warp: hits of the current window of the exact pass
     double wsum[KK_WARPS][8][3];            // per warp: sums of its rows
 };
@@ -171,13 +170,13 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
     __syncthreads();
 
     double ax0 = 0.0, ay0 = 0.0, az0 = 0.0, ax1 = 0.0, ay1 = 0.0, az1 = 0.0;
+    unsigned hits = 0u;
     if (rowbase < nib) {                                // warp-uniform: the group has rows in this block
         const int L = iters << logP;
         {
             const KickBody *pb = &S.body[wi * L + phase];
             const int *ph = &S.hc[wi * L + phase];
-            unsigned *pw = S.hitw[warp];
-            const bool lane0 = lane == 0;
+            unsigned bit = 1u;
 #pragma unroll 2
             for (int t = 0; t < iters; ++t) {
                 const KickBody bj = *pb;
@@ -198,9 +197,8 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
                 const double s30 = bj.gm * fma(p0 * e0, w0, w0), s31 = bj.gm * fma(p1 * e1, w1, w1);   // G m_j y0^3 (1 + 3e/2 + 15 e^2/8)
                 ax0 = fma(s30, dx0, ax0); ay0 = fma(s30, dy0, ay0); az0 = fma(s30, dz0, az0);
                 ax1 = fma(s31, dx1, ax1); ay1 = fma(s31, dy1, ay1); az1 = fma(s31, dz1, az1);
-                const unsigned hm0 = __ballot_sync(0xffffffffu, hit0), hm1 = __ballot_sync(0xffffffffu, hit1);
-                if (lane0) { pw[0] = hm0; pw[1] = hm1; }
-                pw += 2;
+                hits |= (hit0 ? bit : 0u) | (hit1 ? bit << 1 : 0u);     // bit 2 t + s: row s of this lane met body j of iteration t
+                bit <<= 2;
             }
         }
         // the P phases of a row pair: every lane of the pair gets the sums of its two rows
@@ -211,9 +209,9 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
         __syncwarp();
 
         // ---- this warp's pairs inside the precheck sphere: exact weight, candidate list.
-        // Hit word 2 t + s, bit b: row rowbase + 2 (b >> logP) + s, body j = wi L + t P + (b & (P - 1)).  The hits are listed
-        // in (word, b) order, 32 at a time; lane e evaluates entry e; the row pair's first lane adds its entries in list order.
-        const unsigned word = lane < 2 * iters ? S.hitw[warp][lane] : 0u;
+        // Lane l, bit 2 t + s of its hit mask: row rowbase + 2 (l >> logP) + s, body j = wi L + t P + (l & (P - 1)).  The hits are
+        // listed in (lane, bit) order, 32 at a time; lane e evaluates entry e; the row pair's first lane adds its entries in list order.
+        const unsigned word = hits;
         const int cnt = __popc(word);
         int inc = cnt;
 #pragma unroll
@@ -235,7 +233,7 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
             bool cand = false;
             int ci = 0, cj = 0;
             if (lane < nwin) {
-                const int code = S.list[warp][lane].code, b = code >> 8, wd = code & 255;
+                const int code = S.list[warp][lane].code, wd = code >> 8, b = code & 255;      // bit index, lane
                 ci = i0 + rowbase + 2 * (b >> logP) + (wd & 1); cj = wi * L + ((wd >> 1) << logP) + (b & (P - 1));
                 double cx = 0.0, cy = 0.0, cz = 0.0;
                 if (cj != ci) {
@@ -264,9 +262,9 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
             if (phase == 0) {
                 for (int e = 0; e < nwin; ++e) {
                     const int code = S.list[warp][e].code;
-                    if (((code >> 8) >> logP) == rp) {
+                    if (((code & 255) >> logP) == rp) {
                         const double cx = S.list[warp][e].cx, cy = S.list[warp][e].cy, cz = S.list[warp][e].cz;
-                        if (code & 1) { ax1 += cx; ay1 += cy; az1 += cz; } else { ax0 += cx; ay0 += cy; az0 += cz; }
+                        if ((code >> 8) & 1) { ax1 += cx; ay1 += cy; az1 += cz; } else { ax0 += cx; ay0 += cy; az0 += cz; }
                     }
                 }
             }
