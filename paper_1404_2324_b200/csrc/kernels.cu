@@ -533,10 +533,15 @@ __global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset)
         }
         m0 = d.m0[sys];
     } else {
-        for (int k = threadIdx.x; k < d.nm; k += 256) {
-            double m = d.m[k];
-            sx = fma(m, d.vx[k], sx); sy = fma(m, d.vy[k], sy); sz = fma(m, d.vz[k], sz);
+        double lm[KK_MAXN / 256], lx[KK_MAXN / 256], ly[KK_MAXN / 256], lz[KK_MAXN / 256];
+#pragma unroll
+        for (int q = 0; q < KK_MAXN / 256; ++q) {                 // all loads in flight together
+            const int k = threadIdx.x + 256 * q;
+            const bool v = k < d.nm;
+            lm[q] = v ? d.m[k] : 0.0; lx[q] = v ? d.vx[k] : 0.0; ly[q] = v ? d.vy[k] : 0.0; lz[q] = v ? d.vz[k] : 0.0;
         }
+#pragma unroll
+        for (int q = 0; q < KK_MAXN / 256; ++q) { sx = fma(lm[q], lx[q], sx); sy = fma(lm[q], ly[q], sy); sz = fma(lm[q], lz[q], sz); }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             sx += __shfl_xor_sync(0xffffffffu, sx, o); sy += __shfl_xor_sync(0xffffffffu, sy, o); sz += __shfl_xor_sync(0xffffffffu, sz, o);
