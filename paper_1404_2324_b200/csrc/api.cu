@@ -581,9 +581,11 @@ extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ct
             c->launches += 2; per = 2;
         } else if (which == 2) { c->acc = 0; enqueue_kick(c, 0.0, 0, nullptr); per = (int)c->acc; c->launches += c->acc; c->acc = 0; }
         else if (which == 3) {                       // fused particle pass, forwards then backwards
+            k_reset_counters<<<1, 32, 0, c->st>>>(d);     // the candidate list must not run over (as in a step)
             k_tp_front<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, dt, dt, 1);
+            k_reset_counters<<<1, 32, 0, c->st>>>(d);
             k_tp_front<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, -dt, dt, 0);
-            c->launches += 2; per = 2;
+            c->launches += 4; per = 2;
         } else {
             k_tp_back<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, dt);
             k_tp_back<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, -dt);

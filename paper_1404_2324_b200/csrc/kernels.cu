@@ -363,19 +363,31 @@ __device__ __forceinline__ int tp_accel(const DevState &d, const TpMassive &M, i
     int ncand = 0;
     ax = ay = az = 0.0;
     const int nm = d.nm;
+    const unsigned act = __activemask();                        // the live lanes of this warp run the loop together
+    const int lane = threadIdx.x & 31;
     for (int j = 0; j < nm; ++j) {
         double dx = M.x[j] - xi, dy = M.y[j] - yi, dz = M.z[j] - zi;
         double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-        double rcij = fmax(rci, M.rc[j]);
+        double rcij = fmax(rci, M.rc[j]), rc2 = rcij * rcij;
         double s3 = M.gm[j] * rinv3_fast(r2);
-        if (r2 < 9.0 * rcij * rcij) {
+        if (r2 < rc2) {                                         // inside the changeover zone: exact weight (W = 1 outside)
             double r = sqrt(r2);
             s3 = M.gm[j] / (r2 * r) * kick_weight(r, rcij);
-            if (RECORD) {
-                int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
-                if (idx < d.cap) d.cand[idx] = make_int2(j, i);
-                else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
-                ++ncand;
+        }
+        if (RECORD) {                                           // candidates: one atomic per warp
+            const bool cand = r2 < 9.0 * rcij * rcij;
+            const unsigned m = __ballot_sync(act, cand);
+            if (m) {
+                const int leader = __ffs(m) - 1;
+                int base = 0;
+                if (lane == leader) base = atomicAdd(&d.cnt[CI_NCAND], __popc(m));
+                base = __shfl_sync(act, base, leader);
+                if (cand) {
+                    const int idx = base + __popc(m & ((1u << lane) - 1u));
+                    if (idx < d.cap) d.cand[idx] = make_int2(j, i);
+                    else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+                    ++ncand;
+                }
             }
         }
         ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
@@ -456,8 +468,10 @@ __global__ void __launch_bounds__(128) k_kick_multi(DevState d, double h, int re
         double gm = sgm[jt];
         double s3 = gm * rinv3_fast(r2);
         if (r2 < 9.0 * rcij * rcij) {
-            double r = sqrt(r2);
-            s3 = gm / (r2 * r) * kick_weight(r, rcij);
+            if (r2 < rcij * rcij) {                             // W = 1 outside the changeover zone
+                double r = sqrt(r2);
+                s3 = gm / (r2 * r) * kick_weight(r, rcij);
+            }
             const int j = i - t + jt;
             if (record && i < j) {
                 int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
