@@ -346,12 +346,13 @@ __global__ void __launch_bounds__(128) k_tp_kick(DevState d, double h, int recor
 // psum must hold sum m V of the massive bodies after their own kick (front) / after Bulirsch-Stoer (back);
 // the massive bodies must not have been shifted yet (front) / must have been shifted (back): B only sees
 // differences of positions, which a common shift leaves alone.
-struct TpMassive { double x[32], y[32], z[32], gm[32], rc[32]; };
+struct TpMassive { double x[32], y[32], z[32], gm[32], rc[32]; int hc[32]; };
 __device__ __forceinline__ void tp_load_massive(const DevState &d, TpMassive &M)
 {
     if (threadIdx.x < d.nm) {
         int j = threadIdx.x;
         M.x[j] = d.x[j]; M.y[j] = d.y[j]; M.z[j] = d.z[j]; M.gm[j] = d.G * d.m[j]; M.rc[j] = d.rc[j];
+        M.hc[j] = __double2hiint(9.0 * M.rc[j] * M.rc[j]);
     }
     __syncthreads();
 }
@@ -365,17 +366,21 @@ __device__ __forceinline__ int tp_accel(const DevState &d, const TpMassive &M, i
     const int nm = d.nm;
     const unsigned act = __activemask();                        // the live lanes of this warp run the loop together
     const int lane = threadIdx.x & 31;
+    const int hci = __double2hiint(9.0 * rci * rci);            // precheck on the high words (a superset, off the FP64 pipe)
     for (int j = 0; j < nm; ++j) {
         double dx = M.x[j] - xi, dy = M.y[j] - yi, dz = M.z[j] - zi;
         double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-        double rcij = fmax(rci, M.rc[j]), rc2 = rcij * rcij;
         double s3 = M.gm[j] * rinv3_fast(r2);
-        if (r2 < rc2) {                                         // inside the changeover zone: exact weight (W = 1 outside)
-            double r = sqrt(r2);
-            s3 = M.gm[j] / (r2 * r) * kick_weight(r, rcij);
+        bool cand = false;
+        if (__double2hiint(r2) <= max(hci, M.hc[j])) {
+            const double rcij = fmax(rci, M.rc[j]);
+            cand = r2 < 9.0 * rcij * rcij;
+            if (r2 < rcij * rcij) {                             // inside the changeover zone: exact weight (W = 1 outside)
+                double r = sqrt(r2);
+                s3 = M.gm[j] / (r2 * r) * kick_weight(r, rcij);
+            }
         }
         if (RECORD) {                                           // candidates: one atomic per warp
-            const bool cand = r2 < 9.0 * rcij * rcij;
             const unsigned m = __ballot_sync(act, cand);
             if (m) {
                 const int leader = __ffs(m) - 1;
