@@ -103,34 +103,37 @@ __device__ __forceinline__ void bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &
                 float dx = pa.x - mA.x, dy = pa.y - mA.y, dz = pa.z - mA.z;
                 float ex = pb.x - mB.x, ey = pb.y - mB.y, ez = pb.z - mB.z;
                 float d2 = fminf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), fmaf(ez, ez, fmaf(ey, ey, ex * ex)));
-                bool in = (d2 < fmaxf(ft, pa.w) && j != i) || j == n;
+                bool in = d2 < fmaxf(ft, pa.w) && j != i && j != n;
                 mask |= (in ? 1u : 0u) << kk;
             }
+            // pairs that passed: exact test, then both changeover weights in one straight-line block (no branch inside,
+            // so the two dependent chains overlap and the lanes of a warp do not split)
             while (mask) {
                 int j = j0 + (__ffs(mask) - 1) * L;
                 mask &= mask - 1;
-                if (j == n) {
-                    double rA = xA * xA + yA * yA + zA * zA, rB = xB * xB + yB * yB + zB * zB;
-                    double sA = -G * m0 * rinv3_fast(rA), sB = -G * m0 * rinv3_fast(rB);
-                    ax += sA * xA; ay += sA * yA; az += sA * zA;
-                    bx += sB * xB; by += sB * yB; bz += sB * zB;
-                } else {
-                    double rcj = S.rc[j];
-                    double rcij = fmax(my_rc, rcj), rc2 = rcij * rcij;
-                    double dx = pA[0][j] - xA, dy = pA[1][j] - yA, dz = pA[2][j] - zA;
-                    double ex = pB[0][j] - xB, ey = pB[1][j] - yB, ez = pB[2][j] - zB;
-                    double dA = dx * dx + dy * dy + dz * dz, dB = ex * ex + ey * ey + ez * ez;
-                    const bool inA = dA < rc2, inB = dB < rc2;
-                    if (inA || inB) {
-                        const double ir = my_rc >= rcj ? my_irc : S.irc[j], gmj = G * S.m[j];
-                        double scA = direct_scale(inA ? dA : rc2, rcij, ir, gmj);
-                        double scB = direct_scale(inB ? dB : rc2, rcij, ir, gmj);
-                        scA = inA ? scA : 0.0; scB = inB ? scB : 0.0;
-                        ax += scA * dx; ay += scA * dy; az += scA * dz;
-                        bx += scB * ex; by += scB * ey; bz += scB * ez;
-                    }
+                double rcj = S.rc[j];
+                double rcij = fmax(my_rc, rcj), rc2 = rcij * rcij;
+                double dx = pA[0][j] - xA, dy = pA[1][j] - yA, dz = pA[2][j] - zA;
+                double ex = pB[0][j] - xB, ey = pB[1][j] - yB, ez = pB[2][j] - zB;
+                double dA = dx * dx + dy * dy + dz * dz, dB = ex * ex + ey * ey + ez * ez;
+                const bool inA = dA < rc2, inB = dB < rc2;
+                if (inA || inB) {
+                    const double ir = my_rc >= rcj ? my_irc : S.irc[j], gmj = G * S.m[j];
+                    double scA = direct_scale_nb(inA ? dA : rc2, rcij, ir, gmj);
+                    double scB = direct_scale_nb(inB ? dB : rc2, rcij, ir, gmj);
+                    scA = inA ? scA : 0.0; scB = inB ? scB : 0.0;
+                    ax += scA * dx; ay += scA * dy; az += scA * dz;
+                    bx += scB * ex; by += scB * ey; bz += scB * ez;
                 }
             }
+        }
+        // the star (fixed at the origin): every lane of the body computes it, lane 0 keeps it (no split of the warp)
+        {
+            double rA = xA * xA + yA * yA + zA * zA, rB = xB * xB + yB * yB + zB * zB;
+            double sA = -G * m0 * rinv3_fast(rA), sB = -G * m0 * rinv3_fast(rB);
+            sA = t.s == 0 ? sA : 0.0; sB = t.s == 0 ? sB : 0.0;
+            ax += sA * xA; ay += sA * yA; az += sA * zA;
+            bx += sB * xB; by += sB * yB; bz += sB * zB;
         }
     }
     for (int o = t.L >> 1; o > 0; o >>= 1) {

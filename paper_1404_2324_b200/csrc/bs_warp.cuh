@@ -28,22 +28,6 @@ struct BwSmem {
     double tab[BS_KMAX][6][BW_MAXN];     // column results T[k][0], then the diagonal T[k][k]
 };
 
-// G m_j (1 - W(d, rc_ij)) / d^3 as direct_scale(), without a branch (all lanes of a warp run it
-// together; `in` selects afterwards).
-__device__ __forceinline__ double direct_scale_nb(double d2, double rcij, double irc09, double Gmj)
-{
-    double rinv = rsqrt_fast(d2);
-    double dd = d2 * rinv;
-    double y = (dd - 0.1 * rcij) * irc09;
-    double D = fma(2.0 * y, y - 1.0, 1.0);                    // >= 1/2 for every y
-    double iD = rcp_fast(D);
-    double yD = y * iD;                                       // K = y yD
-    double dK = 2.0 * (1.0 - y) * (yD * iD) * irc09;
-    double w1 = 1.0 - fma(y, yD, -dd * dK);
-    w1 = y > 0.0 ? w1 : 1.0;
-    return Gmj * (rinv * rinv) * rinv * w1;
-}
-
 // Forces on this lane's body at TWO positions qA, qB at once; the partners are the other lanes of its
 // S-lane segment (same column): partner t = 0..n-2 sits in segment lane src[t] = (b + 1 + t) mod n and
 // carries rcij[t] = max(rc_b, rc_j) (0 for a massless or missing partner, so that it never passes the

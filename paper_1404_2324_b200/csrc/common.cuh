@@ -80,6 +80,22 @@ __device__ __forceinline__ double direct_scale(double d2, double rcij, double ir
     return Gmj * (rinv * rinv) * rinv * w1;
 }
 
+// G m_j (1 - W(d, rc_ij)) / d^3 as direct_scale(), without a branch (all lanes of a warp run it
+// together; `in` selects afterwards).
+__device__ __forceinline__ double direct_scale_nb(double d2, double rcij, double irc09, double Gmj)
+{
+    double rinv = rsqrt_fast(d2);
+    double dd = d2 * rinv;
+    double y = (dd - 0.1 * rcij) * irc09;
+    double D = fma(2.0 * y, y - 1.0, 1.0);                    // >= 1/2 for every y
+    double iD = rcp_fast(D);
+    double yD = y * iD;                                       // K = y yD
+    double dK = 2.0 * (1.0 - y) * (yD * iD) * irc09;
+    double w1 = 1.0 - fma(y, yD, -dd * dK);
+    w1 = y > 0.0 ? w1 : 1.0;
+    return Gmj * (rinv * rinv) * rinv * w1;
+}
+
 // ---------------------------------------------------------------------------------
 // Stumpff functions c0..c3 at x (Danby 1988; named at L110, L230).  Bounded work:
 // argument quartering down to |x| <= 1 (at most 20 times), degree-9 series, then the
