@@ -315,7 +315,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last)
         enqueue_sun(c, 0.5 * h);
         launch_k(c->pdl, k_drift, nblk(d.ntot, 128), 128, 0, st, d, h); LAUNCH(c);
     }
-    const int pair_blocks = (int)std::min<long long>((d.cap + 127) / 128, 4LL * c->sms);
+    const int pair_blocks = (int)std::min<long long>((d.cap + 127) / 128, 16LL * c->sms);   // grid-stride over the candidates; enough warps to cover the gather latency when there are 10^6 of them (mode 1)
     launch_k(c->pdl, k_confirm, pair_blocks, 128, 0, st, d, h); LAUNCH(c);
     if (d.mode == GENGA_MODE_MULTI_SYSTEM) {                  // modes 0, 1: labelling inside k_build_groups
         launch_k(c->pdl, k_label_init, nblk(d.nmtot, 256), 256, 0, st, d); LAUNCH(c);
