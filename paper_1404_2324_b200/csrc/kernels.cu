@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
                 const KickBody bj = *pb;
                 const int hcj = *ph;
                 pb += P; ph += P;
-                // both pairs' arithmetic first, the two ballots after it: a ballot is a scheduling barrier
+                // both pairs in one straight-line block: their dependent chains overlap
                 const double dx0 = bj.x - xi0, dy0 = bj.y - yi0, dz0 = bj.z - zi0;
                 const double dx1 = bj.x - xi1, dy1 = bj.y - yi1, dz1 = bj.z - zi1;
                 const double r20 = fma(dz0, dz0, fma(dy0, dy0, dx0 * dx0)), r21 = fma(dz1, dz1, fma(dy1, dy1, dx1 * dx1));
