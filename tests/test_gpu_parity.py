@@ -323,6 +323,31 @@ def test_host_and_device_state_paths_agree_and_contexts_are_independent(G):
     g1.close(); g2.close()
 
 
+def test_runs_are_bit_reproducible_with_and_without_dependent_launch(G):
+    """No result depends on the order in which blocks or atomics happen to run: two runs of the same steps, and a run with
+    programmatic dependent launch switched off (GENGA_NO_PDL=1, read at genga_create), give bit-identical states."""
+    import os
+    for make in (lambda: workloads.config1(n=777), lambda: workloads.config2(n_test=4000), lambda: workloads.config3(n_systems=40)):
+        w = make()
+        out = []
+        for env in (None, None, "1"):
+            if env is None:
+                os.environ.pop("GENGA_NO_PDL", None)
+            else:
+                os.environ["GENGA_NO_PDL"] = env
+            g = G.from_workload(w)
+            g.step(7, w["dt"], 4)
+            x, v = g.get_state_host()
+            pairs, ncand, labels = g.encounters()
+            assert g.status() == 0
+            out.append((x.copy(), v.copy(), pairs.copy(), ncand, labels.copy()))
+            g.close()
+        os.environ.pop("GENGA_NO_PDL", None)
+        for o in out[1:]:
+            assert np.array_equal(o[0], out[0][0]) and np.array_equal(o[1], out[0][1])
+            assert np.array_equal(o[2], out[0][2]) and o[3] == out[0][3] and np.array_equal(o[4], out[0][4])
+
+
 def test_full_size_sampled_outputs_config2_and_config3(G):
     """BASELINE sizes in the launch configuration bench.py uses: 1e6 particles / 4096 systems.
     The oracle recomputes a sample: the massive bodies and a slice of particles (particles do not
