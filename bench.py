@@ -38,8 +38,11 @@ def workload(cfg_id):
     return w, name
 
 
-def interactions_per_step(w):
-    nm, evals = w["n_massive"], 2 * {2: 1, 4: 3, 6: 7}[w["order"]]
+def interactions_per_step(w, merged=True):
+    # force evaluations the library makes per step: 2 per map, adjacent kicks of the substeps of one step merged
+    # (modes 0 and 2): 2, 4, 8 for orders 2, 4, 6; the particle mode keeps them apart
+    maps = {2: 1, 4: 3, 6: 7}[w["order"]]
+    nm, evals = w["n_massive"], (2 * maps if (w["mode"] == 1 or not merged) else maps + 1)   # the oracle never merges
     if w["mode"] == 2:
         per = w["n_systems"] * nm * (nm - 1)
     else:
@@ -89,7 +92,7 @@ def oracle_rate(w, budget_s, max_steps):
     """Time the oracle as it stands on one host core; returns (interactions/s, steps, seconds)."""
     import oracle
     sim = oracle.Sim(w, cap=200000)
-    per_step, _ = interactions_per_step(w)
+    per_step, _ = interactions_per_step(w, merged=False)
     sim.step(1)
     t0 = time.perf_counter()
     n = 0
@@ -110,7 +113,7 @@ def run_reference(args):
     for _ in range(min(args.warmup, 2)):
         pass
     rate, n, secs = oracle_rate(w, budget_s=240.0, max_steps=args.steps)
-    per_step, evals = interactions_per_step(w)
+    per_step, evals = interactions_per_step(w, merged=False)
     sample = "%d full steps of %s (%.1f s)" % (n, name, secs)
     line = {
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,

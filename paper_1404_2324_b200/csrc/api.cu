@@ -294,7 +294,11 @@ static cudaError_t launch_bs_cluster(cudaStream_t st, int clusters, const DevSta
 }
 
 // One second-order map S2(h), Eq. 7 (L100), in the order of the bullet list L153-166.
-static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last)
+// hn = size of the NEXT map of the same step (0 after the last): in modes 0 and 2 the closing kick B(h/2) and the
+// opening kick B(hn/2) of the next map act at the same positions with the same critical radii (frozen over the step,
+// DESIGN.md R-4), so they are one kick of (h + hn)/2 that also records the next map's candidates (`L170`: the
+// scheme "applied to each of the substeps"; flags bit 0 keeps them apart).
+static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last, double hn, bool opened)
 {
     DevState &d = c->d;
     cudaStream_t st = c->st;
@@ -311,7 +315,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last)
         launch_k(c->pdl, k_shift, nblk(d.nm, 256), 256, 0, st, dm, d.x, d.y, d.z, 0.5 * h, 0); LAUNCH(c);
         launch_k(c->pdl, k_drift, nblk(d.nm, 128), 128, 0, st, dm, h); LAUNCH(c);
     } else {
-        enqueue_kick(c, 0.5 * h, 1, nullptr);
+        if (!opened) enqueue_kick(c, 0.5 * h, 1, nullptr);        // else: done by the previous map's merged kick
         enqueue_sun(c, 0.5 * h);
         launch_k(c->pdl, k_drift, nblk(d.ntot, 128), 128, 0, st, d, h); LAUNCH(c);
     }
@@ -359,7 +363,8 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last)
         launch_kick(c, 0.5 * h, 0, nullptr); LAUNCH(c);
     } else {
         enqueue_sun(c, 0.5 * h, last ? 0 : 1, true);
-        enqueue_kick(c, 0.5 * h, 0, nullptr);
+        if (hn != 0.0) enqueue_kick(c, 0.5 * (h + hn), 1, nullptr);   // closing kick + opening kick of the next map
+        else enqueue_kick(c, 0.5 * h, 0, nullptr);
     }
 }
 
@@ -377,7 +382,9 @@ static void enqueue_step(genga_ctx *c, double dt, int order)
     } else {
         launch_k(c->pdl, k_rcrit, nblk(d.ntot, 128), 128, 0, c->st, d, dt); LAUNCH(c);
     }
-    for (int k = 0; k < nw; ++k) enqueue_map(c, w[k] * dt, dt, k == 0, k == nw - 1);
+    const bool merge = !(c->cfg.flags & 1) && d.mode != GENGA_MODE_TEST_PARTICLE;
+    for (int k = 0; k < nw; ++k)
+        enqueue_map(c, w[k] * dt, dt, k == 0, k == nw - 1, merge && k + 1 < nw ? w[k + 1] * dt : 0.0, merge && k > 0);
 }
 
 static long long interactions_per_eval(const DevState &d)
@@ -435,7 +442,8 @@ extern "C" __attribute__((visibility("default"))) int genga_step(genga_ctx *c, i
     }
     CK(cudaGetLastError());
     c->steps += n_steps;
-    long long evals = 2LL * maps_per_step(order) * n_steps;
+    const bool merged = !(c->cfg.flags & 1) && c->d.mode != GENGA_MODE_TEST_PARTICLE;
+    long long evals = (merged ? maps_per_step(order) + 1LL : 2LL * maps_per_step(order)) * n_steps;   // force evaluations actually made
     c->force_evals += evals;
     c->interactions += evals * interactions_per_eval(c->d);
     return GENGA_OK;
