@@ -98,7 +98,7 @@ class Genga:
     """One simulation context.  State arrays are (3, Ntot) float64, heliocentric."""
 
     def __init__(self, mode, n_massive, n_test=0, n_systems=1, G=1.0, n1=3.0, n2=0.4, bs_eps=1e-12,
-                 max_pairs=None, device="cuda:0", stream=None):
+                 max_pairs=None, device="cuda:0", stream=None, flags=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1404_2324_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -112,7 +112,7 @@ class Genga:
         self.max_pairs = int(max_pairs)
         with torch.cuda.device(self.device):
             self.stream = stream if stream is not None else torch.cuda.Stream(device=self.device)
-            cfg = genga_config(mode, n_massive, n_test, n_systems, 0, G, n1, n2, bs_eps, self.max_pairs, None, 0,
+            cfg = genga_config(mode, n_massive, n_test, n_systems, int(flags), G, n1, n2, bs_eps, self.max_pairs, None, 0,
                                self.stream.cuda_stream)
             nbytes = self.lib.genga_workspace_bytes(C.byref(cfg))
             if nbytes == 0:

@@ -323,6 +323,26 @@ def test_host_and_device_state_paths_agree_and_contexts_are_independent(G):
     g1.close(); g2.close()
 
 
+def test_merged_and_separate_kicks_are_the_same_map(G):
+    """flags bit 0 keeps the closing kick of a substep and the opening kick of the next apart (orders 4, 6): same map,
+    rounding differs; both agree with the oracle (which never merges)."""
+    w = workloads.config4(n=513, order=6)
+    o = oracle.Sim(w, cap=200000)
+    o.step(3, w["dt"], 6)
+    xo, vo = o.state()
+    res = []
+    for flags in (0, 1):
+        g = G.from_workload(w, flags=flags)
+        g.step(3, w["dt"], 6)
+        x, v = g.get_state_host()
+        assert g.status() == 0
+        assert relerr(x, xo).max() < STATE_TOL and relerr(v, vo).max() < STATE_TOL
+        res.append((x, v, g.counters()["force_evals"]))
+        g.close()
+    assert relerr(res[0][0], res[1][0]).max() < 1e-11
+    assert res[0][2] == 3 * 8 and res[1][2] == 3 * 14       # 7 maps: 8 merged kicks, 14 separate ones
+
+
 def test_runs_are_bit_reproducible_with_and_without_dependent_launch(G):
     """No result depends on the order in which blocks or atomics happen to run: two runs of the same steps, and a run with
     programmatic dependent launch switched off (GENGA_NO_PDL=1, read at genga_create), give bit-identical states."""
