@@ -66,16 +66,16 @@ __device__ __forceinline__ double rcp_fast(double x)
 // Bulirsch-Stoer evaluates it on a latency-bound dependent chain.
 __device__ __forceinline__ double direct_scale(double d2, double rcij, double irc09, double Gmj)
 {
+    // 1 - W = 1 - K + r dK/dr = [D^2 - y^2 D + 2 r y (1 - y) / (0.9 rc)] / D^2,  D = 2 y^2 - 2 y + 1:
+    // one reciprocal (of D^2) at the end of the chain, the numerator is ready before it
     double rinv = rsqrt_fast(d2);
     double dd = d2 * rinv;
     double y = (dd - 0.1 * rcij) * irc09;
     double w1 = 1.0;
     if (y > 0.0) {
         double D = fma(2.0 * y, y - 1.0, 1.0);
-        double iD = rcp_fast(D);
-        double yD = y * iD;                                   // K = y yD
-        double dK = 2.0 * (1.0 - y) * (yD * iD) * irc09;
-        w1 = 1.0 - fma(y, yD, -dd * dK);
+        double N = fma(D, D - y * y, 2.0 * (dd * irc09) * (y * (1.0 - y)));
+        w1 = N * rcp_fast(D * D);
     }
     return Gmj * (rinv * rinv) * rinv * w1;
 }
@@ -88,10 +88,8 @@ __device__ __forceinline__ double direct_scale_nb(double d2, double rcij, double
     double dd = d2 * rinv;
     double y = (dd - 0.1 * rcij) * irc09;
     double D = fma(2.0 * y, y - 1.0, 1.0);                    // >= 1/2 for every y
-    double iD = rcp_fast(D);
-    double yD = y * iD;                                       // K = y yD
-    double dK = 2.0 * (1.0 - y) * (yD * iD) * irc09;
-    double w1 = 1.0 - fma(y, yD, -dd * dK);
+    double N = fma(D, D - y * y, 2.0 * (dd * irc09) * (y * (1.0 - y)));
+    double w1 = N * rcp_fast(D * D);
     w1 = y > 0.0 ? w1 : 1.0;
     return Gmj * (rinv * rinv) * rinv * w1;
 }
