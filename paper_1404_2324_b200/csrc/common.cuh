@@ -68,8 +68,12 @@ __device__ __forceinline__ double direct_scale(double d2, double rcij, double ir
 {
     // 1 - W = 1 - K + r dK/dr = [D^2 - y^2 D + 2 r y (1 - y) / (0.9 rc)] / D^2,  D = 2 y^2 - 2 y + 1:
     // one reciprocal (of D^2) at the end of the chain, the numerator is ready before it
-    double rinv = rsqrt_fast(d2);
-    double dd = d2 * rinv;
+    // d and 1/d from the same seed, d without the extra multiply at the end of the chain
+    const double y0 = rsqrt_seed(d2), t0 = d2 * y0;
+    const double e0 = fma(-t0, y0, 1.0);
+    const double pe = fma(0.375, e0, 0.5) * e0;
+    double dd = fma(pe, t0, t0);                                  // d2 y0 (1 + e/2 + 3 e^2/8) = sqrt(d2)
+    double rinv = fma(pe, y0, y0);
     double y = (dd - 0.1 * rcij) * irc09;
     double w1 = 1.0;
     if (y > 0.0) {
@@ -84,8 +88,12 @@ __device__ __forceinline__ double direct_scale(double d2, double rcij, double ir
 // together; `in` selects afterwards).
 __device__ __forceinline__ double direct_scale_nb(double d2, double rcij, double irc09, double Gmj)
 {
-    double rinv = rsqrt_fast(d2);
-    double dd = d2 * rinv;
+    // d and 1/d from the same seed, d without the extra multiply at the end of the chain
+    const double y0 = rsqrt_seed(d2), t0 = d2 * y0;
+    const double e0 = fma(-t0, y0, 1.0);
+    const double pe = fma(0.375, e0, 0.5) * e0;
+    double dd = fma(pe, t0, t0);                                  // d2 y0 (1 + e/2 + 3 e^2/8) = sqrt(d2)
+    double rinv = fma(pe, y0, y0);
     double y = (dd - 0.1 * rcij) * irc09;
     double D = fma(2.0 * y, y - 1.0, 1.0);                    // >= 1/2 for every y
     double N = fma(D, D - y * y, 2.0 * (dd * irc09) * (y * (1.0 - y)));
