@@ -129,25 +129,24 @@ __device__ __forceinline__ void bw_rhs2_seg8(const double (&qA)[3], const double
 // T[k][0], writes the diagonal T[k][k] back and returns the squared last corrections (T[k][k] - T[k][k-1])^2.
 __device__ __forceinline__ void bw_neville(BwSmem &W, int c, int b, double (&d2)[BS_KMAX])
 {
-    double row[BS_KMAX] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    // column by column, rows from the bottom up, in place: T[k] <- T[k][j] = T[k][j-1] + (T[k][j-1] - T[k-1][j-1]) / ((n_k / n_{k-j})^2 - 1).
+    // The updates of one column are independent of each other, so the dependent chain is 7 steps, not 28.
+    double T[BS_KMAX];
 #pragma unroll
-    for (int k = 0; k < BS_KMAX; ++k) {
-        double cur = W.tab[k][c][b], prev = row[0], diff = 0.0;
-        row[0] = cur;
+    for (int k = 0; k < BS_KMAX; ++k) { T[k] = W.tab[k][c][b]; d2[k] = 0.0; }
 #pragma unroll
-        for (int j = 1; j <= k; ++j) {
+    for (int j = 1; j < BS_KMAX; ++j) {
+#pragma unroll
+        for (int k = BS_KMAX - 1; k >= j; --k) {
             const double ratio = double(k + 1) / double(k - j + 1);
             const double iden = 1.0 / (ratio * ratio - 1.0);
-            double tmp = row[j];
-            double nxt = cur + (cur - prev) * iden;
-            diff = nxt - cur;
-            cur = nxt;
-            row[j] = cur;
-            prev = tmp;
+            const double nxt = T[k] + (T[k] - T[k - 1]) * iden;
+            if (k == j) { const double diff = nxt - T[k]; d2[k] = diff * diff; }
+            T[k] = nxt;
         }
-        W.tab[k][c][b] = cur;                                     // T[k][k]
-        d2[k] = diff * diff;
     }
+#pragma unroll
+    for (int k = 0; k < BS_KMAX; ++k) W.tab[k][c][b] = T[k];      // T[k][k]
 }
 
 // Integrate one group over h.  Lane = S * g + b; Y = state of body b (same in every segment; any
