@@ -57,8 +57,9 @@ typedef struct {
     int32_t n_massive;  /* per system: 1..2048 (mode 0), 1..32 (mode 1), 1..16 (mode 2); L188  */
     int64_t n_test;     /* mode 1 only: 0..10^6 test particles; else 0                        */
     int32_t n_systems;  /* mode 2 only: 1..100000; else 1                                     */
-    int32_t flags;      /* bit 0: do not merge the closing and the next opening kick (L144,
-                           L266); the result is the same map, this only selects the schedule  */
+    int32_t flags;      /* bit 0: do not merge the closing kick of a substep with the opening kick
+                           of the next substep of the same step (orders 4, 6; modes 0, 2; L170);
+                           the result is the same map, this only selects the schedule         */
     double G;           /* gravitational constant                                            */
     double n1, n2;      /* critical-radius parameters of Eq. 6 (L94-96); usually 3 and 0.4   */
     double bs_eps;      /* Bulirsch-Stoer relative tolerance (L116 "machine precision")      */
@@ -74,6 +75,8 @@ size_t genga_workspace_bytes(const genga_config *cfg);
 
 /* Create / destroy a context.  genga_create does not touch the device state arrays;
  * call genga_set_state before anything else. */
+/* Environment: GENGA_NO_PDL=1 (read by genga_create) launches the kernels of a step without programmatic
+ * dependent launch; results are bit-identical either way. */
 int genga_create(const genga_config *cfg, genga_ctx **out);
 int genga_destroy(genga_ctx *ctx);
 
