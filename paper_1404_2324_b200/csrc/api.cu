@@ -306,7 +306,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
     DevState dm = d;                                          // the massive bodies alone (mode 1)
     dm.ntot = d.nm;
     if (d.mode == GENGA_MODE_TEST_PARTICLE) { launch_k(c->pdl, k_begin_map, c->sms, 256, 0, st, d); LAUNCH(c); }
-    if (d.mode == GENGA_MODE_TEST_PARTICLE || first) { launch_k(c->pdl, k_reset_counters, 1, 32, 0, st, d); LAUNCH(c); }   // later maps: closing k_sun
+    if (d.mode == GENGA_MODE_TEST_PARTICLE) { launch_k(c->pdl, k_reset_counters, 1, 32, 0, st, d); LAUNCH(c); }   // modes 0, 2: k_rcrit (first map), closing k_sun (later maps)
     if (tp) {
         // particles: kick, Sun kick and drift in one pass (k_tp_front); the massive bodies as in mode 0
         launch_kick(c, 0.5 * h, 1, nullptr); LAUNCH(c);
@@ -378,9 +378,9 @@ static void enqueue_step(genga_ctx *c, double dt, int order)
     if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {    // the particles' rc: k_tp_front of the first map
         DevState dm = d;
         dm.ntot = d.nm;
-        launch_k(c->pdl, k_rcrit, nblk(d.nm, 128), 128, 0, c->st, dm, dt); LAUNCH(c);
+        launch_k(c->pdl, k_rcrit, nblk(d.nm, 128), 128, 0, c->st, dm, dt, 0); LAUNCH(c);
     } else {
-        launch_k(c->pdl, k_rcrit, nblk(d.ntot, 128), 128, 0, c->st, d, dt); LAUNCH(c);
+        launch_k(c->pdl, k_rcrit, nblk(d.ntot, 128), 128, 0, c->st, d, dt, d.mode != GENGA_MODE_TEST_PARTICLE); LAUNCH(c);
     }
     const bool merge = !(c->cfg.flags & 1) && d.mode != GENGA_MODE_TEST_PARTICLE;
     for (int k = 0; k < nw; ++k)
@@ -545,7 +545,7 @@ extern "C" __attribute__((visibility("default"))) int genga_accelerations(genga_
 {
     if (!c || !a || dt == 0.0) return GENGA_EINVAL;
     DevState &d = c->d;
-    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt);
+    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt, 0);
     if (d.mode == GENGA_MODE_TEST_PARTICLE) { k_begin_map<<<c->sms, 256, 0, c->st>>>(d); c->launches += 1; }
     k_reset_counters<<<1, 32, 0, c->st>>>(d);
     c->launches += 2;
@@ -577,7 +577,7 @@ extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ct
     if (which >= 3 && !(d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm)) return GENGA_EINVAL;
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
-    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt);
+    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt, 0);
     c->launches += 1;
     int per = 1;
     for (int r = -3; r < reps; ++r) {

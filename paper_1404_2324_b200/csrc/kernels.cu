@@ -41,10 +41,14 @@ __global__ void k_reset_counters(DevState d)
 // own velocity (L96), R_H,i = a_i (m_i / 3 m0)^(1/3) with a_i from the vis-viva relation
 // (r_i if unbound); test particles have R_H = 0.  Also stores 9 rc^2, the squared precheck
 // distance (L142: "increasing the critical radius by a factor of three").
-__global__ void k_rcrit(DevState d, double tau)
+__global__ void k_rcrit(DevState d, double tau, int reset)
 {
     pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (reset && i == 0) {                                // start of a step: forget the previous step's lists (modes 0, 2)
+        d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
+        d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0;
+    }
     if (i >= d.ntot) return;
     double x = d.x[i], y = d.y[i], z = d.z[i], vx = d.vx[i], vy = d.vy[i], vz = d.vz[i], m = d.m[i];
     double m0 = d.m0[system_of(d, i)];

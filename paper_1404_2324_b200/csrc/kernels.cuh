@@ -17,7 +17,7 @@ constexpr int BCB_MAXN = 256, BCB_THREADS = 512, BCB_CS = 8;
 
 __global__ void k_begin_map(DevState d);
 __global__ void k_reset_counters(DevState d);
-__global__ void k_rcrit(DevState d, double tau);
+__global__ void k_rcrit(DevState d, double tau, int reset);
 __global__ void k_kick(DevState d, double h, int record, int ni, double *aout);
 size_t kick_smem_bytes();
 __global__ void k_tp_kick(DevState d, double h, int record, double *aout);
