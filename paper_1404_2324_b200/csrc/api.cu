@@ -262,13 +262,13 @@ static void enqueue_kick(genga_ctx *c, double h, int record, double *aout)
     }
 }
 
-static void enqueue_sun(genga_ctx *c, double h, int reset = 0, bool after_bs = false)
+static void enqueue_sun(genga_ctx *c, double h, int reset = 0, bool after_bs = false, double hdrift = 0.0)
 {
     DevState &d = c->d;
     // after Bulirsch-Stoer: a plain launch, so that the kernels behind it are not scheduled (and their blocks do not
     // sit on the SMs) while the groups are still being integrated
     if (d.mode != GENGA_MODE_TEST_PARTICLE) {                 // one launch: every block forms the momentum itself
-        launch_k(c->pdl && !after_bs, k_sun, nblk(d.ntot, 256), 256, 0, c->st, d, h, reset);
+        launch_k(c->pdl && !after_bs, k_sun, nblk(d.ntot, 256), 256, 0, c->st, d, h, reset, hdrift);
         LAUNCH(c);
         return;
     }
@@ -316,8 +316,11 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         launch_k(c->pdl, k_drift, nblk(d.nm, 128), 128, 0, st, dm, h); LAUNCH(c);
     } else {
         if (!opened) enqueue_kick(c, 0.5 * h, 1, nullptr);        // else: done by the previous map's merged kick
-        enqueue_sun(c, 0.5 * h);
-        launch_k(c->pdl, k_drift, nblk(d.ntot, 128), 128, 0, st, d, h); LAUNCH(c);
+        if (d.mode != GENGA_MODE_TEST_PARTICLE) enqueue_sun(c, 0.5 * h, 0, false, h);   // Sun kick and drift in one launch
+        else {
+            enqueue_sun(c, 0.5 * h);
+            launch_k(c->pdl, k_drift, nblk(d.ntot, 128), 128, 0, st, d, h); LAUNCH(c);
+        }
     }
     const int pair_blocks = (int)std::min<long long>((d.cap + 127) / 128, 16LL * c->sms);   // grid-stride over the candidates; enough warps to cover the gather latency when there are 10^6 of them (mode 1)
     launch_k(c->pdl, k_confirm, pair_blocks, 128, 0, st, d, h); LAUNCH(c);

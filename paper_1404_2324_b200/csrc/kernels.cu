@@ -537,7 +537,8 @@ __global__ void k_shift(DevState d, double *ax, double *ay, double *az, double f
 // Sun kick in one launch (modes 0 and 2): every block forms s = sum m V itself -- mode 0: the block sums the
 // massive bodies in a fixed order (at most 8 per thread, then a tree); mode 2: a thread sums the <= 16 bodies of
 // its own system -- and shifts its bodies.  reset != 0: thread 0 also zeroes the per-map counters (the map is over).
-__global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset)
+// hdrift != 0: the Kepler drift over hdrift (operator A, as k_drift) follows in the same thread.
+__global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset, double hdrift)
 {
     pdl_sync();
     __shared__ double red[3][8];
@@ -578,7 +579,14 @@ __global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset)
         if (i >= d.ntot) return;
     }
     const double g = h / m0;
-    d.x[i] = fma(g, sx, d.x[i]); d.y[i] = fma(g, sy, d.y[i]); d.z[i] = fma(g, sz, d.z[i]);
+    double x = fma(g, sx, d.x[i]), y = fma(g, sy, d.y[i]), z = fma(g, sz, d.z[i]);
+    if (hdrift != 0.0) {                                  // opening Sun kick: the Kepler drift follows in the same launch (k_drift)
+        double vx = d.vx[i], vy = d.vy[i], vz = d.vz[i];
+        d.x0[i] = x; d.y0[i] = y; d.z0[i] = z; d.vx0[i] = vx; d.vy0[i] = vy; d.vz0[i] = vz;
+        if (!kepler_drift(d.G * m0, hdrift, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
+        d.vx[i] = vx; d.vy[i] = vy; d.vz[i] = vz;
+    }
+    d.x[i] = x; d.y[i] = y; d.z[i] = z;
 }
 // out = in + f * psum / den  (coordinate maps at the ABI, L69)
 __global__ void k_shift_out(DevState d, const double *ix, const double *iy, const double *iz,
