@@ -534,6 +534,25 @@ __global__ void k_shift(DevState d, double *ax, double *ay, double *az, double f
     double g = f / den;
     ax[i] = fma(g, d.psum[4 * sys], ax[i]); ay[i] = fma(g, d.psum[4 * sys + 1], ay[i]); az[i] = fma(g, d.psum[4 * sys + 2], az[i]);
 }
+// root of i in the union-find forest of the group labels (larger roots hang under smaller ones)
+__device__ __forceinline__ int uf_find(const int *L, int i)
+{
+    int p = L[i];
+    while (p != i) { i = p; p = L[i]; }
+    return i;
+}
+// link the groups of a and b (atomicMin hooks; safe against concurrent links)
+__device__ __forceinline__ void uf_union(int *L, int a, int b)
+{
+    while (true) {
+        a = uf_find(L, a); b = uf_find(L, b);
+        if (a == b) break;
+        int hi = max(a, b), lo = min(a, b);
+        int old = atomicMin(&L[hi], lo);
+        if (old == hi) break;
+        a = old; b = lo;
+    }
+}
 // Sun kick in one launch (modes 0 and 2): every block forms s = sum m V itself -- mode 0: the block sums the
 // massive bodies in a fixed order (at most 8 per thread, then a tree); mode 2: a thread sums the <= 16 bodies of
 // its own system -- and shifts its bodies.  reset != 0: thread 0 also zeroes the per-map counters (the map is over).
@@ -550,6 +569,7 @@ __global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset, do
     double sx = 0.0, sy = 0.0, sz = 0.0, m0;
     if (d.mode == 2) {
         if (i >= d.ntot) return;
+        if (hdrift != 0.0) d.label[i] = i;                    // a new map: every body its own group (k_confirm links them)
         const int sys = i / d.nm, base = sys * d.nm;
         for (int k = 0; k < d.nm; ++k) {
             double m = d.m[base + k];
@@ -649,6 +669,7 @@ __global__ void __launch_bounds__(128) k_confirm(DevState d, double h)
             int idx = atomicAdd(&d.cnt[CI_NENC], 1);
             if (idx < d.cap) d.enc[idx] = p;
             else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+            if (d.mode == 2) uf_union(d.label, i, j);         // multi-system mode: grouping goes with the confirmation
             if (d.mode == 1 && j >= d.nm) {
                 unsigned old = atomicOr(&d.tpmask[j - d.nm], 1u << i);
                 if (old == 0u) {
@@ -665,43 +686,6 @@ __global__ void __launch_bounds__(128) k_confirm(DevState d, double h)
 // label = lowest member index.  Union-find with atomicMin hooks (larger root under smaller
 // root), then pointer jumping to the root -- the LINK iteration of the Appendix without the
 // repeat-until-unchanged sweep.
-__global__ void k_label_init(DevState d)
-{
-    pdl_sync();
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < d.nmtot) d.label[i] = i;
-}
-__device__ __forceinline__ int uf_find(const int *L, int i)
-{
-    int p = L[i];
-    while (p != i) { i = p; p = L[i]; }
-    return i;
-}
-__global__ void k_union(DevState d)
-{
-    pdl_sync();
-    const int ne = min(d.cnt[CI_NENC], (int)d.cap);
-    int *L = d.label;
-    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < ne; e += gridDim.x * blockDim.x) {
-        int2 p = d.enc[e];
-        if (d.mode == 1 && p.y >= d.nm) continue;       // particle pairs do not link massive bodies
-        int a = p.x, b = p.y;
-        while (true) {
-            a = uf_find(L, a); b = uf_find(L, b);
-            if (a == b) break;
-            int hi = max(a, b), lo = min(a, b);
-            int old = atomicMin(&L[hi], lo);
-            if (old == hi) break;
-            a = old; b = lo;
-        }
-    }
-}
-__global__ void k_flatten(DevState d)
-{
-    pdl_sync();
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < d.nmtot) d.label[i] = uf_find(d.label, i);
-}
 
 // exclusive scan of two ints per thread over a 1024-thread block
 __device__ __forceinline__ void block_scan2(int v0, int v1, int &e0, int &e1, int &total, int *wsum)
@@ -728,7 +712,7 @@ __device__ __forceinline__ void block_scan2(int v0, int v1, int &e0, int &e1, in
 // into a matrix", L565 -- here a CSR list), plus `gorder`: the group numbers by DECREASING size
 // (counting sort), the order in which the Bulirsch-Stoer kernels take them from their queue so
 // that the longest integrations start first.  One block of 1024 threads.
-// The labelling itself (k_label_init, k_union, k_flatten: same union-find, in shared memory) runs first in the same block.
+// The labelling itself (the same union-find, in shared memory) runs first in the same block.
 __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
 {
     pdl_sync();
@@ -976,10 +960,12 @@ __global__ void k_list_groups_multi(DevState d)
     pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (d.cnt[CI_NENC] == 0 || i >= d.ntot) return;
-    if (d.label[i] != i) return;
+    const int root = uf_find(d.label, i);                     // flatten on the way (values only move towards the root)
+    d.label[i] = root;
+    if (root != i) return;
     const int nm = d.nm, sys = i / nm, base = sys * nm;
     unsigned mask = 0u;
-    for (int k = 0; k < nm; ++k) if (d.label[base + k] == i) mask |= 1u << k;
+    for (int k = 0; k < nm; ++k) if (uf_find(d.label, base + k) == i) mask |= 1u << k;
     if (__popc(mask) < 2) return;
     int slot = atomicAdd(&d.cnt[CI_NGROUPS], 1);
     d.gorder[2 * slot] = sys; d.gorder[2 * slot + 1] = (int)mask;

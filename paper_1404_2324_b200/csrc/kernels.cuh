@@ -32,9 +32,6 @@ __global__ void k_shift_out(DevState d, const double *ix, const double *iy, cons
 __global__ void k_drift(DevState d, double h);
 __global__ void k_drift_arrays(long long n, double mu, double h, double *x, double *v, int *status);
 __global__ void k_confirm(DevState d, double h);
-__global__ void k_label_init(DevState d);
-__global__ void k_union(DevState d);
-__global__ void k_flatten(DevState d);
 __global__ void k_build_groups(DevState d);
 template <int MAXN, int THREADS, int CS> __global__ void k_bs_cluster(DevState d, double h, int qslot, int endslot);
 __global__ void k_bs_warp(DevState d, double h, int tp);
