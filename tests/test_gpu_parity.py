@@ -50,6 +50,8 @@ CASES = {
     "cfg2_ragged": lambda: workloads.config2(n_massive=5, n_test=1237),
     "cfg2_order4": lambda: dict(workloads.config2(n_test=3000), order=4),
     "cfg2_order6_ragged": lambda: dict(workloads.config2(n_massive=7, n_test=777), order=6),
+    # the paper's second test-particle workload: 32 massive bodies (the mode's maximum)
+    "cfg2_32massive": lambda: workloads.config2(n_massive=32, n_test=4000),
     "cfg3_order4": lambda: dict(workloads.config3(n_systems=17), order=4),
     "cfg3_small": lambda: workloads.config3(n_systems=33),
     "cfg3_7bodies": lambda: workloads.config3(n_systems=10, n_per=7),
@@ -72,7 +74,8 @@ def test_accelerations_rcrit_and_candidates(G, case):
 
 
 STEP_CASES = [("cfg0", 100), ("cfg1_full", 4), ("cfg1_ragged_777", 10), ("cfg4_full", 2), ("cfg4_513", 3),
-              ("cfg2_small", 8), ("cfg2_ragged", 8), ("cfg2_order4", 5), ("cfg2_order6_ragged", 3), ("cfg3_order4", 20), ("cfg3_small", 60), ("cfg3_7bodies", 60)]
+              ("cfg2_small", 8), ("cfg2_ragged", 8), ("cfg2_order4", 5), ("cfg2_order6_ragged", 3), ("cfg2_32massive", 6),
+              ("cfg3_order4", 20), ("cfg3_small", 60), ("cfg3_7bodies", 60)]
 
 
 @pytest.mark.parametrize("case,nsteps", STEP_CASES)
