@@ -30,8 +30,16 @@ FLOP_PER_INTERACTION = 20.0        # Nyland et al. convention, D
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x DFMA/clk/SM x 2 flop x max clock
 
 
-def workload(cfg_id):
-    w = workloads.CONFIGS[cfg_id]()
+def workload(cfg_id, rank=0, world=1):
+    """The configuration of BASELINE.json; under world > 1 the particle and multi-system modes take a global
+    workload world times as large (weak scaling) and this rank's shard of it (workloads.shard: no collective);
+    the massive mode runs replicas."""
+    if world > 1 and cfg_id == 2:
+        w = workloads.shard(workloads.config2(n_test=1_000_000 * world), rank, world)
+    elif world > 1 and cfg_id == 3:
+        w = workloads.shard(workloads.config3(n_systems=4096 * world), rank, world)
+    else:
+        w = workloads.CONFIGS[cfg_id]()
     name = {0: "cfg0 massive N=15", 1: "cfg1 planetesimal disc N=2048 massive, order 2, dt=6d",
             2: "cfg2 8 massive + 1e6 test particles", 3: "cfg3 4096 systems x 16",
             4: "cfg4 annulus N=2048 order 4, dt=2d"}[cfg_id]
@@ -46,7 +54,8 @@ def interactions_per_step(w, merged=True):
     if w["mode"] == 2:
         per = w["n_systems"] * nm * (nm - 1)
     else:
-        per = nm * (nm - 1) + w["n_test"] * nm
+        # the massive bodies are replicated on every rank of a sharded run: counted once, on rank 0
+        per = (nm * (nm - 1) if w.get("shard", (0,))[0] == 0 else 0) + w["n_test"] * nm
     return per * evals, evals
 
 
@@ -156,7 +165,7 @@ def run_gpu(args):
     dev = torch.device("cuda", local)
     torch.cuda.set_device(dev)
 
-    w, name = workload(args.config)
+    w, name = workload(args.config, rank, world)
     per_step, evals = interactions_per_step(w)
     g = G.from_workload(w, device=str(dev))
     dt, order = w["dt"], w["order"]
@@ -288,9 +297,11 @@ def run_gpu(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": name, "n_massive": w["n_massive"], "order": w["order"], "dt_days": w["dt"] / workloads.DAY,
                        "force_evals_per_step": evals, "l2": "flushed (512 MiB fill) before every timed step",
-                       "parallelism": "replicas only" if world > 1 else "1 gpu"},
-            "steps_per_s": args.steps * world / tmax,
-            "resident": {"steps_per_s": nres * world / res_max, "value": res_units / res_max,
+                       "parallelism": ("1 gpu" if world == 1 else "replicas only" if w["mode"] == 0 else
+                                       "particles sharded, massive bodies replicated, no collective" if w["mode"] == 1
+                                       else "systems sharded, no collective")},
+            "steps_per_s": args.steps * (world if w["mode"] == 0 else 1) / tmax,     # replicas step independently
+            "resident": {"steps_per_s": nres * (world if w["mode"] == 0 else 1) / res_max, "value": res_units / res_max,
                          "note": "16-step CUDA graphs back to back, state resident in L2 (no flush)"},
             "e2e": {"value": e2e_units / e2e_max, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": ne2e, "ms_per_step": 1e3 * e2e_max / ne2e},

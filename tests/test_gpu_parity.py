@@ -192,8 +192,7 @@ def test_large_group_block_paths(G, n, n2, min_group):
     g.close()
 
 
-def test_test_particle_groups(G):
-    """particles placed next to a planet: particle groups form, only the particle is written back."""
+def _particles_next_to_a_planet():
     w = workloads.config2(n_massive=3, n_test=400)
     x, v = w["x"].copy(), w["v"].copy()
     V = oracle.helio_to_demo(1.0, w["m"], v, 3)
@@ -202,6 +201,47 @@ def test_test_particle_groups(G):
         f = (0.05 + 0.01 * (k + 1)) * rc1 / np.linalg.norm(x[:, 1])
         x[:, 3 + k] = x[:, 1] * (1 + f); v[:, 3 + k] = v[:, 1] * (1 - 0.5 * f)
     w["x"], w["v"] = x, v
+    return w
+
+
+@pytest.mark.parametrize("case,world", [("tp_groups", 3), ("cfg2_ragged", 4), ("cfg3_small", 5)])
+def test_sharded_runs_are_the_unsharded_run_bit_for_bit(G, case, world):
+    """particles / systems partitioned over ranks with no collective (workloads.shard).  A particle
+    never acts on anything and a system never sees another one, so every shard must reproduce its slice of the
+    unsharded run exactly, the replicated massive bodies included."""
+    full = _particles_next_to_a_planet() if case == "tp_groups" else CASES[case]()
+    nm, nsteps = full["n_massive"], 6
+    g = G.from_workload(full)
+    g.step(nsteps, full["dt"], full["order"])
+    xf, vf = g.get_state_host()
+    assert g.status() == 0
+    nenc_full = len(g.encounters()[0])
+    g.close()
+    nenc = 0
+    for r in range(world):
+        w = workloads.shard(full, r, world)
+        g = G.from_workload(w)
+        g.step(nsteps, w["dt"], w["order"])
+        xs, vs = g.get_state_host()
+        assert g.status() == 0
+        pairs = g.encounters()[0]
+        lo, hi = w["shard"][2:]
+        if full["mode"] == 1:
+            assert np.array_equal(xs[:, :nm], xf[:, :nm]) and np.array_equal(vs[:, :nm], vf[:, :nm])
+            assert np.array_equal(xs[:, nm:], xf[:, nm + lo:nm + hi]) and np.array_equal(vs[:, nm:], vf[:, nm + lo:nm + hi])
+            nenc += sum(1 for p in pairs if p[1] >= nm) + (sum(1 for p in pairs if p[1] < nm) if r == 0 else 0)
+        else:
+            assert np.array_equal(xs, xf[:, lo * nm:hi * nm]) and np.array_equal(vs, vf[:, lo * nm:hi * nm])
+            nenc += len(pairs)
+        g.close()
+    assert nenc == nenc_full
+    if case == "tp_groups":
+        assert nenc_full > 50
+
+
+def test_test_particle_groups(G):
+    """particles placed next to a planet: particle groups form, only the particle is written back."""
+    w = _particles_next_to_a_planet()
     g = G.from_workload(w)
     o = oracle.Sim(w)
     g.step(6, w["dt"], 2)

@@ -137,3 +137,39 @@ def config4(seed=4, n=2048, order=4):
 
 
 CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4}
+
+
+def shard_bounds(n, rank, world):
+    """Balanced contiguous split of n units over world ranks: [lo, hi) of this rank."""
+    return (n * rank) // world, (n * (rank + 1)) // world
+
+
+def shard(w, rank, world):
+    """The part of workload w that rank `rank` of `world` integrates (no data-path collective).
+
+    Test-particle mode: the massive bodies are replicated on every rank and integrated redundantly, the
+    particles are partitioned.  Multi-system mode: the systems are partitioned.  Massive mode does not
+    shard (every force evaluation needs all positions): ValueError -- replicas only.
+    """
+    if not 0 <= rank < world:
+        raise ValueError("rank %d outside world %d" % (rank, world))
+    if w["mode"] == 0:
+        raise ValueError("massive mode does not shard: replicas only")
+    out = dict(w)
+    if w["mode"] == 1:
+        nm = w["n_massive"]
+        lo, hi = shard_bounds(w["n_test"], rank, world)
+        idx = np.concatenate([np.arange(nm), nm + np.arange(lo, hi)])
+        out["n_test"] = hi - lo
+    else:
+        nm = w["n_massive"]
+        lo, hi = shard_bounds(w["n_systems"], rank, world)
+        idx = np.arange(lo * nm, hi * nm)
+        out["n_systems"] = hi - lo
+        out["m0"] = np.ascontiguousarray(w["m0"][lo:hi])
+    out["m"] = np.ascontiguousarray(w["m"][idx])
+    out["radius"] = np.ascontiguousarray(w["radius"][idx])
+    out["x"] = np.ascontiguousarray(w["x"][:, idx])
+    out["v"] = np.ascontiguousarray(w["v"][:, idx])
+    out["shard"] = (rank, world, int(lo), int(hi))
+    return out
