@@ -86,7 +86,10 @@ int genga_destroy(genga_ctx *ctx);
  *   heliocentric positions / velocities.
  * genga_set_state: all pointers DEVICE.  genga_set_state_host: all pointers HOST (pinned
  * or pageable); the copies are enqueued on the stream and the call returns after they and
- * the conversion to democratic coordinates have completed. */
+ * the conversion to democratic coordinates have completed.  States of up to 512 KB (and a
+ * non-NULL radius) are packed into a pinned image owned by the context and moved with ONE
+ * copy (genga_get_state_host likewise); larger ones are copied array by array straight
+ * from the caller's buffers. */
 int genga_set_state(genga_ctx *ctx, const double *m0, const double *m, const double *radius,
                     const double *x, const double *v);
 int genga_set_state_host(genga_ctx *ctx, const double *m0, const double *m, const double *radius,

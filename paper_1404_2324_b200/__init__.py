@@ -91,7 +91,7 @@ def _chk(code, where):
 
 
 def _hp(a):
-    return a.ctypes.data_as(C.c_void_p)
+    return a.ctypes.data          # the address as an int: the argtypes make it a void*; the caller keeps `a` alive
 
 
 class Genga:

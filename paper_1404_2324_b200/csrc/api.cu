@@ -45,6 +45,8 @@ struct genga_ctx {
     int bs_big_clusters;        // grid size (in clusters) of the Bulirsch-Stoer cluster kernel
     int *exp_labels;            // device [np]
     double *eout;               // device [4*nsys]
+    double *hstage;             // pinned host image of x..vz0, m, radius, m0 (small states only, else nullptr)
+    int *hstatus;               // pinned host copy of the status word
     struct GraphEntry { cudaGraphExec_t exec; long long launches; };
     std::map<GraphKey, GraphEntry> graphs;
     long long steps, force_evals, interactions, launches;
@@ -78,10 +80,13 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
     t.mode = c->mode; t.nm = nm; t.ntot = (int)ntot; t.nsys = nsys; t.np = np; t.npm = npm;
     t.nmtot = c->mode == GENGA_MODE_MULTI_SYSTEM ? (int)ntot : nm;
     t.G = c->G; t.n1 = c->n1; t.n2 = c->n2; t.eps = c->bs_eps; t.cap = c->max_pairs;
-    double **arrs[] = {&t.x, &t.y, &t.z, &t.vx, &t.vy, &t.vz, &t.m, &t.radius, &t.rc, &t.c9,
-                       &t.x0, &t.y0, &t.z0, &t.vx0, &t.vy0, &t.vz0};
+    // the arrays the host reads and writes lie in one piece, in this order (np is a multiple of 128, so there are no
+    // gaps): x y z vx0 vy0 vz0 | m radius | m0 -- genga_set_state_host / genga_get_state_host move them with one copy
+    double **arrs[] = {&t.x, &t.y, &t.z, &t.vx0, &t.vy0, &t.vz0, &t.m, &t.radius};
     for (auto a : arrs) *a = (double *)take(sizeof(double) * np);
     t.m0 = (double *)take(sizeof(double) * nsys);
+    double **arrs2[] = {&t.vx, &t.vy, &t.vz, &t.rc, &t.c9, &t.x0, &t.y0, &t.z0};
+    for (auto a : arrs2) *a = (double *)take(sizeof(double) * np);
     t.psum = (double *)take(sizeof(double) * 4 * nsys);
     *eout = (double *)take(sizeof(double) * 4 * nsys);
     if (c->mode != GENGA_MODE_MULTI_SYSTEM) {
@@ -111,6 +116,12 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
     if (d) *d = t;
     return off;
 }
+
+// Host image of the state (the piece of the workspace that starts at d.x): small states go through it, so that a host
+// call is one copy whatever the caller's buffers are (pageable or pinned); large ones are copied array by array
+// straight from the caller's buffers.
+static const size_t HOST_STAGE_MAX = 512u << 10;
+static size_t stage_bytes(const DevState &d) { return sizeof(double) * (8 * (size_t)d.np + (size_t)d.nsys); }
 
 extern "C" __attribute__((visibility("default"))) size_t genga_workspace_bytes(const genga_config *cfg)
 {
@@ -142,6 +153,7 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     c->bs_big_clusters = std::max(1, c->sms / BCB_CS);
     c->steps = c->force_evals = c->interactions = c->launches = 0;
     c->acc = 0;
+    c->hstage = nullptr; c->hstatus = nullptr;
     size_t need = carve(cfg, (char *)cfg->workspace, &c->d, &c->exp_labels, &c->eout, c->sms);
     if (need > cfg->workspace_bytes) { delete c; return GENGA_EINVAL; }
     cudaError_t e = cudaMemsetAsync(cfg->workspace, 0, need, c->st);
@@ -153,6 +165,11 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming);
     }
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaHostAlloc((void **)&c->hstatus, sizeof(int), cudaHostAllocDefault);
+    if (e == cudaSuccess && stage_bytes(c->d) <= HOST_STAGE_MAX) {
+        e = cudaHostAlloc((void **)&c->hstage, stage_bytes(c->d), cudaHostAllocDefault);
+        if (e == cudaSuccess) memset(c->hstage, 0, stage_bytes(c->d));
+    }
     if (e != cudaSuccess) { delete c; snprintf(g_cuda_err, sizeof g_cuda_err, "create: %s", cudaGetErrorString(e)); return GENGA_ECUDA; }
     *out = c;
     return GENGA_OK;
@@ -164,6 +181,8 @@ extern "C" __attribute__((visibility("default"))) int genga_destroy(genga_ctx *c
     for (auto &kv : c->graphs) cudaGraphExecDestroy(kv.second.exec);
     for (int k = 0; k < 2; ++k) { cudaStreamDestroy(c->aux[k]); cudaEventDestroy(c->ev_join[k]); }
     cudaEventDestroy(c->ev_fork);
+    if (c->hstage) cudaFreeHost(c->hstage);
+    if (c->hstatus) cudaFreeHost(c->hstatus);
     delete c;
     return GENGA_OK;
 }
@@ -230,6 +249,23 @@ extern "C" __attribute__((visibility("default"))) int genga_set_state(genga_ctx 
 extern "C" __attribute__((visibility("default"))) int genga_set_state_host(genga_ctx *c, const double *m0, const double *m, const double *radius,
                                     const double *x, const double *v)
 {
+    if (c && c->hstage && m0 && m && radius && x && v) {       // small state: pack, one copy
+        DevState &d = c->d;
+        const size_t n = (size_t)d.ntot, np = (size_t)d.np, B = sizeof(double);
+        double *h = c->hstage;
+        for (int k = 0; k < 3; ++k) {
+            memcpy(h + k * np, x + k * n, B * n);
+            memcpy(h + (3 + k) * np, v + k * n, B * n);
+        }
+        memcpy(h + 6 * np, m, B * n);
+        memcpy(h + 7 * np, radius, B * n);
+        memcpy(h + 8 * np, m0, B * d.nsys);
+        CK(cudaMemcpyAsync(d.x, h, stage_bytes(d), cudaMemcpyHostToDevice, c->st));
+        enqueue_helio_to_demo(c);
+        CK(cudaGetLastError());
+        CK(cudaStreamSynchronize(c->st));
+        return GENGA_OK;
+    }
     int r = set_state_impl(c, m0, m, radius, x, v, cudaMemcpyHostToDevice);
     if (r) return r;
     CK(cudaStreamSynchronize(c->st));
@@ -449,9 +485,9 @@ extern "C" __attribute__((visibility("default"))) int genga_step(genga_ctx *c, i
 
 static int latch(genga_ctx *c)
 {
-    int st = 0;
-    CK(cudaMemcpyAsync(&st, c->d.cnt + CI_STATUS, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaMemcpyAsync(c->hstatus, c->d.cnt + CI_STATUS, sizeof(int), cudaMemcpyDeviceToHost, c->st));
     CK(cudaStreamSynchronize(c->st));
+    const int st = *c->hstatus;
     if (st) {
         CK(cudaMemsetAsync(c->d.cnt + CI_STATUS, 0, sizeof(int), c->st));
         if (st & ERRBIT_KEPLER) return GENGA_EKEPLER;
@@ -494,6 +530,21 @@ extern "C" __attribute__((visibility("default"))) int genga_get_state(genga_ctx 
 }
 extern "C" __attribute__((visibility("default"))) int genga_get_state_host(genga_ctx *c, double *x, double *v)
 {
+    if (c && c->hstage && x && v) {                            // small state: one copy, unpack after the latch's sync
+        DevState &d = c->d;
+        const size_t n = (size_t)d.ntot, np = (size_t)d.np, B = sizeof(double);
+        k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx, d.vy, d.vz);
+        k_shift_out<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0);
+        c->launches += 2;
+        CK(cudaMemcpyAsync(c->hstage, d.x, 6 * B * np, cudaMemcpyDeviceToHost, c->st));
+        CK(cudaGetLastError());
+        int r = latch(c);
+        for (int k = 0; k < 3; ++k) {
+            memcpy(x + k * n, c->hstage + k * np, B * n);
+            memcpy(v + k * n, c->hstage + (3 + k) * np, B * n);
+        }
+        return r;
+    }
     int r = get_state_impl(c, x, v, cudaMemcpyDeviceToHost);
     if (r) return r;
     return latch(c);
