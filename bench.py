@@ -221,7 +221,11 @@ def run_gpu(args):
     xh = torch.empty((3, g.ntot), dtype=torch.float64).pin_memory().numpy()
     vh = torch.empty((3, g.ntot), dtype=torch.float64).pin_memory().numpy()
     xh[:], vh[:] = w["x"], w["v"]
-    m0h, mh, rh = w["m0"], w["m"], w["radius"]
+    def pinned(a):
+        t = torch.empty(a.shape, dtype=torch.float64).pin_memory().numpy()
+        t[...] = a
+        return t
+    m0h, mh, rh = pinned(w["m0"]), pinned(w["m"]), pinned(w["radius"])
     for _ in range(3):
         g.set_state_host(m0h, mh, rh, xh, vh); g.step(1, dt, order); g.get_state_host(xh, vh)
     ne2e = min(args.steps, 200)
