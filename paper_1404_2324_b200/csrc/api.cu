@@ -212,7 +212,7 @@ static int red_threads(int nm) { return std::min(1024, std::max(32, (int)up((siz
 static void enqueue_helio_to_demo(genga_ctx *c)
 {
     DevState &d = c->d;
-    k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx0, d.vy0, d.vz0);
+    k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx0, d.vy0, d.vz0, 0.0);
     k_shift_out<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx0, d.vy0, d.vz0, d.vx, d.vy, d.vz, -1.0, 1);
     c->launches += 2;
 }
@@ -308,7 +308,7 @@ static void enqueue_sun(genga_ctx *c, double h, int reset = 0, bool after_bs = f
         LAUNCH(c);
         return;
     }
-    launch_k(c->pdl, k_momentum, d.nsys, red_threads(d.nm), 0, c->st, d, d.vx, d.vy, d.vz);
+    launch_k(c->pdl, k_momentum, d.nsys, red_threads(d.nm), 0, c->st, d, d.vx, d.vy, d.vz, 0.0);
     launch_k(c->pdl, k_shift, nblk(d.ntot, 256), 256, 0, c->st, d, d.x, d.y, d.z, h, 0);
     LAUNCH(c); LAUNCH(c);
 }
@@ -341,21 +341,22 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
     const bool tp = d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm;
     DevState dm = d;                                          // the massive bodies alone (mode 1)
     dm.ntot = d.nm;
-    if (d.mode == GENGA_MODE_TEST_PARTICLE) { launch_k(c->pdl, k_begin_map, c->sms, 256, 0, st, d); LAUNCH(c); }
-    if (d.mode == GENGA_MODE_TEST_PARTICLE) { launch_k(c->pdl, k_reset_counters, 1, 32, 0, st, d); LAUNCH(c); }   // modes 0, 2: k_rcrit (first map), closing k_sun (later maps)
+    if (d.mode == GENGA_MODE_TEST_PARTICLE && !first) {       // first map: inside k_rcrit; modes 0, 2: k_rcrit (first map), closing k_sun (later maps)
+        launch_k(c->pdl, k_begin_map, c->sms, 256, 0, st, d); LAUNCH(c);
+        launch_k(c->pdl, k_reset_counters, 1, 32, 0, st, d); LAUNCH(c);
+    }
     if (tp) {
         // particles: kick, Sun kick and drift in one pass (k_tp_front); the massive bodies as in mode 0
         launch_kick(c, 0.5 * h, 1, nullptr); LAUNCH(c);
-        launch_k(c->pdl, k_momentum, 1, red_threads(d.nm), 0, st, d, d.vx, d.vy, d.vz); LAUNCH(c);
+        launch_k(c->pdl, k_momentum, 1, red_threads(d.nm), 0, st, d, d.vx, d.vy, d.vz, 0.0); LAUNCH(c);
         launch_k(c->pdl, k_tp_front, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h, tau, first); LAUNCH(c);
-        launch_k(c->pdl, k_shift, nblk(d.nm, 256), 256, 0, st, dm, d.x, d.y, d.z, 0.5 * h, 0); LAUNCH(c);
-        launch_k(c->pdl, k_drift, nblk(d.nm, 128), 128, 0, st, dm, h); LAUNCH(c);
+        launch_k(c->pdl, k_drift, nblk(d.nm, 128), 128, 0, st, dm, h, 0.5 * h); LAUNCH(c);   // Sun kick + drift of the massive bodies
     } else {
         if (!opened) enqueue_kick(c, 0.5 * h, 1, nullptr);        // else: done by the previous map's merged kick
         if (d.mode != GENGA_MODE_TEST_PARTICLE) enqueue_sun(c, 0.5 * h, 0, false, h);   // Sun kick and drift in one launch
         else {
             enqueue_sun(c, 0.5 * h);
-            launch_k(c->pdl, k_drift, nblk(d.ntot, 128), 128, 0, st, d, h); LAUNCH(c);
+            launch_k(c->pdl, k_drift, nblk(d.ntot, 128), 128, 0, st, d, h, 0.0); LAUNCH(c);
         }
     }
     const int pair_blocks = (int)std::min<long long>((d.cap + 127) / 128, 16LL * c->sms);   // grid-stride over the candidates; enough warps to cover the gather latency when there are 10^6 of them (mode 1)
@@ -391,8 +392,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         }
     }
     if (tp) {
-        launch_k(false, k_momentum, 1, red_threads(d.nm), 0, st, d, d.vx, d.vy, d.vz); LAUNCH(c);     // plain: see enqueue_sun
-        launch_k(c->pdl, k_shift, nblk(d.nm, 256), 256, 0, st, dm, d.x, d.y, d.z, 0.5 * h, 0); LAUNCH(c);
+        launch_k(false, k_momentum, 1, red_threads(d.nm), 0, st, d, d.vx, d.vy, d.vz, 0.5 * h); LAUNCH(c);   // + Sun kick of the massive bodies; plain: see enqueue_sun
         launch_k(c->pdl, k_tp_back, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h); LAUNCH(c);
         launch_kick(c, 0.5 * h, 0, nullptr); LAUNCH(c);
     } else {
@@ -409,10 +409,10 @@ static void enqueue_step(genga_ctx *c, double dt, int order)
     DevState &d = c->d;
     double w[7];
     int nw = yoshida_weights(order, w);
-    if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {    // the particles' rc: k_tp_front of the first map
+    if (d.mode == GENGA_MODE_TEST_PARTICLE) {                     // the particles' rc: k_tp_front of the first map
         DevState dm = d;
         dm.ntot = d.nm;
-        launch_k(c->pdl, k_rcrit, nblk(d.nm, 128), 128, 0, c->st, dm, dt, 0); LAUNCH(c);
+        launch_k(c->pdl, k_rcrit, 1, 128, 0, c->st, dm, dt, 2); LAUNCH(c);       // nm <= 32: one block, which also opens the first map
     } else {
         launch_k(c->pdl, k_rcrit, nblk(d.ntot, 128), 128, 0, c->st, d, dt, d.mode != GENGA_MODE_TEST_PARTICLE); LAUNCH(c);
     }
@@ -508,7 +508,7 @@ static int get_state_impl(genga_ctx *c, double *x, double *v, cudaMemcpyKind kin
     if (!c || !x || !v) return GENGA_EINVAL;
     DevState &d = c->d;
     const size_t n = (size_t)d.ntot, B = sizeof(double);
-    k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx, d.vy, d.vz);
+    k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx, d.vy, d.vz, 0.0);
     k_shift_out<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0);
     c->launches += 2;
     const double *src[6] = {d.x, d.y, d.z, d.vx0, d.vy0, d.vz0};
@@ -533,7 +533,7 @@ extern "C" __attribute__((visibility("default"))) int genga_get_state_host(genga
     if (c && c->hstage && x && v) {                            // small state: one copy, unpack after the latch's sync
         DevState &d = c->d;
         const size_t n = (size_t)d.ntot, np = (size_t)d.np, B = sizeof(double);
-        k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx, d.vy, d.vz);
+        k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx, d.vy, d.vz, 0.0);
         k_shift_out<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0);
         c->launches += 2;
         CK(cudaMemcpyAsync(c->hstage, d.x, 6 * B * np, cudaMemcpyDeviceToHost, c->st));
@@ -633,8 +633,8 @@ extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ct
         if (r == 0) CK(cudaEventRecord(e0, c->st));
         if (which == 0) { launch_kick(c, 0.0, 0, nullptr); c->launches += 1; }
         else if (which == 1) {
-            k_drift<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt);
-            k_drift<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, -dt);
+            k_drift<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt, 0.0);
+            k_drift<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, -dt, 0.0);
             c->launches += 2; per = 2;
         } else if (which == 2) { c->acc = 0; enqueue_kick(c, 0.0, 0, nullptr); per = (int)c->acc; c->launches += c->acc; c->acc = 0; }
         else if (which == 3) {                       // fused particle pass, forwards then backwards

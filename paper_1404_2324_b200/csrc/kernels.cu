@@ -45,7 +45,13 @@ __global__ void k_rcrit(DevState d, double tau, int reset)
 {
     pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (reset && i == 0) {                                // start of a step: forget the previous step's lists (modes 0, 2)
+    if (reset == 2) {                                     // mode 1 (ONE block): k_begin_map and k_reset_counters of the first map
+        const int nprev = d.cnt[CI_NTP];
+        for (int k = threadIdx.x; k < nprev; k += blockDim.x) d.tpmask[d.tplist[k] - d.nm] = 0u;
+        __syncthreads();                                  // every thread has read the old count
+        if (threadIdx.x == 0) d.cnt[CI_NTP_PREV] = nprev;
+    }
+    if (reset && i == 0) {                                // start of a step: forget the previous step's lists
         d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
         d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0;
     }
@@ -499,10 +505,11 @@ __global__ void __launch_bounds__(128) k_kick_multi(DevState d, double h, int re
 // bodies of m V (one block per system, fixed-order tree), then q_i += h s / m0 for every
 // body of the system, test particles included.
 // which: 0 = democratic V as stored; used also for the coordinate maps (with other arrays).
-__global__ void k_momentum(DevState d, const double *vx, const double *vy, const double *vz)
+__global__ void k_momentum(DevState d, const double *vx, const double *vy, const double *vz, double fshift)
 {
     pdl_sync();
     __shared__ double red[4][32];
+    __shared__ double tot[4];
     const int sys = blockIdx.x, base = sys * d.nm * (d.mode == 2 ? 1 : 0);
     double s[4] = {0, 0, 0, 0};
     for (int k = threadIdx.x; k < d.nm; k += blockDim.x) {
@@ -521,6 +528,15 @@ __global__ void k_momentum(DevState d, const double *vx, const double *vy, const
         double t = 0;
         for (int k = 0; k < nw; ++k) t += red[threadIdx.x][k];
         d.psum[4 * sys + threadIdx.x] = t;
+        tot[threadIdx.x] = t;
+    }
+    if (fshift != 0.0) {                                  // the Sun kick of these bodies in the same launch (k_shift's arithmetic)
+        __syncthreads();
+        const double g = fshift / d.m0[sys];
+        for (int k = threadIdx.x; k < d.nm; k += blockDim.x) {
+            d.x[base + k] = fma(g, tot[0], d.x[base + k]); d.y[base + k] = fma(g, tot[1], d.y[base + k]);
+            d.z[base + k] = fma(g, tot[2], d.z[base + k]);
+        }
     }
 }
 // q += f * psum / m0   (f = h for the Sun kick)
@@ -624,12 +640,17 @@ __global__ void k_shift_out(DevState d, const double *ix, const double *iy, cons
 // =====================================================================================
 // Kepler drift, the analytic part of operator A (Eq. 9; L195, L208-230): one thread per
 // body, state kept before the drift for the encounter search and for BS.
-__global__ void __launch_bounds__(128) k_drift(DevState d, double h)
+__global__ void __launch_bounds__(128) k_drift(DevState d, double h, double hsun)
 {
     pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= d.ntot) return;
     double x = d.x[i], y = d.y[i], z = d.z[i], vx = d.vx[i], vy = d.vy[i], vz = d.vz[i];
+    if (hsun != 0.0) {                                    // Sun kick first (k_shift's arithmetic, psum from k_momentum)
+        const int sys = system_of(d, i);
+        const double g = hsun / d.m0[sys];
+        x = fma(g, d.psum[4 * sys], x); y = fma(g, d.psum[4 * sys + 1], y); z = fma(g, d.psum[4 * sys + 2], z);
+    }
     d.x0[i] = x; d.y0[i] = y; d.z0[i] = z; d.vx0[i] = vx; d.vy0[i] = vy; d.vz0[i] = vz;
     double mu = d.G * d.m0[system_of(d, i)];
     if (!kepler_drift(mu, h, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
