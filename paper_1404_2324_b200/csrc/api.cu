@@ -347,8 +347,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
     }
     if (tp) {
         // particles: kick, Sun kick and drift in one pass (k_tp_front); the massive bodies as in mode 0
-        launch_kick(c, 0.5 * h, 1, nullptr); LAUNCH(c);
-        launch_k(c->pdl, k_momentum, 1, red_threads(d.nm), 0, st, d, d.vx, d.vy, d.vz, 0.0); LAUNCH(c);
+        launch_k(c->pdl, k_tpm_kick, 1, 32, 0, st, d, 0.5 * h, 1, 0.0); LAUNCH(c);           // kick + momentum sum, one warp
         launch_k(c->pdl, k_tp_front, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h, tau, first); LAUNCH(c);
         launch_k(c->pdl, k_drift, nblk(d.nm, 128), 128, 0, st, dm, h, 0.5 * h); LAUNCH(c);   // Sun kick + drift of the massive bodies
     } else {
@@ -392,9 +391,8 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         }
     }
     if (tp) {
-        launch_k(false, k_momentum, 1, red_threads(d.nm), 0, st, d, d.vx, d.vy, d.vz, 0.5 * h); LAUNCH(c);   // + Sun kick of the massive bodies; plain: see enqueue_sun
+        launch_k(false, k_tpm_kick, 1, 32, 0, st, d, 0.5 * h, 0, 0.5 * h); LAUNCH(c);       // momentum sum, Sun kick, kick of the massive bodies; plain: see enqueue_sun
         launch_k(c->pdl, k_tp_back, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h); LAUNCH(c);
-        launch_kick(c, 0.5 * h, 0, nullptr); LAUNCH(c);
     } else {
         enqueue_sun(c, 0.5 * h, last ? 0 : 1, true);
         if (hn != 0.0) enqueue_kick(c, 0.5 * (h + hn), 1, nullptr);   // closing kick + opening kick of the next map

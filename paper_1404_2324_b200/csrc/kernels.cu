@@ -500,6 +500,70 @@ __global__ void __launch_bounds__(128) k_kick_multi(DevState d, double h, int re
     d.vx[i] = fma(h, ax, vx); d.vy[i] = fma(h, ay, vy); d.vz[i] = fma(h, az, vz);
 }
 
+// The massive bodies of the test-particle mode (nm <= 32, L188): kick, momentum sum and Sun kick of one half map in ONE
+// warp (body = lane).  fshift == 0, opening half: kick, then s = sum m V for the particles' and the massive bodies' Sun kick
+// (k_tp_front, k_drift).  fshift != 0, closing half: s from the velocities as they are, q += fshift s / m0, then the kick at
+// the shifted positions.  Same pair arithmetic as k_kick_multi, same sum order as k_momentum with 32 threads.
+__global__ void __launch_bounds__(32) k_tpm_kick(DevState d, double h, int record, double fshift)
+{
+    pdl_sync();
+    __shared__ double sx[32], sy[32], sz[32], sgm[32], src[32];
+    const int t = threadIdx.x, nm = d.nm;
+    const bool live = t < nm;
+    double xi = 0.0, yi = 0.0, zi = 0.0, rci = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, m = 0.0;
+    if (live) {
+        xi = d.x[t]; yi = d.y[t]; zi = d.z[t]; rci = d.rc[t];
+        vx = d.vx[t]; vy = d.vy[t]; vz = d.vz[t]; m = d.m[t];
+    }
+    auto momentum = [&](double &s0, double &s1, double &s2) {
+        s0 = m * vx; s1 = m * vy; s2 = m * vz;
+        double s3 = m;
+        for (int o = 16; o > 0; o >>= 1) {
+            s0 += __shfl_xor_sync(0xffffffffu, s0, o); s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+            s2 += __shfl_xor_sync(0xffffffffu, s2, o); s3 += __shfl_xor_sync(0xffffffffu, s3, o);
+        }
+        if (t == 0) { d.psum[0] = s0; d.psum[1] = s1; d.psum[2] = s2; d.psum[3] = s3; }
+    };
+    if (fshift != 0.0) {
+        double s0, s1, s2;
+        momentum(s0, s1, s2);
+        const double g = fshift / d.m0[0];
+        xi = fma(g, s0, xi); yi = fma(g, s1, yi); zi = fma(g, s2, zi);
+        if (live) { d.x[t] = xi; d.y[t] = yi; d.z[t] = zi; }
+    }
+    sx[t] = xi; sy[t] = yi; sz[t] = zi; src[t] = rci; sgm[t] = d.G * m;
+    __syncwarp();
+    double ax = 0, ay = 0, az = 0;
+    if (live) {
+        for (int j = 0; j < nm; ++j) {
+            if (j == t) continue;
+            double dx = sx[j] - xi, dy = sy[j] - yi, dz = sz[j] - zi;
+            double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            double rcij = fmax(rci, src[j]);
+            double gm = sgm[j];
+            double s3 = gm * rinv3_fast(r2);
+            if (r2 < 9.0 * rcij * rcij) {
+                if (r2 < rcij * rcij) {                             // W = 1 outside the changeover zone
+                    double r = sqrt(r2);
+                    s3 = gm / (r2 * r) * kick_weight(r, rcij);
+                }
+                if (record && t < j) {
+                    int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
+                    if (idx < d.cap) d.cand[idx] = make_int2(t, j);
+                    else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+                }
+            }
+            ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
+        }
+        vx = fma(h, ax, vx); vy = fma(h, ay, vy); vz = fma(h, az, vz);
+        d.vx[t] = vx; d.vy[t] = vy; d.vz[t] = vz;
+    }
+    if (fshift == 0.0) {
+        double s0, s1, s2;
+        momentum(s0, s1, s2);
+    }
+}
+
 // =====================================================================================
 // Sun kick, operator C (Eq. 3; L196, L232-236, L338, L360-366): s = sum over massive
 // bodies of m V (one block per system, fixed-order tree), then q_i += h s / m0 for every

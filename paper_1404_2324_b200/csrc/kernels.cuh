@@ -25,6 +25,7 @@ __global__ void k_tp_front(DevState d, double h, double tau, int first);
 __global__ void k_tp_back(DevState d, double h);
 __global__ void k_kick_multi(DevState d, double h, int record, double *aout);
 __global__ void k_sun(DevState d, double h, int reset, double hdrift);
+__global__ void k_tpm_kick(DevState d, double h, int record, double fshift);
 __global__ void k_momentum(DevState d, const double *vx, const double *vy, const double *vz, double fshift);
 __global__ void k_shift(DevState d, double *ax, double *ay, double *az, double f, int divide_by_total);
 __global__ void k_shift_out(DevState d, const double *ix, const double *iy, const double *iz,
