@@ -88,8 +88,9 @@ int genga_destroy(genga_ctx *ctx);
  * or pageable); the copies are enqueued on the stream and the call returns after they and
  * the conversion to democratic coordinates have completed.  States of up to 512 KB (and a
  * non-NULL radius) are packed into a pinned image owned by the context and moved with ONE
- * copy (genga_get_state_host likewise); larger ones are copied array by array straight
- * from the caller's buffers. */
+ * copy (genga_get_state_host likewise), and the call returns as soon as the caller's
+ * buffers have been read, the copy still in flight on the stream; larger ones are copied
+ * array by array straight from the caller's buffers. */
 int genga_set_state(genga_ctx *ctx, const double *m0, const double *m, const double *radius,
                     const double *x, const double *v);
 int genga_set_state_host(genga_ctx *ctx, const double *m0, const double *m, const double *radius,

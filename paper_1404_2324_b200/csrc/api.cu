@@ -47,6 +47,8 @@ struct genga_ctx {
     double *eout;               // device [4*nsys]
     double *hstage;             // pinned host image of x..vz0, m, radius, m0 (small states only, else nullptr)
     int *hstatus;               // pinned host copy of the status word
+    cudaEvent_t ev_stage;       // the last copy out of hstage (set_state_host does not wait for it)
+    bool stage_busy;
     struct GraphEntry { cudaGraphExec_t exec; long long launches; };
     std::map<GraphKey, GraphEntry> graphs;
     long long steps, force_evals, interactions, launches;
@@ -153,7 +155,7 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     c->bs_big_clusters = std::max(1, c->sms / BCB_CS);
     c->steps = c->force_evals = c->interactions = c->launches = 0;
     c->acc = 0;
-    c->hstage = nullptr; c->hstatus = nullptr;
+    c->hstage = nullptr; c->hstatus = nullptr; c->ev_stage = nullptr; c->stage_busy = false;
     size_t need = carve(cfg, (char *)cfg->workspace, &c->d, &c->exp_labels, &c->eout, c->sms);
     if (need > cfg->workspace_bytes) { delete c; return GENGA_EINVAL; }
     cudaError_t e = cudaMemsetAsync(cfg->workspace, 0, need, c->st);
@@ -169,6 +171,7 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     if (e == cudaSuccess && stage_bytes(c->d) <= HOST_STAGE_MAX) {
         e = cudaHostAlloc((void **)&c->hstage, stage_bytes(c->d), cudaHostAllocDefault);
         if (e == cudaSuccess) memset(c->hstage, 0, stage_bytes(c->d));
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_stage, cudaEventDisableTiming);
     }
     if (e != cudaSuccess) { delete c; snprintf(g_cuda_err, sizeof g_cuda_err, "create: %s", cudaGetErrorString(e)); return GENGA_ECUDA; }
     *out = c;
@@ -182,6 +185,7 @@ extern "C" __attribute__((visibility("default"))) int genga_destroy(genga_ctx *c
     for (int k = 0; k < 2; ++k) { cudaStreamDestroy(c->aux[k]); cudaEventDestroy(c->ev_join[k]); }
     cudaEventDestroy(c->ev_fork);
     if (c->hstage) cudaFreeHost(c->hstage);
+    if (c->ev_stage) cudaEventDestroy(c->ev_stage);
     if (c->hstatus) cudaFreeHost(c->hstatus);
     delete c;
     return GENGA_OK;
@@ -253,6 +257,7 @@ extern "C" __attribute__((visibility("default"))) int genga_set_state_host(genga
         DevState &d = c->d;
         const size_t n = (size_t)d.ntot, np = (size_t)d.np, B = sizeof(double);
         double *h = c->hstage;
+        if (c->stage_busy) { CK(cudaEventSynchronize(c->ev_stage)); c->stage_busy = false; }   // the image is still being read
         for (int k = 0; k < 3; ++k) {
             memcpy(h + k * np, x + k * n, B * n);
             memcpy(h + (3 + k) * np, v + k * n, B * n);
@@ -261,10 +266,11 @@ extern "C" __attribute__((visibility("default"))) int genga_set_state_host(genga
         memcpy(h + 7 * np, radius, B * n);
         memcpy(h + 8 * np, m0, B * d.nsys);
         CK(cudaMemcpyAsync(d.x, h, stage_bytes(d), cudaMemcpyHostToDevice, c->st));
+        CK(cudaEventRecord(c->ev_stage, c->st));
+        c->stage_busy = true;
         enqueue_helio_to_demo(c);
         CK(cudaGetLastError());
-        CK(cudaStreamSynchronize(c->st));
-        return GENGA_OK;
+        return GENGA_OK;                                       // the caller's buffers have been read: nothing to wait for
     }
     int r = set_state_impl(c, m0, m, radius, x, v, cudaMemcpyHostToDevice);
     if (r) return r;
@@ -537,6 +543,7 @@ extern "C" __attribute__((visibility("default"))) int genga_get_state_host(genga
         CK(cudaMemcpyAsync(c->hstage, d.x, 6 * B * np, cudaMemcpyDeviceToHost, c->st));
         CK(cudaGetLastError());
         int r = latch(c);
+        c->stage_busy = false;
         for (int k = 0; k < 3; ++k) {
             memcpy(x + k * n, c->hstage + k * np, B * n);
             memcpy(v + k * n, c->hstage + (3 + k) * np, B * n);
