@@ -109,6 +109,22 @@ int genga_step(genga_ctx *ctx, int64_t n_steps, double dt, int order);
 int genga_get_state(genga_ctx *ctx, double *x, double *v);
 int genga_get_state_host(genga_ctx *ctx, double *x, double *v);
 
+/* Multi-system mode with a VARIABLE number of bodies per system (L346-354: "no more than 16
+ * bodies" each).  System s holds n_bodies[s] bodies, 1 <= n_bodies[s] <=
+ * n_massive; the packed arrays list the systems one after the other (start index of system
+ * s = sum of n_bodies[0..s-1], Nreal = sum of all): m[Nreal], radius[Nreal] (may be NULL),
+ * x[3*Nreal] = all x, all y, all z, v likewise; m0[n_systems].  HOST pointers.
+ * Inside, every system keeps n_massive slots (body = system * n_massive + k); the unused slots
+ * hold MASSLESS bodies on wide circular orbits (1000 (k + 1) length units from the central
+ * mass): they exert no force, add exact zeros to every sum, never come within a critical
+ * radius of anything, so the real bodies move exactly as in a system of n_bodies[s] slots.
+ * The other calls keep the padded indexing (genga_get_state*, genga_encounters labels);
+ * genga_get_state_ragged_host returns the real bodies in the packed order.  Both synchronise.
+ * GENGA_EINVAL outside multi-system mode, for a size out of range, or (get) before a set. */
+int genga_set_state_ragged_host(genga_ctx *ctx, const int32_t *n_bodies, const double *m0, const double *m,
+                                const double *radius, const double *x, const double *v);
+int genga_get_state_ragged_host(genga_ctx *ctx, double *x, double *v);
+
 /* Total energy E[n_systems] and angular momentum L[3*n_systems] (x,y,z per system) of the
  * current state, Eq. 1-3 summed (L73-80).  HOST pointers; synchronises.  L may be NULL. */
 int genga_energy(genga_ctx *ctx, double *E, double *L);

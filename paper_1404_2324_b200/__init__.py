@@ -67,6 +67,8 @@ def load():
         "genga_step": (i, [vp, l, d, i]),
         "genga_get_state": (i, [vp, dp, dp]),
         "genga_get_state_host": (i, [vp, dp, dp]),
+        "genga_set_state_ragged_host": (i, [vp, vp, dp, dp, dp, dp, dp]),
+        "genga_get_state_ragged_host": (i, [vp, dp, dp]),
         "genga_energy": (i, [vp, dp, dp]),
         "genga_encounters": (i, [vp, vp, l, C.POINTER(l), C.POINTER(l), vp]),
         "genga_status": (i, [vp]),
@@ -177,6 +179,22 @@ class Genga:
         x = np.empty((3, self.ntot)) if x is None else x
         v = np.empty((3, self.ntot)) if v is None else v
         _chk(self.lib.genga_get_state_host(self.h, _hp(x), _hp(v)), "genga_get_state_host")
+        return x, v
+
+    def set_state_ragged_host(self, n_bodies, m0, m, radius, x, v):
+        """Multi-system mode, variable bodies per system: packed arrays, see include/genga.h."""
+        nb = np.ascontiguousarray(n_bodies, dtype=np.int32)
+        if nb.shape != (self.ns,):
+            raise ValueError("n_bodies must have one entry per system")
+        self._nreal = int(nb.sum())
+        arrs = [np.ascontiguousarray(a, dtype=np.float64) for a in (np.atleast_1d(m0), m, radius, x, v)]
+        if arrs[1].size != self._nreal or arrs[2].size != self._nreal or arrs[3].size != 3 * self._nreal or arrs[4].size != 3 * self._nreal:
+            raise ValueError("packed arrays do not match sum(n_bodies)")
+        _chk(self.lib.genga_set_state_ragged_host(self.h, _hp(nb), *[_hp(a) for a in arrs]), "genga_set_state_ragged_host")
+
+    def get_state_ragged_host(self):
+        x, v = np.empty((3, self._nreal)), np.empty((3, self._nreal))
+        _chk(self.lib.genga_get_state_ragged_host(self.h, _hp(x), _hp(v)), "genga_get_state_ragged_host")
         return x, v
 
     def energy(self):

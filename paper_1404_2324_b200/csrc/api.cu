@@ -3,6 +3,7 @@
 // never returns to the host (the paper's Sync/Copy overheads, L204/L274, are designed out:
 // every count stays in device memory and is read by the next kernel).
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -48,6 +49,7 @@ struct genga_ctx {
     double *hstage;             // pinned host image of x..vz0, m, radius, m0 (small states only, else nullptr)
     int *hstatus;               // pinned host copy of the status word
     cudaEvent_t ev_stage;       // the last copy out of hstage (set_state_host does not wait for it)
+    std::vector<int> n_bodies;  // multi-system mode, ragged state: real bodies per system (empty: all slots real)
     bool stage_busy;
     struct GraphEntry { cudaGraphExec_t exec; long long launches; };
     std::map<GraphKey, GraphEntry> graphs;
@@ -553,6 +555,64 @@ extern "C" __attribute__((visibility("default"))) int genga_get_state_host(genga
     int r = get_state_impl(c, x, v, cudaMemcpyDeviceToHost);
     if (r) return r;
     return latch(c);
+}
+
+// Variable number of bodies per system: the packed arrays are scattered into the fixed-stride layout on the host,
+// the unused slots filled with massless bodies on wide circular orbits (include/genga.h).
+extern "C" __attribute__((visibility("default"))) int genga_set_state_ragged_host(genga_ctx *c, const int32_t *n_bodies, const double *m0,
+        const double *m, const double *radius, const double *x, const double *v)
+{
+    if (!c || !n_bodies || !m0 || !m || !x || !v) return GENGA_EINVAL;
+    const DevState &d = c->d;
+    if (d.mode != GENGA_MODE_MULTI_SYSTEM) return GENGA_EINVAL;
+    const size_t nt = (size_t)d.ntot, nm = (size_t)d.nm;
+    size_t nreal = 0;
+    for (int s = 0; s < d.nsys; ++s) {
+        if (n_bodies[s] < 1 || n_bodies[s] > d.nm) return GENGA_EINVAL;
+        nreal += (size_t)n_bodies[s];
+    }
+    std::vector<double> pm(nt, 0.0), pr(nt, 0.0), px(3 * nt, 0.0), pv(3 * nt, 0.0);
+    size_t at = 0;
+    for (int s = 0; s < d.nsys; ++s) {
+        const size_t nb = (size_t)n_bodies[s], base = (size_t)s * nm;
+        for (size_t k = 0; k < nm; ++k) {
+            const size_t i = base + k;
+            if (k < nb) {
+                pm[i] = m[at + k];
+                pr[i] = radius ? radius[at + k] : 0.0;
+                for (int a = 0; a < 3; ++a) { px[a * nt + i] = x[a * nreal + at + k]; pv[a * nt + i] = v[a * nreal + at + k]; }
+            } else {                                              // padding slot: massless, circular, far away
+                const double R = 1000.0 * (double)(k + 1);
+                px[i] = R;
+                pv[nt + i] = std::sqrt(d.G * m0[s] / R);
+            }
+        }
+        at += nb;
+    }
+    int r = genga_set_state_host(c, m0, pm.data(), pr.data(), px.data(), pv.data());
+    if (r) return r;
+    CK(cudaStreamSynchronize(c->st));                         // the padded arrays die with this call
+    c->n_bodies.assign(n_bodies, n_bodies + d.nsys);
+    return GENGA_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_get_state_ragged_host(genga_ctx *c, double *x, double *v)
+{
+    if (!c || !x || !v) return GENGA_EINVAL;
+    const DevState &d = c->d;
+    if (d.mode != GENGA_MODE_MULTI_SYSTEM || (int)c->n_bodies.size() != d.nsys) return GENGA_EINVAL;
+    const size_t nt = (size_t)d.ntot, nm = (size_t)d.nm;
+    std::vector<double> px(3 * nt), pv(3 * nt);
+    int r = genga_get_state_host(c, px.data(), pv.data());
+    size_t nreal = 0, at = 0;
+    for (int nb : c->n_bodies) nreal += (size_t)nb;
+    for (int s = 0; s < d.nsys; ++s) {
+        const size_t nb = (size_t)c->n_bodies[s], base = (size_t)s * nm;
+        for (size_t k = 0; k < nb; ++k)
+            for (int a = 0; a < 3; ++a) { x[a * nreal + at + k] = px[a * nt + base + k]; v[a * nreal + at + k] = pv[a * nt + base + k]; }
+        at += nb;
+    }
+    return r;
 }
 
 extern "C" __attribute__((visibility("default"))) int genga_energy(genga_ctx *c, double *E, double *L)

@@ -440,3 +440,61 @@ def test_full_size_sampled_outputs_config2_and_config3(G):
         xo, vo = o.state()
         assert relerr(x[:, sl], xo).max() < STATE_TOL
     g.close()
+
+
+def _ragged_from(full, sizes):
+    """packed arrays of the first sizes[s] bodies of system s of a fixed-size multi-system workload"""
+    nm = full["n_massive"]
+    idx = np.concatenate([s * nm + np.arange(n) for s, n in enumerate(sizes)])
+    return idx, full["m"][idx], full["radius"][idx], np.ascontiguousarray(full["x"][:, idx]), np.ascontiguousarray(full["v"][:, idx])
+
+
+def test_variable_bodies_per_system_against_the_oracle(G):
+    """systems of different sizes in one context.  Every system is checked
+    against the oracle run of that system alone with exactly its bodies."""
+    full = workloads.config3(n_systems=12, n_per=16)
+    sizes = np.array([16, 7, 3, 12, 2, 16, 9, 5, 11, 4, 13, 8])
+    idx, m, rad, x, v = _ragged_from(full, sizes)
+    g = G.Genga(full["mode"], 16, n_systems=12)
+    g.set_state_ragged_host(sizes, full["m0"], m, rad, x, v)
+    nsteps = 40
+    g.step(nsteps, full["dt"], 2)
+    xg, vg = g.get_state_ragged_host()
+    assert g.status() == 0
+    start = np.concatenate([[0], np.cumsum(sizes)])
+    for s, n in enumerate(sizes):
+        sl = slice(start[s], start[s + 1])
+        w = dict(full, n_systems=1, n_massive=int(n), m0=full["m0"][s:s + 1], m=m[sl], radius=rad[sl],
+                 x=np.ascontiguousarray(x[:, sl]), v=np.ascontiguousarray(v[:, sl]))
+        o = oracle.Sim(w)
+        o.step(nsteps, w["dt"], 2)
+        xo, vo = o.state()
+        assert relerr(xg[:, sl], xo).max() < STATE_TOL and relerr(vg[:, sl], vo).max() < STATE_TOL, (s, n)
+    g.close()
+
+
+def test_padded_systems_move_exactly_as_unpadded_ones(G):
+    """the padding bodies add exact zeros: 7 real bodies in 16 slots == a context with 7 slots, bit for bit"""
+    small = workloads.config3(n_systems=10, n_per=7)
+    g7 = G.from_workload(small)
+    g7.step(60, small["dt"], 2)
+    x7, v7 = g7.get_state_host()
+    g7.close()
+    g = G.Genga(small["mode"], 16, n_systems=10)
+    g.set_state_ragged_host(np.full(10, 7), small["m0"], small["m"], small["radius"], small["x"], small["v"])
+    g.step(60, small["dt"], 2)
+    x, v = g.get_state_ragged_host()
+    assert g.status() == 0
+    assert np.array_equal(x, x7) and np.array_equal(v, v7)
+    # argument checks
+    with pytest.raises(G.GengaError):
+        g.set_state_ragged_host(np.full(10, 17), small["m0"], np.zeros(170), np.zeros(170), np.zeros((3, 170)), np.zeros((3, 170)))
+    with pytest.raises(G.GengaError):
+        g.set_state_ragged_host(np.full(10, 0), small["m0"], np.zeros(0), np.zeros(0), np.zeros((3, 0)), np.zeros((3, 0)))
+    g.close()
+    g0 = G.from_workload(workloads.config0())
+    with pytest.raises(G.GengaError):
+        g0.lib.genga_get_state_ragged_host  # symbol exists
+        x0 = np.zeros((3, 15))
+        G._chk(g0.lib.genga_get_state_ragged_host(g0.h, G._hp(x0), G._hp(x0)), "genga_get_state_ragged_host")
+    g0.close()
