@@ -21,7 +21,8 @@ OK, EINVAL, ECAPACITY, EKEPLER, EBS, ECUDA = 0, -1, -2, -3, -4, -5
 # every symbol include/genga.h declares
 SYMBOLS = [
     "genga_workspace_bytes", "genga_create", "genga_destroy", "genga_set_state", "genga_set_state_host",
-    "genga_step", "genga_get_state", "genga_get_state_host", "genga_energy", "genga_encounters",
+    "genga_step", "genga_get_state", "genga_get_state_host", "genga_set_state_ragged_host", "genga_get_state_ragged_host",
+    "genga_energy", "genga_encounters",
     "genga_status", "genga_accelerations", "genga_kepler_drift", "genga_counters", "genga_time_kernel", "genga_fp64_probe", "genga_strerror",
     "genga_last_cuda_error",
 ]
