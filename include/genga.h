@@ -125,6 +125,13 @@ int genga_set_state_ragged_host(genga_ctx *ctx, const int32_t *n_bodies, const d
                                 const double *radius, const double *x, const double *v);
 int genga_get_state_ragged_host(genga_ctx *ctx, double *x, double *v);
 
+/* Multi-system mode: the n1 and n2 of Eq. 6 (L94-96) of every system (L346-354: among the few
+ * parameters that "can be set individually for the different simulations"; the central mass
+ * is m0[] of genga_set_state).  n1[n_systems], n2[n_systems], HOST pointers, both >= 0; they
+ * replace the configuration's values from the next step on.  Synchronises.  GENGA_EINVAL
+ * outside multi-system mode. */
+int genga_set_system_params_host(genga_ctx *ctx, const double *n1, const double *n2);
+
 /* Total energy E[n_systems] and angular momentum L[3*n_systems] (x,y,z per system) of the
  * current state, Eq. 1-3 summed (L73-80).  HOST pointers; synchronises.  L may be NULL. */
 int genga_energy(genga_ctx *ctx, double *E, double *L);

@@ -21,7 +21,7 @@ OK, EINVAL, ECAPACITY, EKEPLER, EBS, ECUDA = 0, -1, -2, -3, -4, -5
 # every symbol include/genga.h declares
 SYMBOLS = [
     "genga_workspace_bytes", "genga_create", "genga_destroy", "genga_set_state", "genga_set_state_host",
-    "genga_step", "genga_get_state", "genga_get_state_host", "genga_set_state_ragged_host", "genga_get_state_ragged_host",
+    "genga_step", "genga_get_state", "genga_get_state_host", "genga_set_state_ragged_host", "genga_get_state_ragged_host", "genga_set_system_params_host",
     "genga_energy", "genga_encounters",
     "genga_status", "genga_accelerations", "genga_kepler_drift", "genga_counters", "genga_time_kernel", "genga_fp64_probe", "genga_strerror",
     "genga_last_cuda_error",
@@ -70,6 +70,7 @@ def load():
         "genga_get_state_host": (i, [vp, dp, dp]),
         "genga_set_state_ragged_host": (i, [vp, vp, dp, dp, dp, dp, dp]),
         "genga_get_state_ragged_host": (i, [vp, dp, dp]),
+        "genga_set_system_params_host": (i, [vp, dp, dp]),
         "genga_energy": (i, [vp, dp, dp]),
         "genga_encounters": (i, [vp, vp, l, C.POINTER(l), C.POINTER(l), vp]),
         "genga_status": (i, [vp]),
@@ -192,6 +193,11 @@ class Genga:
         if arrs[1].size != self._nreal or arrs[2].size != self._nreal or arrs[3].size != 3 * self._nreal or arrs[4].size != 3 * self._nreal:
             raise ValueError("packed arrays do not match sum(n_bodies)")
         _chk(self.lib.genga_set_state_ragged_host(self.h, _hp(nb), *[_hp(a) for a in arrs]), "genga_set_state_ragged_host")
+
+    def set_system_params_host(self, n1, n2):
+        """Multi-system mode: n1, n2 of Eq. 6 per system."""
+        a, b = (np.ascontiguousarray(np.broadcast_to(np.asarray(q, dtype=np.float64), (self.ns,))) for q in (n1, n2))
+        _chk(self.lib.genga_set_system_params_host(self.h, _hp(a), _hp(b)), "genga_set_system_params_host")
 
     def get_state_ragged_host(self):
         x, v = np.empty((3, self._nreal)), np.empty((3, self._nreal))

@@ -101,6 +101,7 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
         t.gmask = (unsigned *)take(sizeof(unsigned) * 32);
     } else {
         t.gorder = (int *)take(sizeof(int) * np);          // (system, member mask) per group, at most ntot / 2 groups
+        t.n12 = (double *)take(sizeof(double) * 2 * nsys);
     }
     if (c->mode == GENGA_MODE_MASSIVE && nm > BCB_MAXN) {
         t.bss.stride = npm;
@@ -161,6 +162,12 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     size_t need = carve(cfg, (char *)cfg->workspace, &c->d, &c->exp_labels, &c->eout, c->sms);
     if (need > cfg->workspace_bytes) { delete c; return GENGA_EINVAL; }
     cudaError_t e = cudaMemsetAsync(cfg->workspace, 0, need, c->st);
+    if (e == cudaSuccess && c->d.n12) {                       // every system starts with the configuration's n1, n2
+        std::vector<double> p(2 * (size_t)c->d.nsys);
+        for (int s = 0; s < c->d.nsys; ++s) { p[2 * s] = cfg->n1; p[2 * s + 1] = cfg->n2; }
+        e = cudaMemcpyAsync(c->d.n12, p.data(), sizeof(double) * p.size(), cudaMemcpyHostToDevice, c->st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    }
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                    (int)sizeof(BcSmem<BCB_MAXN, BCB_THREADS>));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_kick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kick_smem_bytes());
@@ -555,6 +562,20 @@ extern "C" __attribute__((visibility("default"))) int genga_get_state_host(genga
     int r = get_state_impl(c, x, v, cudaMemcpyDeviceToHost);
     if (r) return r;
     return latch(c);
+}
+
+// n1 and n2 of Eq. 6 per system (multi-system mode, L346-354).
+extern "C" __attribute__((visibility("default"))) int genga_set_system_params_host(genga_ctx *c, const double *n1, const double *n2)
+{
+    if (!c || !n1 || !n2 || c->d.mode != GENGA_MODE_MULTI_SYSTEM) return GENGA_EINVAL;
+    std::vector<double> p(2 * (size_t)c->d.nsys);
+    for (int s = 0; s < c->d.nsys; ++s) {
+        if (!(n1[s] >= 0.0) || !(n2[s] >= 0.0)) return GENGA_EINVAL;
+        p[2 * s] = n1[s]; p[2 * s + 1] = n2[s];
+    }
+    CK(cudaMemcpyAsync(c->d.n12, p.data(), sizeof(double) * p.size(), cudaMemcpyHostToDevice, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    return GENGA_OK;
 }
 
 // Variable number of bodies per system: the packed arrays are scattered into the fixed-stride layout on the host,

@@ -63,8 +63,10 @@ __global__ void k_rcrit(DevState d, double tau, int reset)
     double ainv = 2.0 / r - v2 / (d.G * m0);
     double a = ainv > 0.0 ? 1.0 / ainv : r;
     double rh = m > 0.0 ? a * cbrt(m / (3.0 * m0)) : 0.0;
-    double rv = d.n2 * fabs(tau) * sqrt(v2);
-    double rc = fmax(d.n1 * rh, rv);
+    double n1 = d.n1, n2 = d.n2;
+    if (d.mode == 2) { n1 = d.n12[2 * (i / d.nm)]; n2 = d.n12[2 * (i / d.nm) + 1]; }   // per system (L346-354)
+    double rv = n2 * fabs(tau) * sqrt(v2);
+    double rc = fmax(n1 * rh, rv);
     d.rc[i] = rc;
     d.c9[i] = 9.0 * rc * rc;
 }

@@ -14,6 +14,7 @@ struct DevState {
     int nmtot;       // massive bodies in total (nm, or nsys*nm in mode 2)
     double G, n1, n2, eps;
     double *m0;      // [nsys]
+    double *n12;     // mode 2: [nsys][2] the n1, n2 of every system (L346-354: set individually), else nullptr
     // democratic state, SoA [np]
     double *x, *y, *z, *vx, *vy, *vz, *m, *radius;
     double *rc, *c9;             // critical radius, 9 rc^2 (precheck threshold squared, L142)

@@ -498,3 +498,32 @@ def test_padded_systems_move_exactly_as_unpadded_ones(G):
         x0 = np.zeros((3, 15))
         G._chk(g0.lib.genga_get_state_ragged_host(g0.h, G._hp(x0), G._hp(x0)), "genga_get_state_ragged_host")
     g0.close()
+
+
+def test_n1_n2_per_system_against_the_oracle(G):
+    """n1 and n2 can be set individually for the simulations of the multi-simulation mode."""
+    full = workloads.config3(n_systems=6, n_per=9)
+    n1 = np.array([3.0, 1.0, 5.0, 3.0, 0.0, 8.0])
+    n2 = np.array([0.4, 0.1, 0.4, 1.0, 0.7, 0.0])
+    g = G.from_workload(full)
+    g.set_system_params_host(n1, n2)
+    _, rc = g.accelerations(full["dt"])
+    rc = rc.cpu().numpy()
+    g.set_state(full["m0"], full["m"], full["radius"], full["x"], full["v"])
+    nsteps = 40
+    g.step(nsteps, full["dt"], 2)
+    xg, vg = g.get_state_host()
+    assert g.status() == 0
+    for s in range(6):
+        sl = slice(9 * s, 9 * s + 9)
+        w = dict(full, n_systems=1, m0=full["m0"][s:s + 1], m=full["m"][sl], radius=full["radius"][sl],
+                 x=np.ascontiguousarray(full["x"][:, sl]), v=np.ascontiguousarray(full["v"][:, sl]), n1=n1[s], n2=n2[s])
+        o = oracle.Sim(w)
+        _, rco = oracle_accel(o, w["dt"])
+        assert np.abs(rc[sl] / rco - 1).max() < 2e-15
+        o.step(nsteps, w["dt"], 2)
+        xo, vo = o.state()
+        assert relerr(xg[:, sl], xo).max() < STATE_TOL and relerr(vg[:, sl], vo).max() < STATE_TOL, s
+    with pytest.raises(G.GengaError):
+        g.set_system_params_host(-1.0, 0.4)
+    g.close()
