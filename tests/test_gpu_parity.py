@@ -527,3 +527,28 @@ def test_n1_n2_per_system_against_the_oracle(G):
     with pytest.raises(G.GengaError):
         g.set_system_params_host(-1.0, 0.4)
     g.close()
+
+
+def test_host_image_path_back_to_back_calls(G):
+    """small states go through the context's pinned image with one copy per call and set_state_host does not wait
+    for it: back-to-back host calls must still see their own data; the large-state path (array by array) agrees."""
+    w = workloads.config4(n=300)                      # 300 bodies: the image path (np = 384 > ntot: padded strides)
+    big = workloads.config2(n_massive=4, n_test=40000)   # 2.5 MB of state: the direct path
+    for wl in (w, big):
+        g = G.from_workload(wl)
+        x2 = wl["x"] * (1 + 1e-3)
+        for _ in range(3):                             # the second call must not disturb the first one's copy in flight
+            g.set_state_host(wl["m0"], wl["m"], wl["radius"], x2, wl["v"])
+            g.set_state_host(wl["m0"], wl["m"], wl["radius"], wl["x"], wl["v"])
+        xa, va = g.get_state_host()
+        assert relerr(xa, wl["x"]).max() == 0 and relerr(va, wl["v"]).max() < 1e-15   # v: helio -> demo -> helio
+        g.step(3, wl["dt"], 2)
+        xh, vh = g.get_state_host()
+        xd, vd = g.get_state()
+        assert np.array_equal(xd.cpu().numpy(), xh) and np.array_equal(vd.cpu().numpy(), vh)
+        g2 = G.from_workload(wl)                       # device-pointer path from the start
+        g2.step(3, wl["dt"], 2)
+        x3, v3 = g2.get_state_host()
+        assert np.array_equal(x3, xh) and np.array_equal(v3, vh)
+        assert g.status() == 0
+        g.close(); g2.close()
