@@ -266,6 +266,9 @@ def run_gpu(args):
                          "algorithmic_bytes": 144 * g.ntot,
                          "gbs": 144 * g.ntot / (drift_ms * 1e-3) / 1e9,
                          "note": "launch-latency bound at N = 2048 (295 KB)"}
+        if w["n_massive"] <= 32:
+            roof["note"] = ("N <= 32: the step runs k_tiny_front / k_tiny_back (one warp per half map) and is launch-latency "
+                            "bound; k_kick and k_drift are timed alone here for reference only")
     elif w["mode"] == 1:
         # dominant kernels: the fused particle passes; algorithmic bytes per particle: 48 read + 48 written + 8 (rc)
         nt = w["n_test"]

@@ -349,6 +349,8 @@ static cudaError_t launch_bs_cluster(cudaStream_t st, int clusters, const DevSta
 // opening kick B(hn/2) of the next map act at the same positions with the same critical radii (frozen over the step,
 // DESIGN.md R-4), so they are one kick of (h + hn)/2 that also records the next map's candidates (`L170`: the
 // scheme "applied to each of the substeps"; flags bit 0 keeps them apart).
+static inline bool tiny_mode(const DevState &d) { return d.mode == GENGA_MODE_MASSIVE && d.nm <= 32; }
+
 static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last, double hn, bool opened)
 {
     DevState &d = c->d;
@@ -365,6 +367,8 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         launch_k(c->pdl, k_tpm_kick, 1, 32, 0, st, d, 0.5 * h, 1, 0.0); LAUNCH(c);           // kick + momentum sum, one warp
         launch_k(c->pdl, k_tp_front, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h, tau, first); LAUNCH(c);
         launch_k(c->pdl, k_drift, nblk(d.nm, 128), 128, 0, st, dm, h, 0.5 * h); LAUNCH(c);   // Sun kick + drift of the massive bodies
+    } else if (tiny_mode(d)) {                                // N <= 32: the opening half map in one warp, one launch
+        launch_k(c->pdl, k_tiny_front, 1, 32, 0, st, d, h, tau, first, opened ? 0.0 : 0.5 * h); LAUNCH(c);
     } else {
         if (!opened) enqueue_kick(c, 0.5 * h, 1, nullptr);        // else: done by the previous map's merged kick
         if (d.mode != GENGA_MODE_TEST_PARTICLE) enqueue_sun(c, 0.5 * h, 0, false, h);   // Sun kick and drift in one launch
@@ -408,6 +412,8 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
     if (tp) {
         launch_k(false, k_tpm_kick, 1, 32, 0, st, d, 0.5 * h, 0, 0.5 * h); LAUNCH(c);       // momentum sum, Sun kick, kick of the massive bodies; plain: see enqueue_sun
         launch_k(c->pdl, k_tp_back, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h); LAUNCH(c);
+    } else if (tiny_mode(d)) {                                // plain launch: see enqueue_sun
+        launch_k(false, k_tiny_back, 1, 32, 0, st, d, h, hn != 0.0 ? 0.5 * (h + hn) : 0.5 * h, hn != 0.0 ? 1 : 0, last ? 0 : 1); LAUNCH(c);
     } else {
         enqueue_sun(c, 0.5 * h, last ? 0 : 1, true);
         if (hn != 0.0) enqueue_kick(c, 0.5 * (h + hn), 1, nullptr);   // closing kick + opening kick of the next map
@@ -426,7 +432,7 @@ static void enqueue_step(genga_ctx *c, double dt, int order)
         DevState dm = d;
         dm.ntot = d.nm;
         launch_k(c->pdl, k_rcrit, 1, 128, 0, c->st, dm, dt, 2); LAUNCH(c);       // nm <= 32: one block, which also opens the first map
-    } else {
+    } else if (!tiny_mode(d)) {                                   // N <= 32: inside k_tiny_front of the first map
         launch_k(c->pdl, k_rcrit, nblk(d.ntot, 128), 128, 0, c->st, d, dt, d.mode != GENGA_MODE_TEST_PARTICLE); LAUNCH(c);
     }
     const bool merge = !(c->cfg.flags & 1) && d.mode != GENGA_MODE_TEST_PARTICLE;

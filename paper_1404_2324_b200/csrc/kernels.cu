@@ -41,6 +41,17 @@ __global__ void k_reset_counters(DevState d)
 // own velocity (L96), R_H,i = a_i (m_i / 3 m0)^(1/3) with a_i from the vis-viva relation
 // (r_i if unbound); test particles have R_H = 0.  Also stores 9 rc^2, the squared precheck
 // distance (L142: "increasing the critical radius by a factor of three").
+__device__ __forceinline__ double rcrit_of(double G, double m0, double n1, double n2, double tau,
+                                           double x, double y, double z, double vx, double vy, double vz, double m)
+{
+    double r = sqrt(x * x + y * y + z * z);
+    double v2 = vx * vx + vy * vy + vz * vz;
+    double ainv = 2.0 / r - v2 / (G * m0);
+    double a = ainv > 0.0 ? 1.0 / ainv : r;
+    double rh = m > 0.0 ? a * cbrt(m / (3.0 * m0)) : 0.0;
+    double rv = n2 * fabs(tau) * sqrt(v2);
+    return fmax(n1 * rh, rv);
+}
 __global__ void k_rcrit(DevState d, double tau, int reset)
 {
     pdl_sync();
@@ -58,15 +69,9 @@ __global__ void k_rcrit(DevState d, double tau, int reset)
     if (i >= d.ntot) return;
     double x = d.x[i], y = d.y[i], z = d.z[i], vx = d.vx[i], vy = d.vy[i], vz = d.vz[i], m = d.m[i];
     double m0 = d.m0[system_of(d, i)];
-    double r = sqrt(x * x + y * y + z * z);
-    double v2 = vx * vx + vy * vy + vz * vz;
-    double ainv = 2.0 / r - v2 / (d.G * m0);
-    double a = ainv > 0.0 ? 1.0 / ainv : r;
-    double rh = m > 0.0 ? a * cbrt(m / (3.0 * m0)) : 0.0;
     double n1 = d.n1, n2 = d.n2;
     if (d.mode == 2) { n1 = d.n12[2 * (i / d.nm)]; n2 = d.n12[2 * (i / d.nm) + 1]; }   // per system (L346-354)
-    double rv = n2 * fabs(tau) * sqrt(v2);
-    double rc = fmax(n1 * rh, rv);
+    double rc = rcrit_of(d.G, m0, n1, n2, tau, x, y, z, vx, vy, vz, m);
     d.rc[i] = rc;
     d.c9[i] = 9.0 * rc * rc;
 }
@@ -564,6 +569,101 @@ __global__ void __launch_bounds__(32) k_tpm_kick(DevState d, double h, int recor
         double s0, s1, s2;
         momentum(s0, s1, s2);
     }
+}
+
+// Massive mode with N <= 32 (the paper's small-N regime, L427-433, where a step is launch latency): ONE warp, body = lane,
+// runs a whole half map per launch.  Pair arithmetic as k_kick_multi, critical radius as k_rcrit, Sun kick and drift as k_sun.
+__device__ __forceinline__ void tiny_reset(const DevState &d)
+{
+    d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
+    d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0;
+}
+struct TinySmem { double x[32], y[32], z[32], gm[32], rc[32]; };
+__device__ __forceinline__ void tiny_kick(const DevState &d, TinySmem &S, int t, bool live, double h, int record,
+                                          double xi, double yi, double zi, double rci, double m,
+                                          double &vx, double &vy, double &vz)
+{
+    S.x[t] = xi; S.y[t] = yi; S.z[t] = zi; S.rc[t] = rci; S.gm[t] = d.G * m;
+    __syncwarp();
+    if (live) {
+        double ax = 0, ay = 0, az = 0;
+        for (int j = 0; j < d.nm; ++j) {
+            if (j == t) continue;
+            double dx = S.x[j] - xi, dy = S.y[j] - yi, dz = S.z[j] - zi;
+            double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            double rcij = fmax(rci, S.rc[j]);
+            double gm = S.gm[j];
+            double s3 = gm * rinv3_fast(r2);
+            if (r2 < 9.0 * rcij * rcij) {
+                if (r2 < rcij * rcij) {                             // W = 1 outside the changeover zone
+                    double r = sqrt(r2);
+                    s3 = gm / (r2 * r) * kick_weight(r, rcij);
+                }
+                if (record && t < j) {
+                    int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
+                    if (idx < d.cap) d.cand[idx] = make_int2(t, j);
+                    else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+                }
+            }
+            ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
+        }
+        vx = fma(h, ax, vx); vy = fma(h, ay, vy); vz = fma(h, az, vz);
+    }
+    __syncwarp();
+}
+__device__ __forceinline__ void tiny_momentum(double m, double vx, double vy, double vz, double &s0, double &s1, double &s2)
+{
+    s0 = m * vx; s1 = m * vy; s2 = m * vz;
+    for (int o = 16; o > 0; o >>= 1) {
+        s0 += __shfl_xor_sync(0xffffffffu, s0, o); s1 += __shfl_xor_sync(0xffffffffu, s1, o); s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    }
+}
+// opening half of a map: [critical radii and counter reset at the first map of a step] [kick B(hk), recording the candidates]
+// Sun kick C(h/2), Kepler drift A(h)
+__global__ void __launch_bounds__(32) k_tiny_front(DevState d, double h, double tau, int first, double hk)
+{
+    pdl_sync();
+    __shared__ TinySmem S;
+    const int t = threadIdx.x;
+    const bool live = t < d.nm;
+    double x = 0.0, y = 0.0, z = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, m = 0.0, rc = 0.0;
+    const double m0 = d.m0[0];
+    if (live) { x = d.x[t]; y = d.y[t]; z = d.z[t]; vx = d.vx[t]; vy = d.vy[t]; vz = d.vz[t]; m = d.m[t]; }
+    if (first) {
+        if (t == 0) tiny_reset(d);
+        if (live) { rc = rcrit_of(d.G, m0, d.n1, d.n2, tau, x, y, z, vx, vy, vz, m); d.rc[t] = rc; d.c9[t] = 9.0 * rc * rc; }
+        __syncwarp();
+    } else if (live) rc = d.rc[t];
+    if (hk != 0.0) tiny_kick(d, S, t, live, hk, 1, x, y, z, rc, m, vx, vy, vz);
+    double s0, s1, s2;
+    tiny_momentum(m, vx, vy, vz, s0, s1, s2);
+    if (!live) return;
+    const double g = 0.5 * h / m0;
+    x = fma(g, s0, x); y = fma(g, s1, y); z = fma(g, s2, z);
+    d.x0[t] = x; d.y0[t] = y; d.z0[t] = z; d.vx0[t] = vx; d.vy0[t] = vy; d.vz0[t] = vz;
+    if (!kepler_drift(d.G * m0, h, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
+    d.x[t] = x; d.y[t] = y; d.z[t] = z; d.vx[t] = vx; d.vy[t] = vy; d.vz[t] = vz;
+}
+// closing half of a map: Sun kick C(h/2) [counter reset: the map is over], kick B(hk) [recording the next map's candidates]
+__global__ void __launch_bounds__(32) k_tiny_back(DevState d, double h, double hk, int record, int reset)
+{
+    pdl_sync();
+    __shared__ TinySmem S;
+    const int t = threadIdx.x;
+    const bool live = t < d.nm;
+    double x = 0.0, y = 0.0, z = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, m = 0.0, rc = 0.0;
+    if (live) { x = d.x[t]; y = d.y[t]; z = d.z[t]; vx = d.vx[t]; vy = d.vy[t]; vz = d.vz[t]; m = d.m[t]; rc = d.rc[t]; }
+    if (reset) {
+        if (t == 0) tiny_reset(d);
+        __syncwarp();
+    }
+    double s0, s1, s2;
+    tiny_momentum(m, vx, vy, vz, s0, s1, s2);
+    const double g = 0.5 * h / d.m0[0];
+    x = fma(g, s0, x); y = fma(g, s1, y); z = fma(g, s2, z);
+    tiny_kick(d, S, t, live, hk, record, x, y, z, rc, m, vx, vy, vz);
+    if (!live) return;
+    d.x[t] = x; d.y[t] = y; d.z[t] = z; d.vx[t] = vx; d.vy[t] = vy; d.vz[t] = vz;
 }
 
 // =====================================================================================
