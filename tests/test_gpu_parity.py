@@ -46,6 +46,10 @@ CASES = {
     "cfg1_ragged_777": lambda: workloads.config1(n=777),
     "cfg4_full": lambda: workloads.config4(order=4),
     "cfg4_513": lambda: workloads.config4(n=513, order=6),
+    # N <= 32: the one-warp half-map kernels (k_tiny_front / k_tiny_back); 33 is the first size on the general path
+    "tiny24_order6": lambda: workloads.config4(n=24, order=6),
+    "tiny32_order4": lambda: workloads.config4(n=32, order=4),
+    "n33_order4": lambda: workloads.config4(n=33, order=4),
     "cfg2_small": lambda: workloads.config2(n_test=5000),
     "cfg2_ragged": lambda: workloads.config2(n_massive=5, n_test=1237),
     "cfg2_order4": lambda: dict(workloads.config2(n_test=3000), order=4),
@@ -73,7 +77,7 @@ def test_accelerations_rcrit_and_candidates(G, case):
     g.close()
 
 
-STEP_CASES = [("cfg0", 100), ("cfg1_full", 4), ("cfg1_ragged_777", 10), ("cfg4_full", 2), ("cfg4_513", 3),
+STEP_CASES = [("cfg0", 100), ("cfg1_full", 4), ("cfg1_ragged_777", 10), ("cfg4_full", 2), ("cfg4_513", 3), ("tiny24_order6", 30), ("tiny32_order4", 40), ("n33_order4", 40),
               ("cfg2_small", 8), ("cfg2_ragged", 8), ("cfg2_order4", 5), ("cfg2_order6_ragged", 3), ("cfg2_32massive", 6),
               ("cfg3_order4", 20), ("cfg3_small", 60), ("cfg3_7bodies", 60)]
 
@@ -366,10 +370,11 @@ def test_host_and_device_state_paths_agree_and_contexts_are_independent(G):
     g1.close(); g2.close()
 
 
-def test_merged_and_separate_kicks_are_the_same_map(G):
+@pytest.mark.parametrize("n", [513, 20])                     # 20: the one-warp kernels of N <= 32
+def test_merged_and_separate_kicks_are_the_same_map(G, n):
     """flags bit 0 keeps the closing kick of a substep and the opening kick of the next apart (orders 4, 6): same map,
     rounding differs; both agree with the oracle (which never merges)."""
-    w = workloads.config4(n=513, order=6)
+    w = workloads.config4(n=n, order=6)
     o = oracle.Sim(w, cap=200000)
     o.step(3, w["dt"], 6)
     xo, vo = o.state()
