@@ -378,7 +378,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         }
     }
     const int pair_blocks = (int)std::min<long long>((d.cap + 127) / 128, 16LL * c->sms);   // grid-stride over the candidates; enough warps to cover the gather latency when there are 10^6 of them (mode 1)
-    launch_k(c->pdl, k_confirm, pair_blocks, 128, 0, st, d, h); LAUNCH(c);
+    if (!tiny_mode(d)) { launch_k(c->pdl, k_confirm, pair_blocks, 128, 0, st, d, h); LAUNCH(c); }   // N <= 32: inside k_tiny_front
     const int warp_blocks = 2 * c->sms;                       // 4 warps each; warps take groups from a queue
     if (d.mode == GENGA_MODE_MULTI_SYSTEM) {
         launch_k(c->pdl, k_list_groups_multi, nblk(d.ntot, 256), 256, 0, st, d); LAUNCH(c);

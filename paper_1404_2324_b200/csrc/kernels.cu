@@ -637,12 +637,38 @@ __global__ void __launch_bounds__(32) k_tiny_front(DevState d, double h, double 
     if (hk != 0.0) tiny_kick(d, S, t, live, hk, 1, x, y, z, rc, m, vx, vy, vz);
     double s0, s1, s2;
     tiny_momentum(m, vx, vy, vz, s0, s1, s2);
-    if (!live) return;
-    const double g = 0.5 * h / m0;
-    x = fma(g, s0, x); y = fma(g, s1, y); z = fma(g, s2, z);
-    d.x0[t] = x; d.y0[t] = y; d.z0[t] = z; d.vx0[t] = vx; d.vy0[t] = vy; d.vz0[t] = vz;
-    if (!kepler_drift(d.G * m0, h, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
-    d.x[t] = x; d.y[t] = y; d.z[t] = z; d.vx[t] = vx; d.vy[t] = vy; d.vz[t] = vz;
+    __shared__ double Q[12][32], src[32];                     // state before and after the drift, critical radii
+    if (live) {
+        const double g = 0.5 * h / m0;
+        x = fma(g, s0, x); y = fma(g, s1, y); z = fma(g, s2, z);
+        d.x0[t] = x; d.y0[t] = y; d.z0[t] = z; d.vx0[t] = vx; d.vy0[t] = vy; d.vz0[t] = vz;
+        Q[0][t] = x; Q[1][t] = y; Q[2][t] = z; Q[3][t] = vx; Q[4][t] = vy; Q[5][t] = vz;
+        if (!kepler_drift(d.G * m0, h, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
+        d.x[t] = x; d.y[t] = y; d.z[t] = z; d.vx[t] = vx; d.vy[t] = vy; d.vz[t] = vz;
+        Q[6][t] = x; Q[7][t] = y; Q[8][t] = z; Q[9][t] = vx; Q[10][t] = vy; Q[11][t] = vz;
+        src[t] = rc;
+    }
+    __syncwarp();
+    // encounter search over the candidates (k_confirm's arithmetic; the candidates come from this launch's kick or from
+    // the merged kick of the previous map's k_tiny_back)
+    const int nc = min(atomicAdd(&d.cnt[CI_NCAND], 0), (int)d.cap);
+    for (int e = t; e < nc; e += 32) {
+        const int2 p = __ldcg(&d.cand[e]);
+        const int i = p.x, j = p.y;
+        double dx = Q[0][j] - Q[0][i], dy = Q[1][j] - Q[1][i], dz = Q[2][j] - Q[2][i];
+        double dvx = Q[3][j] - Q[3][i], dvy = Q[4][j] - Q[4][i], dvz = Q[5][j] - Q[5][i];
+        double P0 = dx * dx + dy * dy + dz * dz, Pd0 = 2.0 * (dx * dvx + dy * dvy + dz * dvz);
+        dx = Q[6][j] - Q[6][i]; dy = Q[7][j] - Q[7][i]; dz = Q[8][j] - Q[8][i];
+        dvx = Q[9][j] - Q[9][i]; dvy = Q[10][j] - Q[10][i]; dvz = Q[11][j] - Q[11][i];
+        double P1 = dx * dx + dy * dy + dz * dz, Pd1 = 2.0 * (dx * dvx + dy * dvy + dz * dvz);
+        double rcij = fmax(src[i], src[j]);
+        double D = hermite_min(P0, P1, Pd0, Pd1, h);
+        if (D < rcij * rcij) {
+            int idx = atomicAdd(&d.cnt[CI_NENC], 1);
+            if (idx < d.cap) d.enc[idx] = p;
+            else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+        }
+    }
 }
 // closing half of a map: Sun kick C(h/2) [counter reset: the map is over], kick B(hk) [recording the next map's candidates]
 __global__ void __launch_bounds__(32) k_tiny_back(DevState d, double h, double hk, int record, int reset)
