@@ -369,6 +369,8 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         launch_k(c->pdl, k_drift, nblk(d.nm, 128), 128, 0, st, dm, h, 0.5 * h); LAUNCH(c);   // Sun kick + drift of the massive bodies
     } else if (tiny_mode(d)) {                                // N <= 32: the opening half map in one warp, one launch
         launch_k(c->pdl, k_tiny_front, 1, 32, 0, st, d, h, tau, first, opened ? 0.0 : 0.5 * h); LAUNCH(c);
+    } else if (d.mode == GENGA_MODE_MULTI_SYSTEM) {           // a block holds whole systems: the opening half map in one launch
+        launch_k(c->pdl, k_multi_front, nblk(d.nsys, 128 / d.nm), 128, 0, st, d, h, opened ? 0.0 : 0.5 * h); LAUNCH(c);
     } else {
         if (!opened) enqueue_kick(c, 0.5 * h, 1, nullptr);        // else: done by the previous map's merged kick
         if (d.mode != GENGA_MODE_TEST_PARTICLE) enqueue_sun(c, 0.5 * h, 0, false, h);   // Sun kick and drift in one launch
@@ -414,6 +416,8 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         launch_k(c->pdl, k_tp_back, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h); LAUNCH(c);
     } else if (tiny_mode(d)) {                                // plain launch: see enqueue_sun
         launch_k(false, k_tiny_back, 1, 32, 0, st, d, h, hn != 0.0 ? 0.5 * (h + hn) : 0.5 * h, hn != 0.0 ? 1 : 0, last ? 0 : 1); LAUNCH(c);
+    } else if (d.mode == GENGA_MODE_MULTI_SYSTEM && last) {   // no counter reset after the last map: Sun kick and kick in one launch (plain: see enqueue_sun)
+        launch_k(false, k_multi_back, nblk(d.nsys, 128 / d.nm), 128, 0, st, d, h, 0.5 * h); LAUNCH(c);
     } else {
         enqueue_sun(c, 0.5 * h, last ? 0 : 1, true);
         if (hn != 0.0) enqueue_kick(c, 0.5 * (h + hn), 1, nullptr);   // closing kick + opening kick of the next map

@@ -692,6 +692,104 @@ __global__ void __launch_bounds__(32) k_tiny_back(DevState d, double h, double h
     d.x[t] = x; d.y[t] = y; d.z[t] = z; d.vx[t] = vx; d.vy[t] = vy; d.vz[t] = vz;
 }
 
+// Multi-system mode, half maps in one launch (a block holds whole systems, so nothing crosses blocks): the pair loop of
+// k_kick_multi, the momentum sum, Sun kick and drift of k_sun with the same arithmetic in the same order.
+struct MultiSmem { double x[128], y[128], z[128], gm[128], rc[128], m[128], vx[128], vy[128], vz[128]; };
+__device__ __forceinline__ void multi_pairs(const DevState &d, const MultiSmem &S, int t, int i, int sb, int record,
+                                            double xi, double yi, double zi, double rci, double &ax, double &ay, double &az)
+{
+    ax = ay = az = 0.0;
+    for (int k = 0; k < d.nm; ++k) {
+        const int jt = sb + k;
+        if (jt == t) continue;
+        double dx = S.x[jt] - xi, dy = S.y[jt] - yi, dz = S.z[jt] - zi;
+        double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+        double rcij = fmax(rci, S.rc[jt]);
+        double gm = S.gm[jt];
+        double s3 = gm * rinv3_fast(r2);
+        if (r2 < 9.0 * rcij * rcij) {
+            if (r2 < rcij * rcij) {                             // W = 1 outside the changeover zone
+                double r = sqrt(r2);
+                s3 = gm / (r2 * r) * kick_weight(r, rcij);
+            }
+            const int j = i - t + jt;
+            if (record && i < j) {
+                int idx = atomicAdd(&d.cnt[CI_NCAND], 1);
+                if (idx < d.cap) d.cand[idx] = make_int2(i, j);
+                else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+            }
+        }
+        ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
+    }
+}
+// opening half: [kick B(hk), recording the candidates] Sun kick C(h/2), drift A(h); labels reset for the map's grouping
+__global__ void __launch_bounds__(128) k_multi_front(DevState d, double h, double hk)
+{
+    pdl_sync();
+    __shared__ MultiSmem S;
+    const int nm = d.nm, spb = 128 / nm, t = threadIdx.x;
+    const int i = blockIdx.x * spb * nm + t;
+    const bool live = t < spb * nm && i < d.ntot;
+    double x = 0.0, y = 0.0, z = 0.0, rc = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, m = 0.0;
+    if (live) {
+        x = d.x[i]; y = d.y[i]; z = d.z[i]; rc = d.rc[i]; vx = d.vx[i]; vy = d.vy[i]; vz = d.vz[i]; m = d.m[i];
+        d.label[i] = i;
+        S.x[t] = x; S.y[t] = y; S.z[t] = z; S.rc[t] = rc; S.gm[t] = d.G * m; S.m[t] = m;
+    }
+    __syncthreads();
+    const int sb = (t / nm) * nm;
+    if (live && hk != 0.0) {
+        double ax, ay, az;
+        multi_pairs(d, S, t, i, sb, 1, x, y, z, rc, ax, ay, az);
+        vx = fma(hk, ax, vx); vy = fma(hk, ay, vy); vz = fma(hk, az, vz);
+    }
+    if (live) { S.vx[t] = vx; S.vy[t] = vy; S.vz[t] = vz; }
+    __syncthreads();
+    if (!live) return;
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    for (int k = 0; k < nm; ++k) {
+        const double mk = S.m[sb + k];
+        sx = fma(mk, S.vx[sb + k], sx); sy = fma(mk, S.vy[sb + k], sy); sz = fma(mk, S.vz[sb + k], sz);
+    }
+    const double m0 = d.m0[i / nm], g = 0.5 * h / m0;
+    x = fma(g, sx, x); y = fma(g, sy, y); z = fma(g, sz, z);
+    d.x0[i] = x; d.y0[i] = y; d.z0[i] = z; d.vx0[i] = vx; d.vy0[i] = vy; d.vz0[i] = vz;
+    if (!kepler_drift(d.G * m0, h, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
+    d.x[i] = x; d.y[i] = y; d.z[i] = z; d.vx[i] = vx; d.vy[i] = vy; d.vz[i] = vz;
+}
+// closing half of the LAST map of a step (no counter reset: the step's encounter data stay readable): Sun kick C(h/2), kick B(hk)
+__global__ void __launch_bounds__(128) k_multi_back(DevState d, double h, double hk)
+{
+    pdl_sync();
+    __shared__ MultiSmem S;
+    const int nm = d.nm, spb = 128 / nm, t = threadIdx.x;
+    const int i = blockIdx.x * spb * nm + t;
+    const bool live = t < spb * nm && i < d.ntot;
+    double x = 0.0, y = 0.0, z = 0.0, rc = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, m = 0.0;
+    if (live) {
+        x = d.x[i]; y = d.y[i]; z = d.z[i]; rc = d.rc[i]; vx = d.vx[i]; vy = d.vy[i]; vz = d.vz[i]; m = d.m[i];
+        S.m[t] = m; S.vx[t] = vx; S.vy[t] = vy; S.vz[t] = vz; S.rc[t] = rc; S.gm[t] = d.G * m;
+    }
+    __syncthreads();
+    const int sb = (t / nm) * nm;
+    if (live) {
+        double sx = 0.0, sy = 0.0, sz = 0.0;
+        for (int k = 0; k < nm; ++k) {
+            const double mk = S.m[sb + k];
+            sx = fma(mk, S.vx[sb + k], sx); sy = fma(mk, S.vy[sb + k], sy); sz = fma(mk, S.vz[sb + k], sz);
+        }
+        const double g = 0.5 * h / d.m0[i / nm];
+        x = fma(g, sx, x); y = fma(g, sy, y); z = fma(g, sz, z);
+        S.x[t] = x; S.y[t] = y; S.z[t] = z;
+    }
+    __syncthreads();
+    if (!live) return;
+    double ax, ay, az;
+    multi_pairs(d, S, t, i, sb, 0, x, y, z, rc, ax, ay, az);
+    d.x[i] = x; d.y[i] = y; d.z[i] = z;
+    d.vx[i] = fma(hk, ax, vx); d.vy[i] = fma(hk, ay, vy); d.vz[i] = fma(hk, az, vz);
+}
+
 // =====================================================================================
 // Sun kick, operator C (Eq. 3; L196, L232-236, L338, L360-366): s = sum over massive
 // bodies of m V (one block per system, fixed-order tree), then q_i += h s / m0 for every

@@ -25,6 +25,8 @@ __global__ void k_tp_front(DevState d, double h, double tau, int first);
 __global__ void k_tp_back(DevState d, double h);
 __global__ void k_kick_multi(DevState d, double h, int record, double *aout);
 __global__ void k_sun(DevState d, double h, int reset, double hdrift);
+__global__ void k_multi_front(DevState d, double h, double hk);
+__global__ void k_multi_back(DevState d, double h, double hk);
 __global__ void k_tiny_front(DevState d, double h, double tau, int first, double hk);
 __global__ void k_tiny_back(DevState d, double h, double hk, int record, int reset);
 __global__ void k_tpm_kick(DevState d, double h, int record, double fshift);
