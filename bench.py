@@ -290,7 +290,9 @@ def run_gpu(args):
         roof = {"bound": "alu", "kernel": "k_kick_multi", "achieved": achieved, "peak": peak_probe, "unit": "TFLOP/s",
                 "frac": achieved / peak_probe, "traffic": traffic_tab.get("k_kick_multi"), "ms_per_launch": kick_ms,
                 "interactions_per_launch": inter, "flop_per_interaction": FLOP_PER_INTERACTION,
-                "peak_source": "DFMA probe measured in this run (genga_fp64_probe)"}
+                "peak_source": "DFMA probe measured in this run (genga_fp64_probe)",
+                "note": "the pair loop timed alone; inside a step it runs within k_multi_front / k_multi_back (kick + Sun kick "
+                        "[+ drift] in one launch), and the step is bound by the Bulirsch-Stoer chain of k_bs_warp"}
 
     # ---- aggregate over ranks (replicas: no data-path collective)
     tmax, units = reduce_max_and_sum(elapsed, per_step * args.steps, dev)
