@@ -225,9 +225,8 @@ static int red_threads(int nm) { return std::min(1024, std::max(32, (int)up((siz
 static void enqueue_helio_to_demo(genga_ctx *c)
 {
     DevState &d = c->d;
-    k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx0, d.vy0, d.vz0, 0.0);
-    k_shift_out<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx0, d.vy0, d.vz0, d.vx, d.vy, d.vz, -1.0, 1);
-    c->launches += 2;
+    k_coord_map<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx0, d.vy0, d.vz0, d.vx, d.vy, d.vz, -1.0, 1);
+    c->launches += 1;
 }
 
 static int set_state_impl(genga_ctx *c, const double *m0, const double *m, const double *radius,
@@ -531,9 +530,8 @@ static int get_state_impl(genga_ctx *c, double *x, double *v, cudaMemcpyKind kin
     if (!c || !x || !v) return GENGA_EINVAL;
     DevState &d = c->d;
     const size_t n = (size_t)d.ntot, B = sizeof(double);
-    k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx, d.vy, d.vz, 0.0);
-    k_shift_out<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0);
-    c->launches += 2;
+    k_coord_map<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0);
+    c->launches += 1;
     const double *src[6] = {d.x, d.y, d.z, d.vx0, d.vy0, d.vz0};
     if ((size_t)d.np == n) {
         CK(cudaMemcpyAsync(x, d.x, 3 * B * n, kind, c->st));
@@ -556,9 +554,8 @@ extern "C" __attribute__((visibility("default"))) int genga_get_state_host(genga
     if (c && c->hstage && x && v) {                            // small state: one copy, unpack after the latch's sync
         DevState &d = c->d;
         const size_t n = (size_t)d.ntot, np = (size_t)d.np, B = sizeof(double);
-        k_momentum<<<d.nsys, red_threads(d.nm), 0, c->st>>>(d, d.vx, d.vy, d.vz, 0.0);
-        k_shift_out<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0);
-        c->launches += 2;
+        k_coord_map<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0);
+        c->launches += 1;
         CK(cudaMemcpyAsync(c->hstage, d.x, 6 * B * np, cudaMemcpyDeviceToHost, c->st));
         CK(cudaGetLastError());
         int r = latch(c);

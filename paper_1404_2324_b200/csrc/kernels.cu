@@ -914,17 +914,52 @@ __global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset, do
     }
     d.x[i] = x; d.y[i] = y; d.z[i] = z;
 }
-// out = in + f * psum / den  (coordinate maps at the ABI, L69)
-__global__ void k_shift_out(DevState d, const double *ix, const double *iy, const double *iz,
-                            double *ox, double *oy, double *oz, double f, int divide_by_total)
+// Coordinate maps at the ABI in ONE launch (L69): out = in + f * s / den, s = sum m * in over the massive bodies of the
+// system, den = m0 (+ sum m if divide_by_total).  Every block forms s itself, in a fixed order: modes 0, 1 as k_sun
+// (at most 8 bodies per thread, then a tree), mode 2 a thread sums the bodies of its own system.
+__global__ void __launch_bounds__(256) k_coord_map(DevState d, const double *ix, const double *iy, const double *iz,
+                                                   double *ox, double *oy, double *oz, double f, int divide_by_total)
 {
     pdl_sync();
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= d.ntot) return;
-    int sys = system_of(d, i);
-    double den = divide_by_total ? d.m0[sys] + d.psum[4 * sys + 3] : d.m0[sys];
-    double g = f / den;
-    ox[i] = fma(g, d.psum[4 * sys], ix[i]); oy[i] = fma(g, d.psum[4 * sys + 1], iy[i]); oz[i] = fma(g, d.psum[4 * sys + 2], iz[i]);
+    __shared__ double red[4][8];
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    double sx = 0.0, sy = 0.0, sz = 0.0, sm = 0.0, m0;
+    if (d.mode == 2) {
+        if (i >= d.ntot) return;
+        const int sys = i / d.nm, base = sys * d.nm;
+        for (int k = 0; k < d.nm; ++k) {
+            double m = d.m[base + k];
+            sx = fma(m, ix[base + k], sx); sy = fma(m, iy[base + k], sy); sz = fma(m, iz[base + k], sz);
+            sm += m;
+        }
+        m0 = d.m0[sys];
+    } else {
+#pragma unroll
+        for (int q = 0; q < KK_MAXN / 256; ++q) {
+            const int k = threadIdx.x + 256 * q;
+            if (k < d.nm) {
+                double m = d.m[k];
+                sx = fma(m, ix[k], sx); sy = fma(m, iy[k], sy); sz = fma(m, iz[k], sz);
+                sm += m;
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            sx += __shfl_xor_sync(0xffffffffu, sx, o); sy += __shfl_xor_sync(0xffffffffu, sy, o);
+            sz += __shfl_xor_sync(0xffffffffu, sz, o); sm += __shfl_xor_sync(0xffffffffu, sm, o);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            red[0][threadIdx.x >> 5] = sx; red[1][threadIdx.x >> 5] = sy; red[2][threadIdx.x >> 5] = sz; red[3][threadIdx.x >> 5] = sm;
+        }
+        __syncthreads();
+        sx = sy = sz = sm = 0.0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) { sx += red[0][w]; sy += red[1][w]; sz += red[2][w]; sm += red[3][w]; }
+        m0 = d.m0[0];
+        if (i >= d.ntot) return;
+    }
+    const double g = f / (divide_by_total ? m0 + sm : m0);
+    ox[i] = fma(g, sx, ix[i]); oy[i] = fma(g, sy, iy[i]); oz[i] = fma(g, sz, iz[i]);
 }
 
 // =====================================================================================

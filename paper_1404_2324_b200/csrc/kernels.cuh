@@ -27,13 +27,12 @@ __global__ void k_kick_multi(DevState d, double h, int record, double *aout);
 __global__ void k_sun(DevState d, double h, int reset, double hdrift);
 __global__ void k_multi_front(DevState d, double h, double hk);
 __global__ void k_multi_back(DevState d, double h, double hk);
+__global__ void k_coord_map(DevState d, const double *ix, const double *iy, const double *iz, double *ox, double *oy, double *oz, double f, int divide_by_total);
 __global__ void k_tiny_front(DevState d, double h, double tau, int first, double hk);
 __global__ void k_tiny_back(DevState d, double h, double hk, int record, int reset);
 __global__ void k_tpm_kick(DevState d, double h, int record, double fshift);
 __global__ void k_momentum(DevState d, const double *vx, const double *vy, const double *vz, double fshift);
 __global__ void k_shift(DevState d, double *ax, double *ay, double *az, double f, int divide_by_total);
-__global__ void k_shift_out(DevState d, const double *ix, const double *iy, const double *iz,
-                            double *ox, double *oy, double *oz, double f, int divide_by_total);
 __global__ void k_drift(DevState d, double h, double hsun);
 __global__ void k_drift_arrays(long long n, double mu, double h, double *x, double *v, int *status);
 __global__ void k_confirm(DevState d, double h);
