@@ -63,7 +63,7 @@ typedef struct {
     double G;           /* gravitational constant                                            */
     double n1, n2;      /* critical-radius parameters of Eq. 6 (L94-96); usually 3 and 0.4   */
     double bs_eps;      /* Bulirsch-Stoer relative tolerance (L116 "machine precision")      */
-    int64_t max_pairs;  /* capacity of the candidate list and of the encounter list          */
+    int64_t max_pairs;  /* capacity of the candidate list and of the encounter list, 1 .. 2^31 - 1 */
     void *workspace;    /* device memory, >= genga_workspace_bytes(), 256-byte aligned        */
     size_t workspace_bytes;
     void *stream;       /* cudaStream_t; NULL = the legacy default stream                     */
@@ -160,9 +160,10 @@ int genga_accelerations(genga_ctx *ctx, double dt, double *a, double *rcrit);
  * x[3*n], v[3*n] DEVICE, updated in place.  Stand-alone: needs no state in the context. */
 int genga_kepler_drift(genga_ctx *ctx, int64_t n, double mu, double h, double *x, double *v);
 
-/* Counters accumulated since genga_create, HOST out[8]:
+/* Counters accumulated since genga_create, HOST out[16]:
  *  0 steps, 1 force evaluations, 2 ordered pair interactions evaluated, 3 kernel launches,
- *  4 groups integrated, 5 largest group, 6 BS steps accepted, 7 candidates seen.
+ *  4 groups integrated, 5 largest group, 6 BS steps accepted, 7 candidates seen,
+ *  8 BS attempts rejected (all eight extrapolation columns failed, step halved), 9..15 reserved (0).
  * Synchronises. */
 int genga_counters(genga_ctx *ctx, int64_t *out);
 
@@ -176,6 +177,22 @@ int genga_counters(genga_ctx *ctx, int64_t *out);
  * The state is left unchanged up to rounding (3, 4: up to the integration error of the
  * pass and its inverse).  Synchronises. */
 int genga_time_kernel(genga_ctx *ctx, int which, int reps, double dt, double *ms_per_launch);
+
+/* Run n_steps (1..4096) time steps exactly as genga_step does, but as plain launches with a CUDA event at every
+ * phase boundary instead of a graph replay, and report the time per step of each phase, HOST ms[8]:
+ *   0 critical radii (Eq. 6)   1 kicks (Eq. 2; every pair-force launch of the step)
+ *   2 opening half map: Sun kick + Kepler drift (Eq. 3, Eq. 9; the fused half-map kernels of the small-N,
+ *     particle and multi-system layouts count here as a whole, their kick included)
+ *   3 encounter search (Eq. 10-12)   4 grouping (Appendix)   5 Bulirsch-Stoer (L116), all layouts
+ *   6 closing half map: Sun kick (and kick where fused)   7 sum of the phases.
+ * The state advances by n_steps steps.  Synchronises. */
+int genga_profile_step(genga_ctx *ctx, int64_t n_steps, double dt, int order, double *ms);
+
+/* out[i] = f(in[i]) with the library's reciprocal routines built on the hardware seeds, in FP64:
+ * which = 0: x^(-1/2), 1: x^(-3/2), 2: 1/x, for positive normal x.  The paper keeps IEEE sqrt and divide for fear of a
+ * biased error (L228, L264); tests/test_gpu_fastmath.py measures the signed error of these in ulps.
+ * in, out: DEVICE pointers to n doubles.  Enqueues, no sync. */
+int genga_eval_fast(genga_ctx *ctx, int which, int64_t n, const double *in, double *out);
 
 /* Measure the device's FP64 FMA throughput with independent DFMA chains on every SM:
  * *tflops (HOST out) = 2 * DFMAs / time.  The ALU-roofline denominator.  Synchronises. */

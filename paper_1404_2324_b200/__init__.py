@@ -23,7 +23,8 @@ SYMBOLS = [
     "genga_workspace_bytes", "genga_create", "genga_destroy", "genga_set_state", "genga_set_state_host",
     "genga_step", "genga_get_state", "genga_get_state_host", "genga_set_state_ragged_host", "genga_get_state_ragged_host", "genga_set_system_params_host",
     "genga_energy", "genga_encounters",
-    "genga_status", "genga_accelerations", "genga_kepler_drift", "genga_counters", "genga_time_kernel", "genga_fp64_probe", "genga_strerror",
+    "genga_status", "genga_accelerations", "genga_kepler_drift", "genga_counters", "genga_time_kernel", "genga_profile_step",
+    "genga_eval_fast", "genga_fp64_probe", "genga_strerror",
     "genga_last_cuda_error",
 ]
 
@@ -78,6 +79,8 @@ def load():
         "genga_kepler_drift": (i, [vp, l, d, d, dp, dp]),
         "genga_counters": (i, [vp, vp]),
         "genga_time_kernel": (i, [vp, i, i, d, C.POINTER(d)]),
+        "genga_profile_step": (i, [vp, l, d, i, vp]),
+        "genga_eval_fast": (i, [vp, i, l, dp, dp]),
         "genga_fp64_probe": (i, [vp, C.POINTER(d)]),
         "genga_strerror": (C.c_char_p, [i]),
         "genga_last_cuda_error": (C.c_char_p, []),
@@ -150,6 +153,14 @@ class Genga:
             a = t.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device=self.device)
         return a
 
+    def _order_before(self):
+        """the context's stream waits for the work the caller queued on torch's current stream (the tensors passed in)"""
+        self.stream.wait_stream(self.torch.cuda.current_stream(self.device))
+
+    def _order_after(self):
+        """torch's current stream waits for the work this call queued on the context's stream"""
+        self.torch.cuda.current_stream(self.device).wait_stream(self.stream)
+
     def set_state(self, m0, m, radius, x, v):
         """Device path: arguments are moved to the device first (if they are not there),
         then handed to genga_set_state as device pointers."""
@@ -173,6 +184,7 @@ class Genga:
         t = self.torch
         x = t.empty((3, self.ntot), dtype=t.float64, device=self.device)
         v = t.empty((3, self.ntot), dtype=t.float64, device=self.device)
+        self._order_before()
         _chk(self.lib.genga_get_state(self.h, x.data_ptr(), v.data_ptr()), "genga_get_state")
         self.stream.synchronize()
         return x, v
@@ -224,6 +236,7 @@ class Genga:
         t = self.torch
         a = t.empty((3, self.ntot), dtype=t.float64, device=self.device)
         rc = t.empty(self.ntot, dtype=t.float64, device=self.device)
+        self._order_before()
         _chk(self.lib.genga_accelerations(self.h, float(dt), a.data_ptr(), rc.data_ptr()), "genga_accelerations")
         self.stream.synchronize()
         return a, rc
@@ -231,13 +244,31 @@ class Genga:
     def kepler_drift(self, mu, h, x, v):
         """In-place drift of device tensors x, v of shape (3, n)."""
         n = x.shape[1]
+        self._order_before()
         _chk(self.lib.genga_kepler_drift(self.h, n, float(mu), float(h), x.data_ptr(), v.data_ptr()), "genga_kepler_drift")
+        self._order_after()
 
     def counters(self):
-        out = np.zeros(8, dtype=np.int64)
+        out = np.zeros(16, dtype=np.int64)
         _chk(self.lib.genga_counters(self.h, _hp(out)), "genga_counters")
-        keys = ["steps", "force_evals", "interactions", "launches", "groups", "max_group", "bs_steps", "candidates"]
+        keys = ["steps", "force_evals", "interactions", "launches", "groups", "max_group", "bs_steps", "candidates", "bs_rejects"]
         return dict(zip(keys, map(int, out)))
+
+    PHASES = ["rcrit", "kick", "front", "confirm", "group", "bs", "back", "total"]
+
+    def profile_step(self, n_steps, dt, order=2):
+        """ms per step of each phase (genga_profile_step)."""
+        ms = np.zeros(8)
+        _chk(self.lib.genga_profile_step(self.h, int(n_steps), float(dt), int(order), _hp(ms)), "genga_profile_step")
+        return dict(zip(self.PHASES, map(float, ms)))
+
+    def eval_fast(self, which, x):
+        """x: device float64 tensor; returns f(x) for f = x^-1/2, x^-3/2, 1/x (which = 0, 1, 2)."""
+        out = self.torch.empty_like(x)
+        self._order_before()
+        _chk(self.lib.genga_eval_fast(self.h, int(which), x.numel(), x.data_ptr(), out.data_ptr()), "genga_eval_fast")
+        self.stream.synchronize()
+        return out
 
     def time_kernel(self, which, reps, dt):
         ms = C.c_double()

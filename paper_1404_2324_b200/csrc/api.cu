@@ -55,7 +55,28 @@ struct genga_ctx {
     std::map<GraphKey, GraphEntry> graphs;
     long long steps, force_evals, interactions, launches;
     long long acc;              // launches enqueued (or captured) since last reset
+    // genga_profile_step: events at the phase boundaries of plain (uncaptured) launches
+    bool prof;
+    std::vector<cudaEvent_t> prof_ev;
+    std::vector<int> prof_phase;
+    size_t prof_used;
 };
+
+// phases of a step as genga_profile_step reports them (include/genga.h)
+enum : int { PH_RCRIT = 0, PH_KICK = 1, PH_FRONT = 2, PH_CONFIRM = 3, PH_GROUP = 4, PH_BS = 5, PH_BACK = 6, PH_TOTAL = 7, PH_COUNT = 8 };
+
+static void mark(genga_ctx *c, int phase)
+{
+    if (!c->prof) return;
+    if (c->prof_used == c->prof_ev.size()) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return;
+        c->prof_ev.push_back(e);
+        c->prof_phase.push_back(0);
+    }
+    c->prof_phase[c->prof_used] = phase;
+    cudaEventRecord(c->prof_ev[c->prof_used++], c->st);
+}
 
 static inline size_t up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -66,7 +87,8 @@ static bool valid_cfg(const genga_config *c)
     else if (c->mode == GENGA_MODE_TEST_PARTICLE) { if (c->n_massive < 1 || c->n_massive > 32 || c->n_test < 0 || c->n_test > 1000000) return false; }
     else if (c->mode == GENGA_MODE_MULTI_SYSTEM) { if (c->n_massive < 1 || c->n_massive > 16 || c->n_systems < 1 || c->n_systems > 100000 || c->n_test != 0) return false; }
     else return false;
-    if (!(c->G > 0.0) || c->n1 < 0.0 || c->n2 < 0.0 || !(c->bs_eps > 0.0) || c->max_pairs < 1) return false;
+    if (!(c->G > 0.0) || c->n1 < 0.0 || c->n2 < 0.0 || !(c->bs_eps > 0.0)) return false;
+    if (c->max_pairs < 1 || c->max_pairs > 0x7fffffffLL) return false;      // the device counters and list indices are int
     return true;
 }
 
@@ -106,6 +128,10 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
     if (c->mode == GENGA_MODE_MASSIVE && nm > BCB_MAXN) {
         t.bss.stride = npm;
         t.bss.base = (double *)take(sizeof(double) * (size_t)BSA_COUNT * npm);
+    }
+    if (c->mode == GENGA_MODE_TEST_PARTICLE && nm + 1 > 32) {  // a particle group of 33 bodies: k_tp_bs_big's scratch
+        t.bss.stride = 64 * TPBIG_BLOCKS;
+        t.bss.base = (double *)take(sizeof(double) * (size_t)BSA_COUNT * t.bss.stride);
     }
     if (c->mode == GENGA_MODE_TEST_PARTICLE) {
         size_t nt = (size_t)std::max<long long>(c->n_test, 1);
@@ -158,6 +184,7 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     c->bs_big_clusters = std::max(1, c->sms / BCB_CS);
     c->steps = c->force_evals = c->interactions = c->launches = 0;
     c->acc = 0;
+    c->prof = false; c->prof_used = 0;
     c->hstage = nullptr; c->hstatus = nullptr; c->ev_stage = nullptr; c->stage_busy = false;
     size_t need = carve(cfg, (char *)cfg->workspace, &c->d, &c->exp_labels, &c->eout, c->sms);
     if (need > cfg->workspace_bytes) { delete c; return GENGA_EINVAL; }
@@ -191,6 +218,7 @@ extern "C" __attribute__((visibility("default"))) int genga_destroy(genga_ctx *c
 {
     if (!c) return GENGA_EINVAL;
     for (auto &kv : c->graphs) cudaGraphExecDestroy(kv.second.exec);
+    for (auto e : c->prof_ev) cudaEventDestroy(e);
     for (int k = 0; k < 2; ++k) { cudaStreamDestroy(c->aux[k]); cudaEventDestroy(c->ev_join[k]); }
     cudaEventDestroy(c->ev_fork);
     if (c->hstage) cudaFreeHost(c->hstage);
@@ -288,15 +316,17 @@ extern "C" __attribute__((visibility("default"))) int genga_set_state_host(genga
 
 // ---------------------------------------------------------------------------------------
 // kick of the massive bodies: one block per SM owning ni bodies i, TJ bodies j per thread
-static void launch_kick(genga_ctx *c, double h, int record, double *aout)
+static void launch_kick(genga_ctx *c, double h, int record, double *aout, int to0 = 0)
 {
     DevState &d = c->d;
     const int ni = std::min(KK_NI, (d.nm + c->sms - 1) / c->sms);
     const int grid = (d.nm + ni - 1) / ni;
-    launch_k(c->pdl, k_kick, grid, KK_THREADS, kick_smem_bytes(), c->st, d, h, record, ni, aout);
+    launch_k(c->pdl, k_kick, grid, KK_THREADS, kick_smem_bytes(), c->st, d, h, record, ni, aout, to0);
 }
 
-static void enqueue_kick(genga_ctx *c, double h, int record, double *aout)
+// to0 (mode 0): the kick is followed by the fused Sun kick + drift (k_sun with hdrift != 0), which reads the kicked
+// velocities from the pre-drift arrays vx0.. and writes the drifted ones to vx..
+static void enqueue_kick(genga_ctx *c, double h, int record, double *aout, int to0 = 0)
 {
     DevState &d = c->d;
     if (d.mode == GENGA_MODE_MULTI_SYSTEM) {
@@ -304,7 +334,7 @@ static void enqueue_kick(genga_ctx *c, double h, int record, double *aout)
         LAUNCH(c);
         return;
     }
-    launch_kick(c, h, record, aout);
+    launch_kick(c, h, record, aout, d.mode == GENGA_MODE_MASSIVE ? to0 : 0);
     LAUNCH(c);
     if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {
         launch_k(c->pdl, k_tp_kick, nblk(d.ntot - d.nm, 128), 128, 0, c->st, d, h, record, aout);
@@ -322,7 +352,7 @@ static void enqueue_sun(genga_ctx *c, double h, int reset = 0, bool after_bs = f
         LAUNCH(c);
         return;
     }
-    launch_k(c->pdl, k_momentum, d.nsys, red_threads(d.nm), 0, c->st, d, d.vx, d.vy, d.vz, 0.0);
+    launch_k(c->pdl && !after_bs, k_momentum, d.nsys, red_threads(d.nm), 0, c->st, d, d.vx, d.vy, d.vz, 0.0);
     launch_k(c->pdl, k_shift, nblk(d.ntot, 256), 256, 0, c->st, d, d.x, d.y, d.z, h, 0);
     LAUNCH(c); LAUNCH(c);
 }
@@ -357,6 +387,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
     const bool tp = d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm;
     DevState dm = d;                                          // the massive bodies alone (mode 1)
     dm.ntot = d.nm;
+    mark(c, PH_FRONT);
     if (d.mode == GENGA_MODE_TEST_PARTICLE && !first) {       // first map: inside k_rcrit; modes 0, 2: k_rcrit (first map), closing k_sun (later maps)
         launch_k(c->pdl, k_begin_map, c->sms, 256, 0, st, d); LAUNCH(c);
         launch_k(c->pdl, k_reset_counters, 1, 32, 0, st, d); LAUNCH(c);
@@ -371,7 +402,9 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
     } else if (d.mode == GENGA_MODE_MULTI_SYSTEM) {           // a block holds whole systems: the opening half map in one launch
         launch_k(c->pdl, k_multi_front, nblk(d.nsys, 128 / d.nm), 128, 0, st, d, h, opened ? 0.0 : 0.5 * h); LAUNCH(c);
     } else {
-        if (!opened) enqueue_kick(c, 0.5 * h, 1, nullptr);        // else: done by the previous map's merged kick
+        mark(c, PH_KICK);
+        if (!opened) enqueue_kick(c, 0.5 * h, 1, nullptr, 1);     // else: done by the previous map's merged kick
+        mark(c, PH_FRONT);
         if (d.mode != GENGA_MODE_TEST_PARTICLE) enqueue_sun(c, 0.5 * h, 0, false, h);   // Sun kick and drift in one launch
         else {
             enqueue_sun(c, 0.5 * h);
@@ -379,14 +412,18 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         }
     }
     const int pair_blocks = (int)std::min<long long>((d.cap + 127) / 128, 16LL * c->sms);   // grid-stride over the candidates; enough warps to cover the gather latency when there are 10^6 of them (mode 1)
+    mark(c, PH_CONFIRM);
     if (!tiny_mode(d)) { launch_k(c->pdl, k_confirm, pair_blocks, 128, 0, st, d, h); LAUNCH(c); }   // N <= 32: inside k_tiny_front
     const int warp_blocks = 2 * c->sms;                       // 4 warps each; warps take groups from a queue
+    mark(c, PH_GROUP);
     if (d.mode == GENGA_MODE_MULTI_SYSTEM) {
         launch_k(c->pdl, k_list_groups_multi, nblk(d.ntot, 256), 256, 0, st, d); LAUNCH(c);
+        mark(c, PH_BS);
         launch_k(c->pdl, k_bs_warp, warp_blocks, 32 * BW_WARPS, 0, st, d, h, 0); LAUNCH(c);
         if (d.nm > BW_MAXN) { launch_k(c->pdl, k_bs_multi, nblk(d.nsys, 8), 128, 0, st, d, h); LAUNCH(c); }
     } else {
         launch_k(c->pdl, k_build_groups, 1, 1024, 0, st, d); LAUNCH(c);
+        mark(c, PH_BS);
         // the Bulirsch-Stoer layouts work on disjoint parts of the size-ordered group queue: side by side
         const bool mid = d.nm > BW_MAXN;
         if (mid) {
@@ -394,7 +431,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
             cudaStreamWaitEvent(c->aux[0], c->ev_fork, 0);
             launch_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>(c->aux[0], c->bs_big_clusters, d, h, CI_QBIG, CI_NMIDEND); LAUNCH(c);
             cudaEventRecord(c->ev_join[0], c->aux[0]);
-            if (d.bss.base) {
+            if (d.bss.base && d.mode == GENGA_MODE_MASSIVE) {
                 cudaStreamWaitEvent(c->aux[1], c->ev_fork, 0);
                 k_bs_block<<<16, 256, 0, c->aux[1]>>>(d, h); LAUNCH(c);
                 cudaEventRecord(c->ev_join[1], c->aux[1]);
@@ -403,13 +440,15 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         launch_k(c->pdl, k_bs_warp, warp_blocks, 32 * BW_WARPS, 0, st, d, h, 0); LAUNCH(c);
         if (mid) {
             cudaStreamWaitEvent(st, c->ev_join[0], 0);
-            if (d.bss.base) cudaStreamWaitEvent(st, c->ev_join[1], 0);
+            if (d.bss.base && d.mode == GENGA_MODE_MASSIVE) cudaStreamWaitEvent(st, c->ev_join[1], 0);
         }
         if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {
             launch_k(c->pdl, k_bs_warp, warp_blocks, 32 * BW_WARPS, 0, st, d, h, 1); LAUNCH(c);
             if (d.nm + 1 > BW_MAXN) { k_tp_bs<32><<<2 * c->sms, 128, 0, st>>>(d, h, BW_MAXN); LAUNCH(c); }
+            if (d.nm + 1 > 32) { k_tp_bs_big<<<TPBIG_BLOCKS, 64, 0, st>>>(d, h); LAUNCH(c); }
         }
     }
+    mark(c, PH_BACK);
     if (tp) {
         launch_k(false, k_tpm_kick, 1, 32, 0, st, d, 0.5 * h, 0, 0.5 * h); LAUNCH(c);       // momentum sum, Sun kick, kick of the massive bodies; plain: see enqueue_sun
         launch_k(c->pdl, k_tp_back, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h); LAUNCH(c);
@@ -419,7 +458,8 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         launch_k(false, k_multi_back, nblk(d.nsys, 128 / d.nm), 128, 0, st, d, h, 0.5 * h); LAUNCH(c);
     } else {
         enqueue_sun(c, 0.5 * h, last ? 0 : 1, true);
-        if (hn != 0.0) enqueue_kick(c, 0.5 * (h + hn), 1, nullptr);   // closing kick + opening kick of the next map
+        mark(c, PH_KICK);
+        if (hn != 0.0) enqueue_kick(c, 0.5 * (h + hn), 1, nullptr, 1);   // closing kick + opening kick of the next map
         else enqueue_kick(c, 0.5 * h, 0, nullptr);
     }
 }
@@ -431,6 +471,7 @@ static void enqueue_step(genga_ctx *c, double dt, int order)
     DevState &d = c->d;
     double w[7];
     int nw = yoshida_weights(order, w);
+    mark(c, PH_RCRIT);
     if (d.mode == GENGA_MODE_TEST_PARTICLE) {                     // the particles' rc: k_tp_front of the first map
         DevState dm = d;
         dm.ntot = d.nm;
@@ -441,6 +482,7 @@ static void enqueue_step(genga_ctx *c, double dt, int order)
     const bool merge = !(c->cfg.flags & 1) && d.mode != GENGA_MODE_TEST_PARTICLE;
     for (int k = 0; k < nw; ++k)
         enqueue_map(c, w[k] * dt, dt, k == 0, k == nw - 1, merge && k + 1 < nw ? w[k + 1] * dt : 0.0, merge && k > 0);
+    mark(c, PH_TOTAL);
 }
 
 static long long interactions_per_eval(const DevState &d)
@@ -502,6 +544,35 @@ extern "C" __attribute__((visibility("default"))) int genga_step(genga_ctx *c, i
     long long evals = (merged ? maps_per_step(order) + 1LL : 2LL * maps_per_step(order)) * n_steps;   // force evaluations actually made
     c->force_evals += evals;
     c->interactions += evals * interactions_per_eval(c->d);
+    return GENGA_OK;
+}
+
+// The steps of genga_step as plain launches with an event at every phase boundary (no CUDA graph; an event between
+// two kernels also keeps them from overlapping by programmatic dependent launch, so the phases add up to a little more
+// than a graph-replayed step).  ms[PH_COUNT]: time per step of each phase, averaged over n_steps.
+extern "C" __attribute__((visibility("default"))) int genga_profile_step(genga_ctx *c, int64_t n_steps, double dt, int order, double *ms)
+{
+    if (!c || !ms || n_steps < 1 || n_steps > 4096 || dt == 0.0 || !(dt == dt) || (order != 2 && order != 4 && order != 6)) return GENGA_EINVAL;
+    c->prof = true; c->prof_used = 0; c->acc = 0;
+    for (int64_t s = 0; s < n_steps; ++s) enqueue_step(c, dt, order);
+    c->prof = false;
+    c->launches += c->acc; c->acc = 0;
+    c->steps += n_steps;
+    const bool merged = !(c->cfg.flags & 1) && c->d.mode != GENGA_MODE_TEST_PARTICLE;
+    const long long evals = (merged ? maps_per_step(order) + 1LL : 2LL * maps_per_step(order)) * n_steps;
+    c->force_evals += evals;
+    c->interactions += evals * interactions_per_eval(c->d);
+    CK(cudaStreamSynchronize(c->st));
+    CK(cudaGetLastError());
+    for (int k = 0; k < PH_COUNT; ++k) ms[k] = 0.0;
+    for (size_t k = 0; k + 1 < c->prof_used; ++k) {
+        if (c->prof_phase[k] == PH_TOTAL) continue;           // the gap between two steps
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, c->prof_ev[k], c->prof_ev[k + 1]));
+        ms[c->prof_phase[k]] += t;
+        ms[PH_TOTAL] += t;
+    }
+    for (int k = 0; k < PH_COUNT; ++k) ms[k] /= (double)n_steps;
     return GENGA_OK;
 }
 
@@ -752,6 +823,16 @@ extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ct
     return GENGA_OK;
 }
 
+extern "C" __attribute__((visibility("default"))) int genga_eval_fast(genga_ctx *c, int which, int64_t n, const double *in, double *out)
+{
+    if (!c || !in || !out || n < 0 || which < 0 || which > 2) return GENGA_EINVAL;
+    if (n == 0) return GENGA_OK;
+    k_eval_fast<<<nblk(n, 256), 256, 0, c->st>>>(which, n, in, out);
+    c->launches += 1;
+    CK(cudaGetLastError());
+    return GENGA_OK;
+}
+
 extern "C" __attribute__((visibility("default"))) int genga_fp64_probe(genga_ctx *c, double *tflops)
 {
     if (!c || !tflops) return GENGA_EINVAL;
@@ -783,6 +864,8 @@ extern "C" __attribute__((visibility("default"))) int genga_counters(genga_ctx *
     CK(cudaStreamSynchronize(c->st));
     out[0] = c->steps; out[1] = c->force_evals; out[2] = c->interactions; out[3] = c->launches;
     out[4] = st[CNT_GROUPS]; out[5] = st[CNT_MAXGROUP]; out[6] = st[CNT_BSSTEPS]; out[7] = st[CNT_CAND];
+    out[8] = st[CNT_BSREJECTS];
+    for (int k = 9; k < 16; ++k) out[k] = 0;
     return GENGA_OK;
 }
 

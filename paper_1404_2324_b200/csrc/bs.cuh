@@ -9,11 +9,13 @@
 // row, accept at <= eps^2; on failure after 8 columns H <- H/2, after an accept within five
 // columns H <- 1.5 H, the last step is cut to land exactly on h.
 //
-// Two layouts (the paper's Table 3, picked block sizes for cc 2.x; here):
+// Two layouts in this file (the paper's Table 3, picked block sizes for cc 2.x; the warp and
+// cluster layouts are in bs_warp.cuh and bs_cluster.cuh):
 //   * team of TW lanes of one warp, one body per lane, everything in registers, positions
 //     exchanged through double-buffered shared memory (one __syncwarp per force evaluation);
 //   * one thread block per large group, bodies strided over the threads, tableau in a
 //     global scratch area (any group size, up to all 2048 bodies, Fig. 15).
+// Every integrator counts into nsteps[2]: [0] accepted steps, [1] rejected attempts (all 8 columns failed).
 #pragma once
 #include "common.cuh"
 
@@ -166,7 +168,7 @@ __device__ bool bs_team(const WarpTeam<TW> &t, TeamSmem<TW> &sm, int nb, bool ac
 #pragma unroll
                         for (int c = 0; c < 3; ++c) { q[c] = row[k][c]; V[c] = row[k][3 + c]; }
                         done += H;
-                        if (nsteps) ++*nsteps;
+                        if (nsteps) ++nsteps[0];
                         if (k <= 4) H *= 1.5;
                         accepted = true;
                     }
@@ -174,218 +176,11 @@ __device__ bool bs_team(const WarpTeam<TW> &t, TeamSmem<TW> &sm, int nb, bool ac
             }
             if (!accepted) {
                 H *= 0.5; last = false;
+                if (nsteps) ++nsteps[1];
                 if (fabs(H) < BS_HMIN * fabs(h)) return false;
             }
         }
     }
-    return true;
-}
-
-// ---------------------------------------------------------------------------------
-// Shared-memory block layout for groups of BSW_MAXN < n <= BSS_MAXN bodies: one block of
-// BSS_THREADS threads per group.  The paper gives each body p threads that share its partner
-// loop and reduce (Table 3); here body i owns L = BSS_THREADS / pow2ceil(n) adjacent
-// lanes of one warp (L <= 32), lane s of the segment takes partners j = s, s+L, ... and the
-// star as partner j = n, the segment sum is an xor-butterfly of shuffles (fixed order), and
-// lane 0 of the segment ("owner") carries the modified-midpoint state of the body in
-// registers.  Positions are exchanged through a double-buffered shared array (one
-// __syncthreads per force evaluation); the extrapolation tableau lives in shared memory.
-constexpr int BSW_MAXN = 16;        // largest group the warp-team layout takes
-constexpr int BSS_MAXN = 256;       // largest group the shared-memory block layout takes
-constexpr int BSS_THREADS = 512;
-
-struct BssSmem {
-    double pos[2][3][BSS_MAXN];
-    float pf[2][3][BSS_MAXN];       // the same positions rounded to FP32, for the conservative pretest
-    float thr2[BSS_MAXN];           // (rc_i + margin)^2 rounded up: FP32 pretest threshold of body i
-    double m[BSS_MAXN], rc[BSS_MAXN], irc[BSS_MAXN];
-    double Y[6][BSS_MAXN];
-    double acc0[3][BSS_MAXN];
-    double tab[BS_KMAX][6][BSS_MAXN];
-    double red[BSS_THREADS / 32];
-};
-
-struct BssLane {
-    int n, L, i, s;     // group size, lanes per body, my body, my lane in the segment
-    bool owner;
-};
-
-// Force on body t.i at the positions q of the owners (Eq. 1 L73-74 through Eq. 8; star fixed
-// at the origin, L314).  Every pair of the group is examined at every evaluation (L505); to make
-// the n^2 examinations cheap they are done first in FP32 against a threshold widened by more than
-// the FP32 rounding of the positions, so the test can only err towards "inside"; the pairs that
-// pass take the exact FP64 test and weight.  The result is identical to testing in FP64 only.
-__device__ __forceinline__ void bss_rhs(BssSmem &S, const BssLane &t, int &buf, double G, double m0,
-                                        const double q[3], double a[3])
-{
-    GENGA_BS_RHS_HOOK();
-    double(*p)[BSS_MAXN] = S.pos[buf];
-    float(*pf)[BSS_MAXN] = S.pf[buf];
-    if (t.owner) {
-        p[0][t.i] = q[0]; p[1][t.i] = q[1]; p[2][t.i] = q[2];
-        pf[0][t.i] = (float)q[0]; pf[1][t.i] = (float)q[1]; pf[2][t.i] = (float)q[2];
-    }
-    __syncthreads();
-    buf ^= 1;
-    double ax = 0.0, ay = 0.0, az = 0.0;
-    if (t.i < t.n) {
-        const int n = t.n, L = t.L, i = t.i;
-        const float fx = pf[0][i], fy = pf[1][i], fz = pf[2][i], ft = S.thr2[i];
-        const double qx = p[0][i], qy = p[1][i], qz = p[2][i];
-        const double my_rc = S.rc[i], my_irc = S.irc[i];
-        for (int j0 = t.s; j0 <= n; j0 += 32 * L) {              // partner j = n is the star
-            unsigned mask = 0u;
-#pragma unroll 4
-            for (int kk = 0; kk < 32; ++kk) {
-                int j = j0 + kk * L;
-                if (j > n) break;
-                int jc = j < n ? j : i;                           // star / self: computed, not used
-                float dx = pf[0][jc] - fx, dy = pf[1][jc] - fy, dz = pf[2][jc] - fz;
-                float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                bool in = (d2 < fmaxf(ft, S.thr2[jc]) && j != i) || j == n;
-                mask |= (in ? 1u : 0u) << kk;
-            }
-            while (mask) {
-                int j = j0 + (__ffs(mask) - 1) * L;
-                mask &= mask - 1;
-                if (j == n) {
-                    double r2 = qx * qx + qy * qy + qz * qz;
-                    double s0 = -G * m0 * rinv3_fast(r2);
-                    ax += s0 * qx; ay += s0 * qy; az += s0 * qz;
-                } else {
-                    double rcj = S.rc[j];
-                    double rcij = fmax(my_rc, rcj);
-                    double dx = p[0][j] - qx, dy = p[1][j] - qy, dz = p[2][j] - qz;
-                    double d2 = dx * dx + dy * dy + dz * dz;
-                    if (d2 < rcij * rcij) {
-                        double sc = direct_scale(d2, rcij, my_rc >= rcj ? my_irc : S.irc[j], G * S.m[j]);
-                        ax += sc * dx; ay += sc * dy; az += sc * dz;
-                    }
-                }
-            }
-        }
-    }
-    for (int o = t.L >> 1; o > 0; o >>= 1) {
-        ax += __shfl_xor_sync(0xffffffffu, ax, o);
-        ay += __shfl_xor_sync(0xffffffffu, ay, o);
-        az += __shfl_xor_sync(0xffffffffu, az, o);
-    }
-    a[0] = ax; a[1] = ay; a[2] = az;
-}
-
-__device__ __forceinline__ double bss_block_max(BssSmem &S, double v)
-{
-    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-    __syncthreads();
-    if ((threadIdx.x & 31) == 0) S.red[threadIdx.x >> 5] = v;
-    __syncthreads();
-    double r = S.red[0];
-#pragma unroll
-    for (int w = 1; w < BSS_THREADS / 32; ++w) r = fmax(r, S.red[w]);
-    return r;
-}
-
-// S.Y, S.m, S.rc, S.irc hold the group (entries [0, n)) on entry; S.Y holds the result on return.
-__device__ inline bool bss_integrate(BssSmem &S, const BssLane &t, double G, double m0, double h, double eps, int *nsteps)
-{
-    int buf = 0;
-    double done = 0.0, H = h;
-    bool last = false;
-    const double eps2 = eps * eps;
-    const int i = t.i;
-    __syncthreads();
-    {
-        // FP32 pretest thresholds: positions stay within Q = 2 max_i(|q_i| + |h| |V_i|) (max norms) of
-        // the origin during the step, so rounding them to FP32 moves a separation by < 2^-22 Q and
-        // the FP32 evaluation of its square adds < 2^-21 relative; thr = (rc + 2^-20 Q)^2 (1 + 2^-18).
-        double qm = 0.0;
-        if (t.owner) {
-            qm = fmax(fmax(fabs(S.Y[0][i]), fabs(S.Y[1][i])), fabs(S.Y[2][i])) +
-                 fabs(h) * fmax(fmax(fabs(S.Y[3][i]), fabs(S.Y[4][i])), fabs(S.Y[5][i]));
-        }
-        const double Q = 2.0 * bss_block_max(S, qm);
-        if (t.owner) {
-            double w = S.rc[i] + 0x1.0p-20 * Q;
-            S.thr2[i] = __double2float_ru(w * w * (1.0 + 0x1.0p-18));
-        }
-        __syncthreads();
-    }
-    while (!last) {
-        double rem = h - done;
-        if (fabs(H) >= fabs(rem)) { H = rem; last = true; }
-        double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0}, isq = 0.0, isv = 0.0, acc0[3];
-        if (t.owner) {
-#pragma unroll
-            for (int c = 0; c < 3; ++c) { q[c] = S.Y[c][i]; V[c] = S.Y[3 + c][i]; }
-            isq = 1.0 / (q[0] * q[0] + q[1] * q[1] + q[2] * q[2]);
-            isv = 1.0 / (V[0] * V[0] + V[1] * V[1] + V[2] * V[2]);
-        }
-        bss_rhs(S, t, buf, G, m0, q, acc0);
-        bool accepted = false;
-        while (!accepted) {
-#pragma unroll 1
-            for (int k = 0; k < BS_KMAX && !accepted; ++k) {
-                const int nk = 2 * (k + 1);
-                const double eta = H / nk;
-                double qa[3], Va[3], qb[3], Vb[3], acc[3];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    qa[c] = q[c]; Va[c] = V[c];
-                    qb[c] = q[c] + eta * V[c]; Vb[c] = V[c] + eta * acc0[c];
-                }
-#pragma unroll 1
-                for (int ms = 1; ms < nk; ++ms) {
-                    bss_rhs(S, t, buf, G, m0, qb, acc);
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        double qn = qa[c] + 2.0 * eta * Vb[c];
-                        double vn = Va[c] + 2.0 * eta * acc[c];
-                        qa[c] = qb[c]; Va[c] = Vb[c]; qb[c] = qn; Vb[c] = vn;
-                    }
-                }
-                bss_rhs(S, t, buf, G, m0, qb, acc);
-                double e = 0.0;
-                if (t.owner) {
-                    double dq2 = 0.0, dv2 = 0.0;
-#pragma unroll
-                    for (int c = 0; c < 6; ++c) {
-                        double T = c < 3 ? 0.5 * (qb[c] + qa[c] + eta * Vb[c]) : 0.5 * (Vb[c - 3] + Va[c - 3] + eta * acc[c - 3]);
-                        double prev = S.tab[0][c][i], cur = T, diff = 0.0;
-                        S.tab[0][c][i] = T;
-                        for (int j = 1; j <= k; ++j) {
-                            const double iden = c_bs_iden.v[k][j];
-                            double tmp = S.tab[j][c][i];
-                            double nxt = cur + (cur - prev) * iden;
-                            diff = nxt - cur;
-                            cur = nxt;
-                            S.tab[j][c][i] = cur;
-                            prev = tmp;
-                        }
-                        if (c < 3) dq2 += diff * diff; else dv2 += diff * diff;
-                    }
-                    e = fmax(dq2 * isq, dv2 * isv);
-                }
-                if (k >= 1) {
-                    e = bss_block_max(S, e);
-                    if (e <= eps2) {
-                        if (t.owner) {
-#pragma unroll
-                            for (int c = 0; c < 6; ++c) S.Y[c][i] = S.tab[k][c][i];
-                        }
-                        done += H;
-                        if (nsteps && threadIdx.x == 0) ++*nsteps;
-                        if (k <= 4) H *= 1.5;
-                        accepted = true;
-                    }
-                }
-            }
-            if (!accepted) {
-                H *= 0.5; last = false;
-                if (fabs(H) < BS_HMIN * fabs(h)) return false;
-            }
-        }
-    }
-    __syncthreads();
     return true;
 }
 
@@ -519,7 +314,7 @@ __device__ inline bool bs_block(const BsScratch &S, int off, int nb, double G, d
                         for (int b = threadIdx.x; b < nb; b += blockDim.x)
                             for (int c = 0; c < 6; ++c) S.arr(BSA_Y + c)[off + b] = S.arr(BSA_ROW + 6 * k + c)[off + b];
                         done += H;
-                        if (nsteps && threadIdx.x == 0) ++*nsteps;
+                        if (nsteps && threadIdx.x == 0) ++nsteps[0];
                         if (k <= 4) H *= 1.5;
                         accepted = true;
                     }
@@ -527,6 +322,7 @@ __device__ inline bool bs_block(const BsScratch &S, int off, int nb, double G, d
                 __syncthreads();
             }
             if (!accepted) {
+                if (nsteps && threadIdx.x == 0) ++nsteps[1];
                 H *= 0.5; last = false;
                 if (fabs(H) < BS_HMIN * fabs(h)) return false;
             }

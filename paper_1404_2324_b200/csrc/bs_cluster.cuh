@@ -316,11 +316,12 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, BcSmem<MA
                 __syncthreads();
             }
             done += H;
-            if (nsteps) ++*nsteps;
+            if (nsteps) ++nsteps[0];
             if (kstar <= 4) H *= 1.5;
             fresh = true;
         } else {
             H *= 0.5; last = false;
+            if (nsteps) ++nsteps[1];
             if (fabs(H) < BS_HMIN * fabs(h)) return false;
         }
     }

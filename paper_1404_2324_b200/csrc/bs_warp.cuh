@@ -275,11 +275,12 @@ __device__ __forceinline__ bool bw_integrate(BwSmem &W, const int lane, const in
             }
             __syncwarp();
             done += H;
-            if (nsteps) ++*nsteps;
+            if (nsteps) ++nsteps[0];
             if (kstar <= 4) H *= 1.5;
             fresh = true;
         } else {
             H *= 0.5; last = false;
+            if (nsteps) ++nsteps[1];
             if (fabs(H) < BS_HMIN * fabs(h)) return false;
         }
     }

@@ -131,7 +131,7 @@ struct KickSmem {
     double wsum[KK_WARPS][8][3];            // per warp: sums of its rows
 };
 
-__global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, int record, int ni, double *aout)
+__global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, int record, int ni, double *aout, int to0)
 {
     pdl_sync();
     extern __shared__ __align__(32) unsigned char kk_raw[];
@@ -308,7 +308,9 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
         a += __shfl_xor_sync(0xffffffffu, a, 1);
         a += __shfl_xor_sync(0xffffffffu, a, 2);
         if (live && part == 0) {
-            double *vel = c == 0 ? d.vx : c == 1 ? d.vy : d.vz;
+            // to0: the kicked velocities go to the pre-drift arrays, which the fused Sun kick + drift (k_sun, hdrift != 0)
+            // only reads -- no block of that launch may read a velocity array another block is overwriting
+            double *vel = to0 ? (c == 0 ? d.vx0 : c == 1 ? d.vy0 : d.vz0) : (c == 0 ? d.vx : c == 1 ? d.vy : d.vz);
             vel[i0 + r] = fma(h, a, vel0);
             if (aout) aout[(size_t)c * d.ntot + i0 + r] = a;
         }
@@ -883,12 +885,15 @@ __global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset, do
         }
         m0 = d.m0[sys];
     } else {
+        // hdrift != 0: the velocities after the kick are in vx0.. (k_kick with to0): this launch only reads them, while
+        // vx.. receive the drifted velocities -- a block never sums an array another block of the launch is overwriting
+        const double *svx = hdrift != 0.0 ? d.vx0 : d.vx, *svy = hdrift != 0.0 ? d.vy0 : d.vy, *svz = hdrift != 0.0 ? d.vz0 : d.vz;
         double lm[KK_MAXN / 256], lx[KK_MAXN / 256], ly[KK_MAXN / 256], lz[KK_MAXN / 256];
 #pragma unroll
         for (int q = 0; q < KK_MAXN / 256; ++q) {                 // all loads in flight together
             const int k = threadIdx.x + 256 * q;
             const bool v = k < d.nm;
-            lm[q] = v ? d.m[k] : 0.0; lx[q] = v ? d.vx[k] : 0.0; ly[q] = v ? d.vy[k] : 0.0; lz[q] = v ? d.vz[k] : 0.0;
+            lm[q] = v ? d.m[k] : 0.0; lx[q] = v ? svx[k] : 0.0; ly[q] = v ? svy[k] : 0.0; lz[q] = v ? svz[k] : 0.0;
         }
 #pragma unroll
         for (int q = 0; q < KK_MAXN / 256; ++q) { sx = fma(lm[q], lx[q], sx); sy = fma(lm[q], ly[q], sy); sz = fma(lm[q], lz[q], sz); }
@@ -907,8 +912,10 @@ __global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset, do
     const double g = h / m0;
     double x = fma(g, sx, d.x[i]), y = fma(g, sy, d.y[i]), z = fma(g, sz, d.z[i]);
     if (hdrift != 0.0) {                                  // opening Sun kick: the Kepler drift follows in the same launch (k_drift)
-        double vx = d.vx[i], vy = d.vy[i], vz = d.vz[i];
-        d.x0[i] = x; d.y0[i] = y; d.z0[i] = z; d.vx0[i] = vx; d.vy0[i] = vy; d.vz0[i] = vz;
+        double vx, vy, vz;
+        if (d.mode == 2) { vx = d.vx[i]; vy = d.vy[i]; vz = d.vz[i]; d.vx0[i] = vx; d.vy0[i] = vy; d.vz0[i] = vz; }
+        else { vx = d.vx0[i]; vy = d.vy0[i]; vz = d.vz0[i]; }   // mode 0: already there (read-only in this launch)
+        d.x0[i] = x; d.y0[i] = y; d.z0[i] = z;
         if (!kepler_drift(d.G * m0, hdrift, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
         d.vx[i] = vx; d.vy[i] = vy; d.vz[i] = vz;
     }
@@ -1194,8 +1201,8 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
             double rc = d.rc[i];
             S.m[b] = d.m[i]; S.rc[b] = rc; S.irc[b] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
         }
-        int nsteps = 0;
-        bool ok = bc_integrate<MAXN, THREADS, CS>(S, S0, rank, t, d.G, d.m0[0], h, d.eps, &nsteps);
+        int nsteps[2] = {0, 0};
+        bool ok = bc_integrate<MAXN, THREADS, CS>(S, S0, rank, t, d.G, d.m0[0], h, d.eps, nsteps);
         if (rank == 0) {
             __syncthreads();
             for (int b = threadIdx.x; b < n; b += THREADS) {
@@ -1205,7 +1212,8 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
             }
             if (threadIdx.x == 0) {
                 if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
-                atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
+                atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps[0]);
+                atomicAdd((unsigned long long *)&d.stat[CNT_BSREJECTS], (unsigned long long)nsteps[1]);
             }
         }
     }
@@ -1270,7 +1278,7 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
             rc = d.rc[i]; m = d.m[i];
         }
         const double Gm0 = d.G * d.m0[sys];
-        int nsteps = 0;
+        int nsteps[2] = {0, 0};
         bool ok;
         if (n <= 4) {
             // segments of 2 or 4 lanes: slot b = lane % S takes body b from lane b of the 8-slot layout
@@ -1278,10 +1286,10 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
 #pragma unroll
             for (int c = 0; c < 6; ++c) Y[c] = __shfl_sync(0xffffffffu, Y[c], src);
             rc = __shfl_sync(0xffffffffu, rc, src); m = __shfl_sync(0xffffffffu, m, src);
-            if (n == 2) ok = bw_integrate<2>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, &nsteps);
-            else ok = bw_integrate<4>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, &nsteps);
+            if (n == 2) ok = bw_integrate<2>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, nsteps);
+            else ok = bw_integrate<4>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, nsteps);
         } else {
-            ok = bw_integrate<8>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, &nsteps);
+            ok = bw_integrate<8>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, nsteps);
         }
         if (lane < 8 && writeback) {
             d.x[i] = Y[0]; d.y[i] = Y[1]; d.z[i] = Y[2]; d.vx[i] = Y[3]; d.vy[i] = Y[4]; d.vz[i] = Y[5];
@@ -1289,7 +1297,8 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
         }
         if (lane == 0) {
             if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
-            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps[0]);
+                atomicAdd((unsigned long long *)&d.stat[CNT_BSREJECTS], (unsigned long long)nsteps[1]);
             if (tp || d.mode == 2) {
                 atomicAdd((unsigned long long *)&d.stat[CNT_GROUPS], 1ull);
                 atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)n);
@@ -1323,21 +1332,21 @@ __global__ void __launch_bounds__(256) k_bs_block(DevState d, double h)
 {
     pdl_sync();
     __shared__ double red[32];
-    __shared__ int nsteps;
+    __shared__ int nsteps[2];
     if (d.cnt[CI_NBIG] == 0) return;
     const int ng = d.cnt[CI_NGROUPS];
     for (int g = blockIdx.x; g < ng; g += gridDim.x) {
         const int nb = d.gsize[g];
         if (nb <= BCB_MAXN) continue;
         const int off = d.gstart[g];
-        if (threadIdx.x == 0) nsteps = 0;
+        if (threadIdx.x == 0) { nsteps[0] = 0; nsteps[1] = 0; }
         for (int b = threadIdx.x; b < nb; b += blockDim.x) {
             int i = d.gmem[off + b];
             d.bss.arr(BSA_Y + 0)[off + b] = d.x0[i]; d.bss.arr(BSA_Y + 1)[off + b] = d.y0[i]; d.bss.arr(BSA_Y + 2)[off + b] = d.z0[i];
             d.bss.arr(BSA_Y + 3)[off + b] = d.vx0[i]; d.bss.arr(BSA_Y + 4)[off + b] = d.vy0[i]; d.bss.arr(BSA_Y + 5)[off + b] = d.vz0[i];
             d.bss.arr(BSA_M)[off + b] = d.m[i]; d.bss.arr(BSA_RC)[off + b] = d.rc[i];
         }
-        bool ok = bs_block(d.bss, off, nb, d.G, d.m0[0], h, d.eps, red, &nsteps);
+        bool ok = bs_block(d.bss, off, nb, d.G, d.m0[0], h, d.eps, red, nsteps);
         __syncthreads();
         for (int b = threadIdx.x; b < nb; b += blockDim.x) {
             int i = d.gmem[off + b];
@@ -1346,7 +1355,8 @@ __global__ void __launch_bounds__(256) k_bs_block(DevState d, double h)
         }
         if (threadIdx.x == 0) {
             if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
-            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps[0]);
+                atomicAdd((unsigned long long *)&d.stat[CNT_BSREJECTS], (unsigned long long)nsteps[1]);
         }
         __syncthreads();
     }
@@ -1377,10 +1387,7 @@ __global__ void __launch_bounds__(128) k_tp_bs(DevState d, double h, int lo)
             lab = min(lab, d.label[j]);
         }
         const int nb = __popc(full) + 1;
-        if (nb > TW || nb <= lo) {
-            if (nb > 32 && TW == 32 && lane == 0) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);  // 32 massive + particle
-            continue;
-        }
+        if (nb > TW || nb <= lo) continue;            // 32 massive bodies + the particle: k_tp_bs_big
         const bool active = lane < nb;
         int i = p;
         if (lane < nb - 1) {                         // lane-th set bit of full
@@ -1397,20 +1404,66 @@ __global__ void __launch_bounds__(128) k_tp_bs(DevState d, double h, int lo)
             sm[team].m[lane] = d.m[i]; sm[team].rc[lane] = rc; sm[team].irc[lane] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
         }
         t.sync();
-        int nsteps = 0;
+        int nsteps[2] = {0, 0};
         unsigned srcmask = nb >= 32 ? 0xffffffffu : ((1u << nb) - 1u);
-        bool ok = bs_team<TW>(t, sm[team], nb, active, srcmask, d.G, d.m0[0], rc, q, V, h, d.eps, &nsteps);
+        bool ok = bs_team<TW>(t, sm[team], nb, active, srcmask, d.G, d.m0[0], rc, q, V, h, d.eps, nsteps);
         if (lane == nb - 1) {
             d.x[p] = q[0]; d.y[p] = q[1]; d.z[p] = q[2]; d.vx[p] = V[0]; d.vy[p] = V[1]; d.vz[p] = V[2];
             d.label[p] = lab;
             if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
-            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps[0]);
+                atomicAdd((unsigned long long *)&d.stat[CNT_BSREJECTS], (unsigned long long)nsteps[1]);
             atomicAdd((unsigned long long *)&d.stat[CNT_GROUPS], 1ull);
             atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)nb);
         }
     }
 }
 template __global__ void k_tp_bs<32>(DevState, double, int);
+
+// Test-particle groups of 33 bodies: all 32 massive bodies of the mode's maximum (L188) in one group, plus the particle
+// (L342).  One more body than a warp holds: one block per listed particle with the tableau in global scratch (bs_block,
+// 64 entries per block); rare, so the slow layout is enough.  Only the particle is written back.
+__global__ void __launch_bounds__(64) k_tp_bs_big(DevState d, double h)
+{
+    pdl_sync();
+    __shared__ double red[32];
+    __shared__ int nsteps[2];
+    const int ntp = d.cnt[CI_NTP];
+    const int off = blockIdx.x * 64;
+    for (int k = blockIdx.x; k < ntp; k += gridDim.x) {
+        const int p = d.tplist[k];
+        unsigned mask = d.tpmask[p - d.nm], full = 0u;
+        int lab = p;
+        for (unsigned mm = mask; mm; mm &= mm - 1) {
+            int j = __ffs(mm) - 1;
+            full |= d.gmask[j];
+            lab = min(lab, d.label[j]);
+        }
+        const int nb = __popc(full) + 1;
+        if (nb <= 32) continue;                           // k_bs_warp / k_tp_bs<32> (uniform over the block)
+        if (threadIdx.x == 0) { nsteps[0] = 0; nsteps[1] = 0; }
+        for (int b = threadIdx.x; b < nb; b += blockDim.x) {
+            const int i = b < nb - 1 ? __fns(full, 0, b + 1) : p;
+            d.bss.arr(BSA_Y + 0)[off + b] = d.x0[i]; d.bss.arr(BSA_Y + 1)[off + b] = d.y0[i]; d.bss.arr(BSA_Y + 2)[off + b] = d.z0[i];
+            d.bss.arr(BSA_Y + 3)[off + b] = d.vx0[i]; d.bss.arr(BSA_Y + 4)[off + b] = d.vy0[i]; d.bss.arr(BSA_Y + 5)[off + b] = d.vz0[i];
+            d.bss.arr(BSA_M)[off + b] = d.m[i]; d.bss.arr(BSA_RC)[off + b] = d.rc[i];
+        }
+        const bool ok = bs_block(d.bss, off, nb, d.G, d.m0[0], h, d.eps, red, nsteps);
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const int b = nb - 1;
+            d.x[p] = d.bss.arr(BSA_Y + 0)[off + b]; d.y[p] = d.bss.arr(BSA_Y + 1)[off + b]; d.z[p] = d.bss.arr(BSA_Y + 2)[off + b];
+            d.vx[p] = d.bss.arr(BSA_Y + 3)[off + b]; d.vy[p] = d.bss.arr(BSA_Y + 4)[off + b]; d.vz[p] = d.bss.arr(BSA_Y + 5)[off + b];
+            d.label[p] = lab;
+            if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps[0]);
+                atomicAdd((unsigned long long *)&d.stat[CNT_BSREJECTS], (unsigned long long)nsteps[1]);
+            atomicAdd((unsigned long long *)&d.stat[CNT_GROUPS], 1ull);
+            atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)nb);
+        }
+        __syncthreads();
+    }
+}
 
 // Multi-system mode (L372-376), groups of more than BW_MAXN bodies (the others: k_bs_warp): 16 lanes
 // per system; the groups of a system are the sets of equal labels among its bodies.
@@ -1440,7 +1493,7 @@ __global__ void __launch_bounds__(128) k_bs_multi(DevState d, double h)
     double rc = have ? d.rc[i] : 0.0;
     sm[team].m[lane] = have ? d.m[i] : 0.0; sm[team].rc[lane] = rc; sm[team].irc[lane] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
     t.sync();
-    int ngroups = 0, nsteps_tot = 0, big = 0;
+    int ngroups = 0, nsteps_tot = 0, nrej_tot = 0, big = 0;
     bool ok = true;
     while (todo) {
         int root = __ffs(todo) - 1;
@@ -1449,14 +1502,15 @@ __global__ void __launch_bounds__(128) k_bs_multi(DevState d, double h)
         bool active = (gm >> lane) & 1u;
         double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0};
         if (active) { q[0] = d.x0[i]; q[1] = d.y0[i]; q[2] = d.z0[i]; V[0] = d.vx0[i]; V[1] = d.vy0[i]; V[2] = d.vz0[i]; }
-        int nsteps = 0;
-        ok = bs_team<TW>(t, sm[team], TW, active, gm, d.G, d.m0[sys], rc, q, V, h, d.eps, &nsteps) && ok;
+        int nsteps[2] = {0, 0};
+        ok = bs_team<TW>(t, sm[team], TW, active, gm, d.G, d.m0[sys], rc, q, V, h, d.eps, nsteps) && ok;
         if (active) { d.x[i] = q[0]; d.y[i] = q[1]; d.z[i] = q[2]; d.vx[i] = V[0]; d.vy[i] = V[1]; d.vz[i] = V[2]; }
-        ++ngroups; nsteps_tot += nsteps; big = max(big, __popc(gm));
+        ++ngroups; nsteps_tot += nsteps[0]; nrej_tot += nsteps[1]; big = max(big, __popc(gm));
     }
     if (lane == 0) {
         if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
         atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps_tot);
+        atomicAdd((unsigned long long *)&d.stat[CNT_BSREJECTS], (unsigned long long)nrej_tot);
         atomicAdd((unsigned long long *)&d.stat[CNT_GROUPS], (unsigned long long)ngroups);
         atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)big);
     }
@@ -1522,6 +1576,15 @@ __global__ void __launch_bounds__(256) k_fp64_probe(double *out, int iters)
     }
     double r = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
     if (r == 0.12345) out[threadIdx.x] = r;      // never true: keeps the chains alive without a per-thread output array
+}
+
+// The reciprocal routines of common.cuh on caller arrays (genga_eval_fast): the bias test of tests/test_gpu_fastmath.py.
+__global__ void k_eval_fast(int which, long long n, const double *in, double *out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double x = in[i];
+    out[i] = which == 0 ? rsqrt_fast(x) : which == 1 ? rinv3_fast(x) : rcp_fast(x);
 }
 
 // labels for genga_encounters: body's own index unless it is in a group

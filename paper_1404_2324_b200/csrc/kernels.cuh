@@ -18,7 +18,7 @@ constexpr int BCB_MAXN = 256, BCB_THREADS = 512, BCB_CS = 8;
 __global__ void k_begin_map(DevState d);
 __global__ void k_reset_counters(DevState d);
 __global__ void k_rcrit(DevState d, double tau, int reset);
-__global__ void k_kick(DevState d, double h, int record, int ni, double *aout);
+__global__ void k_kick(DevState d, double h, int record, int ni, double *aout, int to0);
 size_t kick_smem_bytes();
 __global__ void k_tp_kick(DevState d, double h, int record, double *aout);
 __global__ void k_tp_front(DevState d, double h, double tau, int first);
@@ -42,9 +42,12 @@ __global__ void k_bs_warp(DevState d, double h, int tp);
 __global__ void k_list_groups_multi(DevState d);
 __global__ void k_bs_block(DevState d, double h);
 template <int TW> __global__ void k_tp_bs(DevState d, double h, int lo);
+__global__ void k_tp_bs_big(DevState d, double h);
+constexpr int TPBIG_BLOCKS = 16;   // blocks of k_tp_bs_big, 64 scratch entries each
 __global__ void k_bs_multi(DevState d, double h);
 __global__ void k_energy(DevState d, double *out);
 __global__ void k_export_labels(DevState d, int *out);
 __global__ void k_fp64_probe(double *out, int iters);
+__global__ void k_eval_fast(int which, long long n, const double *in, double *out);
 
 }  // namespace genga

@@ -55,7 +55,7 @@ def test_workspace_size_and_limits(lib):
     assert all(s > 0 and s % 256 == 0 for s in sizes)
     assert sizes[1] > sizes[0] and sizes[2] > 16 * 8 * 1_000_000
     bad = [_cfg(0, 0), _cfg(0, 2049), _cfg(0, 10, 5), _cfg(1, 33, 10), _cfg(1, 8, 1_000_001), _cfg(2, 17, 0, 10),
-           _cfg(2, 16, 0, 100_001), _cfg(3, 5), _cfg(0, 5, G=0.0), _cfg(0, 5, bs_eps=0.0), _cfg(0, 5, max_pairs=0)]
+           _cfg(2, 16, 0, 100_001), _cfg(3, 5), _cfg(0, 5, G=0.0), _cfg(0, 5, bs_eps=0.0), _cfg(0, 5, max_pairs=0), _cfg(0, 5, max_pairs=2**31)]
     for c in bad:
         assert lib.genga_workspace_bytes(C.byref(c)) == 0
     assert lib.genga_workspace_bytes(None) == 0

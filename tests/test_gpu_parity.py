@@ -45,6 +45,7 @@ CASES = {
     "cfg1_full": lambda: workloads.config1(),
     "cfg1_ragged_777": lambda: workloads.config1(n=777),
     "cfg4_full": lambda: workloads.config4(order=4),
+    "cfg4_full_order6": lambda: workloads.config4(order=6),
     "cfg4_513": lambda: workloads.config4(n=513, order=6),
     # N <= 32: the one-warp half-map kernels (k_tiny_front / k_tiny_back); 33 is the first size on the general path
     "tiny24_order6": lambda: workloads.config4(n=24, order=6),
@@ -77,7 +78,10 @@ def test_accelerations_rcrit_and_candidates(G, case):
     g.close()
 
 
-STEP_CASES = [("cfg0", 100), ("cfg1_full", 4), ("cfg1_ragged_777", 10), ("cfg4_full", 2), ("cfg4_513", 3), ("tiny24_order6", 30), ("tiny32_order4", 40), ("n33_order4", 40),
+# cfg1_full, 100 steps: the largest group grows from ~30 to ~60 bodies (the regime bench.py times); cfg4 at full size at
+# both of its orders
+STEP_CASES = [("cfg0", 100), ("cfg1_full", 4), ("cfg1_full", 100), ("cfg1_ragged_777", 10), ("cfg4_full", 2), ("cfg4_full", 10),
+              ("cfg4_full_order6", 10), ("cfg4_513", 3), ("tiny24_order6", 30), ("tiny32_order4", 40), ("n33_order4", 40),
               ("cfg2_small", 8), ("cfg2_ragged", 8), ("cfg2_order4", 5), ("cfg2_order6_ragged", 3), ("cfg2_32massive", 6),
               ("cfg3_order4", 20), ("cfg3_small", 60), ("cfg3_7bodies", 60)]
 
@@ -110,6 +114,109 @@ def test_trajectories_encounters_and_energy(G, case, nsteps):
     xd, vd = g.get_state()
     assert np.array_equal(xd.cpu().numpy(), x) and np.array_equal(vd.cpu().numpy(), v)
     g.close()
+
+
+def _annulus_particles(mult, n1, nt):
+    """32 massive bodies (the mode's maximum) packed in the annulus of config 4 with masses inflated so
+    that they form large encounter groups, plus nt test particles in the same annulus."""
+    w4 = workloads.config4(n=32 + nt)
+    m = w4["m"].copy()
+    m[:32] *= mult
+    m[32:] = 0.0
+    return dict(w4, mode=1, m=m, n_massive=32, n_test=nt, order=2, n1=n1)
+
+
+@pytest.mark.parametrize("name,make,nsteps,min_group,max_group", [
+    # multi-system groups of 9..16 bodies: k_bs_multi (16 lanes per system)
+    ("multi_big_groups", lambda: dict(workloads.config3(n_systems=12), n2=1.5, m=workloads.config3(n_systems=12)["m"] * 3000), 10, 9, 16),
+    # particle groups {particle} + a massive group of 9..31 bodies: k_tp_bs<32>
+    ("tp_mid_groups", lambda: _annulus_particles(10000, 3.0, 200), 4, 10, 32),
+    # all 32 massive bodies in one group + the particle = 33 bodies: k_tp_bs_big
+    ("tp_33_bodies", lambda: _annulus_particles(3000, 20.0, 40), 3, 33, 33),
+])
+def test_bulirsch_stoer_layouts_reached_by_large_groups(G, name, make, nsteps, min_group, max_group):
+    """Every Bulirsch-Stoer layout the library ships is reached by a real group and agrees with the oracle:
+    state, pair lists and labels."""
+    w = make()
+    g = G.from_workload(w, max_pairs=200000)
+    o = oracle.Sim(w, cap=200000)
+    for _ in range(nsteps):
+        g.step(1, w["dt"], w["order"])
+        o.step(1, w["dt"], w["order"])
+        pairs, ncand, labels = g.encounters()
+        co, eo, lo = o.encounters()
+        assert ncand == len(co) and np.array_equal(pairs, eo) and np.array_equal(labels, lo)
+    x, v = g.get_state_host()
+    assert g.status() == 0
+    xo, vo = o.state()
+    assert relerr(x, xo).max() < STATE_TOL and relerr(v, vo).max() < STATE_TOL
+    big = g.counters()["max_group"]
+    assert min_group <= big <= max_group, big
+    assert big == max(s.stats()["max_group"] for s in o.sys)
+    g.close()
+
+
+@pytest.mark.parametrize("order", [2, 4])
+def test_1e4_steps_energy_with_encounters(G, order):
+    """north_star: |dE/E| after 10^4 steps within 2x of the oracle's -- on a run WITH encounters (config 4's annulus,
+    64 bodies, masses x 30: ~3 to ~10 groups per step, Bulirsch-Stoer in every map), the parts that can break
+    symplecticity.  The system is chaotic: a relative perturbation of 1e-14 of the initial positions changes the
+    oracle's own end-of-run |dE/E| by up to 2x (the error is dominated by a few close approaches), and the GPU run is
+    one more rounding-level perturbation.  So the quantity compared is the MAXIMUM of |dE/E| over the run, sampled
+    every 100 steps, and the oracle's figure is the largest over three runs (unperturbed, positions x (1 +- 1e-14))."""
+    def make(pert=0.0):
+        w = workloads.config4(n=64)
+        w["m"] = w["m"] * 30
+        w["x"] = w["x"] * (1.0 + pert)
+        return w
+    w = make()
+    g = G.from_workload(w)
+    E0, _ = g.energy()
+    worst_g = 0.0
+    for _ in range(100):
+        g.step(100, w["dt"], order)
+        worst_g = max(worst_g, abs((g.energy()[0] - E0) / E0)[0])
+    assert g.status() == 0
+    assert g.counters()["groups"] > 1000
+    g.close()
+    worst_o = 0.0
+    for pert in (0.0, 1e-14, -1e-14):
+        wo = make(pert)
+        o = oracle.Sim(wo)
+        Eo0, _ = o.energy()
+        for _ in range(100):
+            o.step(100, wo["dt"], order)
+            worst_o = max(worst_o, abs((o.energy()[0] - Eo0) / Eo0)[0])
+        assert o.sys[0].stats()["groups"] > 1000
+    assert worst_g <= 2 * worst_o, (order, worst_g, worst_o)
+
+
+def test_bit_reproducible_under_sm_contention(G):
+    """The fused Sun kick + drift launch of the massive mode sums m V over ALL bodies in every block while the same
+    launch writes the drifted velocities: the sums are taken from the pre-drift arrays, which that launch only reads, so
+    the result cannot depend on when a block becomes resident.  N = 2048 (8 blocks), steps run while another stream
+    keeps every SM busy, compared bit for bit with the run on an idle GPU."""
+    import torch
+    w = workloads.config1()
+    ref = None
+    for load in (False, True, True):
+        g = G.from_workload(w)
+        stop = False
+        if load:
+            side = torch.cuda.Stream()
+            a = torch.randn(4096, 4096, device="cuda")
+            with torch.cuda.stream(side):
+                for _ in range(60):
+                    a = torch.tanh(a @ a * 1e-3)
+        g.step(32, w["dt"], 2)
+        x, v = g.get_state_host()
+        torch.cuda.synchronize()
+        assert g.status() == 0
+        if ref is None:
+            ref = (x.copy(), v.copy())
+        else:
+            assert np.array_equal(x, ref[0]) and np.array_equal(v, ref[1])
+        g.close()
 
 
 def test_config0_1000_steps_energy_and_state(G):

@@ -94,6 +94,28 @@ def test_kick_plus_bs_weights_sum_to_newton():
     assert np.all(a0 == 0.0)
 
 
+def test_kick_plus_bs_right_hand_side_is_newton():
+    """W_kick + W_BS = 1 on the FORCES: the right-hand side Bulirsch-Stoer integrates (Eq. 1 L73-74 through Eq. 8:
+    star + (1 - W)-weighted group pairs) is read off ora_bs_group itself as dV/dt at t = 0 (central difference of two
+    tiny integrations, +h and -h); added to the kick acceleration it must give the plain Newtonian sum of the star and
+    all pairs, written here with numpy.  A wrong sign or weight in the BS right-hand side fails this."""
+    m, q, V, rc = _cluster(seed=7)
+    G, m0, h = 1.0, 1.0, 1e-5
+    a_kick, _ = oracle.accel(G, m, q, rc)
+    _, Vp, _ = oracle.bs_group(G, m0, m, rc, q, V, h)
+    _, Vm, _ = oracle.bs_group(G, m0, m, rc, q, V, -h)
+    a_bs = (Vp - Vm) / (2 * h)
+    d = q[:, None, :] - q[:, :, None]                      # d[:, i, j] = q_j - q_i
+    r3 = (d**2).sum(0) ** 1.5
+    np.fill_diagonal(r3, np.inf)
+    newton = (G * m[None, None, :] * d / r3[None]).sum(2) - G * m0 * q / np.linalg.norm(q, axis=0) ** 3
+    err = np.linalg.norm(a_kick + a_bs - newton, axis=0) / np.linalg.norm(newton, axis=0)
+    assert err.max() < 1e-7, err
+    # not trivial: the BS part carries a real share of the pair force
+    pair = newton + G * m0 * q / np.linalg.norm(q, axis=0) ** 3
+    assert (np.linalg.norm(a_kick - pair, axis=0) / np.linalg.norm(pair, axis=0)).max() > 0.05
+
+
 def test_pair_forces_antisymmetric_and_torque_free():
     w = workloads.config4(n=64)
     m, q = w["m"], w["x"]

@@ -59,12 +59,19 @@ def test_single_drift_matches_analytic_orbit(e, frac):
     assert 0 < it <= 60
 
 
-def test_invariants_over_1e4_orbits():
-    """Repeated 6-day drifts over 1e4 orbits at 1 AU: energy, angular momentum and the
-    eccentricity vector hold to 1e-13 relative (SURVEY 8(c) caveat: the along-track PHASE
-    cannot, it random-walks; it is reported, not asserted)."""
+def test_invariants_and_phase_over_1e4_orbits():
+    """north_star: "two-body drift must match the analytic orbit to 1e-13 relative over 1e4 orbits" (reading R-18).
+    650 146 repeated 6-day drifts = 1e4 orbits at a = 1.04 AU, e = 0.043.
+    (i) The invariants -- energy, angular momentum vector, eccentricity vector -- hold to a few 1e-13: they random-walk
+        with the ~6.5e5 roundings.  Measured on this oracle: |dE/E| = 1.9e-13, |dL|/|L| = 9.1e-14, |dA| = 1.5e-13
+        (absolute, |A| = e = 0.043); the bounds below are ~2.5x those, not the 1e-13 of a single drift.
+    (ii) The along-track PHASE cannot hold 1e-13 in FP64: the mean anomaly alone carries eps * 2 pi * 1e4 = 1.4e-11, and
+        an energy error dE shifts the mean motion by 1.5 dE/E, so the phase error is bounded by 1.5 * (2 pi 1e4) *
+        max|dE/E| over the run.  The position against the analytic orbit (mpmath, 40 digits, Kepler's equation solved
+        at the final time) is asserted against that bound.  Measured: 1.2e-9 relative (bound 1.9e-8)."""
     mu, h = 1.0, 6 * 0.01720209895
     q = np.array([1.0, 0.0, 0.0]); V = np.array([0.0, 1.02, 0.05])
+    q0, V0 = q.copy(), V.copy()
     def inv(q, V):
         E = 0.5 * V @ V - mu / np.linalg.norm(q)
         L = np.cross(q, V)
@@ -72,14 +79,39 @@ def test_invariants_over_1e4_orbits():
         return E, L, A
     E0, L0, A0 = inv(q, V)
     a = -mu / (2 * E0)
-    nsteps = int(1e4 * 2 * np.pi * a**1.5 / h)
+    norbits = 1e4
+    nsteps = int(norbits * 2 * np.pi * a**1.5 / h)
     lib = oracle.lib()
-    for _ in range(nsteps):
+    worst_dE = 0.0
+    for k in range(nsteps):
         assert lib.ora_kepler_drift(mu, h, q, V) > 0
+        if k % 1000 == 999:
+            worst_dE = max(worst_dE, abs(inv(q, V)[0] - E0) / abs(E0))
     E1, L1, A1 = inv(q, V)
-    assert abs(E1 - E0) <= 1e-13 * abs(E0) * 5  # random walk of ~6e5 roundings: a few 1e-14
-    assert np.linalg.norm(L1 - L0) <= 5e-13 * np.linalg.norm(L0)
-    assert np.linalg.norm(A1 - A0) <= 5e-12  # |e|~0.04; absolute
+    worst_dE = max(worst_dE, abs(E1 - E0) / abs(E0))
+    assert worst_dE <= 5e-13
+    assert np.linalg.norm(L1 - L0) <= 2.5e-13 * np.linalg.norm(L0)
+    assert np.linalg.norm(A1 - A0) <= 4e-13
+    # analytic position at t = nsteps * h from the initial state, in mpmath: elements, Kepler's equation, f and g
+    mq, mv = [mp.mpf(x) for x in q0], [mp.mpf(x) for x in V0]
+    dot = lambda u, w: sum(x * y for x, y in zip(u, w))
+    r0 = mp.sqrt(dot(mq, mq))
+    am = 1 / (2 / r0 - dot(mv, mv) / mu)
+    n = mp.sqrt(mu / am**3)
+    ecosE, esinE = 1 - r0 / am, dot(mq, mv) / mp.sqrt(mu * am)
+    ecc = mp.sqrt(ecosE**2 + esinE**2)
+    Ea = mp.atan2(esinE, ecosE)
+    T = mp.mpf(h) * nsteps
+    M1 = Ea - esinE + n * T
+    Eb = mp.findroot(lambda E: E - ecc * mp.sin(E) - M1, M1, tol=mp.mpf(10) ** -35)
+    dE = Eb - Ea
+    f, g = 1 - am / r0 * (1 - mp.cos(dE)), T - (dE - mp.sin(dE)) / n
+    q1 = [f * x + g * v for x, v in zip(mq, mv)]
+    err = float(mp.sqrt(sum((mp.mpf(float(u)) - w) ** 2 for u, w in zip(q, q1))) / mp.sqrt(dot(q1, q1)))
+    bound = 1.5 * 2 * np.pi * norbits * worst_dE + 2.2e-16 * 2 * np.pi * norbits
+    print("phase error after 1e4 orbits: %.3e relative (bound %.3e, max |dE/E| %.3e)" % (err, bound, worst_dE))
+    assert err <= bound
+    assert err <= 2e-8
 
 
 def test_drift_group_property_and_reversal():

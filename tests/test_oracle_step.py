@@ -47,17 +47,19 @@ def _close_pair_system():
     return dict(m=m, x=np.ascontiguousarray(x), v=np.ascontiguousarray(v))
 
 
-def test_energy_error_scaling_with_pairs_inside_rcrit():
-    """n2 = 0 so r_crit does not depend on dt; the pair spends the whole run inside 3 R_H.
-    Order 2 must show ~dt^2; order 4 must be far better than order 2 at the same dt [R-4]."""
+@pytest.mark.parametrize("order,dt_days,lo,hi", [(2, 2.0, 3.5, 4.6), (4, 4.0, 13, 20), (6, 8.0, 45, 90)])
+def test_energy_error_scaling_with_pairs_inside_rcrit(order, dt_days, lo, hi):
+    """|dE/E| ~ dt^p for p = 2, 4, 6 on a run WITH pairs inside r_crit (n2 = 0, so r_crit does not
+    depend on dt; the pair spends the whole run inside 3 R_H and Bulirsch-Stoer runs in every map).  Halving dt must
+    divide the error by 2^p: this is what constrains reading R-4 (r_crit frozen over the substeps of a step -- a
+    substep that moved the changeover boundary would not be the same one-parameter map and the h^3 / h^5 terms of the
+    composition would not cancel).  Measured: 4.00, 16.04, 64.7 (dt chosen per order above the 1e-14 floor)."""
     w = _close_pair_system()
     kw = dict(n1=6.0, n2=0.0)
-    e2a, s = _max_energy_error(w, 2, 2.0, 120, **kw)
-    assert s.stats()["groups"] > 10          # BS really ran
-    e2b, _ = _max_energy_error(w, 2, 1.0, 120, **kw)
-    assert 2.8 < e2a / e2b < 5.5, (e2a, e2b)
-    e4a, _ = _max_energy_error(w, 4, 2.0, 120, **kw)
-    assert e4a < 0.2 * e2a
+    ea, s = _max_energy_error(w, order, dt_days, 120, **kw)
+    assert s.stats()["groups"] >= 15          # BS really ran, in every map
+    eb, _ = _max_energy_error(w, order, dt_days / 2, 120, **kw)
+    assert lo < ea / eb < hi, (order, ea, eb, ea / eb)
 
 
 def test_time_reversal_of_the_map_with_frozen_rcrit():
