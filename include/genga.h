@@ -146,6 +146,13 @@ int genga_energy(genga_ctx *ctx, double *E, double *L);
 int genga_encounters(genga_ctx *ctx, int32_t *pairs, int64_t cap, int64_t *n_pairs,
                      int64_t *n_candidates, int32_t *group_label);
 
+/* One record per encounter group that Bulirsch-Stoer integrated in the LAST drift substep executed (L116, L286-314;
+ * at most 4096 are kept): out[4*k + 0] = group size | layout << 16 (layout 0: one warp, 1: cluster),
+ * out[4*k + 1] = accepted steps | rejected attempts << 16, out[4*k + 2] = SM clock cycles the integration took,
+ * out[4*k + 3] = a member's body index.  *n = number of records made (may exceed cap and 4096).  The step time of an
+ * encounter-heavy run is the longest of these chains; bench.py reports it.  HOST pointers; synchronises. */
+int genga_bs_trace(genga_ctx *ctx, int32_t *out, int64_t cap, int64_t *n);
+
 /* Synchronise the stream and return (and clear) the latched device error, or GENGA_OK. */
 int genga_status(genga_ctx *ctx);
 

@@ -22,7 +22,7 @@ OK, EINVAL, ECAPACITY, EKEPLER, EBS, ECUDA = 0, -1, -2, -3, -4, -5
 SYMBOLS = [
     "genga_workspace_bytes", "genga_create", "genga_destroy", "genga_set_state", "genga_set_state_host",
     "genga_step", "genga_get_state", "genga_get_state_host", "genga_set_state_ragged_host", "genga_get_state_ragged_host", "genga_set_system_params_host",
-    "genga_energy", "genga_encounters",
+    "genga_energy", "genga_encounters", "genga_bs_trace",
     "genga_status", "genga_accelerations", "genga_kepler_drift", "genga_counters", "genga_time_kernel", "genga_profile_step",
     "genga_eval_fast", "genga_fp64_probe", "genga_strerror",
     "genga_last_cuda_error",
@@ -74,6 +74,7 @@ def load():
         "genga_set_system_params_host": (i, [vp, dp, dp]),
         "genga_energy": (i, [vp, dp, dp]),
         "genga_encounters": (i, [vp, vp, l, C.POINTER(l), C.POINTER(l), vp]),
+        "genga_bs_trace": (i, [vp, vp, l, C.POINTER(l)]),
         "genga_status": (i, [vp]),
         "genga_accelerations": (i, [vp, d, dp, dp]),
         "genga_kepler_drift": (i, [vp, l, d, d, dp, dp]),
@@ -228,6 +229,14 @@ class Genga:
         _chk(self.lib.genga_encounters(self.h, _hp(pairs), self.max_pairs, C.byref(npairs), C.byref(ncand),
                                        _hp(labels) if with_labels else None), "genga_encounters")
         return pairs[: npairs.value].copy(), int(ncand.value), labels
+
+    def bs_trace(self):
+        """records (n, layout, accepted, rejected, cycles, member) of the groups integrated in the last substep"""
+        out = np.zeros((4096, 4), dtype=np.int32)
+        n = C.c_int64()
+        _chk(self.lib.genga_bs_trace(self.h, _hp(out), 4096, C.byref(n)), "genga_bs_trace")
+        r = out[: min(n.value, 4096)]
+        return np.stack([r[:, 0] & 0xffff, r[:, 0] >> 16, r[:, 1] & 0xffff, r[:, 1] >> 16, r[:, 2], r[:, 3]], axis=1)
 
     def status(self):
         return self.lib.genga_status(self.h)

@@ -142,6 +142,7 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
     t.enc = (int2 *)take(sizeof(int2) * (size_t)c->max_pairs);
     t.cnt = (int *)take(sizeof(int) * CI_COUNT);
     t.stat = (long long *)take(sizeof(long long) * CNT_N);
+    t.bstrace = (int4 *)take(sizeof(int4) * BS_TRACE_CAP);
     t.label = (int *)take(sizeof(int) * np);
     *exp_labels = (int *)take(sizeof(int) * np);
     if (d) *d = t;
@@ -752,6 +753,21 @@ extern "C" __attribute__((visibility("default"))) int genga_encounters(genga_ctx
     if (n_pairs) *n_pairs = cnt[CI_NENC];
     if (n_candidates) *n_candidates = cnt[CI_NCAND];
     return r;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_bs_trace(genga_ctx *c, int32_t *out, int64_t cap, int64_t *n)
+{
+    if (!c || !n || cap < 0 || (cap > 0 && !out)) return GENGA_EINVAL;
+    int cnt = 0;
+    CK(cudaMemcpyAsync(&cnt, c->d.cnt + CI_NTRACE, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    *n = cnt;
+    const int64_t m = std::min<int64_t>(std::min<int64_t>(cnt, BS_TRACE_CAP), cap);
+    if (m > 0) {
+        CK(cudaMemcpyAsync(out, c->d.bstrace, sizeof(int4) * (size_t)m, cudaMemcpyDeviceToHost, c->st));
+        CK(cudaStreamSynchronize(c->st));
+    }
+    return GENGA_OK;
 }
 
 extern "C" __attribute__((visibility("default"))) int genga_accelerations(genga_ctx *c, double dt, double *a, double *rcrit)

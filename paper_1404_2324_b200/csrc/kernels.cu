@@ -3,6 +3,7 @@
 #include "kernels.cuh"
 #include "bs_cluster.cuh"
 #include "bs_warp.cuh"
+#include "bs_small.cuh"
 
 namespace genga {
 
@@ -12,6 +13,19 @@ __device__ __forceinline__ void pdl_sync()
 {
     asm volatile("griddepcontrol.launch_dependents;");
     asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
+// the per-map counters: candidates, encounter pairs, groups, listed particles, the Bulirsch-Stoer queues and trace
+__device__ __forceinline__ void reset_map_counters(const DevState &d)
+{
+    d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
+    d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0; d.cnt[CI_NTRACE] = 0;
+}
+// one record per integrated group (genga_bs_trace): size, layout, accepted steps, rejected attempts, SM cycles
+__device__ __forceinline__ void bs_trace(const DevState &d, int n, int layout, const int *nsteps, long long t0, int first)
+{
+    const int k = atomicAdd(&d.cnt[CI_NTRACE], 1);
+    if (k < BS_TRACE_CAP) d.bstrace[k] = make_int4(n | (layout << 16), nsteps[0] | (nsteps[1] << 16), (int)(clock64() - t0), first);
 }
 
 // =====================================================================================
@@ -31,8 +45,7 @@ __global__ void k_reset_counters(DevState d)
 {
     pdl_sync();
     if (threadIdx.x == 0) {
-        d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
-        d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0;
+        reset_map_counters(d);
     }
 }
 
@@ -63,8 +76,7 @@ __global__ void k_rcrit(DevState d, double tau, int reset)
         if (threadIdx.x == 0) d.cnt[CI_NTP_PREV] = nprev;
     }
     if (reset && i == 0) {                                // start of a step: forget the previous step's lists
-        d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
-        d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0;
+        reset_map_counters(d);
     }
     if (i >= d.ntot) return;
     double x = d.x[i], y = d.y[i], z = d.z[i], vx = d.vx[i], vy = d.vy[i], vz = d.vz[i], m = d.m[i];
@@ -577,8 +589,7 @@ __global__ void __launch_bounds__(32) k_tpm_kick(DevState d, double h, int recor
 // runs a whole half map per launch.  Pair arithmetic as k_kick_multi, critical radius as k_rcrit, Sun kick and drift as k_sun.
 __device__ __forceinline__ void tiny_reset(const DevState &d)
 {
-    d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
-    d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0;
+    reset_map_counters(d);
 }
 struct TinySmem { double x[32], y[32], z[32], gm[32], rc[32]; };
 __device__ __forceinline__ void tiny_kick(const DevState &d, TinySmem &S, int t, bool live, double h, int record,
@@ -871,8 +882,7 @@ __global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset, do
     __shared__ double red[3][8];
     const int i = blockIdx.x * 256 + threadIdx.x;
     if (reset && i == 0) {
-        d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
-        d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0;
+        reset_map_counters(d);
     }
     double sx = 0.0, sy = 0.0, sz = 0.0, m0;
     if (d.mode == 2) {
@@ -1202,6 +1212,7 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
             S.m[b] = d.m[i]; S.rc[b] = rc; S.irc[b] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
         }
         int nsteps[2] = {0, 0};
+        const long long t0 = clock64();
         bool ok = bc_integrate<MAXN, THREADS, CS>(S, S0, rank, t, d.G, d.m0[0], h, d.eps, nsteps);
         if (rank == 0) {
             __syncthreads();
@@ -1214,6 +1225,7 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
                 if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
                 atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps[0]);
                 atomicAdd((unsigned long long *)&d.stat[CNT_BSREJECTS], (unsigned long long)nsteps[1]);
+                bs_trace(d, n, 1, nsteps, t0, d.gmem[off]);
             }
         }
     }
@@ -1221,8 +1233,9 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
 }
 template __global__ void k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>(DevState, double, int, int);
 
-// Bulirsch-Stoer on the SMALL groups (2..BW_MAXN bodies) of every mode: one warp per group, the
-// extrapolation columns side by side in its lanes (bs_warp.cuh).  Warps take groups from a queue:
+// Bulirsch-Stoer on the SMALL groups (2..BW_MAXN bodies) of every mode: one block of 4 warps per group, the
+// extrapolation columns and several trial step sizes side by side in its lanes (bs_small.cuh).  Blocks take groups
+// from a queue:
 //   mode 0/1: entries [cnt[CI_QSMALL], cnt[CI_NGROUPS]) of gorder (groups by decreasing size);
 //   mode 2  : entries [0, cnt[CI_NGROUPS]) of gorder, each (system, 16-bit member mask);
 //   particles (tp = 1, mode 1): entries [0, cnt[CI_NTP]) of tplist; group = {particle} + the massive
@@ -1230,16 +1243,17 @@ template __global__ void k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>(DevState, d
 __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h, int tp)
 {
     pdl_sync();
-    __shared__ BwSmem sm[BW_WARPS];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    BwSmem &W = sm[warp];
+    __shared__ BsmSmem W;
+    __shared__ int s_qi;
+    const int lane = threadIdx.x & 31;
     const int qslot = tp ? CI_QTP : CI_QWARP;
     const int qend = tp ? d.cnt[CI_NTP] : d.cnt[CI_NGROUPS];
     if (!tp && d.mode != 2 && d.cnt[CI_QSMALL] >= qend) return;
     while (true) {
-        int qi = 0;
-        if (lane == 0) qi = atomicAdd(&d.cnt[qslot], 1);
-        qi = __shfl_sync(0xffffffffu, qi, 0);
+        __syncthreads();                                   // the previous group is finished with s_qi and W
+        if (threadIdx.x == 0) s_qi = atomicAdd(&d.cnt[qslot], 1);
+        __syncthreads();
+        int qi = s_qi;
         if (!tp && d.mode != 2) qi += d.cnt[CI_QSMALL];
         if (qi >= qend) break;
         // ---- members of the group: body index of slot b = lane % 8
@@ -1279,6 +1293,7 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
         }
         const double Gm0 = d.G * d.m0[sys];
         int nsteps[2] = {0, 0};
+        const long long t0 = clock64();
         bool ok;
         if (n <= 4) {
             // segments of 2 or 4 lanes: slot b = lane % S takes body b from lane b of the 8-slot layout
@@ -1286,25 +1301,25 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
 #pragma unroll
             for (int c = 0; c < 6; ++c) Y[c] = __shfl_sync(0xffffffffu, Y[c], src);
             rc = __shfl_sync(0xffffffffu, rc, src); m = __shfl_sync(0xffffffffu, m, src);
-            if (n == 2) ok = bw_integrate<2>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, nsteps);
-            else ok = bw_integrate<4>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, nsteps);
+            if (n == 2) ok = bsm_integrate<2, BW_WARPS>(W, n, Gm0, rc, m, d.G, Y, h, d.eps, nsteps);
+            else ok = bsm_integrate<4, BW_WARPS>(W, n, Gm0, rc, m, d.G, Y, h, d.eps, nsteps);
         } else {
-            ok = bw_integrate<8>(W, lane, n, Gm0, rc, m, d.G, Y, h, d.eps, nsteps);
+            ok = bsm_integrate<8, BW_WARPS>(W, n, Gm0, rc, m, d.G, Y, h, d.eps, nsteps);
         }
-        if (lane < 8 && writeback) {
+        if (threadIdx.x < 8 && writeback) {
             d.x[i] = Y[0]; d.y[i] = Y[1]; d.z[i] = Y[2]; d.vx[i] = Y[3]; d.vy[i] = Y[4]; d.vz[i] = Y[5];
             if (tp) d.label[i] = plabel;
         }
-        if (lane == 0) {
+        if (threadIdx.x == 0) {
             if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
             atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps[0]);
-                atomicAdd((unsigned long long *)&d.stat[CNT_BSREJECTS], (unsigned long long)nsteps[1]);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSREJECTS], (unsigned long long)nsteps[1]);
             if (tp || d.mode == 2) {
                 atomicAdd((unsigned long long *)&d.stat[CNT_GROUPS], 1ull);
                 atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)n);
             }
+            bs_trace(d, n, 0, nsteps, t0, i);
         }
-        __syncwarp();
     }
 }
 
