@@ -196,7 +196,7 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
         e = cudaMemcpyAsync(c->d.n12, p.data(), sizeof(double) * p.size(), cudaMemcpyHostToDevice, c->st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
     }
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_LV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                    (int)sizeof(BcSmem<BCB_MAXN, BCB_THREADS>));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_kick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kick_smem_bytes());
     for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
@@ -358,9 +358,10 @@ static void enqueue_sun(genga_ctx *c, double h, int reset = 0, bool after_bs = f
     LAUNCH(c); LAUNCH(c);
 }
 
-template <int MAXN, int THREADS, int CS>
+template <int MAXN, int THREADS, int LV>
 static cudaError_t launch_bs_cluster(cudaStream_t st, int clusters, const DevState &d, double h, int qslot, int endslot)
 {
+    constexpr int CS = 8 * LV;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(clusters * CS);
     cfg.blockDim = dim3(THREADS);
@@ -371,7 +372,7 @@ static cudaError_t launch_bs_cluster(cudaStream_t st, int clusters, const DevSta
     at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = CS > 1 ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, k_bs_cluster<MAXN, THREADS, CS>, d, h, qslot, endslot);
+    return cudaLaunchKernelEx(&cfg, k_bs_cluster<MAXN, THREADS, LV>, d, h, qslot, endslot);
 }
 
 // One second-order map S2(h), Eq. 7 (L100), in the order of the bullet list L153-166.
@@ -430,7 +431,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         if (mid) {
             cudaEventRecord(c->ev_fork, st);
             cudaStreamWaitEvent(c->aux[0], c->ev_fork, 0);
-            launch_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>(c->aux[0], c->bs_big_clusters, d, h, CI_QBIG, CI_NMIDEND); LAUNCH(c);
+            launch_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_LV>(c->aux[0], c->bs_big_clusters, d, h, CI_QBIG, CI_NMIDEND); LAUNCH(c);
             cudaEventRecord(c->ev_join[0], c->aux[0]);
             if (d.bss.base && d.mode == GENGA_MODE_MASSIVE) {
                 cudaStreamWaitEvent(c->aux[1], c->ev_fork, 0);

@@ -1181,24 +1181,26 @@ __global__ void __launch_bounds__(1024) k_build_groups(DevState d)
 // members start from the state before the drift and overwrite the drift result (L163, L301-314).
 // Clusters take groups from a queue in order of decreasing size: entries [cnt[qslot], cnt[endslot])
 // of gorder (two instantiations run side by side on the two halves of the queue).
-template <int MAXN, int THREADS, int CS>
+template <int MAXN, int THREADS, int LV>
 __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, int qslot, int endslot)
 {
     pdl_sync();
     extern __shared__ __align__(16) unsigned char bc_raw[];
     using Smem = BcSmem<MAXN, THREADS>;
     Smem &S = *reinterpret_cast<Smem *>(bc_raw);
-    int rank = 0;
-    Smem *S0 = &S;
-    if constexpr (CS > 1) {
-        cg::cluster_group cluster = cg::this_cluster();
-        rank = (int)cluster.block_rank();
-        S0 = cluster.map_shared_rank(&S, 0);
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank();
+    Smem *S0 = cluster.map_shared_rank(&S, 0);
+    if (threadIdx.x == 0) {
+        S.seq_begin = 0; S.seq_end = 0; S.rec_state = 0;
+        for (int k = 0; k < BS_KMAX; ++k) S.ready[k] = 0;
+        for (int k = 0; k < 4; ++k) S.lev_result[k] = 0;
     }
+    int seq = 0;                                    // round numbers of the cluster's protocol run on from group to group
     const int qend = d.cnt[endslot];
     while (true) {
         if (rank == 0 && threadIdx.x == 0) S.cur = atomicAdd(&d.cnt[qslot], 1);
-        bc_sync<CS>();
+        cluster.sync();                             // also: everybody has left the previous group, its shared memory may be reused
         const int qi = S0->cur;
         if (qi >= qend) break;
         const int g = d.gorder[qi];
@@ -1213,7 +1215,8 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
         }
         int nsteps[2] = {0, 0};
         const long long t0 = clock64();
-        bool ok = bc_integrate<MAXN, THREADS, CS>(S, S0, rank, t, d.G, d.m0[0], h, d.eps, nsteps);
+        cluster.sync();                             // S0->cur has been read by everybody (the master may pop the next group)
+        bool ok = bc_integrate<MAXN, THREADS, LV>(S, rank, t, d.G, d.m0[0], h, d.eps, nsteps, seq);
         if (rank == 0) {
             __syncthreads();
             for (int b = threadIdx.x; b < n; b += THREADS) {
@@ -1229,9 +1232,9 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
             }
         }
     }
-    bc_sync<CS>();      // nobody leaves while its shared memory may still be read
+    cluster.sync();     // nobody leaves while its shared memory may still be read
 }
-template __global__ void k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_CS>(DevState, double, int, int);
+template __global__ void k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_LV>(DevState, double, int, int);
 
 // Bulirsch-Stoer on the SMALL groups (2..BW_MAXN bodies) of every mode: one block of 4 warps per group, the
 // extrapolation columns and several trial step sizes side by side in its lanes (bs_small.cuh).  Blocks take groups

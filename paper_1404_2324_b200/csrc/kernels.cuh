@@ -13,7 +13,7 @@ constexpr int KK_MAXN = 2048;     // massive bodies of one system (L188)
 
 // Bulirsch-Stoer layouts: groups of 2..8 bodies on one warp (bs_warp.cuh), of 9..256 bodies on a
 // cluster of 8 CTAs (bs_cluster.cuh), larger ones on one block with a global-memory tableau (bs.cuh)
-constexpr int BCB_MAXN = 256, BCB_THREADS = 512, BCB_CS = 8;
+constexpr int BCB_MAXN = 256, BCB_THREADS = 512, BCB_LV = 1, BCB_CS = 8 * BCB_LV;   // BCB_LV trial step sizes side by side, 8 CTAs each
 
 __global__ void k_begin_map(DevState d);
 __global__ void k_reset_counters(DevState d);
@@ -37,7 +37,7 @@ __global__ void k_drift(DevState d, double h, double hsun);
 __global__ void k_drift_arrays(long long n, double mu, double h, double *x, double *v, int *status);
 __global__ void k_confirm(DevState d, double h);
 __global__ void k_build_groups(DevState d);
-template <int MAXN, int THREADS, int CS> __global__ void k_bs_cluster(DevState d, double h, int qslot, int endslot);
+template <int MAXN, int THREADS, int LV> __global__ void k_bs_cluster(DevState d, double h, int qslot, int endslot);
 __global__ void k_bs_warp(DevState d, double h, int tp);
 __global__ void k_list_groups_multi(DevState d);
 __global__ void k_bs_block(DevState d, double h);
