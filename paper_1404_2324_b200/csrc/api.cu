@@ -198,6 +198,19 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     }
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_LV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                    (int)sizeof(BcSmem<BCB_MAXN, BCB_THREADS>));
+    if (e == cudaSuccess && BCB_CS > 8) e = cudaFuncSetAttribute(k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_LV>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e == cudaSuccess) {                                    // clusters of BCB_CS CTAs the device can hold at once
+        cudaLaunchConfig_t q = {};
+        q.gridDim = dim3(BCB_CS * 32); q.blockDim = dim3(BCB_THREADS); q.dynamicSmemBytes = sizeof(BcSmem<BCB_MAXN, BCB_THREADS>);
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = BCB_CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        q.attrs = at; q.numAttrs = 1;
+        int nc = 0;
+        e = cudaOccupancyMaxActiveClusters(&nc, k_bs_cluster<BCB_MAXN, BCB_THREADS, BCB_LV>, &q);
+        if (e == cudaSuccess) c->bs_big_clusters = std::max(1, nc);
+        if (getenv("GENGA_VERBOSE")) fprintf(stderr, "genga: %d clusters of %d CTAs active at once\n", nc, BCB_CS);
+    }
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_kick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kick_smem_bytes());
     for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
         e = cudaStreamCreateWithFlags(&c->aux[k], cudaStreamNonBlocking);

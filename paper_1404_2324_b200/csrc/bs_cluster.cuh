@@ -22,6 +22,7 @@
 // __syncthreads per force evaluation.
 #pragma once
 #include <cooperative_groups.h>
+#include <cstdio>
 
 #include "bs.cuh"
 
@@ -96,6 +97,13 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
                                        const volatile int *watch)
 {
     GENGA_BS_RHS_HOOK();
+#ifdef GENGA_BC_PROF
+    long long ph_[8]; int phn_ = 0;
+#define RHS_PROF() ph_[phn_++] = clock64();
+#else
+#define RHS_PROF()
+#endif
+    RHS_PROF()
     double(*pA)[MAXN] = S.pos[buf][0];
     double(*pB)[MAXN] = S.pos[buf][1];
     float4 *fA = S.pf[buf][0];
@@ -112,6 +120,7 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
     if (threadIdx.x == 0) S.bc[buf] = *watch;
     __syncthreads();
     const int seen = S.bc[buf];
+    RHS_PROF()
     buf ^= 1;
     double ax = 0.0, ay = 0.0, az = 0.0, bx = 0.0, by = 0.0, bz = 0.0;
     const int n = t.n, L = t.L, i = t.i;
@@ -142,7 +151,9 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
         if (lane == 31) S.wtot[warp] = inc;
+        RHS_PROF()
         __syncthreads();
+        RHS_PROF()
         int base = 0, total = 0;
 #pragma unroll
         for (int w = 0; w < THREADS / 32; ++w) { const int v = S.wtot[w]; base += w < warp ? v : 0; total += v; }
@@ -154,6 +165,7 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
             const int start = __shfl_sync(0xffffffffu, at, lane & ~(L - 1));
             for (unsigned mm = mask; mm; mm &= mm - 1) S.plist[at++] = make_int2(i, t.s + (__ffs(mm) - 1) * L);
             __syncthreads();
+            RHS_PROF()
             // ---- one thread per listed pair: exact test and both changeover weights, without the partner's mass
             for (int p = threadIdx.x; p < total; p += THREADS) {
                 const int2 pr = S.plist[p];
@@ -170,7 +182,9 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
                 S.pres[p][0] = wA * dx; S.pres[p][1] = wA * dy; S.pres[p][2] = wA * dz;
                 S.pres[p][3] = wB * ex; S.pres[p][4] = wB * ey; S.pres[p][5] = wB * ez;
             }
+            RHS_PROF()
             __syncthreads();
+            RHS_PROF()
             // ---- body i: its own range, lane s takes every L-th entry
             if (live) {
                 for (int p = start + t.s; p < start + cseg; p += L) {
@@ -257,6 +271,14 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
     }
     aA[0] = ax; aA[1] = ay; aA[2] = az;
     aB[0] = bx; aB[1] = by; aB[2] = bz;
+#ifdef GENGA_BC_PROF
+    RHS_PROF()
+    if (threadIdx.x == 0 && t.n == 55 && (blockIdx.x & 7) < 2 && seen < 4) {
+        printf("rhs n=%d blk=%d seq=%d phases:", t.n, blockIdx.x & 7, seen);
+        for (int k = 1; k < phn_; ++k) printf(" %d", (int)(ph_[k] - ph_[k - 1]));
+        printf("\n");
+    }
+#endif
     return seen;
 }
 
@@ -380,6 +402,12 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, const int
         for (int r = 0; r < NCTA; ++r) cluster.map_shared_rank(&S, r)->seq_end = seq + 1;
     }
     bool ok = true;
+#ifdef GENGA_BC_PROF
+    long long pf_t = clock64(), pf_acc[6] = {0, 0, 0, 0, 0, 0};   // record, rhs, wait, check, publish, calls
+#define BC_PROF(k) { const long long now_ = clock64(); pf_acc[k] += now_ - pf_t; pf_t = now_; }
+#else
+#define BC_PROF(k)
+#endif
     while (true) {
         // ---- the newest record (sequence lock: the master may be rewriting it)
         int e, state;
@@ -405,6 +433,7 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, const int
             consistent = __syncthreads_and(S.seq_begin == e) != 0;
         } while (!consistent);
         seq = e;
+        BC_PROF(0)
         if (state != 0) { ok = state == 1; break; }
         const double Hl = ldexp(Hr, -lev);
         const bool under = lev > 0 && fabs(Hl) < BS_HMIN * fabs(h);
@@ -444,6 +473,7 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, const int
                 if (tid == 0) SC->ready[col] = seq;
             }
         }
+        BC_PROF(1)
         if (!checker) continue;
         // ---- checker of this level: rows 1.. as their columns arrive; first row whose error passes
         int code = under ? 0 : 1;                 // 0 underflow, 1 rejected, 2 + k passed at row k
@@ -459,7 +489,9 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, const int
                 __syncthreads();
                 if (S.bc[0] == 0) { dropped = true; break; }
                 __threadfence();
+                BC_PROF(2)
                 const double err = bc_check_row(S, n, k);
+                BC_PROF(3)
                 if (err <= eps2) { code = 2 + k; break; }
             }
         }
@@ -541,7 +573,11 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, const int
             __threadfence();
             for (int r = 0; r < NCTA; ++r) cluster.map_shared_rank(&S, r)->seq_end = ns;
         }
+        BC_PROF(4)
     }
+#ifdef GENGA_BC_PROF
+    if (master && tid == 0 && nsteps) { for (int k = 0; k < 5; ++k) nsteps[2 + k] = (int)(pf_acc[k] >> 4); }
+#endif
     return ok;
 }
 

@@ -27,17 +27,24 @@
 namespace genga {
 
 constexpr int BSM_MAXL = 8;
+constexpr int BSM_SLOTS = 16;        // levels x lanes per segment: 8 x 2, 4 x 4 or 2 x 8
 
 struct BsmSmem {
-    double tab[BSM_MAXL][BS_KMAX][6][BW_MAXN];   // [level][column][component][body]: column results T[k][0]
-    double Y[6][BW_MAXN];                        // state at the start of the round / the accepted state
-    double werr[BSM_MAXL][6][BW_MAXN];           // scaled squared corrections of the row under test
+    double tab[BS_KMAX][6][BSM_SLOTS];           // [column][component][level * S + body]: column results T[k][0], then T[k][k]
+    double werr[BS_KMAX][6][BSM_SLOTS];          // scaled squared corrections of the rows under test
+    double Y[6][BW_MAXN];                        // state at the start of the round
     int status[BSM_MAXL];                        // 0 running, 1 + k accepted at row k, -1 rejected, -2 step size underflow
 };
 
 // Integrate one group over h with NW warps (the whole block).  Lane layout as above; Y = state of body b = lane % S
 // (any finite dummy for b >= n), the same in every segment.  On return Y holds the result in every lane.
 // nsteps[0] += accepted steps, nsteps[1] += rejected attempts (as the sequential rule counts them).
+//
+// The tableau is not tested after every evaluation: a test costs about as much as two evaluations (two block barriers,
+// a trip through shared memory, a reduction over the bodies).  It is tested when the row the previous step of this
+// group was accepted at has become complete (row 4 at first), then every second row, and at the end; a test looks at all
+// the rows completed since the last one and takes the FIRST that passes, so the accepted row is the sequential
+// algorithm's whatever the schedule of the tests.
 template <int S, int NW>
 __device__ __forceinline__ bool bsm_integrate(BsmSmem &W, const int n, const double Gm0, const double my_rc, const double my_m,
                                               const double G, double (&Y)[6], const double h, const double eps, int *nsteps)
@@ -46,7 +53,7 @@ __device__ __forceinline__ bool bsm_integrate(BsmSmem &W, const int n, const dou
     constexpr int L = NW * SPW / BS_KMAX;             // speculation levels
     constexpr int LL = (8 * S < 32) ? 8 * S : 32;     // lanes of a level inside its first warp
     constexpr int NROUND = (6 * S + LL - 1) / LL;     // tableau entries (component, body) per checking lane
-    static_assert(L >= 1 && L <= BSM_MAXL, "levels");
+    static_assert(L >= 1 && L <= BSM_MAXL && L * S <= BSM_SLOTS, "levels");
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int slot = warp * SPW + lane / S, lev = slot / BS_KMAX, col = slot % BS_KMAX, b = lane % S;
@@ -79,6 +86,7 @@ __device__ __forceinline__ bool bsm_integrate(BsmSmem &W, const int n, const dou
     const double eps2 = eps * eps;
     double q[3], V[3], acc0[3];
     double wsc[NROUND];                               // checker: 1 / |q_b|^2 or 1 / |V_b|^2 of its entries
+    int hint = 4;                                     // the row to test first
     while (!last) {
         double rem = h - done;
         if (fabs(rem) <= 8.0 * 2.220446049250313e-16 * fabs(h)) break;     // a remainder of a few ulp of h: done
@@ -124,14 +132,14 @@ __device__ __forceinline__ bool bsm_integrate(BsmSmem &W, const int n, const dou
         for (int r = 0; r < NROUND; ++r)
 #pragma unroll
             for (int j = 0; j < BS_KMAX; ++j) prow[r][j] = 0.0;
-        int winner = -1, wrow = 0;
+        if (checker && cl == 0) W.status[lev] = mystat;           // read after the barriers of the first test
+        int winner = -1, wrow = 0, tested = -1, next_test = hint;
         bool resolved = false;
 #pragma unroll 1
         for (int it = 0; it < BS_KMAX && !resolved; ++it) {
             // ---- my column: Gragg's modified midpoint rule, two substeps per evaluation (bs_warp.cuh)
             const bool work = mystat == 0;            // my level is still undecided
-            // warp-uniform: some column of this warp still runs
-            if (__any_sync(full, work && it <= col)) {
+            if (__any_sync(full, work && it <= col)) {            // warp-uniform: some column of this warp still runs
                 double qc[3], A[3], C[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) qc[c] = qa[c] + 2.0 * eta * Vb[c];
@@ -142,8 +150,8 @@ __device__ __forceinline__ bool bsm_integrate(BsmSmem &W, const int n, const dou
                 for (int c = 0; c < 3; ++c) {
                     double vc = Va[c] + 2.0 * eta * A[c];
                     if (fin && body && work) {
-                        W.tab[lev][col][c][b] = 0.5 * (qc[c] + qb[c] + eta * vc);
-                        W.tab[lev][col][3 + c][b] = 0.5 * (vc + Vb[c] + eta * C[c]);
+                        W.tab[col][c][lev * S + b] = 0.5 * (qc[c] + qb[c] + eta * vc);
+                        W.tab[col][3 + c][lev * S + b] = 0.5 * (vc + Vb[c] + eta * C[c]);
                     }
                     double qd = qb[c] + 2.0 * eta * vc, vd = Vb[c] + 2.0 * eta * C[c];
                     qa[c] = qc[c]; Va[c] = vc; qb[c] = qd; Vb[c] = vd;
@@ -154,51 +162,58 @@ __device__ __forceinline__ bool bsm_integrate(BsmSmem &W, const int n, const dou
                     eta = 0.0;
                 }
             }
+            if (it < next_test && it < BS_KMAX - 1) continue;     // no test after this evaluation (uniform over the block)
             __syncthreads();
-            // ---- the tableau row that became complete: T[it][j] = T[it][j-1] + (T[it][j-1] - T[it-1][j-1]) / ((n_it / n_{it-j})^2 - 1)
+            // ---- the tableau rows completed since the last test: T[r][j] = T[r][j-1] + (T[r][j-1] - T[r-1][j-1]) / ((n_r / n_{r-j})^2 - 1)
             if (checker && mystat == 0) {
-                double wv[NROUND];
+#pragma unroll 1
+                for (int row = tested + 1; row <= it; ++row) {
 #pragma unroll
-                for (int r = 0; r < NROUND; ++r) {
-                    const int item = cl + LL * r, c = item / S, bb = item % S;
-                    wv[r] = 0.0;
-                    if (item < 6 * S && bb < n) {
-                        double cur = W.tab[lev][it][c][bb], prev = prow[r][0], diff = 0.0;
-                        prow[r][0] = cur;
+                    for (int r = 0; r < NROUND; ++r) {
+                        const int item = cl + LL * r, c = item / S, bb = item % S;
+                        if (item < 6 * S && bb < n) {
+                            double cur = W.tab[row][c][lev * S + bb], prev = prow[r][0], diff = 0.0;
+                            prow[r][0] = cur;
 #pragma unroll
-                        for (int j = 1; j < BS_KMAX; ++j) {
-                            if (j <= it) {
-                                const double tmp = prow[r][j];
-                                const double nxt = cur + (cur - prev) * c_bs_iden.v[it][j];
-                                diff = nxt - cur;
-                                cur = nxt;
-                                prow[r][j] = cur;
-                                prev = tmp;
+                            for (int j = 1; j < BS_KMAX; ++j) {
+                                if (j <= row) {
+                                    const double tmp = prow[r][j];
+                                    const double nxt = cur + (cur - prev) * c_bs_iden.v[row][j];
+                                    diff = nxt - cur;
+                                    cur = nxt;
+                                    prow[r][j] = cur;
+                                    prev = tmp;
+                                }
                             }
+                            W.tab[row][c][lev * S + bb] = cur;    // T[row][row]: the state if this row is accepted
+                            W.werr[row][c][lev * S + bb] = diff * diff * wsc[r];
                         }
-                        wv[r] = diff * diff * wsc[r];
-                        W.tab[lev][it][c][bb] = cur;              // T[it][it]: the state if this row is accepted
-                        W.werr[lev][c][bb] = wv[r];
                     }
                 }
             }
             __syncwarp();
-            if (checker && mystat == 0 && it >= 1) {
-                double e = 0.0;
-                if (cl < n) {
-                    const double dq = W.werr[lev][0][cl] + W.werr[lev][1][cl] + W.werr[lev][2][cl];
-                    const double dv = W.werr[lev][3][cl] + W.werr[lev][4][cl] + W.werr[lev][5][cl];
-                    e = fmax(dq, dv);
-                }
-                // the first S lanes of the level hold the bodies' errors
+            if (checker && mystat == 0) {
+                int pass = -1;                        // first row, among the new ones, whose error passes
+#pragma unroll 1
+                for (int row = max(tested + 1, 1); row <= it; ++row) {
+                    double e = 0.0;
+                    if (cl < n) {
+                        const double dq = W.werr[row][0][lev * S + cl] + W.werr[row][1][lev * S + cl] + W.werr[row][2][lev * S + cl];
+                        const double dv = W.werr[row][3][lev * S + cl] + W.werr[row][4][lev * S + cl] + W.werr[row][5][lev * S + cl];
+                        e = fmax(dq, dv);
+                    }
 #pragma unroll
-                for (int o = S / 2; o > 0; o >>= 1) e = fmax(e, __shfl_xor_sync(lmask, e, o, S));
+                    for (int o = S / 2; o > 0; o >>= 1) e = fmax(e, __shfl_xor_sync(lmask, e, o, S));   // the first S lanes of the level hold the bodies' errors
+                    e = __shfl_sync(lmask, e, lfirst);
+                    if (pass < 0 && e <= eps2) pass = row;
+                }
                 if (cl == 0) {
-                    if (e <= eps2) W.status[lev] = 1 + it;
+                    if (pass >= 0) W.status[lev] = 1 + pass;
                     else if (it == BS_KMAX - 1) W.status[lev] = -1;
                 }
             }
-            if (it == 0 && checker && cl == 0) W.status[lev] = mystat;          // round start: running (or underflow)
+            tested = it;
+            next_test = min(it + 2, BS_KMAX - 1);
             __syncthreads();
             // ---- decision, the same in every thread: the first level, in the order H, H/2, ..., that passed
             mystat = W.status[lev];
@@ -215,7 +230,7 @@ __device__ __forceinline__ bool bsm_integrate(BsmSmem &W, const int n, const dou
         if (winner >= 0) {
             if (body) {
 #pragma unroll
-                for (int c = 0; c < 6; ++c) Y[c] = W.tab[winner][wrow][c][b];
+                for (int c = 0; c < 6; ++c) Y[c] = W.tab[wrow][c][winner * S + b];
             }
             const double Hw = ldexp(H, -winner);
             done += Hw;
@@ -224,6 +239,7 @@ __device__ __forceinline__ bool bsm_integrate(BsmSmem &W, const int n, const dou
             if (wrow <= 4) H *= 1.5;
             if (winner > 0) last = false;
             fresh = true;
+            hint = max(2, wrow);
         } else {                                      // every level rejected
             if (nsteps) nsteps[1] += L;
             H = ldexp(H, -L); last = false;

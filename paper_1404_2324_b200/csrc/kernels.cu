@@ -1213,9 +1213,9 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
             double rc = d.rc[i];
             S.m[b] = d.m[i]; S.rc[b] = rc; S.irc[b] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
         }
-        int nsteps[2] = {0, 0};
-        const long long t0 = clock64();
+        int nsteps[8] = {0, 0, 0, 0, 0, 0, 0, 0};
         cluster.sync();                             // S0->cur has been read by everybody (the master may pop the next group)
+        const long long t0 = clock64();
         bool ok = bc_integrate<MAXN, THREADS, LV>(S, rank, t, d.G, d.m0[0], h, d.eps, nsteps, seq);
         if (rank == 0) {
             __syncthreads();
@@ -1229,6 +1229,15 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
                 atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps[0]);
                 atomicAdd((unsigned long long *)&d.stat[CNT_BSREJECTS], (unsigned long long)nsteps[1]);
                 bs_trace(d, n, 1, nsteps, t0, d.gmem[off]);
+#ifdef GENGA_BC_PROF
+                {   // cycles / 16 by phase: record, rhs, wait, check, publish
+                    const int k = atomicAdd(&d.cnt[CI_NTRACE], 2);
+                    if (k + 1 < BS_TRACE_CAP) {
+                        d.bstrace[k] = make_int4(n | (2 << 16), nsteps[2], nsteps[3], nsteps[4]);
+                        d.bstrace[k + 1] = make_int4(n | (3 << 16), nsteps[5], nsteps[6], 0);
+                    }
+                }
+#endif
             }
         }
     }
