@@ -59,7 +59,9 @@ typedef struct {
     int32_t n_systems;  /* mode 2 only: 1..100000; else 1                                     */
     int32_t flags;      /* bit 0: do not merge the closing kick of a substep with the opening kick
                            of the next substep of the same step (orders 4, 6; modes 0, 2; L170);
-                           the result is the same map, this only selects the schedule         */
+                           the result is the same map, this only selects the schedule;
+                           bit 1: mode 0, do not reuse the far-pair sums of a step's closing kick in the
+                           opening kick of the next step (L266-274); same map, schedule only        */
     double G;           /* gravitational constant                                            */
     double n1, n2;      /* critical-radius parameters of Eq. 6 (L94-96); usually 3 and 0.4   */
     double bs_eps;      /* Bulirsch-Stoer relative tolerance (L116 "machine precision")      */
@@ -96,7 +98,10 @@ int genga_set_state(genga_ctx *ctx, const double *m0, const double *m, const dou
 int genga_set_state_host(genga_ctx *ctx, const double *m0, const double *m, const double *radius,
                          const double *x, const double *v);
 
-/* Advance n_steps time steps of length dt (dt < 0 integrates backwards) with the hybrid
+/* The kernel sequence of (dt, order) is captured into CUDA graphs (16 steps, 1 step) the first time it is used and
+ * replayed afterwards; the cache is keyed on the exact value of dt and holds 16 entries (a 17th clears it), so a
+ * caller that changes dt at every call pays a capture (~1 ms) per call.
+ * Advance n_steps time steps of length dt (dt < 0 integrates backwards) with the hybrid
  * symplectic scheme of order 2 (Eq. 7; per-step algorithm), 4 or 6
  * (Yoshida compositions, L168-170).  Each step: critical radii (Eq. 6), kick with the
  * changeover weight and prechecker (Eq. 2), Sun kick (Eq. 3), Kepler drift (Eq. 9),

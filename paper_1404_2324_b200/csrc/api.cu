@@ -31,8 +31,8 @@ static thread_local char g_cuda_err[256] = "";
     } while (0)
 
 struct GraphKey {
-    double dt; int order; int nsteps;
-    bool operator<(const GraphKey &o) const { return std::tie(dt, order, nsteps) < std::tie(o.dt, o.order, o.nsteps); }
+    double dt; int order; int nsteps; int reuse;     // reuse: the first step of the graph opens with the stored hit masks (S2')
+    bool operator<(const GraphKey &o) const { return std::tie(dt, order, nsteps, reuse) < std::tie(o.dt, o.order, o.nsteps, o.reuse); }
 };
 
 struct genga_ctx {
@@ -55,6 +55,7 @@ struct genga_ctx {
     std::map<GraphKey, GraphEntry> graphs;
     long long steps, force_evals, interactions, launches;
     long long acc;              // launches enqueued (or captured) since last reset
+    bool far_valid;             // the stored hit masks / far sums of the last closing kick belong to the current positions (S2')
     // genga_profile_step: events at the phase boundaries of plain (uncaptured) launches
     bool prof;
     std::vector<cudaEvent_t> prof_ev;
@@ -143,6 +144,10 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
     t.cnt = (int *)take(sizeof(int) * CI_COUNT);
     t.stat = (long long *)take(sizeof(long long) * CNT_N);
     t.bstrace = (int4 *)take(sizeof(int4) * BS_TRACE_CAP);
+    if (c->mode == GENGA_MODE_MASSIVE && nm > 32) {
+        t.khits = (unsigned *)take(sizeof(unsigned) * (size_t)sms * KK_THREADS);
+        t.kfar = (double *)take(sizeof(double) * 6 * (size_t)sms * KK_THREADS);
+    }
     t.label = (int *)take(sizeof(int) * np);
     *exp_labels = (int *)take(sizeof(int) * np);
     if (d) *d = t;
@@ -185,7 +190,7 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     c->bs_big_clusters = std::max(1, c->sms / BCB_CS);
     c->steps = c->force_evals = c->interactions = c->launches = 0;
     c->acc = 0;
-    c->prof = false; c->prof_used = 0;
+    c->prof = false; c->prof_used = 0; c->far_valid = false;
     c->hstage = nullptr; c->hstatus = nullptr; c->ev_stage = nullptr; c->stage_busy = false;
     size_t need = carve(cfg, (char *)cfg->workspace, &c->d, &c->exp_labels, &c->eout, c->sms);
     if (need > cfg->workspace_bytes) { delete c; return GENGA_EINVAL; }
@@ -267,6 +272,7 @@ static int red_threads(int nm) { return std::min(1024, std::max(32, (int)up((siz
 static void enqueue_helio_to_demo(genga_ctx *c)
 {
     DevState &d = c->d;
+    c->far_valid = false;                                     // new positions: the stored hit masks are void
     k_coord_map<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx0, d.vy0, d.vz0, d.vx, d.vy, d.vz, -1.0, 1);
     c->launches += 1;
 }
@@ -330,17 +336,18 @@ extern "C" __attribute__((visibility("default"))) int genga_set_state_host(genga
 
 // ---------------------------------------------------------------------------------------
 // kick of the massive bodies: one block per SM owning ni bodies i, TJ bodies j per thread
-static void launch_kick(genga_ctx *c, double h, int record, double *aout, int to0 = 0)
+static void launch_kick(genga_ctx *c, double h, int record, double *aout, int to0 = 0, int s2p = 0)
 {
     DevState &d = c->d;
     const int ni = std::min(KK_NI, (d.nm + c->sms - 1) / c->sms);
     const int grid = (d.nm + ni - 1) / ni;
-    launch_k(c->pdl, k_kick, grid, KK_THREADS, kick_smem_bytes(), c->st, d, h, record, ni, aout, to0);
+    launch_k(c->pdl, k_kick, grid, KK_THREADS, kick_smem_bytes(), c->st, d, h, record, ni, aout, to0, s2p);
 }
 
 // to0 (mode 0): the kick is followed by the fused Sun kick + drift (k_sun with hdrift != 0), which reads the kicked
 // velocities from the pre-drift arrays vx0.. and writes the drifted ones to vx..
-static void enqueue_kick(genga_ctx *c, double h, int record, double *aout, int to0 = 0)
+// s2p (mode 0): bit 0 = keep the hit masks and far sums for the next opening kick, bit 1 = use the stored ones
+static void enqueue_kick(genga_ctx *c, double h, int record, double *aout, int to0 = 0, int s2p = 0)
 {
     DevState &d = c->d;
     if (d.mode == GENGA_MODE_MULTI_SYSTEM) {
@@ -348,7 +355,7 @@ static void enqueue_kick(genga_ctx *c, double h, int record, double *aout, int t
         LAUNCH(c);
         return;
     }
-    launch_kick(c, h, record, aout, d.mode == GENGA_MODE_MASSIVE ? to0 : 0);
+    launch_kick(c, h, record, aout, d.mode == GENGA_MODE_MASSIVE ? to0 : 0, d.mode == GENGA_MODE_MASSIVE ? s2p : 0);
     LAUNCH(c);
     if (d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm) {
         launch_k(c->pdl, k_tp_kick, nblk(d.ntot - d.nm, 128), 128, 0, c->st, d, h, record, aout);
@@ -395,7 +402,7 @@ static cudaError_t launch_bs_cluster(cudaStream_t st, int clusters, const DevSta
 // scheme "applied to each of the substeps"; flags bit 0 keeps them apart).
 static inline bool tiny_mode(const DevState &d) { return d.mode == GENGA_MODE_MASSIVE && d.nm <= 32; }
 
-static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last, double hn, bool opened)
+static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last, double hn, bool opened, bool reuse)
 {
     DevState &d = c->d;
     cudaStream_t st = c->st;
@@ -418,7 +425,7 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         launch_k(c->pdl, k_multi_front, nblk(d.nsys, 128 / d.nm), 128, 0, st, d, h, opened ? 0.0 : 0.5 * h); LAUNCH(c);
     } else {
         mark(c, PH_KICK);
-        if (!opened) enqueue_kick(c, 0.5 * h, 1, nullptr, 1);     // else: done by the previous map's merged kick
+        if (!opened) enqueue_kick(c, 0.5 * h, 1, nullptr, 1, reuse ? 2 : 0);     // else: done by the previous map's merged kick
         mark(c, PH_FRONT);
         if (d.mode != GENGA_MODE_TEST_PARTICLE) enqueue_sun(c, 0.5 * h, 0, false, h);   // Sun kick and drift in one launch
         else {
@@ -475,28 +482,41 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
         enqueue_sun(c, 0.5 * h, last ? 0 : 1, true);
         mark(c, PH_KICK);
         if (hn != 0.0) enqueue_kick(c, 0.5 * (h + hn), 1, nullptr, 1);   // closing kick + opening kick of the next map
-        else enqueue_kick(c, 0.5 * h, 0, nullptr);
+        else enqueue_kick(c, 0.5 * h, 0, nullptr, 0, 1);          // closing kick of the step: keeps its hit masks for the next step (S2')
     }
 }
 
 static int maps_per_step(int order) { return order == 2 ? 1 : order == 4 ? 3 : 7; }
 
-static void enqueue_step(genga_ctx *c, double dt, int order)
+// Full force evaluations (all-pairs loops) n_steps steps make: 2 per map; adjacent kicks of the maps of one step are one
+// evaluation (modes 0, 2); with S2' the opening kick of a step is no evaluation either (it adds the stored sums).
+static long long evals_of(const genga_ctx *c, int order, long long n_steps, bool reused_first)
+{
+    const int maps = maps_per_step(order);
+    const bool merged = !(c->cfg.flags & 1) && c->d.mode != GENGA_MODE_TEST_PARTICLE;
+    const long long per = merged ? maps + 1LL : 2LL * maps;
+    const bool s2p = c->d.khits != nullptr && !(c->cfg.flags & 2);
+    return per * n_steps - (s2p ? (n_steps - 1) + (reused_first ? 1 : 0) : 0);
+}
+
+// reuse: the positions are those of the previous step's closing kick and its hit masks are stored (S2', L266-274)
+static void enqueue_step(genga_ctx *c, double dt, int order, bool reuse)
 {
     DevState &d = c->d;
     double w[7];
     int nw = yoshida_weights(order, w);
+    reuse = reuse && d.khits != nullptr && !(c->cfg.flags & 2);
     mark(c, PH_RCRIT);
     if (d.mode == GENGA_MODE_TEST_PARTICLE) {                     // the particles' rc: k_tp_front of the first map
         DevState dm = d;
         dm.ntot = d.nm;
-        launch_k(c->pdl, k_rcrit, 1, 128, 0, c->st, dm, dt, 2); LAUNCH(c);       // nm <= 32: one block, which also opens the first map
+        launch_k(c->pdl, k_rcrit, 1, 128, 0, c->st, dm, dt, 2, 0); LAUNCH(c);    // nm <= 32: one block, which also opens the first map
     } else if (!tiny_mode(d)) {                                   // N <= 32: inside k_tiny_front of the first map
-        launch_k(c->pdl, k_rcrit, nblk(d.ntot, 128), 128, 0, c->st, d, dt, d.mode != GENGA_MODE_TEST_PARTICLE); LAUNCH(c);
+        launch_k(c->pdl, k_rcrit, nblk(d.ntot, 128), 128, 0, c->st, d, dt, d.mode != GENGA_MODE_TEST_PARTICLE, reuse ? 1 : 0); LAUNCH(c);
     }
     const bool merge = !(c->cfg.flags & 1) && d.mode != GENGA_MODE_TEST_PARTICLE;
     for (int k = 0; k < nw; ++k)
-        enqueue_map(c, w[k] * dt, dt, k == 0, k == nw - 1, merge && k + 1 < nw ? w[k + 1] * dt : 0.0, merge && k > 0);
+        enqueue_map(c, w[k] * dt, dt, k == 0, k == nw - 1, merge && k + 1 < nw ? w[k + 1] * dt : 0.0, merge && k > 0, reuse && k == 0);
     mark(c, PH_TOTAL);
 }
 
@@ -507,15 +527,15 @@ static long long interactions_per_eval(const DevState &d)
     return nm * (nm - 1) + (long long)(d.ntot - d.nm) * nm;
 }
 
-static int get_graph(genga_ctx *c, double dt, int order, int nsteps, genga_ctx::GraphEntry *out)
+static int get_graph(genga_ctx *c, double dt, int order, int nsteps, bool reuse, genga_ctx::GraphEntry *out)
 {
-    GraphKey key{dt, order, nsteps};
+    GraphKey key{dt, order, nsteps, reuse ? 1 : 0};
     auto it = c->graphs.find(key);
     if (it == c->graphs.end()) {
         cudaGraph_t g;
         CK(cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal));
         c->acc = 0;
-        for (int s = 0; s < nsteps; ++s) enqueue_step(c, dt, order);
+        for (int s = 0; s < nsteps; ++s) enqueue_step(c, dt, order, s > 0 || reuse);
         long long n = c->acc;
         c->acc = 0;
         CK(cudaStreamEndCapture(c->st, &g));
@@ -536,9 +556,10 @@ extern "C" __attribute__((visibility("default"))) int genga_step(genga_ctx *c, i
 {
     if (!c || n_steps < 0 || dt == 0.0 || !(dt == dt) || (order != 2 && order != 4 && order != 6)) return GENGA_EINVAL;
     if (n_steps == 0) return GENGA_OK;
+    const bool reused_first = c->far_valid;
     if (c->st == nullptr) {                       // legacy stream cannot be captured: plain launches
         c->acc = 0;
-        for (int64_t s = 0; s < n_steps; ++s) enqueue_step(c, dt, order);
+        for (int64_t s = 0; s < n_steps; ++s) enqueue_step(c, dt, order, s > 0 || c->far_valid);
         c->launches += c->acc; c->acc = 0;
     } else {
         const int chunk = 16;
@@ -546,17 +567,18 @@ extern "C" __attribute__((visibility("default"))) int genga_step(genga_ctx *c, i
         while (left > 0) {
             int n = left >= chunk ? chunk : 1;
             genga_ctx::GraphEntry ge;
-            int r = get_graph(c, dt, order, n, &ge);
+            int r = get_graph(c, dt, order, n, c->far_valid, &ge);
             if (r) return r;
             CK(cudaGraphLaunch(ge.exec, c->st));
             c->launches += ge.launches;
+            c->far_valid = true;
             left -= n;
         }
     }
     CK(cudaGetLastError());
+    c->far_valid = true;
     c->steps += n_steps;
-    const bool merged = !(c->cfg.flags & 1) && c->d.mode != GENGA_MODE_TEST_PARTICLE;
-    long long evals = (merged ? maps_per_step(order) + 1LL : 2LL * maps_per_step(order)) * n_steps;   // force evaluations actually made
+    long long evals = evals_of(c, order, n_steps, reused_first);   // force evaluations actually made
     c->force_evals += evals;
     c->interactions += evals * interactions_per_eval(c->d);
     return GENGA_OK;
@@ -568,13 +590,14 @@ extern "C" __attribute__((visibility("default"))) int genga_step(genga_ctx *c, i
 extern "C" __attribute__((visibility("default"))) int genga_profile_step(genga_ctx *c, int64_t n_steps, double dt, int order, double *ms)
 {
     if (!c || !ms || n_steps < 1 || n_steps > 4096 || dt == 0.0 || !(dt == dt) || (order != 2 && order != 4 && order != 6)) return GENGA_EINVAL;
+    const bool reused_first = c->far_valid;
     c->prof = true; c->prof_used = 0; c->acc = 0;
-    for (int64_t s = 0; s < n_steps; ++s) enqueue_step(c, dt, order);
+    for (int64_t s = 0; s < n_steps; ++s) enqueue_step(c, dt, order, s > 0 || c->far_valid);
     c->prof = false;
+    c->far_valid = true;
     c->launches += c->acc; c->acc = 0;
     c->steps += n_steps;
-    const bool merged = !(c->cfg.flags & 1) && c->d.mode != GENGA_MODE_TEST_PARTICLE;
-    const long long evals = (merged ? maps_per_step(order) + 1LL : 2LL * maps_per_step(order)) * n_steps;
+    const long long evals = evals_of(c, order, n_steps, reused_first);
     c->force_evals += evals;
     c->interactions += evals * interactions_per_eval(c->d);
     CK(cudaStreamSynchronize(c->st));
@@ -788,7 +811,8 @@ extern "C" __attribute__((visibility("default"))) int genga_accelerations(genga_
 {
     if (!c || !a || dt == 0.0) return GENGA_EINVAL;
     DevState &d = c->d;
-    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt, 0);
+    c->far_valid = false;
+    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt, 0, 0);
     if (d.mode == GENGA_MODE_TEST_PARTICLE) { k_begin_map<<<c->sms, 256, 0, c->st>>>(d); c->launches += 1; }
     k_reset_counters<<<1, 32, 0, c->st>>>(d);
     c->launches += 2;
@@ -820,7 +844,8 @@ extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ct
     if (which >= 3 && !(d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm)) return GENGA_EINVAL;
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
-    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt, 0);
+    c->far_valid = false;
+    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt, 0, 0);
     c->launches += 1;
     int per = 1;
     for (int r = -3; r < reps; ++r) {

@@ -65,7 +65,7 @@ __device__ __forceinline__ double rcrit_of(double G, double m0, double n1, doubl
     double rv = n2 * fabs(tau) * sqrt(v2);
     return fmax(n1 * rh, rv);
 }
-__global__ void k_rcrit(DevState d, double tau, int reset)
+__global__ void k_rcrit(DevState d, double tau, int reset, int check)
 {
     pdl_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -84,6 +84,9 @@ __global__ void k_rcrit(DevState d, double tau, int reset)
     double n1 = d.n1, n2 = d.n2;
     if (d.mode == 2) { n1 = d.n12[2 * (i / d.nm)]; n2 = d.n12[2 * (i / d.nm) + 1]; }   // per system (L346-354)
     double rc = rcrit_of(d.G, m0, n1, n2, tau, x, y, z, vx, vy, vz, m);
+    // S2': the hit masks of the previous closing kick cover r < 3.3 rc_old; they serve the coming opening kick only if
+    // 3 rc_new <= 3.3 rc_old for every body
+    if (check && rc > KK_GROW * d.rc[i]) d.cnt[CI_S2PMISS] = 1;
     d.rc[i] = rc;
     d.c9[i] = 9.0 * rc * rc;
 }
@@ -143,7 +146,7 @@ struct KickSmem {
     double wsum[KK_WARPS][8][3];            // per warp: sums of its rows
 };
 
-__global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, int record, int ni, double *aout, int to0)
+__global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, int record, int ni, double *aout, int to0, int s2p)
 {
     pdl_sync();
     extern __shared__ __align__(32) unsigned char kk_raw[];
@@ -181,7 +184,7 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
                 b.x = lx[q]; b.y = ly[q]; b.z = lz[q]; b.gm = d.G * lm[q];
                 S.body[j] = b;
                 S.rc[j] = lr[q];
-                S.hc[j] = lr[q] >= 0.0 ? __double2hiint(9.0 * lr[q] * lr[q]) : -1;
+                S.hc[j] = lr[q] >= 0.0 ? __double2hiint(KK_WIDE2 * lr[q] * lr[q]) : -1;
             }
         }
     }
@@ -189,7 +192,7 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
     const double xi0 = ok0 ? d.x[i] : 1e150, yi0 = ok0 ? d.y[i] : 1e150, zi0 = ok0 ? d.z[i] : 1e150;
     const double xi1 = ok1 ? d.x[i + 1] : 1e150, yi1 = ok1 ? d.y[i + 1] : 1e150, zi1 = ok1 ? d.z[i + 1] : 1e150;
     const double rci0 = ok0 ? d.rc[i] : 0.0, rci1 = ok1 ? d.rc[i + 1] : 0.0;
-    const int hci0 = ok0 ? __double2hiint(9.0 * rci0 * rci0) : -1, hci1 = ok1 ? __double2hiint(9.0 * rci1 * rci1) : -1;
+    const int hci0 = ok0 ? __double2hiint(KK_WIDE2 * rci0 * rci0) : -1, hci1 = ok1 ? __double2hiint(KK_WIDE2 * rci1 * rci1) : -1;
     // the velocity component this thread will kick at the end: loaded now, off the critical path
     double vel0 = 0.0;
     if ((tid & 3) == 0 && (tid >> 2) < 3 * nib) {
@@ -200,9 +203,20 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
 
     double ax0 = 0.0, ay0 = 0.0, az0 = 0.0, ax1 = 0.0, ay1 = 0.0, az1 = 0.0;
     unsigned hits = 0u;
+    // S2' (L266-274): s2p & 2 = this is the opening kick of a step at the positions of the previous step's closing kick,
+    // whose hit masks and far-pair sums are stored (s2p & 1 there); they hold as long as no critical radius grew past the
+    // margin of the wide precheck (k_rcrit latches that in CI_S2PMISS, then the pair loop runs again)
+    const bool stored = (s2p & 2) && d.cnt[CI_S2PMISS] == 0;
+    if ((s2p & 1) && blockIdx.x == 0 && tid == 0) d.cnt[CI_S2PMISS] = 0;      // read by the k_rcrit of the next step
     if (rowbase < nib) {                                // warp-uniform: the group has rows in this block
         const int L = iters << logP;
-        {
+        if (stored) {
+            hits = d.khits[(size_t)blockIdx.x * KK_THREADS + tid];
+            if (phase == 0) {
+                const double *f = d.kfar + ((size_t)blockIdx.x * KK_THREADS + tid) * 6;
+                ax0 = f[0]; ay0 = f[1]; az0 = f[2]; ax1 = f[3]; ay1 = f[4]; az1 = f[5];
+            }
+        } else {
             const KickBody *pb = &S.body[wi * L + phase];
             const int *ph = &S.hc[wi * L + phase];
             unsigned bit = 1u;
@@ -231,9 +245,18 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
             }
         }
         // the P phases of a row pair: every lane of the pair gets the sums of its two rows
-        for (int o = 1; o < P; o <<= 1) {
-            ax0 += __shfl_xor_sync(0xffffffffu, ax0, o); ay0 += __shfl_xor_sync(0xffffffffu, ay0, o); az0 += __shfl_xor_sync(0xffffffffu, az0, o);
-            ax1 += __shfl_xor_sync(0xffffffffu, ax1, o); ay1 += __shfl_xor_sync(0xffffffffu, ay1, o); az1 += __shfl_xor_sync(0xffffffffu, az1, o);
+        if (!stored) {
+            for (int o = 1; o < P; o <<= 1) {
+                ax0 += __shfl_xor_sync(0xffffffffu, ax0, o); ay0 += __shfl_xor_sync(0xffffffffu, ay0, o); az0 += __shfl_xor_sync(0xffffffffu, az0, o);
+                ax1 += __shfl_xor_sync(0xffffffffu, ax1, o); ay1 += __shfl_xor_sync(0xffffffffu, ay1, o); az1 += __shfl_xor_sync(0xffffffffu, az1, o);
+            }
+            if (s2p & 1) {                              // keep the sums over the far pairs and the hit masks for the next opening kick
+                d.khits[(size_t)blockIdx.x * KK_THREADS + tid] = hits;
+                if (phase == 0) {
+                    double *f = d.kfar + ((size_t)blockIdx.x * KK_THREADS + tid) * 6;
+                    f[0] = ax0; f[1] = ay0; f[2] = az0; f[3] = ax1; f[4] = ay1; f[5] = az1;
+                }
+            }
         }
         __syncwarp();
 

@@ -10,6 +10,10 @@ constexpr int KK_THREADS = 896;   // threads per block of the kick kernel: 28 wa
 constexpr int KK_WARPS = KK_THREADS / 32;
 constexpr int KK_NI = 14;         // bodies i a block owns at most: ceil(2048 / 148)
 constexpr int KK_MAXN = 2048;     // massive bodies of one system (L188)
+// Squared radius of the kick's branch-free precheck in units of rc_ij^2: 3.3^2 instead of the 3^2 of the candidate test
+// (L142).  The 10 % margin is what lets the opening kick of the NEXT step reuse the hit masks (S2', L266-274): its
+// candidates r < 3 rc' are all hits as long as no critical radius grew by more than 10 % (k_rcrit checks).
+constexpr double KK_WIDE2 = 10.89, KK_GROW = 1.0999;
 
 // Bulirsch-Stoer layouts: groups of 2..8 bodies on one warp (bs_warp.cuh), of 9..256 bodies on a
 // cluster of 8 CTAs (bs_cluster.cuh), larger ones on one block with a global-memory tableau (bs.cuh)
@@ -17,8 +21,8 @@ constexpr int BCB_MAXN = 256, BCB_THREADS = 512, BCB_LV = 2, BCB_CS = 8 * BCB_LV
 
 __global__ void k_begin_map(DevState d);
 __global__ void k_reset_counters(DevState d);
-__global__ void k_rcrit(DevState d, double tau, int reset);
-__global__ void k_kick(DevState d, double h, int record, int ni, double *aout, int to0);
+__global__ void k_rcrit(DevState d, double tau, int reset, int check);
+__global__ void k_kick(DevState d, double h, int record, int ni, double *aout, int to0, int s2p);
 size_t kick_smem_bytes();
 __global__ void k_tp_kick(DevState d, double h, int record, double *aout);
 __global__ void k_tp_front(DevState d, double h, double tau, int first);

@@ -31,13 +31,15 @@ struct DevState {
     unsigned *tpmask;            // mode 1: per particle, massive bodies it meets
     int *tplist;                 // mode 1: particles with encounters in this substep
     long long *stat;             // CNT_* accumulators
+    unsigned *khits;             // mode 0: hit masks of the last closing kick, [blocks][KK_THREADS] (S2', k_kick)
+    double *kfar;                // mode 0: its sums over the far pairs, [blocks][KK_THREADS][6]
     int4 *bstrace;               // [BS_TRACE_CAP] one record per group integrated in the last map (bs_trace in kernels.cu)
     BsScratch bss;
 };
 
 // indices into DevState::cnt
 enum : int { CI_NCAND = 0, CI_NENC = 1, CI_NGROUPS = 2, CI_NTP = 3, CI_STATUS = 4, CI_NTP_PREV = 5,
-             CI_NBIG = 6, CI_QBIG = 7, CI_NMIDEND = 8, CI_QSMALL = 9, CI_QWARP = 10, CI_QTP = 11, CI_NTRACE = 12, CI_COUNT = 16 };
+             CI_NBIG = 6, CI_QBIG = 7, CI_NMIDEND = 8, CI_QSMALL = 9, CI_QWARP = 10, CI_QTP = 11, CI_NTRACE = 12, CI_S2PMISS = 13, CI_COUNT = 16 };
 constexpr int BS_TRACE_CAP = 4096;   // records of genga_bs_trace kept per map
 
 __device__ __forceinline__ int system_of(const DevState &d, int i) { return d.mode == 2 ? i / d.nm : 0; }
