@@ -67,6 +67,11 @@ def lib():
         "ora_get_stats": (None, [vp, _lp]),
         "ora_system_energy": (d, [vp, _dp]),
         "ora_accel_now": (i, [vp, d, _dp, _dp]),
+        "ora_set_collisions": (None, [vp, vp, i, d, d, i]),
+        "ora_get_events": (l, [vp, vp, l]),
+        "ora_get_bodies": (None, [vp, vp, vp, vp, vp]),
+        "ora_internal_energy": (d, [vp]),
+        "ora_bs_group_collide": (i, [i, d, d, _dp, _dp, _dp, _ip, _dp, _dp, _dp, d, d, _dp, _dp, l, _lp]),
     }
     for name, (res, args) in sig.items():
         f = getattr(L, name)
@@ -81,6 +86,9 @@ ERR = {0: "ok", -1: "invalid argument", -2: "pair list capacity exceeded",
 
 class OracleError(RuntimeError):
     pass
+
+
+EV = 24          # doubles per event record: step, kind, i, j, m_i, m_j, R_i, R_j, q_i[3], V_i[3], q_j[3], V_j[3], U, spin[3]
 
 
 def _chk(rc):
@@ -158,6 +166,18 @@ def bs_group(G, m0, m, rc, q, V, h, eps=1e-12):
                             np.ascontiguousarray(rc, dtype=np.float64), q, V, h, eps,
                             stats.ctypes.data))
     return q, V, stats
+
+
+def bs_group_collide(G, m0, m, rc, R, q, V, h, kind=None, eps=1e-12):
+    """one group integrated over h with collisions; returns q, V, m, R, kind, spin, U, events"""
+    ng = len(m)
+    m = np.array(m, dtype=np.float64); R = np.array(R, dtype=np.float64)
+    q = np.array(q, dtype=np.float64, order="C"); V = np.array(V, dtype=np.float64, order="C")
+    kind = np.zeros(ng, dtype=np.int32) if kind is None else np.array(kind, dtype=np.int32)
+    spin = np.zeros((3, ng)); U = np.zeros(1); ev = np.zeros((64, EV)); nev = np.zeros(1, dtype=np.int64)
+    _chk(lib().ora_bs_group_collide(ng, G, m0, m, np.ascontiguousarray(rc, dtype=np.float64), R, kind, spin, q, V, h, eps,
+                                    U, ev, 64, nev))
+    return q, V, m, R, kind, spin, U[0], ev[: nev[0]]
 
 
 def energy(G, m0, m, q, V, rc=None, n_massive=None):
@@ -253,6 +273,26 @@ class System:
         enc = enc[np.lexsort((enc[:, 1], enc[:, 0]))] if len(enc) else enc
         return cand.copy(), enc.copy(), label
 
+    # ---- collisions, ejections, removal
+    def set_collisions(self, radius, collisions=True, rcut=0.0, rcut_sun=0.0, nmin=0):
+        R = np.ascontiguousarray(radius, dtype=np.float64)
+        lib().ora_set_collisions(self.h, R.ctypes.data, int(collisions), float(rcut), float(rcut_sun), int(nmin))
+
+    def events(self):
+        """event records (EV doubles each, see genga_oracle.c): all events since creation"""
+        n = lib().ora_get_events(self.h, None, 0)
+        buf = np.zeros((max(n, 1), EV))
+        lib().ora_get_events(self.h, buf.ctypes.data, n)
+        return buf[:n]
+
+    def bodies(self):
+        m, R, kind, spin = np.zeros(self.n), np.zeros(self.n), np.zeros(self.n, dtype=np.int32), np.zeros((3, self.n))
+        lib().ora_get_bodies(self.h, m.ctypes.data, R.ctypes.data, kind.ctypes.data, spin.ctypes.data)
+        return m, R, kind, spin
+
+    def internal_energy(self):
+        return lib().ora_internal_energy(self.h)
+
     def stats(self):
         out = np.zeros(6, dtype=np.int64)
         lib().ora_get_stats(self.h, out)
@@ -276,6 +316,29 @@ class Sim:
             nm = w["n_massive"] if w["mode"] != 2 else self.per
             self.sys.append(System(w["m0"][s], w["m"][sl], w["x"][:, sl], w["v"][:, sl],
                                    n_massive=nm, **kw))
+
+    def set_collisions(self, collisions=True, rcut=0.0, rcut_sun=0.0, nmin=0):
+        for k, s in enumerate(self.sys):
+            sl = slice(k * self.per, (k + 1) * self.per)
+            s.set_collisions(self.w["radius"][sl], collisions, rcut, rcut_sun, nmin)
+
+    def events(self):
+        """all events, body indices global, in the order (system, occurrence)"""
+        out = []
+        for k, s in enumerate(self.sys):
+            e = s.events().copy()
+            if len(e):
+                e[:, 2] += k * self.per
+                e[:, 3] = np.where(e[:, 3] >= 0, e[:, 3] + k * self.per, e[:, 3])
+                out.append(e)
+        return np.concatenate(out) if out else np.zeros((0, EV))
+
+    def bodies(self):
+        m, R, kind, spin = zip(*[s.bodies() for s in self.sys])
+        return np.concatenate(m), np.concatenate(R), np.concatenate(kind), np.concatenate(spin, axis=1)
+
+    def internal_energy(self):
+        return np.array([s.internal_energy() for s in self.sys])
 
     def step(self, n_steps, dt=None, order=None):
         dt = self.w["dt"] if dt is None else dt

@@ -391,8 +391,113 @@ static void bs_midpoint(int ng, double G, double m0, const double *m, const doub
  * land exactly on h; ORA_EBS when |H| < 1e-12 |h|.
  * q,V: [3*ng] SoA, overwritten.  stats[0] += BS steps, stats[1] += RHS calls. */
 #define BS_KMAX 8
+
+/* Collisions (L316-328, section 3.2.7).  "To find collisions between the Bulirsch-Stoer time steps, we use the same
+ * code as in the close encounter detection" (L328): after every ACCEPTED Bulirsch-Stoer step of a group the minimum of
+ * the cubic Hermite interpolant of the squared separation (Eq. 10-12) over that step is compared, pair by pair, with
+ * (R_i + R_j)^2.  A colliding pair merges as perfectly inelastic bodies at the END of that step [reading R-19]:
+ *   m = m_i + m_j, q = (m_i q_i + m_j q_j)/m, V = (m_i V_i + m_j V_j)/m   (linear momentum conserved, L316),
+ *   R = (R_i^3 + R_j^3)^(1/3)                                             [R-20: the paper does not say; same density],
+ *   U += 1/2 m_i m_j/(m_i + m_j) v_ij^2 - G m_i m_j / r_ij                (L318-322, at the merge state),
+ *   spin += spin_i + spin_j + m_i m_j/m (q_i - q_j) x (V_i - V_j)          (angular momentum conservation, L324),
+ * the new body keeps the index of the more massive one, the smaller index if the masses are equal (L324); the other
+ * becomes a massless ghost (L324) and is parked on a circular orbit of radius 1000 (index + 1) about the star, where
+ * it meets nothing and adds exact zeros to every sum [R-21: "removed later" -- the caller compacts].  A test particle
+ * that hits a massive body is reported and removed, with no effect on the body (L336); particles do not collide with
+ * each other.  Pairs are visited in the order of the group's member list (a < b); a body removed earlier in the
+ * same step is skipped.  The report holds the two states at the START of that Bulirsch-Stoer step, "the last time
+ * step before the collision happens" (L326).  The integration of the group then goes on from the merged state. */
+#define ORA_EV 24                 /* doubles per event record */
+typedef struct {
+    int enabled;
+    const int *gidx;              /* global index of every member */
+    const int *kind;              /* 0 massive, 1 test particle, 2 removed (updated here) */
+    double *R;                    /* physical radii of the members (updated) */
+    double *mm;                   /* masses of the members (updated; the const m passed to the integrator is this array) */
+    double *spin;                 /* [3 ng] spins of the members (updated) */
+    double *U;                    /* internal energy accumulator */
+    double *ev; int64_t *nev, evcap;   /* event records */
+    double step_id;
+    int *kindw;                   /* writable alias of kind */
+} ora_coll;
+
+double ora_hermite_min(double P0, double P1, double Pd0, double Pd1, double h);
+
+static void coll_scan(int ng, double G, double m0, ora_coll *cc, const double *q0, const double *V0,
+                      double *q1, double *V1, double H)
+{
+    for (int a = 0; a < ng; ++a)
+        for (int b = a + 1; b < ng; ++b) {
+            if (cc->kindw[a] == 2 || cc->kindw[b] == 2) continue;
+            if (cc->kindw[a] == 1 && cc->kindw[b] == 1) continue;            /* particles do not see each other (L336) */
+            double d0[3], w0[3], d1[3], w1[3];
+            for (int c = 0; c < 3; ++c) {
+                d0[c] = q0[c * ng + b] - q0[c * ng + a]; w0[c] = V0[c * ng + b] - V0[c * ng + a];
+                d1[c] = q1[c * ng + b] - q1[c * ng + a]; w1[c] = V1[c * ng + b] - V1[c * ng + a];
+            }
+            double P0 = d0[0] * d0[0] + d0[1] * d0[1] + d0[2] * d0[2], Pd0 = 2.0 * (d0[0] * w0[0] + d0[1] * w0[1] + d0[2] * w0[2]);
+            double P1 = d1[0] * d1[0] + d1[1] * d1[1] + d1[2] * d1[2], Pd1 = 2.0 * (d1[0] * w1[0] + d1[1] * w1[1] + d1[2] * w1[2]);
+            double D = ora_hermite_min(P0, P1, Pd0, Pd1, H);
+            double Rs = cc->R[a] + cc->R[b];
+            if (!(D < Rs * Rs)) continue;
+            /* survivor s, removed d */
+            int sv = a, dd = b, kindev = 0;
+            if (cc->kindw[a] == 1) { sv = b; dd = a; kindev = 1; }
+            else if (cc->kindw[b] == 1) { sv = a; dd = b; kindev = 1; }
+            else if (cc->mm[b] > cc->mm[a]) { sv = b; dd = a; }               /* equal masses: the smaller index (a) */
+            double ma = cc->mm[sv], mb = cc->mm[dd], mt = ma + mb, Uev = 0.0;
+            if (*cc->nev < cc->evcap) {
+                double *e = cc->ev + ORA_EV * (*cc->nev);
+                e[0] = cc->step_id; e[1] = kindev; e[2] = cc->gidx[sv]; e[3] = cc->gidx[dd];
+                e[4] = ma; e[5] = mb; e[6] = cc->R[sv]; e[7] = cc->R[dd];
+                for (int c = 0; c < 3; ++c) {
+                    e[8 + c] = q0[c * ng + sv]; e[11 + c] = V0[c * ng + sv];
+                    e[14 + c] = q0[c * ng + dd]; e[17 + c] = V0[c * ng + dd];
+                }
+            }
+            if (kindev == 0) {
+                double dq[3], dv[3], r2 = 0.0, v2 = 0.0;
+                for (int c = 0; c < 3; ++c) {
+                    dq[c] = q1[c * ng + sv] - q1[c * ng + dd]; dv[c] = V1[c * ng + sv] - V1[c * ng + dd];
+                    r2 += dq[c] * dq[c]; v2 += dv[c] * dv[c];
+                }
+                double mu = ma * mb / mt;
+                Uev = 0.5 * mu * v2 - G * ma * mb / sqrt(r2);
+                *cc->U += Uev;
+                double lx = mu * (dq[1] * dv[2] - dq[2] * dv[1]), ly = mu * (dq[2] * dv[0] - dq[0] * dv[2]), lz = mu * (dq[0] * dv[1] - dq[1] * dv[0]);
+                cc->spin[sv] += cc->spin[dd] + lx; cc->spin[ng + sv] += cc->spin[ng + dd] + ly; cc->spin[2 * ng + sv] += cc->spin[2 * ng + dd] + lz;
+                for (int c = 0; c < 3; ++c) {
+                    q1[c * ng + sv] = (ma * q1[c * ng + sv] + mb * q1[c * ng + dd]) / mt;
+                    V1[c * ng + sv] = (ma * V1[c * ng + sv] + mb * V1[c * ng + dd]) / mt;
+                }
+                cc->R[sv] = cbrt(cc->R[sv] * cc->R[sv] * cc->R[sv] + cc->R[dd] * cc->R[dd] * cc->R[dd]);
+                cc->mm[sv] = mt;
+            }
+            if (*cc->nev < cc->evcap) {
+                double *e = cc->ev + ORA_EV * (*cc->nev);
+                e[20] = Uev; e[21] = cc->spin[sv]; e[22] = cc->spin[ng + sv]; e[23] = cc->spin[2 * ng + sv];
+            }
+            ++*cc->nev;
+            /* the ghost: massless, parked far away on a circular orbit */
+            double Rp = 1000.0 * (double)(cc->gidx[dd] + 1);
+            cc->mm[dd] = 0.0; cc->R[dd] = 0.0; cc->kindw[dd] = 2;
+            cc->spin[dd] = cc->spin[ng + dd] = cc->spin[2 * ng + dd] = 0.0;
+            q1[dd] = Rp; q1[ng + dd] = 0.0; q1[2 * ng + dd] = 0.0;
+            V1[dd] = 0.0; V1[ng + dd] = sqrt(G * m0 / Rp); V1[2 * ng + dd] = 0.0;
+        }
+}
+
+static int bs_group_impl(int ng, double G, double m0, const double *m, const double *rc,
+                         double *q, double *V, double h, double eps, int64_t *stats, ora_coll *cc);
+
 int ora_bs_group(int ng, double G, double m0, const double *m, const double *rc,
                  double *q, double *V, double h, double eps, int64_t *stats)
+{
+    return bs_group_impl(ng, G, m0, m, rc, q, V, h, eps, stats, NULL);
+}
+
+static int bs_group_impl(int ng, double G, double m0, const double *m, const double *rc,
+                         double *q, double *V, double h, double eps, int64_t *stats, ora_coll *cc)
 {
     int N3 = 3 * ng, N6 = 6 * ng;
     if (h == 0.0 || ng == 0) return ORA_OK;
@@ -443,6 +548,7 @@ int ora_bs_group(int ng, double G, double m0, const double *m, const double *rc,
                         if (e2 > err2) err2 = e2;
                     }
                     if (err2 <= eps * eps) {
+                        if (cc && cc->enabled) coll_scan(ng, G, m0, cc, q, V, Tkk, Tkk + N3, H);   /* may merge bodies in Tkk */
                         memcpy(q, Tkk, sizeof(double) * N3);
                         memcpy(V, Tkk + N3, sizeof(double) * N3);
                         done += H;
@@ -460,6 +566,23 @@ int ora_bs_group(int ng, double G, double m0, const double *m, const double *rc,
     }
 out:
     free(T); free(work); free(acc0); free(sq);
+    return rcode;
+}
+
+/* One group with collisions, for the pins: kind[ng] (0 massive, 1 test particle, 2 removed), R[ng], spin[3 ng], m[ng]
+ * are updated; events are appended to ev (ORA_EV doubles each, member numbers as indices). */
+int ora_bs_group_collide(int ng, double G, double m0, double *m, const double *rc, double *R, int32_t *kind, double *spin,
+                         double *q, double *V, double h, double eps, double *U, double *ev, int64_t evcap, int64_t *nev)
+{
+    int *gidx = (int *)malloc(sizeof(int) * (size_t)ng), *k2 = (int *)malloc(sizeof(int) * (size_t)ng);
+    for (int i = 0; i < ng; ++i) { gidx[i] = i; k2[i] = kind[i]; }
+    ora_coll cc;
+    memset(&cc, 0, sizeof cc);
+    cc.enabled = 1; cc.gidx = gidx; cc.kind = k2; cc.kindw = k2; cc.R = R; cc.mm = m; cc.spin = spin;
+    cc.U = U; cc.ev = ev; cc.nev = nev; cc.evcap = evcap; cc.step_id = 0.0;
+    int rcode = bs_group_impl(ng, G, m0, m, rc, q, V, h, eps, NULL, &cc);
+    for (int i = 0; i < ng; ++i) kind[i] = k2[i];
+    free(gidx); free(k2);
     return rcode;
 }
 
@@ -539,6 +662,15 @@ typedef struct {
     int64_t cap, n_cand, n_enc;
     int32_t *cand, *enc, *label;
     int64_t stat_kepler_iters, stat_bs[2], stat_force_evals, stat_groups, stat_maxgroup;
+    /* collisions, ejections, removal (L316-332, L336, L378-384); off unless ora_set_collisions() switches them on */
+    int coll;                 /* 1: collisions are looked for between the Bulirsch-Stoer steps */
+    double rcut, rcut_sun;    /* ejection limits (L330-332); 0 = none */
+    int nmin;                 /* the system is stopped when fewer bodies are left (L378-384); 0 = never */
+    double *R, *spin;         /* [n] physical radii, [3n] spins */
+    int *kind;                /* [n] 0 massive, 1 test particle, 2 removed */
+    double U;                 /* internal energy of the collisions so far (L318-322) */
+    double *ev; int64_t nev, evcap;
+    int64_t step_id;
 } ora_sys;
 
 ora_sys *ora_create(int n, int n_massive, double G, double m0, double n1, double n2,
@@ -554,14 +686,39 @@ ora_sys *ora_create(int n, int n_massive, double G, double m0, double n1, double
     s->a = (double *)calloc(3 * (size_t)n, 8);
     s->cand = (int32_t *)calloc(2 * (size_t)cap, 4); s->enc = (int32_t *)calloc(2 * (size_t)cap, 4);
     s->label = (int32_t *)calloc(n, 4);
+    s->R = (double *)calloc(n, 8); s->spin = (double *)calloc(3 * (size_t)n, 8);
+    s->kind = (int *)calloc(n, sizeof(int));
+    for (int i = n_massive; i < n; ++i) s->kind[i] = 1;
+    s->evcap = 4096; s->ev = (double *)calloc((size_t)s->evcap * ORA_EV, 8);
     return s;
 }
 void ora_destroy(ora_sys *s)
 {
     if (!s) return;
     free(s->m); free(s->rc); free(s->q); free(s->V); free(s->q0); free(s->V0); free(s->a);
-    free(s->cand); free(s->enc); free(s->label); free(s);
+    free(s->cand); free(s->enc); free(s->label); free(s->R); free(s->spin); free(s->kind); free(s->ev); free(s);
 }
+/* radii [n]; coll: look for collisions; rcut, rcut_sun: ejection limits (0 = none); nmin: stop limit (0 = never) */
+void ora_set_collisions(ora_sys *s, const double *R, int coll, double rcut, double rcut_sun, int nmin)
+{
+    if (R) memcpy(s->R, R, 8 * (size_t)s->n);
+    s->coll = coll; s->rcut = rcut; s->rcut_sun = rcut_sun; s->nmin = nmin;
+}
+int64_t ora_get_events(const ora_sys *s, double *buf, int64_t cap)
+{
+    int64_t k = s->nev < s->evcap ? s->nev : s->evcap;
+    if (k > cap) k = cap;
+    if (buf && k > 0) memcpy(buf, s->ev, 8 * (size_t)k * ORA_EV);
+    return s->nev;
+}
+void ora_get_bodies(const ora_sys *s, double *m, double *R, int32_t *kind, double *spin)
+{
+    if (m) memcpy(m, s->m, 8 * (size_t)s->n);
+    if (R) memcpy(R, s->R, 8 * (size_t)s->n);
+    if (kind) for (int i = 0; i < s->n; ++i) kind[i] = s->kind[i];
+    if (spin) memcpy(spin, s->spin, 24 * (size_t)s->n);
+}
+double ora_internal_energy(const ora_sys *s) { return s->U; }
 void ora_set_cull(ora_sys *s, int cull) { s->cull = cull; }
 
 /* x, v heliocentric, SoA [3n] */
@@ -627,6 +784,18 @@ static int do_groups(ora_sys *s, double h)
     int *idx = (int *)malloc(sizeof(int) * (size_t)(nm + 1));
     double *gm = (double *)malloc(8 * (size_t)(nm + 1)), *grc = (double *)malloc(8 * (size_t)(nm + 1));
     double *gq = (double *)malloc(24 * (size_t)(nm + 1)), *gV = (double *)malloc(24 * (size_t)(nm + 1));
+    /* collisions: every group starts from the bodies as they were before this substep's groups were integrated (a particle's
+       group re-integrates the massive bodies it contains, merges included, and must see them unmerged) */
+    double *gR = (double *)malloc(8 * (size_t)(nm + 1)), *gspin = (double *)malloc(24 * (size_t)(nm + 1));
+    int *gkind = (int *)malloc(sizeof(int) * (size_t)(nm + 1));
+    double *m_pre = (double *)malloc(8 * (size_t)n), *R_pre = (double *)malloc(8 * (size_t)n), *spin_pre = (double *)malloc(24 * (size_t)n);
+    int *kind_pre = (int *)malloc(sizeof(int) * (size_t)n);
+    memcpy(m_pre, s->m, 8 * (size_t)n); memcpy(R_pre, s->R, 8 * (size_t)n); memcpy(spin_pre, s->spin, 24 * (size_t)n);
+    memcpy(kind_pre, s->kind, sizeof(int) * (size_t)n);
+    ora_coll cc;
+    memset(&cc, 0, sizeof cc);
+    cc.enabled = s->coll; cc.gidx = idx; cc.kind = gkind; cc.kindw = gkind; cc.R = gR; cc.mm = gm; cc.spin = gspin;
+    cc.U = &s->U; cc.ev = s->ev; cc.nev = &s->nev; cc.evcap = s->evcap; cc.step_id = (double)s->step_id;
     /* results of massive groups are collected first and written after the
        particle groups have read the pre-drift state (they only use q0,V0). */
     for (int root = 0; root < nm && rcode == ORA_OK; ++root) {
@@ -635,12 +804,20 @@ static int do_groups(ora_sys *s, double h)
         for (int i = root; i < nm; ++i) if (s->label[i] == root) idx[ng++] = i;
         if (ng < 2) continue;
         for (int k = 0; k < ng; ++k) {
-            gm[k] = s->m[idx[k]]; grc[k] = s->rc[idx[k]];
-            for (int c = 0; c < 3; ++c) { gq[c * ng + k] = s->q0[c * n + idx[k]]; gV[c * ng + k] = s->V0[c * n + idx[k]]; }
+            gm[k] = m_pre[idx[k]]; grc[k] = s->rc[idx[k]]; gR[k] = R_pre[idx[k]]; gkind[k] = kind_pre[idx[k]];
+            for (int c = 0; c < 3; ++c) {
+                gq[c * ng + k] = s->q0[c * n + idx[k]]; gV[c * ng + k] = s->V0[c * n + idx[k]];
+                gspin[c * ng + k] = spin_pre[c * n + idx[k]];
+            }
         }
-        rcode = ora_bs_group(ng, s->G, s->m0, gm, grc, gq, gV, h, s->bs_eps, s->stat_bs);
-        for (int k = 0; k < ng; ++k)
-            for (int c = 0; c < 3; ++c) { s->q[c * n + idx[k]] = gq[c * ng + k]; s->V[c * n + idx[k]] = gV[c * ng + k]; }
+        rcode = bs_group_impl(ng, s->G, s->m0, gm, grc, gq, gV, h, s->bs_eps, s->stat_bs, &cc);
+        for (int k = 0; k < ng; ++k) {
+            for (int c = 0; c < 3; ++c) {
+                s->q[c * n + idx[k]] = gq[c * ng + k]; s->V[c * n + idx[k]] = gV[c * ng + k];
+                s->spin[c * n + idx[k]] = gspin[c * ng + k];
+            }
+            s->m[idx[k]] = gm[k]; s->R[idx[k]] = gR[k]; s->kind[idx[k]] = gkind[k];
+        }
         s->stat_groups++;
         if (ng > s->stat_maxgroup) s->stat_maxgroup = ng;
     }
@@ -665,18 +842,73 @@ static int do_groups(ora_sys *s, double h)
             for (int i = 0; i < nm; ++i) if (in[i]) idx[ng++] = i;
             idx[ng++] = p;
             for (int k = 0; k < ng; ++k) {
-                gm[k] = s->m[idx[k]]; grc[k] = s->rc[idx[k]];
-                for (int c = 0; c < 3; ++c) { gq[c * ng + k] = s->q0[c * n + idx[k]]; gV[c * ng + k] = s->V0[c * n + idx[k]]; }
+                gm[k] = m_pre[idx[k]]; grc[k] = s->rc[idx[k]]; gR[k] = R_pre[idx[k]]; gkind[k] = kind_pre[idx[k]];
+                for (int c = 0; c < 3; ++c) {
+                    gq[c * ng + k] = s->q0[c * n + idx[k]]; gV[c * ng + k] = s->V0[c * n + idx[k]];
+                    gspin[c * ng + k] = spin_pre[c * n + idx[k]];
+                }
             }
-            rcode = ora_bs_group(ng, s->G, s->m0, gm, grc, gq, gV, h, s->bs_eps, s->stat_bs);
+            /* the massive bodies' own collisions were reported (and their energy counted) by their massive group: here
+               they are only re-enacted; the particle's collision is new */
+            double U_dummy = 0.0;
+            int64_t nev0 = s->nev;
+            cc.U = &U_dummy;
+            rcode = bs_group_impl(ng, s->G, s->m0, gm, grc, gq, gV, h, s->bs_eps, s->stat_bs, &cc);
+            cc.U = &s->U;
+            {   /* keep only the particle's events of this group */
+                int64_t w = nev0;
+                for (int64_t e = nev0; e < s->nev && e < s->evcap; ++e)
+                    if (s->ev[ORA_EV * e + 1] == 1.0) { if (w != e) memcpy(s->ev + ORA_EV * w, s->ev + ORA_EV * e, 8 * ORA_EV); ++w; }
+                s->nev = w;
+            }
             for (int c = 0; c < 3; ++c) { s->q[c * n + p] = gq[c * ng + ng - 1]; s->V[c * n + p] = gV[c * ng + ng - 1]; }
+            s->R[p] = gR[ng - 1]; s->kind[p] = gkind[ng - 1];
             s->stat_groups++;
             if (ng > s->stat_maxgroup) s->stat_maxgroup = ng;
         }
         free(in); free(head); free(next);
     }
     free(idx); free(gm); free(grc); free(gq); free(gV);
+    free(gR); free(gspin); free(gkind); free(m_pre); free(R_pre); free(spin_pre); free(kind_pre);
     return rcode;
+}
+
+/* End of a time step: ejections (L330-332) -- a body farther from the central mass than Rcut, or closer than RcutSun,
+ * is reported and removed -- and the stop of the system (L378-384): when fewer than Nmin bodies are left, all of them
+ * are removed.  Removed bodies are parked as the ghosts of the collisions are.  Event kinds: 2 = beyond Rcut,
+ * 3 = inside RcutSun, 4 = removed because the system stopped. */
+static void remove_body(ora_sys *s, int i, int kind_ev)
+{
+    int n = s->n;
+    if (s->nev < s->evcap) {
+        double *e = s->ev + ORA_EV * s->nev;
+        memset(e, 0, 8 * ORA_EV);
+        e[0] = (double)s->step_id; e[1] = kind_ev; e[2] = i; e[3] = -1; e[4] = s->m[i]; e[6] = s->R[i];
+        for (int c = 0; c < 3; ++c) { e[8 + c] = s->q[c * n + i]; e[11 + c] = s->V[c * n + i]; e[21 + c] = s->spin[c * n + i]; }
+    }
+    s->nev++;
+    double Rp = 1000.0 * (double)(i + 1);
+    s->m[i] = 0.0; s->R[i] = 0.0; s->kind[i] = 2;
+    s->spin[i] = s->spin[n + i] = s->spin[2 * n + i] = 0.0;
+    s->q[i] = Rp; s->q[n + i] = 0.0; s->q[2 * n + i] = 0.0;
+    s->V[i] = 0.0; s->V[n + i] = sqrt(s->G * s->m0 / Rp); s->V[2 * n + i] = 0.0;
+}
+static void end_of_step(ora_sys *s)
+{
+    int n = s->n;
+    if (s->rcut > 0.0 || s->rcut_sun > 0.0)
+        for (int i = 0; i < n; ++i) {
+            if (s->kind[i] == 2) continue;
+            double r2 = s->q[i] * s->q[i] + s->q[n + i] * s->q[n + i] + s->q[2 * n + i] * s->q[2 * n + i];
+            if (s->rcut > 0.0 && r2 > s->rcut * s->rcut) remove_body(s, i, 2);
+            else if (s->rcut_sun > 0.0 && r2 < s->rcut_sun * s->rcut_sun) remove_body(s, i, 3);
+        }
+    if (s->nmin > 0) {
+        int left = 0;
+        for (int i = 0; i < s->n_massive; ++i) left += s->kind[i] != 2;
+        if (left < s->nmin && left > 0)
+            for (int i = 0; i < n; ++i) if (s->kind[i] != 2) remove_body(s, i, 4);
+    }
 }
 
 /* Second-order map S2(h), Eq. 7 (L100), in the order of the bullet list
@@ -729,6 +961,8 @@ int ora_step(ora_sys *s, int64_t n_steps, double dt, int order)
             int rcode = ora_map_s2(s, w[k] * dt);
             if (rcode) return rcode;
         }
+        end_of_step(s);
+        s->step_id++;
     }
     return ORA_OK;
 }
