@@ -84,7 +84,7 @@ int genga_destroy(genga_ctx *ctx);
 
 /* Load the state (problem statement: L69, L188, L316-324, L352).
  *   m0[n_systems]  central masses; m[Ntot] masses (0 for test particles); radius[Ntot]
- *   physical radii (stored; collisions are not on this path); x[3*Ntot], v[3*Ntot]
+ *   physical radii (used once genga_set_collisions switches collisions on); x[3*Ntot], v[3*Ntot]
  *   heliocentric positions / velocities.
  * genga_set_state: all pointers DEVICE.  genga_set_state_host: all pointers HOST (pinned
  * or pageable); the copies are enqueued on the stream and the call returns after they and
@@ -150,6 +150,34 @@ int genga_energy(genga_ctx *ctx, double *E, double *L);
  * HOST pointers; synchronises. */
 int genga_encounters(genga_ctx *ctx, int32_t *pairs, int64_t cap, int64_t *n_pairs,
                      int64_t *n_candidates, int32_t *group_label);
+
+/* Collisions, ejections and removal of bodies (L316-332 sections 3.2.7-3.2.8, L336, L378-384; SURVEY 8(f) NEXT-1..3).
+ * Off after genga_create: bodies are point masses.  genga_set_collisions switches on
+ *   collisions != 0: between the Bulirsch-Stoer steps of every group the minimum of the cubic Hermite interpolant of the
+ *     squared separation over the step (Eq. 10-12; "the same code as in the close encounter detection", L328) is compared
+ *     with (R_i + R_j)^2.  A colliding pair merges as perfectly inelastic bodies at the end of that step: mass and linear
+ *     momentum conserved, position = centre of mass, radius (R_i^3 + R_j^3)^(1/3), internal energy U += 1/2 m_i m_j /
+ *     (m_i + m_j) v_ij^2 - G m_i m_j / r_ij (L318-322), spin from angular momentum conservation, the new body keeps the
+ *     index of the more massive one (the smaller index if equal); the other becomes a massless ghost parked on a
+ *     circular orbit of radius 1000 (k + 1) (k = its index within its system), where it meets nothing and adds exact
+ *     zeros to every sum -- "removed later" (L324): the caller compacts by reloading the state without the removed
+ *     bodies.  A test particle that hits a massive body is reported and removed, with no effect on the body (L336).
+ *   rcut, rcut_sun > 0: at the end of a time step a body farther from the central mass than rcut, or closer than
+ *     rcut_sun, is reported and removed (L330-332).
+ *   n_min > 0: a system with fewer than n_min massive bodies left is stopped: all its bodies are removed (L378-384).
+ * Synchronises; drops the cached CUDA graphs.
+ * genga_events: the records since the last genga_set_state*, at most 4096 are kept; *n = number made.  A record is 24
+ * doubles: [0] steps completed before the event's step, [1] kind (0 collision, 1 test particle hit a massive body,
+ * 2 beyond rcut, 3 inside rcut_sun, 4 removed because its system stopped), [2] surviving body (or the body removed by
+ * kinds 2-4), [3] removed body (-1 for kinds 2-4), [4..5] masses, [6..7] radii, [8..10], [11..13] heliocentric position
+ * and BARYCENTRIC velocity of body [2] at the start of the Bulirsch-Stoer step in which the collision happened ("the
+ * last time step before the collision", L326; kinds 2-4: at the end of the step), [14..19] the same of body [3],
+ * [20] the internal energy of this collision, [21..23] spin of the new body.  Order of the records: not defined.
+ * genga_bodies: current m[Ntot], radius[Ntot], kind[Ntot] (0 massive, 1 test particle, 2 removed), spin[3*Ntot],
+ * U[n_systems]; any pointer may be NULL.  HOST pointers; both synchronise. */
+int genga_set_collisions(genga_ctx *ctx, int collisions, double rcut, double rcut_sun, int n_min);
+int genga_events(genga_ctx *ctx, double *records, int64_t cap, int64_t *n);
+int genga_bodies(genga_ctx *ctx, double *m, double *radius, int32_t *kind, double *spin, double *U);
 
 /* One record per encounter group that Bulirsch-Stoer integrated in the LAST drift substep executed (L116, L286-314;
  * at most 4096 are kept): out[4*k + 0] = group size | layout << 16 (layout 0: one warp, 1: cluster),

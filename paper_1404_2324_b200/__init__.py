@@ -22,7 +22,7 @@ OK, EINVAL, ECAPACITY, EKEPLER, EBS, ECUDA = 0, -1, -2, -3, -4, -5
 SYMBOLS = [
     "genga_workspace_bytes", "genga_create", "genga_destroy", "genga_set_state", "genga_set_state_host",
     "genga_step", "genga_get_state", "genga_get_state_host", "genga_set_state_ragged_host", "genga_get_state_ragged_host", "genga_set_system_params_host",
-    "genga_energy", "genga_encounters", "genga_bs_trace",
+    "genga_energy", "genga_encounters", "genga_bs_trace", "genga_set_collisions", "genga_events", "genga_bodies",
     "genga_status", "genga_accelerations", "genga_kepler_drift", "genga_counters", "genga_time_kernel", "genga_profile_step",
     "genga_eval_fast", "genga_fp64_probe", "genga_strerror",
     "genga_last_cuda_error",
@@ -75,6 +75,9 @@ def load():
         "genga_energy": (i, [vp, dp, dp]),
         "genga_encounters": (i, [vp, vp, l, C.POINTER(l), C.POINTER(l), vp]),
         "genga_bs_trace": (i, [vp, vp, l, C.POINTER(l)]),
+        "genga_set_collisions": (i, [vp, i, d, d, i]),
+        "genga_events": (i, [vp, vp, l, C.POINTER(l)]),
+        "genga_bodies": (i, [vp, vp, vp, vp, vp, vp]),
         "genga_status": (i, [vp]),
         "genga_accelerations": (i, [vp, d, dp, dp]),
         "genga_kepler_drift": (i, [vp, l, d, d, dp, dp]),
@@ -229,6 +232,24 @@ class Genga:
         _chk(self.lib.genga_encounters(self.h, _hp(pairs), self.max_pairs, C.byref(npairs), C.byref(ncand),
                                        _hp(labels) if with_labels else None), "genga_encounters")
         return pairs[: npairs.value].copy(), int(ncand.value), labels
+
+    def set_collisions(self, collisions=True, rcut=0.0, rcut_sun=0.0, n_min=0):
+        _chk(self.lib.genga_set_collisions(self.h, int(collisions), float(rcut), float(rcut_sun), int(n_min)), "genga_set_collisions")
+
+    def events(self):
+        """event records (n, 24), see include/genga.h"""
+        buf = np.zeros((4096, 24))
+        n = C.c_int64()
+        _chk(self.lib.genga_events(self.h, _hp(buf), 4096, C.byref(n)), "genga_events")
+        return buf[: min(n.value, 4096)].copy()
+
+    def bodies(self):
+        """(m, radius, kind, spin, U) as they are now"""
+        ns = self.ns if self.mode == MODE_MULTI_SYSTEM else 1
+        m, R, kind = np.zeros(self.ntot), np.zeros(self.ntot), np.zeros(self.ntot, dtype=np.int32)
+        spin, U = np.zeros((3, self.ntot)), np.zeros(ns)
+        _chk(self.lib.genga_bodies(self.h, _hp(m), _hp(R), _hp(kind), _hp(spin), _hp(U)), "genga_bodies")
+        return m, R, kind, spin, U
 
     def bs_trace(self):
         """records (n, layout, accepted, rejected, cycles, member) of the groups integrated in the last substep"""

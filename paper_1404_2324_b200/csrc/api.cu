@@ -80,6 +80,7 @@ static void mark(genga_ctx *c, int phase)
 }
 
 static inline size_t up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+static const long long GENGA_EVENT_CAP = 4096;    // event records kept until genga_events reads them
 
 static bool valid_cfg(const genga_config *c)
 {
@@ -139,6 +140,19 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
         t.tpmask = (unsigned *)take(sizeof(unsigned) * nt);
         t.tplist = (int *)take(sizeof(int) * nt);
     }
+    // collisions, ejections, removal (genga_set_collisions)
+    t.kind = (int *)take(sizeof(int) * np);
+    t.spin = (double *)take(sizeof(double) * 3 * np);
+    t.U = (double *)take(sizeof(double) * nsys);
+    t.evcap = GENGA_EVENT_CAP;
+    t.ev = (double *)take(sizeof(double) * GENGA_EV * (size_t)t.evcap);
+    t.redo = (int2 *)take(sizeof(int2) * (size_t)c->max_pairs);
+    if (c->mode != GENGA_MODE_MULTI_SYSTEM) {
+        t.genA.stride = npm;
+        t.genA.base = (double *)take(sizeof(double) * (size_t)BSA_COUNT2 * npm);
+    }
+    t.genB.stride = 64 * GEN_BLOCKS;
+    t.genB.base = (double *)take(sizeof(double) * (size_t)BSA_COUNT2 * t.genB.stride);
     t.cand = (int2 *)take(sizeof(int2) * (size_t)c->max_pairs);
     t.enc = (int2 *)take(sizeof(int2) * (size_t)c->max_pairs);
     t.cnt = (int *)take(sizeof(int) * CI_COUNT);
@@ -273,6 +287,8 @@ static void enqueue_helio_to_demo(genga_ctx *c)
 {
     DevState &d = c->d;
     c->far_valid = false;                                     // new positions: the stored hit masks are void
+    k_init_bodies<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d);   // kinds, spins, internal energy, event list: a new run
+    c->launches += 1;
     k_coord_map<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx0, d.vy0, d.vz0, d.vx, d.vy, d.vz, -1.0, 1);
     c->launches += 1;
 }
@@ -470,6 +486,10 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
             if (d.nm + 1 > 32) { k_tp_bs_big<<<TPBIG_BLOCKS, 64, 0, st>>>(d, h); LAUNCH(c); }
         }
     }
+    if (d.coll) {                                             // groups in which a pair collides: integrated again, with the merge
+        k_bs_generic<<<GEN_BLOCKS, 256, 0, st>>>(d, h, 0); LAUNCH(c);
+        k_bs_generic<<<GEN_BLOCKS, 256, 0, st>>>(d, h, 1); LAUNCH(c);
+    }
     mark(c, PH_BACK);
     if (tp) {
         launch_k(false, k_tpm_kick, 1, 32, 0, st, d, 0.5 * h, 0, 0.5 * h); LAUNCH(c);       // momentum sum, Sun kick, kick of the massive bodies; plain: see enqueue_sun
@@ -517,6 +537,10 @@ static void enqueue_step(genga_ctx *c, double dt, int order, bool reuse)
     const bool merge = !(c->cfg.flags & 1) && d.mode != GENGA_MODE_TEST_PARTICLE;
     for (int k = 0; k < nw; ++k)
         enqueue_map(c, w[k] * dt, dt, k == 0, k == nw - 1, merge && k + 1 < nw ? w[k + 1] * dt : 0.0, merge && k > 0, reuse && k == 0);
+    if (d.coll || d.rcut2 > 0.0 || d.rcutsun2 > 0.0 || d.nmin > 0) {      // ejections, stop of a system, step counter of the events
+        k_end_step<<<nblk(d.mode == GENGA_MODE_MULTI_SYSTEM ? d.nsys : d.ntot, 128), 128, 0, c->st>>>(d); LAUNCH(c);
+        k_end_step2<<<1, 256, 0, c->st>>>(d); LAUNCH(c);
+    }
     mark(c, PH_TOTAL);
 }
 
@@ -728,6 +752,13 @@ extern "C" __attribute__((visibility("default"))) int genga_set_state_ragged_hos
     }
     int r = genga_set_state_host(c, m0, pm.data(), pr.data(), px.data(), pv.data());
     if (r) return r;
+    {   // the padding slots are no bodies: "removed" from the start (no ejection report, not counted against Nmin)
+        std::vector<int> kd(nt, 0);
+        for (int s = 0; s < d.nsys; ++s)
+            for (size_t k = (size_t)n_bodies[s]; k < nm; ++k) kd[(size_t)s * nm + k] = 2;
+        CK(cudaMemcpyAsync(d.kind, kd.data(), sizeof(int) * nt, cudaMemcpyHostToDevice, c->st));
+        CK(cudaStreamSynchronize(c->st));
+    }
     CK(cudaStreamSynchronize(c->st));                         // the padded arrays die with this call
     c->n_bodies.assign(n_bodies, n_bodies + d.nsys);
     return GENGA_OK;
@@ -790,6 +821,45 @@ extern "C" __attribute__((visibility("default"))) int genga_encounters(genga_ctx
     if (n_pairs) *n_pairs = cnt[CI_NENC];
     if (n_candidates) *n_candidates = cnt[CI_NCAND];
     return r;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_set_collisions(genga_ctx *c, int collisions, double rcut, double rcut_sun, int n_min)
+{
+    if (!c || !(rcut >= 0.0) || !(rcut_sun >= 0.0) || n_min < 0 || n_min > c->d.nm) return GENGA_EINVAL;
+    CK(cudaStreamSynchronize(c->st));
+    c->d.coll = collisions ? 1 : 0; c->d.rcut2 = rcut * rcut; c->d.rcutsun2 = rcut_sun * rcut_sun; c->d.nmin = n_min;
+    for (auto &kv : c->graphs) cudaGraphExecDestroy(kv.second.exec);      // the kernel sequence of a step changes
+    c->graphs.clear();
+    return GENGA_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_events(genga_ctx *c, double *buf, int64_t cap, int64_t *n)
+{
+    if (!c || !n || cap < 0 || (cap > 0 && !buf)) return GENGA_EINVAL;
+    long long st[CNT_N];
+    CK(cudaMemcpyAsync(st, c->d.stat, sizeof st, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    *n = st[CNT_NEV];
+    const int64_t m = std::min<int64_t>(std::min<int64_t>(st[CNT_NEV], c->d.evcap), cap);
+    if (m > 0) {
+        CK(cudaMemcpyAsync(buf, c->d.ev, sizeof(double) * GENGA_EV * (size_t)m, cudaMemcpyDeviceToHost, c->st));
+        CK(cudaStreamSynchronize(c->st));
+    }
+    return GENGA_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) int genga_bodies(genga_ctx *c, double *m, double *radius, int32_t *kind, double *spin, double *U)
+{
+    if (!c) return GENGA_EINVAL;
+    const DevState &d = c->d;
+    const size_t n = (size_t)d.ntot;
+    if (m) CK(cudaMemcpyAsync(m, d.m, sizeof(double) * n, cudaMemcpyDeviceToHost, c->st));
+    if (radius) CK(cudaMemcpyAsync(radius, d.radius, sizeof(double) * n, cudaMemcpyDeviceToHost, c->st));
+    if (kind) CK(cudaMemcpyAsync(kind, d.kind, sizeof(int) * n, cudaMemcpyDeviceToHost, c->st));
+    if (spin) for (int k = 0; k < 3; ++k) CK(cudaMemcpyAsync(spin + k * n, d.spin + (size_t)k * d.np, sizeof(double) * n, cudaMemcpyDeviceToHost, c->st));
+    if (U) CK(cudaMemcpyAsync(U, d.U, sizeof(double) * (size_t)d.nsys, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    return GENGA_OK;
 }
 
 extern "C" __attribute__((visibility("default"))) int genga_bs_trace(genga_ctx *c, int32_t *out, int64_t cap, int64_t *n)

@@ -194,7 +194,133 @@ struct BsScratch {
 };
 enum : int { BSA_Y = 0, BSA_QA = 6, BSA_VA = 9, BSA_QB = 12, BSA_VB = 15, BSA_ACC0 = 18,
              BSA_ACC = 21, BSA_ISQ = 24, BSA_ISV = 25, BSA_M = 26, BSA_RC = 27, BSA_ROW = 28,
-             BSA_COUNT = 28 + 6 * BS_KMAX };
+             BSA_COUNT = 28 + 6 * BS_KMAX,
+             // the layout with collisions (k_bs_generic) carries radius, kind (0 massive, 1 test particle, 2 removed), spin
+             // and the member's index within its system as well
+             BSA_R = BSA_COUNT, BSA_KIND = BSA_COUNT + 1, BSA_SPIN = BSA_COUNT + 2, BSA_GIDX = BSA_COUNT + 5,
+             BSA_COUNT2 = BSA_COUNT + 6 };
+
+// ---------------------------------------------------------------------------------
+// Collisions (section 3.2.7; readings R-19..R-21).  "To find collisions between the
+// Bulirsch-Stoer time steps, we use the same code as in the close encounter detection" (L328): after every accepted
+// Bulirsch-Stoer step the minimum of the cubic Hermite interpolant of the squared separation over that step (Eq. 10-12)
+// is compared, pair by pair, with (R_i + R_j)^2.
+constexpr int GENGA_EV = 24;        // doubles per event record (include/genga.h)
+
+// a cheap lower bound of the Hermite interpolant first: P(t) = h00 P0 + h01 P1 + h10 h Pd0 + h11 h Pd1 with
+// h00 + h01 = 1 and |h10|, |h11| <= 4/27 on [0, 1]
+__device__ __forceinline__ bool pair_collides(double P0, double P1, double Pd0, double Pd1, double H, double Rs)
+{
+    const double Rs2 = Rs * Rs;
+    if (fmin(P0, P1) - (4.0 / 27.0) * (fabs(H * Pd0) + fabs(H * Pd1)) > Rs2) return false;
+    return hermite_min(P0, P1, Pd0, Pd1, H) < Rs2;
+}
+
+struct BsColl {
+    double *ev;                     // event records, GENGA_EV doubles each
+    long long evcap;
+    unsigned long long *nev;        // events so far (device counter)
+    double *U;                      // internal energy of this system (L318-322)
+    double step_id;
+    int base;                       // global index of the system's first body
+    int record_massive;             // 0: a test particle's group re-enacts the massive bodies' collisions silently (L342)
+};
+
+// The merges of one accepted step, in the order of the member list (a < b), a body removed earlier in the step
+// skipped: ONE thread, exactly the oracle's loop.  Old state in BSA_Y, new state in BSA_ROW + 6 k.
+__device__ inline void bs_collisions_seq(const BsScratch &S, int off, int nb, int k, double H, double G, double m0, const BsColl &cc)
+{
+    double *m = S.arr(BSA_M) + off, *R = S.arr(BSA_R) + off, *kind = S.arr(BSA_KIND) + off, *gidx = S.arr(BSA_GIDX) + off;
+    double *q0[3], *V0[3], *q1[3], *V1[3], *sp[3];
+    for (int c = 0; c < 3; ++c) {
+        q0[c] = S.arr(BSA_Y + c) + off; V0[c] = S.arr(BSA_Y + 3 + c) + off;
+        q1[c] = S.arr(BSA_ROW + 6 * k + c) + off; V1[c] = S.arr(BSA_ROW + 6 * k + 3 + c) + off;
+        sp[c] = S.arr(BSA_SPIN + c) + off;
+    }
+    for (int a = 0; a < nb; ++a)
+        for (int b = a + 1; b < nb; ++b) {
+            if (kind[a] == 2.0 || kind[b] == 2.0) continue;
+            if (kind[a] == 1.0 && kind[b] == 1.0) continue;
+            double d0[3], w0[3], d1[3], w1[3];
+            for (int c = 0; c < 3; ++c) {
+                d0[c] = q0[c][b] - q0[c][a]; w0[c] = V0[c][b] - V0[c][a];
+                d1[c] = q1[c][b] - q1[c][a]; w1[c] = V1[c][b] - V1[c][a];
+            }
+            const double P0 = d0[0] * d0[0] + d0[1] * d0[1] + d0[2] * d0[2], Pd0 = 2.0 * (d0[0] * w0[0] + d0[1] * w0[1] + d0[2] * w0[2]);
+            const double P1 = d1[0] * d1[0] + d1[1] * d1[1] + d1[2] * d1[2], Pd1 = 2.0 * (d1[0] * w1[0] + d1[1] * w1[1] + d1[2] * w1[2]);
+            if (!pair_collides(P0, P1, Pd0, Pd1, H, R[a] + R[b])) continue;
+            int sv = a, dd = b, kev = 0;
+            if (kind[a] == 1.0) { sv = b; dd = a; kev = 1; }
+            else if (kind[b] == 1.0) { sv = a; dd = b; kev = 1; }
+            else if (m[b] > m[a]) { sv = b; dd = a; }
+            const double ma = m[sv], mb = m[dd], mt = ma + mb;
+            const bool rec = kev == 1 || cc.record_massive;
+            double *e = nullptr;
+            if (rec) {
+                const unsigned long long slot = atomicAdd(cc.nev, 1ull);
+                if ((long long)slot < cc.evcap) {
+                    e = cc.ev + GENGA_EV * slot;
+                    e[0] = cc.step_id; e[1] = kev; e[2] = cc.base + gidx[sv]; e[3] = cc.base + gidx[dd];
+                    e[4] = ma; e[5] = mb; e[6] = R[sv]; e[7] = R[dd];
+                    for (int c = 0; c < 3; ++c) { e[8 + c] = q0[c][sv]; e[11 + c] = V0[c][sv]; e[14 + c] = q0[c][dd]; e[17 + c] = V0[c][dd]; }
+                }
+            }
+            double Uev = 0.0;
+            if (kev == 0) {
+                double dq[3], dv[3], r2 = 0.0, v2 = 0.0;
+                for (int c = 0; c < 3; ++c) {
+                    dq[c] = q1[c][sv] - q1[c][dd]; dv[c] = V1[c][sv] - V1[c][dd];
+                    r2 += dq[c] * dq[c]; v2 += dv[c] * dv[c];
+                }
+                const double mu = ma * mb / mt;
+                Uev = 0.5 * mu * v2 - G * ma * mb / sqrt(r2);
+                if (cc.record_massive) atomicAdd(cc.U, Uev);
+                sp[0][sv] += sp[0][dd] + mu * (dq[1] * dv[2] - dq[2] * dv[1]);
+                sp[1][sv] += sp[1][dd] + mu * (dq[2] * dv[0] - dq[0] * dv[2]);
+                sp[2][sv] += sp[2][dd] + mu * (dq[0] * dv[1] - dq[1] * dv[0]);
+                for (int c = 0; c < 3; ++c) {
+                    q1[c][sv] = (ma * q1[c][sv] + mb * q1[c][dd]) / mt;
+                    V1[c][sv] = (ma * V1[c][sv] + mb * V1[c][dd]) / mt;
+                }
+                R[sv] = cbrt(R[sv] * R[sv] * R[sv] + R[dd] * R[dd] * R[dd]);
+                m[sv] = mt;
+            }
+            if (e) { e[20] = Uev; e[21] = sp[0][sv]; e[22] = sp[1][sv]; e[23] = sp[2][sv]; }
+            // the ghost: massless, parked far away on a circular orbit (it meets nothing and adds exact zeros to every sum)
+            const double Rp = 1000.0 * (gidx[dd] + 1.0);
+            m[dd] = 0.0; R[dd] = 0.0; kind[dd] = 2.0;
+            sp[0][dd] = sp[1][dd] = sp[2][dd] = 0.0;
+            q1[0][dd] = Rp; q1[1][dd] = 0.0; q1[2][dd] = 0.0;
+            V1[0][dd] = 0.0; V1[1][dd] = sqrt(G * m0 / Rp); V1[2][dd] = 0.0;
+        }
+}
+
+// Does any pair of the group collide in the step just accepted (old state BSA_Y, new state BSA_ROW + 6 k)?  All
+// threads of the block; the same answer in every thread.
+__device__ inline bool bs_any_collision(const BsScratch &S, int off, int nb, int k, double H)
+{
+    const double *R = S.arr(BSA_R) + off, *kind = S.arr(BSA_KIND) + off;
+    int hit = 0;
+    for (int a = threadIdx.x; a < nb && !hit; a += blockDim.x) {
+        if (kind[a] == 2.0) continue;
+        double qa0[3], va0[3], qa1[3], va1[3];
+        for (int c = 0; c < 3; ++c) {
+            qa0[c] = S.arr(BSA_Y + c)[off + a]; va0[c] = S.arr(BSA_Y + 3 + c)[off + a];
+            qa1[c] = S.arr(BSA_ROW + 6 * k + c)[off + a]; va1[c] = S.arr(BSA_ROW + 6 * k + 3 + c)[off + a];
+        }
+        for (int b = a + 1; b < nb; ++b) {
+            if (kind[b] == 2.0 || (kind[a] == 1.0 && kind[b] == 1.0)) continue;
+            double P0 = 0.0, Pd0 = 0.0, P1 = 0.0, Pd1 = 0.0;
+            for (int c = 0; c < 3; ++c) {
+                const double d0 = S.arr(BSA_Y + c)[off + b] - qa0[c], w0 = S.arr(BSA_Y + 3 + c)[off + b] - va0[c];
+                const double d1 = S.arr(BSA_ROW + 6 * k + c)[off + b] - qa1[c], w1 = S.arr(BSA_ROW + 6 * k + 3 + c)[off + b] - va1[c];
+                P0 += d0 * d0; Pd0 += 2.0 * d0 * w0; P1 += d1 * d1; Pd1 += 2.0 * d1 * w1;
+            }
+            if (pair_collides(P0, P1, Pd0, Pd1, H, R[a] + R[b])) { hit = 1; break; }
+        }
+    }
+    return __syncthreads_or(hit) != 0;
+}
 
 __device__ inline void bsb_rhs(const BsScratch &S, int off, int nb, double G, double m0, int posarr, int accarr)
 {
@@ -239,7 +365,7 @@ __device__ inline double block_max(double v, double *red)
 
 // state Y (arrays BSA_Y..+5), m, rc must be loaded at [off, off+nb) before the call.
 __device__ inline bool bs_block(const BsScratch &S, int off, int nb, double G, double m0, double h,
-                                double eps, double *red, int *nsteps)
+                                double eps, double *red, int *nsteps, const BsColl *cc = nullptr)
 {
     double done = 0.0, H = h;
     bool last = false;
@@ -311,6 +437,13 @@ __device__ inline bool bs_block(const BsScratch &S, int off, int nb, double G, d
                 if (k >= 1) {
                     e = block_max(e, red);
                     if (e <= eps2) {
+                        if (cc) {                    // collisions between the Bulirsch-Stoer steps (L328): may merge bodies in row k
+                            __syncthreads();
+                            if (bs_any_collision(S, off, nb, k, H)) {
+                                if (threadIdx.x == 0) bs_collisions_seq(S, off, nb, k, H, G, m0, *cc);
+                                __syncthreads();
+                            }
+                        }
                         for (int b = threadIdx.x; b < nb; b += blockDim.x)
                             for (int c = 0; c < 6; ++c) S.arr(BSA_Y + c)[off + b] = S.arr(BSA_ROW + 6 * k + c)[off + b];
                         done += H;

@@ -39,6 +39,7 @@ struct BcSmem {
     double isq[MAXN], isv[MAXN];    // checker: 1 / |q|^2, 1 / |V|^2 of the round's starting state (error norm)
     float thr2[MAXN];               // (rc_i + margin)^2 rounded up
     double m[MAXN], rc[MAXN], irc[MAXN];
+    double R[MAXN];                 // physical radii (collision test; < 0: none)
     double Y[6][MAXN];              // state the current round starts from (pushed by the master)
     double tab[BS_KMAX][6][MAXN];   // checker: column results T[k][0] of its level
     double diag[6][MAXN];           // checker: T[k][k] of the row tested last
@@ -51,7 +52,7 @@ struct BcSmem {
     // run on from group to group, so a flag of an older round never equals a current one.
     volatile int seq_begin, seq_end;
     volatile double rec_H;          // the round's largest trial step (level l tries rec_H / 2^l)
-    volatile int rec_state;         // 0 run the round, 1 group finished, 2 step size underflow
+    volatile int rec_state;         // 0 run the round, 1 group finished, 2 step size underflow, 3 a pair collides
     volatile int ready[BS_KMAX];    // checker: ready[k] = round whose column k has arrived
     volatile int lev_result[4];     // master: (round << 8) | code of level l; code 0 underflow, 1 rejected, 2 + k passed at row k
     int bc[2];                      // block-local broadcast of what thread 0 saw
@@ -354,14 +355,40 @@ __device__ __forceinline__ double bc_check_row(BcSmem<MAXN, THREADS> &S, const i
     return bc_block_max(S, e);
 }
 
+// Master: does a pair of the group collide in the step just accepted (L328: the Hermite minimum of Eq. 10-12 over the
+// step against (R_a + R_b)^2)?  Old state S.Y, new state SW->diag.  The same answer in every thread.
+template <int MAXN, int THREADS>
+__device__ __noinline__ bool bc_any_collision(BcSmem<MAXN, THREADS> &S, const BcSmem<MAXN, THREADS> *SW, const int n, const double H)
+{
+    int hit = 0;
+    for (int a = threadIdx.x; a < n && !hit; a += THREADS) {
+        if (S.R[a] < 0.0) continue;
+        double qa0[3], va0[3], qa1[3], va1[3];
+        for (int c = 0; c < 3; ++c) { qa0[c] = S.Y[c][a]; va0[c] = S.Y[3 + c][a]; qa1[c] = SW->diag[c][a]; va1[c] = SW->diag[3 + c][a]; }
+        for (int b = a + 1; b < n; ++b) {
+            if (S.R[b] < 0.0) continue;
+            double P0 = 0.0, Pd0 = 0.0, P1 = 0.0, Pd1 = 0.0;
+            for (int c = 0; c < 3; ++c) {
+                const double d0 = S.Y[c][b] - qa0[c], w0 = S.Y[3 + c][b] - va0[c];
+                const double d1 = SW->diag[c][b] - qa1[c], w1 = SW->diag[3 + c][b] - va1[c];
+                P0 += d0 * d0; Pd0 += 2.0 * d0 * w0; P1 += d1 * d1; Pd1 += 2.0 * d1 * w1;
+            }
+            if (pair_collides(P0, P1, Pd0, Pd1, H, S.R[a] + S.R[b])) { hit = 1; break; }
+        }
+    }
+    return __syncthreads_or(hit) != 0;
+}
+
 // One group, integrated over h by the whole cluster of 8 LV CTAs (rank = this CTA's rank in it: level rank / 8,
 // column rank % 8).  On entry S.Y, S.m, S.rc, S.irc of EVERY CTA hold the group; seq = the last round number used (the
 // same in every CTA; 0 and the protocol words of S zero at kernel start), updated on return.  On return S.Y of the
 // master (rank 0) holds the result.  Returns false on step-size underflow (uniform over the cluster).  nsteps (master
 // only): [0] accepted steps, [1] rejected attempts as the sequential rule counts them.
+// Returns 0: step size underflow, 1: done, 2 (coll != 0): a pair of the group collides in an accepted step; the group is
+// abandoned (k_bs_generic integrates it again and merges the pair).
 template <int MAXN, int THREADS, int LV>
-__device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, const int rank, const BcLane &t, double G, double m0,
-                                             double h, double eps, int *nsteps, int &seq)
+__device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int rank, const BcLane &t, double G, double m0,
+                                            double h, double eps, int *nsteps, int &seq, const int coll)
 {
     using Smem = BcSmem<MAXN, THREADS>;
     cg::cluster_group cluster = cg::this_cluster();
@@ -401,7 +428,7 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, const int
         __threadfence();
         for (int r = 0; r < NCTA; ++r) cluster.map_shared_rank(&S, r)->seq_end = seq + 1;
     }
-    bool ok = true;
+    int ok = 1;
 #ifdef GENGA_BC_PROF
     long long pf_t = clock64(), pf_acc[6] = {0, 0, 0, 0, 0, 0};   // record, rhs, wait, check, publish, calls
 #define BC_PROF(k) { const long long now_ = clock64(); pf_acc[k] += now_ - pf_t; pf_t = now_; }
@@ -434,7 +461,7 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, const int
         } while (!consistent);
         seq = e;
         BC_PROF(0)
-        if (state != 0) { ok = state == 1; break; }
+        if (state != 0) { ok = state == 1 ? 1 : state == 3 ? 2 : 0; break; }
         const double Hl = ldexp(Hr, -lev);
         const bool under = lev > 0 && fabs(Hl) < BS_HMIN * fabs(h);
         bool dropped = false;
@@ -524,6 +551,7 @@ __device__ __forceinline__ bool bc_integrate(BcSmem<MAXN, THREADS> &S, const int
         __threadfence();
         int next_state = 0;
         if (fail) next_state = 2;
+        else if (winner >= 0 && coll && bc_any_collision(S, cluster.map_shared_rank(&S, winner * BS_KMAX), n, ldexp(Hr, -winner))) next_state = 3;
         else if (winner >= 0) {
             const Smem *SW = cluster.map_shared_rank(&S, winner * BS_KMAX);
             for (int b = tid; b < 6 * n; b += THREADS) {

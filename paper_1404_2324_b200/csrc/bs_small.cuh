@@ -34,7 +34,36 @@ struct BsmSmem {
     double werr[BS_KMAX][6][BSM_SLOTS];          // scaled squared corrections of the rows under test
     double Y[6][BW_MAXN];                        // state at the start of the round
     int status[BSM_MAXL];                        // 0 running, 1 + k accepted at row k, -1 rejected, -2 step size underflow
+    double R[BW_MAXN];                           // physical radii (collision test; < 0: none)
+    int coll;                                    // look for collisions in every accepted step (L328)
 };
+
+// Does a pair of the group collide in the step just accepted (L328: the Hermite minimum of Eq. 10-12 over the step
+// against (R_a + R_b)^2)?  Old state W.Y, new state row `wrow` of level `winner`.  The whole block; the same answer in
+// every thread.  A group with a collision is handed to k_bs_generic, which integrates it again and merges the pair.
+template <int S>
+__device__ __noinline__ bool bsm_any_collision(BsmSmem &W, const int n, const int wrow, const int winner, const double H)
+{
+    int hit = 0;
+    const int p = threadIdx.x;                   // pair number: (a, b), a < b < n <= 8: at most 28
+    if (p < n * (n - 1) / 2) {
+        int a = 0, rest = p;
+        while (rest >= n - 1 - a) { rest -= n - 1 - a; ++a; }
+        const int b = a + 1 + rest;
+        if (W.R[a] >= 0.0 && W.R[b] >= 0.0) {
+            double P0 = 0.0, Pd0 = 0.0, P1 = 0.0, Pd1 = 0.0;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double d0 = W.Y[c][b] - W.Y[c][a], w0 = W.Y[3 + c][b] - W.Y[3 + c][a];
+                const double d1 = W.tab[wrow][c][winner * S + b] - W.tab[wrow][c][winner * S + a];
+                const double w1 = W.tab[wrow][3 + c][winner * S + b] - W.tab[wrow][3 + c][winner * S + a];
+                P0 += d0 * d0; Pd0 += 2.0 * d0 * w0; P1 += d1 * d1; Pd1 += 2.0 * d1 * w1;
+            }
+            hit = pair_collides(P0, P1, Pd0, Pd1, H, W.R[a] + W.R[b]) ? 1 : 0;
+        }
+    }
+    return __syncthreads_or(hit) != 0;
+}
 
 // Integrate one group over h with NW warps (the whole block).  Lane layout as above; Y = state of body b = lane % S
 // (any finite dummy for b >= n), the same in every segment.  On return Y holds the result in every lane.
@@ -45,8 +74,9 @@ struct BsmSmem {
 // group was accepted at has become complete (row 4 at first), then every second row, and at the end; a test looks at all
 // the rows completed since the last one and takes the FIRST that passes, so the accepted row is the sequential
 // algorithm's whatever the schedule of the tests.
+// Returns 0: step size underflow, 1: done, 2: a pair of the group collides (nothing written; see bsm_any_collision).
 template <int S, int NW>
-__device__ __forceinline__ bool bsm_integrate(BsmSmem &W, const int n, const double Gm0, const double my_rc, const double my_m,
+__device__ __forceinline__ int bsm_integrate(BsmSmem &W, const int n, const double Gm0, const double my_rc, const double my_m,
                                               const double G, double (&Y)[6], const double h, const double eps, int *nsteps)
 {
     constexpr int SPW = 32 / S;                       // slots (columns) per warp
@@ -226,8 +256,9 @@ __device__ __forceinline__ bool bsm_integrate(BsmSmem &W, const int n, const dou
                 else if (st == -2) { resolved = true; winner = -2; }
             }
         }
-        if (winner == -2) return false;
+        if (winner == -2) return 0;
         if (winner >= 0) {
+            if (W.coll && bsm_any_collision<S>(W, n, wrow, winner, ldexp(H, -winner))) return 2;
             if (body) {
 #pragma unroll
                 for (int c = 0; c < 6; ++c) Y[c] = W.tab[wrow][c][winner * S + b];
@@ -243,11 +274,11 @@ __device__ __forceinline__ bool bsm_integrate(BsmSmem &W, const int n, const dou
         } else {                                      // every level rejected
             if (nsteps) nsteps[1] += L;
             H = ldexp(H, -L); last = false;
-            if (fabs(H) < BS_HMIN * fabs(h)) return false;
+            if (fabs(H) < BS_HMIN * fabs(h)) return 0;
         }
         __syncthreads();                              // the tableau and the statuses may be overwritten
     }
-    return true;
+    return 1;
 }
 
 }  // namespace genga

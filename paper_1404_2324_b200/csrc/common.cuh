@@ -10,7 +10,7 @@ namespace genga {
 enum : int { ERRBIT_CAPACITY = 1, ERRBIT_KEPLER = 2, ERRBIT_BS = 4 };
 
 // device counters (int64 slots in DevCounters::c)
-enum : int { CNT_GROUPS = 0, CNT_MAXGROUP = 1, CNT_BSSTEPS = 2, CNT_CAND = 3, CNT_BSREJECTS = 4, CNT_N = 8 };
+enum : int { CNT_GROUPS = 0, CNT_MAXGROUP = 1, CNT_BSSTEPS = 2, CNT_CAND = 3, CNT_BSREJECTS = 4, CNT_NEV = 5, CNT_STEPID = 6, CNT_N = 8 };
 
 // ---------------------------------------------------------------------------------
 // Changeover function K (Eq. 4-5) and the weight of the Newtonian pair force

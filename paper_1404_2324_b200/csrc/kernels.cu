@@ -19,13 +19,21 @@ __device__ __forceinline__ void pdl_sync()
 __device__ __forceinline__ void reset_map_counters(const DevState &d)
 {
     d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
-    d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0; d.cnt[CI_NTRACE] = 0;
+    d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0; d.cnt[CI_NTRACE] = 0; d.cnt[CI_NREDO] = 0;
 }
 // one record per integrated group (genga_bs_trace): size, layout, accepted steps, rejected attempts, SM cycles
 __device__ __forceinline__ void bs_trace(const DevState &d, int n, int layout, const int *nsteps, long long t0, int first)
 {
     const int k = atomicAdd(&d.cnt[CI_NTRACE], 1);
     if (k < BS_TRACE_CAP) d.bstrace[k] = make_int4(n | (layout << 16), nsteps[0] | (nsteps[1] << 16), (int)(clock64() - t0), first);
+}
+
+// a group for k_bs_generic (collisions switched on): kind 0 massive group g, 1 particle p, 2 multi-system (system, member mask)
+__device__ __forceinline__ void push_redo(const DevState &d, int kind, int id, int mask)
+{
+    const int k = atomicAdd(&d.cnt[CI_NREDO], 1);
+    if (k < d.cap) d.redo[k] = make_int2((kind << 28) | id, mask);
+    else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
 }
 
 // =====================================================================================
@@ -1235,11 +1243,16 @@ __global__ void __launch_bounds__(THREADS) k_bs_cluster(DevState d, double h, in
             S.Y[3][b] = d.vx0[i]; S.Y[4][b] = d.vy0[i]; S.Y[5][b] = d.vz0[i];
             double rc = d.rc[i];
             S.m[b] = d.m[i]; S.rc[b] = rc; S.irc[b] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
+            S.R[b] = d.coll && d.kind[i] != 2 ? d.radius[i] : -1.0;
         }
         int nsteps[8] = {0, 0, 0, 0, 0, 0, 0, 0};
         cluster.sync();                             // S0->cur has been read by everybody (the master may pop the next group)
         const long long t0 = clock64();
-        bool ok = bc_integrate<MAXN, THREADS, LV>(S, rank, t, d.G, d.m0[0], h, d.eps, nsteps, seq);
+        const int ok = bc_integrate<MAXN, THREADS, LV>(S, rank, t, d.G, d.m0[0], h, d.eps, nsteps, seq, d.coll);
+        if (ok == 2) {                                  // a collision inside this group: k_bs_generic integrates it again, with the merge
+            if (rank == 0 && threadIdx.x == 0) push_redo(d, 0, g, 0);
+            continue;
+        }
         if (rank == 0) {
             __syncthreads();
             for (int b = threadIdx.x; b < n; b += THREADS) {
@@ -1326,10 +1339,14 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
             Y[0] = d.x0[i]; Y[1] = d.y0[i]; Y[2] = d.z0[i]; Y[3] = d.vx0[i]; Y[4] = d.vy0[i]; Y[5] = d.vz0[i];
             rc = d.rc[i]; m = d.m[i];
         }
+        if (d.coll && threadIdx.x < 8) {                   // radii for the collision test (a removed body: none)
+            W.R[threadIdx.x] = i >= 0 && d.kind[i] != 2 ? d.radius[i] : -1.0;
+            W.coll = 1;
+        } else if (threadIdx.x == 0) W.coll = 0;
         const double Gm0 = d.G * d.m0[sys];
         int nsteps[2] = {0, 0};
         const long long t0 = clock64();
-        bool ok;
+        int ok;
         if (n <= 4) {
             // segments of 2 or 4 lanes: slot b = lane % S takes body b from lane b of the 8-slot layout
             const int src = n == 2 ? (lane & 1) : (lane & 3);
@@ -1340,6 +1357,14 @@ __global__ void __launch_bounds__(32 * BW_WARPS) k_bs_warp(DevState d, double h,
             else ok = bsm_integrate<4, BW_WARPS>(W, n, Gm0, rc, m, d.G, Y, h, d.eps, nsteps);
         } else {
             ok = bsm_integrate<8, BW_WARPS>(W, n, Gm0, rc, m, d.G, Y, h, d.eps, nsteps);
+        }
+        if (ok == 2) {                                     // a collision inside this group: k_bs_generic integrates it again, with the merge
+            if (threadIdx.x == 0) {
+                if (tp) push_redo(d, 1, d.tplist[qi], 0);
+                else if (d.mode == 2) push_redo(d, 2, sys, d.gorder[2 * qi + 1]);
+                else push_redo(d, 0, d.gorder[qi], 0);
+            }
+            continue;
         }
         if (threadIdx.x < 8 && writeback) {
             d.x[i] = Y[0]; d.y[i] = Y[1]; d.z[i] = Y[2]; d.vx[i] = Y[3]; d.vy[i] = Y[4]; d.vz[i] = Y[5];
@@ -1388,6 +1413,7 @@ __global__ void __launch_bounds__(256) k_bs_block(DevState d, double h)
     for (int g = blockIdx.x; g < ng; g += gridDim.x) {
         const int nb = d.gsize[g];
         if (nb <= BCB_MAXN) continue;
+        if (d.coll) { if (threadIdx.x == 0) push_redo(d, 0, g, 0); continue; }   // collisions: the generic layout takes it
         const int off = d.gstart[g];
         if (threadIdx.x == 0) { nsteps[0] = 0; nsteps[1] = 0; }
         for (int b = threadIdx.x; b < nb; b += blockDim.x) {
@@ -1438,6 +1464,7 @@ __global__ void __launch_bounds__(128) k_tp_bs(DevState d, double h, int lo)
         }
         const int nb = __popc(full) + 1;
         if (nb > TW || nb <= lo) continue;            // 32 massive bodies + the particle: k_tp_bs_big
+        if (d.coll) { if (lane == 0) push_redo(d, 1, p, 0); continue; }      // collisions: the generic layout takes it
         const bool active = lane < nb;
         int i = p;
         if (lane < nb - 1) {                         // lane-th set bit of full
@@ -1491,6 +1518,7 @@ __global__ void __launch_bounds__(64) k_tp_bs_big(DevState d, double h)
         }
         const int nb = __popc(full) + 1;
         if (nb <= 32) continue;                           // k_bs_warp / k_tp_bs<32> (uniform over the block)
+        if (d.coll) { if (threadIdx.x == 0) push_redo(d, 1, p, 0); continue; }
         if (threadIdx.x == 0) { nsteps[0] = 0; nsteps[1] = 0; }
         for (int b = threadIdx.x; b < nb; b += blockDim.x) {
             const int i = b < nb - 1 ? __fns(full, 0, b + 1) : p;
@@ -1513,6 +1541,140 @@ __global__ void __launch_bounds__(64) k_tp_bs_big(DevState d, double h)
         }
         __syncthreads();
     }
+}
+
+// Bulirsch-Stoer WITH collisions (L316-328): one block per listed group, any size, tableau in global scratch (bs_block).
+// The fast layouts only notice that a pair of a group collides in an accepted step (same test, same steps) and hand the
+// group over; here it is integrated again from the state before the drift, and the pair merges at the end of that
+// step.  pass 0: particle groups (only the particle is written back; the massive bodies' merges are re-enacted silently,
+// L342) and multi-system groups; pass 1: groups of massive bodies of modes 0, 1, which change masses the particle groups
+// must still see unchanged.
+__global__ void __launch_bounds__(256) k_bs_generic(DevState d, double h, int pass)
+{
+    pdl_sync();
+    __shared__ double red[32];
+    __shared__ int nsteps[2];
+    const int nredo = min(d.cnt[CI_NREDO], (int)d.cap);
+    for (int e = blockIdx.x; e < nredo; e += gridDim.x) {
+        const int2 en = d.redo[e];
+        const int kind = (unsigned)en.x >> 28, id = en.x & 0x0fffffff;
+        if ((kind == 0) != (pass == 1)) continue;
+        int nb, off, sys = 0, p = -1, lab = 0;
+        unsigned full = 0u;
+        const BsScratch &S = kind == 0 ? d.genA : d.genB;
+        if (kind == 0) { nb = d.gsize[id]; off = d.gstart[id]; }
+        else if (kind == 1) {
+            p = id; lab = p;
+            for (unsigned mm = d.tpmask[p - d.nm]; mm; mm &= mm - 1) {
+                const int j = __ffs(mm) - 1;
+                full |= d.gmask[j];
+                lab = min(lab, d.label[j]);
+            }
+            nb = __popc(full) + 1; off = blockIdx.x * 64;
+        } else { sys = id; full = (unsigned)en.y; nb = __popc(full); off = blockIdx.x * 64; }
+        const int base = d.mode == 2 ? sys * d.nm : 0;
+        if (threadIdx.x == 0) { nsteps[0] = 0; nsteps[1] = 0; }
+        for (int b = threadIdx.x; b < nb; b += blockDim.x) {
+            const int i = kind == 0 ? d.gmem[off + b] : kind == 1 ? (b < nb - 1 ? __fns(full, 0, b + 1) : p) : base + __fns(full, 0, b + 1);
+            S.arr(BSA_Y + 0)[off + b] = d.x0[i]; S.arr(BSA_Y + 1)[off + b] = d.y0[i]; S.arr(BSA_Y + 2)[off + b] = d.z0[i];
+            S.arr(BSA_Y + 3)[off + b] = d.vx0[i]; S.arr(BSA_Y + 4)[off + b] = d.vy0[i]; S.arr(BSA_Y + 5)[off + b] = d.vz0[i];
+            S.arr(BSA_M)[off + b] = d.m[i]; S.arr(BSA_RC)[off + b] = d.rc[i];
+            S.arr(BSA_R)[off + b] = d.radius[i]; S.arr(BSA_KIND)[off + b] = (double)d.kind[i];
+            for (int c = 0; c < 3; ++c) S.arr(BSA_SPIN + c)[off + b] = d.spin[(size_t)c * d.np + i];
+            S.arr(BSA_GIDX)[off + b] = (double)(i - base);
+        }
+        BsColl cc;
+        cc.ev = d.ev; cc.evcap = d.evcap; cc.nev = (unsigned long long *)&d.stat[CNT_NEV]; cc.U = d.U + sys;
+        cc.step_id = (double)d.stat[CNT_STEPID]; cc.base = base; cc.record_massive = kind != 1;
+        const bool ok = bs_block(S, off, nb, d.G, d.m0[sys], h, d.eps, red, nsteps, &cc);
+        __syncthreads();
+        for (int b = threadIdx.x; b < nb; b += blockDim.x) {
+            const int i = kind == 0 ? d.gmem[off + b] : kind == 1 ? (b < nb - 1 ? __fns(full, 0, b + 1) : p) : base + __fns(full, 0, b + 1);
+            if (kind == 1 && b < nb - 1) continue;                   // only the particle (L342)
+            d.x[i] = S.arr(BSA_Y + 0)[off + b]; d.y[i] = S.arr(BSA_Y + 1)[off + b]; d.z[i] = S.arr(BSA_Y + 2)[off + b];
+            d.vx[i] = S.arr(BSA_Y + 3)[off + b]; d.vy[i] = S.arr(BSA_Y + 4)[off + b]; d.vz[i] = S.arr(BSA_Y + 5)[off + b];
+            d.m[i] = S.arr(BSA_M)[off + b]; d.radius[i] = S.arr(BSA_R)[off + b]; d.kind[i] = (int)S.arr(BSA_KIND)[off + b];
+            for (int c = 0; c < 3; ++c) d.spin[(size_t)c * d.np + i] = S.arr(BSA_SPIN + c)[off + b];
+            if (kind == 1) d.label[i] = lab;
+        }
+        if (threadIdx.x == 0) {
+            if (!ok) atomicOr(&d.cnt[CI_STATUS], ERRBIT_BS);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSSTEPS], (unsigned long long)nsteps[0]);
+            atomicAdd((unsigned long long *)&d.stat[CNT_BSREJECTS], (unsigned long long)nsteps[1]);
+            if (kind != 0) {
+                atomicAdd((unsigned long long *)&d.stat[CNT_GROUPS], 1ull);
+                atomicMax((unsigned long long *)&d.stat[CNT_MAXGROUP], (unsigned long long)nb);
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// End of a time step with collisions / ejections switched on: ejections (L330-332: a body farther from the central mass
+// than Rcut or closer than RcutSun is reported and removed), the stop of a system with fewer than Nmin bodies left
+// (L378-384: all its bodies are removed), the step counter of the event records.  One thread per system does the
+// system's bodies in index order (events of a system in a fixed order); removed bodies are parked like the ghosts.
+__device__ inline void remove_body(const DevState &d, int i, int base, int sys, int kev)
+{
+    const unsigned long long slot = atomicAdd((unsigned long long *)&d.stat[CNT_NEV], 1ull);
+    if ((long long)slot < d.evcap) {
+        double *e = d.ev + GENGA_EV * slot;
+        for (int k = 0; k < GENGA_EV; ++k) e[k] = 0.0;
+        e[0] = (double)d.stat[CNT_STEPID]; e[1] = kev; e[2] = i; e[3] = -1.0; e[4] = d.m[i]; e[6] = d.radius[i];
+        e[8] = d.x[i]; e[9] = d.y[i]; e[10] = d.z[i]; e[11] = d.vx[i]; e[12] = d.vy[i]; e[13] = d.vz[i];
+        for (int c = 0; c < 3; ++c) e[21 + c] = d.spin[(size_t)c * d.np + i];
+    }
+    const double Rp = 1000.0 * (double)(i - base + 1);
+    d.m[i] = 0.0; d.radius[i] = 0.0; d.kind[i] = 2;
+    for (int c = 0; c < 3; ++c) d.spin[(size_t)c * d.np + i] = 0.0;
+    d.x[i] = Rp; d.y[i] = 0.0; d.z[i] = 0.0;
+    d.vx[i] = 0.0; d.vy[i] = sqrt(d.G * d.m0[sys] / Rp); d.vz[i] = 0.0;
+    d.cnt[CI_S2PMISS] = 1;                                        // positions changed after the closing kick: its stored sums are void
+}
+__global__ void k_end_step(DevState d)
+{
+    pdl_sync();
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (d.mode == 2) {
+        if (t < d.nsys) {
+            const int base = t * d.nm;
+            int left = 0;
+            for (int k = 0; k < d.nm; ++k) {
+                const int i = base + k;
+                if (d.kind[i] == 2) continue;
+                const double r2 = d.x[i] * d.x[i] + d.y[i] * d.y[i] + d.z[i] * d.z[i];
+                if (d.rcut2 > 0.0 && r2 > d.rcut2) remove_body(d, i, base, t, 2);
+                else if (d.rcutsun2 > 0.0 && r2 < d.rcutsun2) remove_body(d, i, base, t, 3);
+                else ++left;
+            }
+            if (d.nmin > 0 && left < d.nmin && left > 0)
+                for (int k = 0; k < d.nm; ++k) if (d.kind[base + k] != 2) remove_body(d, base + k, base, t, 4);
+        }
+    } else {
+        // massive bodies and particles: one thread per body; the stop of the (single) system by thread 0 of a second launch
+        if (t < d.ntot && d.kind[t] != 2) {
+            const double r2 = d.x[t] * d.x[t] + d.y[t] * d.y[t] + d.z[t] * d.z[t];
+            if (d.rcut2 > 0.0 && r2 > d.rcut2) remove_body(d, t, 0, 0, 2);
+            else if (d.rcutsun2 > 0.0 && r2 < d.rcutsun2) remove_body(d, t, 0, 0, 3);
+        }
+    }
+}
+// single system (modes 0, 1): the stop at fewer than Nmin massive bodies, and the step counter
+__global__ void k_end_step2(DevState d)
+{
+    pdl_sync();
+    if (d.mode != 2 && d.nmin > 0) {
+        __shared__ int left;
+        if (threadIdx.x == 0) left = 0;
+        __syncthreads();
+        int mine = 0;
+        for (int i = threadIdx.x; i < d.nm; i += blockDim.x) mine += d.kind[i] != 2;
+        atomicAdd(&left, mine);
+        __syncthreads();
+        if (left < d.nmin && left > 0 && threadIdx.x == 0)
+            for (int i = 0; i < d.ntot; ++i) if (d.kind[i] != 2) remove_body(d, i, 0, 0, 4);
+    }
+    if (threadIdx.x == 0) d.stat[CNT_STEPID] += 1;
 }
 
 // Multi-system mode (L372-376), groups of more than BW_MAXN bodies (the others: k_bs_warp): 16 lanes
@@ -1549,6 +1711,7 @@ __global__ void __launch_bounds__(128) k_bs_multi(DevState d, double h)
         int root = __ffs(todo) - 1;
         todo &= todo - 1;
         unsigned gm = __shfl_sync(tmask, grp, root, TW);
+        if (d.coll) { if (lane == 0) push_redo(d, 2, sys, (int)gm); continue; }   // collisions: the generic layout takes it
         bool active = (gm >> lane) & 1u;
         double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0};
         if (active) { q[0] = d.x0[i]; q[1] = d.y0[i]; q[2] = d.z0[i]; V[0] = d.vx0[i]; V[1] = d.vy0[i]; V[2] = d.vz0[i]; }
@@ -1635,6 +1798,18 @@ __global__ void k_eval_fast(int which, long long n, const double *in, double *ou
     if (i >= n) return;
     const double x = in[i];
     out[i] = which == 0 ? rsqrt_fast(x) : which == 1 ? rinv3_fast(x) : rcp_fast(x);
+}
+
+// A new state has been loaded: every body is what its slot says (massive / test particle), no spin, no internal
+// energy, no events, step 0 (genga_set_state*).
+__global__ void k_init_bodies(DevState d)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) { d.stat[CNT_NEV] = 0; d.stat[CNT_STEPID] = 0; }
+    if (i < d.nsys) d.U[i] = 0.0;
+    if (i >= d.ntot) return;
+    d.kind[i] = (d.mode == 1 && i >= d.nm) ? 1 : 0;
+    for (int c = 0; c < 3; ++c) d.spin[(size_t)c * d.np + i] = 0.0;
 }
 
 // labels for genga_encounters: body's own index unless it is in a group

@@ -49,6 +49,10 @@ template <int TW> __global__ void k_tp_bs(DevState d, double h, int lo);
 __global__ void k_tp_bs_big(DevState d, double h);
 constexpr int TPBIG_BLOCKS = 16;   // blocks of k_tp_bs_big, 64 scratch entries each
 __global__ void k_bs_multi(DevState d, double h);
+__global__ void k_bs_generic(DevState d, double h, int pass);
+__global__ void k_end_step(DevState d);
+__global__ void k_end_step2(DevState d);
+__global__ void k_init_bodies(DevState d);
 __global__ void k_energy(DevState d, double *out);
 __global__ void k_export_labels(DevState d, int *out);
 __global__ void k_fp64_probe(double *out, int iters);

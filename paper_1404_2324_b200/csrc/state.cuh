@@ -35,11 +35,23 @@ struct DevState {
     double *kfar;                // mode 0: its sums over the far pairs, [blocks][KK_THREADS][6]
     int4 *bstrace;               // [BS_TRACE_CAP] one record per group integrated in the last map (bs_trace in kernels.cu)
     BsScratch bss;
+    // ---- collisions, ejections, removal (L316-332, L336, L378-384); off unless genga_set_collisions switches them on
+    int coll;                    // collisions are looked for between the Bulirsch-Stoer steps
+    int nmin;                    // a system with fewer bodies left is stopped (0 = never)
+    double rcut2, rcutsun2;      // squared ejection limits (0 = none)
+    int *kind;                   // [np] 0 massive, 1 test particle, 2 removed
+    double *spin;                // [3][np]
+    double *U;                   // [nsys] internal energy of the collisions (L318-322)
+    double *ev;                  // event records, GENGA_EV doubles each (include/genga.h)
+    long long evcap;
+    int2 *redo;                  // groups k_bs_generic integrates: (kind << 28 | id, member mask); kinds: 0 massive group, 1 particle, 2 multi-system group
+    BsScratch genA, genB;        // its scratch: genA indexed like gmem (massive groups are disjoint), genB 64 entries per block
 };
 
 // indices into DevState::cnt
 enum : int { CI_NCAND = 0, CI_NENC = 1, CI_NGROUPS = 2, CI_NTP = 3, CI_STATUS = 4, CI_NTP_PREV = 5,
-             CI_NBIG = 6, CI_QBIG = 7, CI_NMIDEND = 8, CI_QSMALL = 9, CI_QWARP = 10, CI_QTP = 11, CI_NTRACE = 12, CI_S2PMISS = 13, CI_COUNT = 16 };
+             CI_NBIG = 6, CI_QBIG = 7, CI_NMIDEND = 8, CI_QSMALL = 9, CI_QWARP = 10, CI_QTP = 11, CI_NTRACE = 12, CI_S2PMISS = 13, CI_NREDO = 14, CI_COUNT = 16 };
+constexpr int GEN_BLOCKS = 64;        // blocks of k_bs_generic
 constexpr int BS_TRACE_CAP = 4096;   // records of genga_bs_trace kept per map
 
 __device__ __forceinline__ int system_of(const DevState &d, int i) { return d.mode == 2 ? i / d.nm : 0; }
