@@ -61,7 +61,9 @@ typedef struct {
                            of the next substep of the same step (orders 4, 6; modes 0, 2; L170);
                            the result is the same map, this only selects the schedule;
                            bit 1: mode 0, do not reuse the far-pair sums of a step's closing kick in the
-                           opening kick of the next step (L266-274); same map, schedule only        */
+                           opening kick of the next step (L266-274); same map, schedule only;
+                           bit 2: mode 2, run a step as one launch per operator over all systems instead of
+                           one launch per call in which every block runs its own systems ahead          */
     double G;           /* gravitational constant                                            */
     double n1, n2;      /* critical-radius parameters of Eq. 6 (L94-96); usually 3 and 0.4   */
     double bs_eps;      /* Bulirsch-Stoer relative tolerance (L116 "machine precision")      */

@@ -581,6 +581,24 @@ extern "C" __attribute__((visibility("default"))) int genga_step(genga_ctx *c, i
     if (!c || n_steps < 0 || dt == 0.0 || !(dt == dt) || (order != 2 && order != 4 && order != 6)) return GENGA_EINVAL;
     if (n_steps == 0) return GENGA_OK;
     const bool reused_first = c->far_valid;
+    if (c->d.mode == GENGA_MODE_MULTI_SYSTEM && n_steps >= 4 && !c->d.coll && c->d.rcut2 == 0.0 && c->d.rcutsun2 == 0.0 && c->d.nmin == 0 && !(c->cfg.flags & 5)) {
+        // systems never interact: all the steps of this call (4 or more) in one launch, every block runs its own systems ahead
+        // (multi_persist.cuh); collisions / ejections and flags bit 2 keep the per-operator pipeline below
+        int64_t left = n_steps;
+        while (left > 0) {
+            const int n = (int)std::min<int64_t>(left, 1 << 20);
+            k_reset_counters<<<1, 32, 0, c->st>>>(c->d);
+            k_multi_persist<<<nblk(c->d.nsys, MP_SYS), MP_THREADS, 0, c->st>>>(c->d, dt, order, n);
+            c->launches += 2;
+            left -= n;
+        }
+        CK(cudaGetLastError());
+        c->steps += n_steps;
+        const long long evals = evals_of(c, order, n_steps, false);
+        c->force_evals += evals;
+        c->interactions += evals * interactions_per_eval(c->d);
+        return GENGA_OK;
+    }
     if (c->st == nullptr) {                       // legacy stream cannot be captured: plain launches
         c->acc = 0;
         for (int64_t s = 0; s < n_steps; ++s) enqueue_step(c, dt, order, s > 0 || c->far_valid);

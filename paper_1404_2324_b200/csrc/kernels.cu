@@ -1,5 +1,6 @@
 // Kernels of the hybrid symplectic step, sm_100a.
 // Each kernel states the operator it implements and the passage that defines it.
+#define GENGA_KERNELS_CU 1
 #include "kernels.cuh"
 #include "bs_cluster.cuh"
 #include "bs_warp.cuh"

@@ -3,6 +3,7 @@
 #include "state.cuh"
 #include "bs_cluster.cuh"
 #include "bs_warp.cuh"
+#include "multi_persist.cuh"
 
 namespace genga {
 

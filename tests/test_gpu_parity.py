@@ -511,6 +511,32 @@ def test_merged_and_separate_kicks_are_the_same_map(G, n):
     assert res[0][2] == 3 * 8 - (2 if n > 32 else 0) and res[1][2] == 3 * 14 - (2 if n > 32 else 0)   # 7 maps: 8 merged kicks, 14 separate ones; n > 32: the opening kick of steps 2, 3 from the stored sums
 
 
+@pytest.mark.parametrize("order,npart", [(2, 16), (4, 11), (6, 16)])
+def test_multi_system_one_launch_per_call_is_the_same_integration(G, order, npart):
+    """Multi-system mode runs all the steps of a call in one launch in which every block runs its own systems ahead
+    (multi_persist.cuh); flags bit 2 keeps one launch per operator.  Same maps: both agree with the oracle, and with
+    each other to rounding; the lists of the last substep are the oracle's."""
+    w = dict(workloads.config3(n_systems=37, n_per=npart), order=order)
+    w["m"] = w["m"] * 30                                   # a few groups of 3+ bodies
+    o = oracle.Sim(w)
+    o.step(24, w["dt"], order)
+    xo, vo = o.state()
+    co, eo, lo = o.encounters()
+    res = []
+    for flags in (0, 4):
+        g = G.from_workload(w, flags=flags)
+        g.step(24, w["dt"], order)
+        x, v = g.get_state_host()
+        assert g.status() == 0
+        assert relerr(x, xo).max() < STATE_TOL and relerr(v, vo).max() < STATE_TOL
+        pairs, ncand, labels = g.encounters()
+        assert ncand == len(co) and np.array_equal(pairs, eo) and np.array_equal(labels, lo)
+        res.append((x, v, g.counters()))
+        g.close()
+    assert relerr(res[0][0], res[1][0]).max() < 1e-11
+    assert res[0][2]["groups"] == res[1][2]["groups"] > 0 and res[0][2]["launches"] < res[1][2]["launches"] / 10
+
+
 def test_opening_kick_from_the_stored_sums_is_the_same_kick(G):
     """S2': the closing kick of a step keeps its sums over the far pairs and its hit masks, the opening
     kick of the next step adds them to the near pairs re-weighted with the new critical radii.  Same map as evaluating
