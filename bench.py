@@ -116,10 +116,21 @@ def oracle_rate(w, budget_s, max_steps):
     return per_step * n / dt, n, dt
 
 
+def lib_evals(w):
+    """full force evaluations (all-pairs loops) the library makes per step: 2 per map in the particle mode; adjacent kicks
+    of the maps of a step are one evaluation (modes 0, 2); in massive mode with N > 32 the opening kick of a step is
+    none either (S2': it adds the sums the previous closing kick stored)"""
+    maps = {2: 1, 4: 3, 6: 7}[w["order"]]
+    if w["mode"] == 1:
+        return 2 * maps
+    return maps if (w["mode"] == 0 and w["n_massive"] > 32) else maps + 1
+
+
 def config_dict(w, name, evals, world=1):
     """the `config` object of the JSON line: the benchmark configuration, the same object on both arms"""
+    evals = lib_evals(w)
     return {"workload": name, "n_massive": w["n_massive"], "order": w["order"], "dt_days": w["dt"] / workloads.DAY,
-            "force_evals_per_step": evals,
+            "force_evals_per_step": evals, "steps_per_timed_call": 16 if w["mode"] == 2 else 1,
             "l2": "flushed (512 MiB fill) before every timed step",
             "parallelism": ("1 gpu" if world == 1 else "replicas only" if w["mode"] == 0 else
                             "particles sharded, massive bodies replicated, no collective" if w["mode"] == 1
@@ -205,20 +216,31 @@ def measure(torch, G, dev, cfg_id, order, steps, warmup, rank, world, clocks=Non
     assert g.status() == 0
     c0 = g.counters()
 
-    # ---- timed: K steps, each timed with events on the library's stream, L2 flushed between
+    # ---- timed: K steps, timed with events on the library's stream, L2 flushed between the timed calls.  A timed call is
+    # one step; in multi-system mode 16 steps, because there all the steps of a call run in ONE launch in which every
+    # block runs its own systems ahead (a call of one step would time the per-operator pipeline instead)
+    chunk = 16 if w["mode"] == 2 else 1
+    steps = max(chunk, steps // chunk * chunk)
     barrier()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps // chunk)]
     with torch.cuda.stream(g.stream):
-        for k in range(steps):
+        for k in range(steps // chunk):
             flush.fill_(k & 255)               # evicts the state from L2; outside the timed events
             ev[k][0].record(g.stream)
-            g.step(1, dt, order)
+            g.step(chunk, dt, order)
             ev[k][1].record(g.stream)
     barrier()
     ms = [a.elapsed_time(b) for a, b in ev]
     elapsed = sum(ms) * 1e-3
     c1 = g.counters()
     status = g.status()
+    trace = g.bs_trace()                       # the groups of the last substep: the longest chain sets the step time
+    # pair interactions the library evaluated per step (its own count of full force evaluations: adjacent kicks merged,
+    # the opening kick of a step taken from the stored sums of the previous closing kick)
+    evals = (c1["force_evals"] - c0["force_evals"]) / steps
+    per_step = (c1["interactions"] - c0["interactions"]) / steps
+    if w.get("shard", (0,))[0] != 0 and w["mode"] == 1:      # the replicated massive bodies are counted once, on rank 0
+        per_step -= w["n_massive"] * (w["n_massive"] - 1) * evals
 
     # ---- back-to-back (state resident in L2, 16-step graphs): the production loop
     nres = max(16, (steps // 16) * 16)
@@ -279,13 +301,16 @@ def measure(torch, G, dev, cfg_id, order, steps, warmup, rank, world, clocks=Non
           "in_step_ms": phases["bs"], "share_of_step": phases["bs"] / phases["total"] if phases["total"] else None,
           "groups_per_step": groups_ps, "accepted_steps_per_step": acc_ps, "rejected_attempts_per_step": rej_ps,
           "group_steps_per_s": acc_ps / (phases["bs"] * 1e-3) if phases["bs"] > 0 else None,
+          "longest_chain": ({"group_size": int(trace[np.argmax(trace[:, 4]), 0]), "accepted": int(trace[np.argmax(trace[:, 4]), 2]),
+                             "rejected": int(trace[np.argmax(trace[:, 4]), 3]), "us": float(trace[:, 4].max()) / 1965.0,
+                             "note": "last substep of the timed run (genga_bs_trace), SM cycles at 1965 MHz"} if len(trace) else None),
           "fp64_pipe_pct_ncu": tab.get("fp64_pipe_pct", {}).get("bs"),
           "note": "time = the longest dependent chain of one group, not arithmetic: ncu's FP64-pipe share (profiles/) is the utilisation figure"}
     if w["mode"] == 0:
         kick_ms = g.time_kernel(0, 200, dt)
         inter = w["n_massive"] * (w["n_massive"] - 1)
         achieved = FLOP_PER_INTERACTION * inter / (kick_ms * 1e-3) / 1e12
-        nk = maps + 1                                            # kick launches per step (adjacent kicks merged)
+        nk = maps + 1                                            # kick launches per step: `maps` full ones + the near-pair one of S2' (N > 32)
         kin = phases["kick"] / nk
         roof = {"bound": "alu", "kernel": "k_kick", "achieved": achieved, "peak": peak_probe,
                 "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": tab.get("k_kick"),
