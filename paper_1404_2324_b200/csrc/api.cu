@@ -433,8 +433,8 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
     if (tp) {
         // particles: kick, Sun kick and drift in one pass (k_tp_front); the massive bodies as in mode 0
         launch_k(c->pdl, k_tpm_kick, 1, 32, 0, st, d, 0.5 * h, 1, 0.0); LAUNCH(c);           // kick + momentum sum, one warp
-        launch_k(c->pdl, k_tp_front, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h, tau, first); LAUNCH(c);
         launch_k(c->pdl, k_drift, nblk(d.nm, 128), 128, 0, st, dm, h, 0.5 * h); LAUNCH(c);   // Sun kick + drift of the massive bodies
+        launch_k(c->pdl, k_tp_front, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h, tau, first); LAUNCH(c);   // the particles, encounter search included
     } else if (tiny_mode(d)) {                                // N <= 32: the opening half map in one warp, one launch
         launch_k(c->pdl, k_tiny_front, 1, 32, 0, st, d, h, tau, first, opened ? 0.0 : 0.5 * h); LAUNCH(c);
     } else if (d.mode == GENGA_MODE_MULTI_SYSTEM) {           // a block holds whole systems: the opening half map in one launch
@@ -837,7 +837,7 @@ extern "C" __attribute__((visibility("default"))) int genga_encounters(genga_ctx
     std::sort(h.begin(), h.end(), [](const int2 &a, const int2 &b) { return a.x != b.x ? a.x < b.x : a.y < b.y; });
     for (long long k = 0; k < ne && k < cap; ++k) { pairs[2 * k] = h[k].x; pairs[2 * k + 1] = h[k].y; }
     if (n_pairs) *n_pairs = cnt[CI_NENC];
-    if (n_candidates) *n_candidates = cnt[CI_NCAND];
+    if (n_candidates) *n_candidates = (int64_t)cnt[CI_NCAND] + cnt[CI_NCAND_TP];
     return r;
 }
 

@@ -20,7 +20,7 @@ __device__ __forceinline__ void pdl_sync()
 __device__ __forceinline__ void reset_map_counters(const DevState &d)
 {
     d.cnt[CI_NCAND] = 0; d.cnt[CI_NENC] = 0; d.cnt[CI_NGROUPS] = 0; d.cnt[CI_NTP] = 0; d.cnt[CI_NBIG] = 0;
-    d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0; d.cnt[CI_NTRACE] = 0; d.cnt[CI_NREDO] = 0;
+    d.cnt[CI_QWARP] = 0; d.cnt[CI_QTP] = 0; d.cnt[CI_NTRACE] = 0; d.cnt[CI_NREDO] = 0; d.cnt[CI_NCAND_TP] = 0;
 }
 // one record per integrated group (genga_bs_trace): size, layout, accepted steps, rejected attempts, SM cycles
 __device__ __forceinline__ void bs_trace(const DevState &d, int n, int layout, const int *nsteps, long long t0, int first)
@@ -410,62 +410,51 @@ __global__ void __launch_bounds__(128) k_tp_kick(DevState d, double h, int recor
 // the massive bodies must not have been shifted yet (front) / must have been shifted (back): B only sees
 // differences of positions, which a common shift leaves alone.
 struct TpMassive { double x[32], y[32], z[32], gm[32], rc[32]; int hc[32]; };
-__device__ __forceinline__ void tp_load_massive(const DevState &d, TpMassive &M)
+__device__ __forceinline__ void tp_load_massive(const DevState &d, TpMassive &M, const double *px, const double *py, const double *pz)
 {
     if (threadIdx.x < d.nm) {
         int j = threadIdx.x;
-        M.x[j] = d.x[j]; M.y[j] = d.y[j]; M.z[j] = d.z[j]; M.gm[j] = d.G * d.m[j]; M.rc[j] = d.rc[j];
+        M.x[j] = px[j]; M.y[j] = py[j]; M.z[j] = pz[j]; M.gm[j] = d.G * d.m[j]; M.rc[j] = d.rc[j];
         M.hc[j] = __double2hiint(9.0 * M.rc[j] * M.rc[j]);
     }
     __syncthreads();
 }
-// acceleration of a particle at (xi, yi, zi) by the massive bodies; returns the number of candidates recorded
-template <bool RECORD>
-__device__ __forceinline__ int tp_accel(const DevState &d, const TpMassive &M, int i, double xi, double yi, double zi, double rci,
-                                        double &ax, double &ay, double &az)
+// acceleration of a particle at (xi, yi, zi) by the massive bodies; returns the mask of the massive bodies inside the
+// precheck sphere (the particle's candidates, L142)
+__device__ __forceinline__ unsigned tp_accel(const DevState &d, const TpMassive &M, double xi, double yi, double zi, double rci,
+                                             double &ax, double &ay, double &az)
 {
-    int ncand = 0;
+    unsigned cmask = 0u;
     ax = ay = az = 0.0;
     const int nm = d.nm;
-    const unsigned act = __activemask();                        // the live lanes of this warp run the loop together
-    const int lane = threadIdx.x & 31;
     const int hci = __double2hiint(9.0 * rci * rci);            // precheck on the high words (a superset, off the FP64 pipe)
     for (int j = 0; j < nm; ++j) {
         double dx = M.x[j] - xi, dy = M.y[j] - yi, dz = M.z[j] - zi;
         double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
         double s3 = M.gm[j] * rinv3_fast(r2);
-        bool cand = false;
         if (__double2hiint(r2) <= max(hci, M.hc[j])) {
             const double rcij = fmax(rci, M.rc[j]);
-            cand = r2 < 9.0 * rcij * rcij;
+            if (r2 < 9.0 * rcij * rcij) cmask |= 1u << j;
             if (r2 < rcij * rcij) {                             // inside the changeover zone: exact weight (W = 1 outside)
                 double r = sqrt(r2);
                 s3 = M.gm[j] / (r2 * r) * kick_weight(r, rcij);
             }
         }
-        if (RECORD) {                                           // candidates: one atomic per warp
-            const unsigned m = __ballot_sync(act, cand);
-            if (m) {
-                const int leader = __ffs(m) - 1;
-                int base = 0;
-                if (lane == leader) base = atomicAdd(&d.cnt[CI_NCAND], __popc(m));
-                base = __shfl_sync(act, base, leader);
-                if (cand) {
-                    const int idx = base + __popc(m & ((1u << lane) - 1u));
-                    if (idx < d.cap) d.cand[idx] = make_int2(j, i);
-                    else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
-                    ++ncand;
-                }
-            }
-        }
         ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
     }
-    return ncand;
+    return cmask;
 }
+// The massive bodies have been kicked, Sun-kicked and drifted before this launch (k_tpm_kick, k_drift): x0.. hold them
+// after the Sun kick, x.. after the drift.  The particle takes its Sun kick FIRST and its kick against the shifted massive
+// bodies (B and C commute exactly: B only sees differences of positions, R-11), drifts, and tests its candidates by the
+// Hermite minimum (Eq. 10-12) right here, from registers and shared memory: no candidate list, no gather, and the state
+// before the drift is stored only for the few particles that do have an encounter.
+struct TpMassive2 { double x1[32], y1[32], z1[32], vx0[32], vy0[32], vz0[32], vx1[32], vy1[32], vz1[32]; };
 __global__ void __launch_bounds__(128) k_tp_front(DevState d, double h, double tau, int first)
 {
     pdl_sync();
     __shared__ TpMassive M;
+    __shared__ TpMassive2 M2;
     const int i = d.nm + blockIdx.x * blockDim.x + threadIdx.x;
     const bool live = i < d.ntot;
     // the particle's own loads go out before the block waits for the massive bodies: one memory round trip
@@ -474,19 +463,53 @@ __global__ void __launch_bounds__(128) k_tp_front(DevState d, double h, double t
         x = d.x[i]; y = d.y[i]; z = d.z[i]; vx = d.vx[i]; vy = d.vy[i]; vz = d.vz[i];
         if (!first) rci = d.rc[i];
     }
-    tp_load_massive(d, M);
-    if (!live) return;
-    if (first) {
+    if (threadIdx.x < d.nm) {
+        const int j = threadIdx.x;
+        M2.x1[j] = d.x[j]; M2.y1[j] = d.y[j]; M2.z1[j] = d.z[j];
+        M2.vx0[j] = d.vx0[j]; M2.vy0[j] = d.vy0[j]; M2.vz0[j] = d.vz0[j];
+        M2.vx1[j] = d.vx[j]; M2.vy1[j] = d.vy[j]; M2.vz1[j] = d.vz[j];
+    }
+    tp_load_massive(d, M, d.x0, d.y0, d.z0);
+    if (first && live) {
         rci = fmax(d.n1 * 0.0, d.n2 * fabs(tau) * sqrt(vx * vx + vy * vy + vz * vz));
         d.rc[i] = rci;
     }
-    double ax, ay, az;
-    const int ncand = tp_accel<true>(d, M, i, x, y, z, rci, ax, ay, az);
     const double hh = 0.5 * h, g = hh / d.m0[0];
-    vx = fma(hh, ax, vx); vy = fma(hh, ay, vy); vz = fma(hh, az, vz);
     x = fma(g, d.psum[0], x); y = fma(g, d.psum[1], y); z = fma(g, d.psum[2], z);
-    if (ncand) { d.x0[i] = x; d.y0[i] = y; d.z0[i] = z; d.vx0[i] = vx; d.vy0[i] = vy; d.vz0[i] = vz; }
-    if (!kepler_drift(d.G * d.m0[0], h, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
+    double ax, ay, az;
+    const unsigned cmask = live ? tp_accel(d, M, x, y, z, rci, ax, ay, az) : 0u;
+    if (live) { vx = fma(hh, ax, vx); vy = fma(hh, ay, vy); vz = fma(hh, az, vz); }
+    const double x0 = x, y0 = y, z0 = z, vx0 = vx, vy0 = vy, vz0 = vz;
+    if (live && !kepler_drift(d.G * d.m0[0], h, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
+    // candidates of this warp: one atomic
+    {
+        int nc = __popc(cmask);
+        for (int o = 16; o > 0; o >>= 1) nc += __shfl_xor_sync(0xffffffffu, nc, o);
+        if ((threadIdx.x & 31) == 0 && nc) atomicAdd(&d.cnt[CI_NCAND_TP], nc);
+    }
+    if (!live) return;
+    unsigned emask = 0u;
+    for (unsigned cm = cmask; cm; cm &= cm - 1) {
+        const int j = __ffs(cm) - 1;
+        double dx = x0 - M.x[j], dy = y0 - M.y[j], dz = z0 - M.z[j];
+        double dvx = vx0 - M2.vx0[j], dvy = vy0 - M2.vy0[j], dvz = vz0 - M2.vz0[j];
+        const double P0 = dx * dx + dy * dy + dz * dz, Pd0 = 2.0 * (dx * dvx + dy * dvy + dz * dvz);
+        dx = x - M2.x1[j]; dy = y - M2.y1[j]; dz = z - M2.z1[j];
+        dvx = vx - M2.vx1[j]; dvy = vy - M2.vy1[j]; dvz = vz - M2.vz1[j];
+        const double P1 = dx * dx + dy * dy + dz * dz, Pd1 = 2.0 * (dx * dvx + dy * dvy + dz * dvz);
+        const double rcij = fmax(rci, M.rc[j]);
+        if (hermite_min(P0, P1, Pd0, Pd1, h) < rcij * rcij) {
+            emask |= 1u << j;
+            const int idx = atomicAdd(&d.cnt[CI_NENC], 1);
+            if (idx < d.cap) d.enc[idx] = make_int2(j, i);
+            else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+        }
+    }
+    if (emask) {                                                // Bulirsch-Stoer needs the state before the drift
+        d.x0[i] = x0; d.y0[i] = y0; d.z0[i] = z0; d.vx0[i] = vx0; d.vy0[i] = vy0; d.vz0[i] = vz0;
+        d.tpmask[i - d.nm] = emask;
+        d.tplist[atomicAdd(&d.cnt[CI_NTP], 1)] = i;
+    }
     d.x[i] = x; d.y[i] = y; d.z[i] = z; d.vx[i] = vx; d.vy[i] = vy; d.vz[i] = vz;
 }
 __global__ void __launch_bounds__(128) k_tp_back(DevState d, double h)
@@ -497,12 +520,12 @@ __global__ void __launch_bounds__(128) k_tp_back(DevState d, double h)
     const bool live = i < d.ntot;
     double x = 0.0, y = 0.0, z = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, rci = 0.0;
     if (live) { x = d.x[i]; y = d.y[i]; z = d.z[i]; vx = d.vx[i]; vy = d.vy[i]; vz = d.vz[i]; rci = d.rc[i]; }
-    tp_load_massive(d, M);
+    tp_load_massive(d, M, d.x, d.y, d.z);
     if (!live) return;
     const double hh = 0.5 * h, g = hh / d.m0[0];
     x = fma(g, d.psum[0], x); y = fma(g, d.psum[1], y); z = fma(g, d.psum[2], z);
     double ax, ay, az;
-    tp_accel<false>(d, M, i, x, y, z, rci, ax, ay, az);
+    tp_accel(d, M, x, y, z, rci, ax, ay, az);
     d.x[i] = x; d.y[i] = y; d.z[i] = z;
     d.vx[i] = fma(hh, ax, vx); d.vy[i] = fma(hh, ay, vy); d.vz[i] = fma(hh, az, vz);
 }

@@ -50,7 +50,7 @@ struct DevState {
 
 // indices into DevState::cnt
 enum : int { CI_NCAND = 0, CI_NENC = 1, CI_NGROUPS = 2, CI_NTP = 3, CI_STATUS = 4, CI_NTP_PREV = 5,
-             CI_NBIG = 6, CI_QBIG = 7, CI_NMIDEND = 8, CI_QSMALL = 9, CI_QWARP = 10, CI_QTP = 11, CI_NTRACE = 12, CI_S2PMISS = 13, CI_NREDO = 14, CI_COUNT = 16 };
+             CI_NBIG = 6, CI_QBIG = 7, CI_NMIDEND = 8, CI_QSMALL = 9, CI_QWARP = 10, CI_QTP = 11, CI_NTRACE = 12, CI_S2PMISS = 13, CI_NREDO = 14, CI_NCAND_TP = 15, CI_COUNT = 16 };   // CI_NCAND_TP: particle candidates (counted, not listed: k_tp_front)
 constexpr int GEN_BLOCKS = 64;        // blocks of k_bs_generic
 constexpr int BS_TRACE_CAP = 4096;   // records of genga_bs_trace kept per map
 
