@@ -80,7 +80,9 @@ size_t genga_workspace_bytes(const genga_config *cfg);
 /* Create / destroy a context.  genga_create does not touch the device state arrays;
  * call genga_set_state before anything else. */
 /* Environment: GENGA_NO_PDL=1 (read by genga_create) launches the kernels of a step without programmatic
- * dependent launch; results are bit-identical either way. */
+ * dependent launch; GENGA_TMA=1 makes the pair kernel of the kick stage the records of its partner tile with bulk copies
+ * (cp.async.bulk + one mbarrier per slice) instead of through registers (measured on B200 at N = 2048: 12.4 against
+ * 11.7 us per launch, so it is not the default); results are bit-identical either way. */
 int genga_create(const genga_config *cfg, genga_ctx **out);
 int genga_destroy(genga_ctx *ctx);
 

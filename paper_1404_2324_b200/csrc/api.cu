@@ -43,6 +43,7 @@ struct genga_ctx {
     cudaEvent_t ev_fork, ev_join[2];
     int sms;
     bool pdl;                   // programmatic dependent launch on the main stream (GENGA_NO_PDL=1 switches it off)
+    bool tma;                   // k_kick stages its j-tile with bulk copies (GENGA_TMA=1; default: loads through registers, measured faster)
     int bs_big_clusters;        // grid size (in clusters) of the Bulirsch-Stoer cluster kernel
     int *exp_labels;            // device [np]
     double *eout;               // device [4*nsys]
@@ -159,6 +160,8 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
     t.stat = (long long *)take(sizeof(long long) * CNT_N);
     t.bstrace = (int4 *)take(sizeof(int4) * BS_TRACE_CAP);
     if (c->mode == GENGA_MODE_MASSIVE && nm > 32) {
+        t.kb = (double *)take(sizeof(double) * 4 * (size_t)npm);
+        t.hcw = (int *)take(sizeof(int) * (size_t)npm);
         t.khits = (unsigned *)take(sizeof(unsigned) * (size_t)sms * KK_THREADS);
         t.kfar = (double *)take(sizeof(double) * 6 * (size_t)sms * KK_THREADS);
     }
@@ -201,6 +204,7 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     c->st = (cudaStream_t)cfg->stream;
     c->sms = std::min(prop.multiProcessorCount, 148);
     { const char *e = getenv("GENGA_NO_PDL"); c->pdl = !(e && e[0] == '1'); }
+    { const char *e = getenv("GENGA_TMA"); c->tma = e && e[0] == '1'; }
     c->bs_big_clusters = std::max(1, c->sms / BCB_CS);
     c->steps = c->force_evals = c->interactions = c->launches = 0;
     c->acc = 0;
@@ -357,6 +361,7 @@ static void launch_kick(genga_ctx *c, double h, int record, double *aout, int to
     DevState &d = c->d;
     const int ni = std::min(KK_NI, (d.nm + c->sms - 1) / c->sms);
     const int grid = (d.nm + ni - 1) / ni;
+    if (!d.kb || !c->tma) s2p |= 4;                           // no packed j-tile (N <= 32, mode 1) or switched off: stage through registers
     launch_k(c->pdl, k_kick, grid, KK_THREADS, kick_smem_bytes(), c->st, d, h, record, ni, aout, to0, s2p);
 }
 
@@ -533,6 +538,7 @@ static void enqueue_step(genga_ctx *c, double dt, int order, bool reuse)
         launch_k(c->pdl, k_rcrit, 1, 128, 0, c->st, dm, dt, 2, 0); LAUNCH(c);    // nm <= 32: one block, which also opens the first map
     } else if (!tiny_mode(d)) {                                   // N <= 32: inside k_tiny_front of the first map
         launch_k(c->pdl, k_rcrit, nblk(d.ntot, 128), 128, 0, c->st, d, dt, d.mode != GENGA_MODE_TEST_PARTICLE, reuse ? 1 : 0); LAUNCH(c);
+        if (d.kb && !reuse) { launch_k(c->pdl, k_pack_kb, nblk(d.npm, 128), 128, 0, c->st, d); LAUNCH(c); }   // a state that did not come out of a step
     }
     const bool merge = !(c->cfg.flags & 1) && d.mode != GENGA_MODE_TEST_PARTICLE;
     for (int k = 0; k < nw; ++k)
@@ -901,6 +907,7 @@ extern "C" __attribute__((visibility("default"))) int genga_accelerations(genga_
     DevState &d = c->d;
     c->far_valid = false;
     k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt, 0, 0);
+    if (d.kb) { k_pack_kb<<<nblk(d.npm, 128), 128, 0, c->st>>>(d); c->launches += 1; }
     if (d.mode == GENGA_MODE_TEST_PARTICLE) { k_begin_map<<<c->sms, 256, 0, c->st>>>(d); c->launches += 1; }
     k_reset_counters<<<1, 32, 0, c->st>>>(d);
     c->launches += 2;
@@ -934,6 +941,7 @@ extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ct
     CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
     c->far_valid = false;
     k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt, 0, 0);
+    if (d.kb) { k_pack_kb<<<nblk(d.npm, 128), 128, 0, c->st>>>(d); c->launches += 1; }
     c->launches += 1;
     int per = 1;
     for (int r = -3; r < reps; ++r) {

@@ -98,6 +98,7 @@ __global__ void k_rcrit(DevState d, double tau, int reset, int check)
     if (check && rc > KK_GROW * d.rc[i]) d.cnt[CI_S2PMISS] = 1;
     d.rc[i] = rc;
     d.c9[i] = 9.0 * rc * rc;
+    if (d.hcw && i < d.nm) d.hcw[i] = __double2hiint(KK_WIDE2 * rc * rc);
 }
 
 // =====================================================================================
@@ -153,7 +154,48 @@ struct KickSmem {
     double rc[KK_MAXN];                     // critical radius (exact pass)
     KickHit list[KK_WARPS][32];             // per warp: hits of the current window of the exact pass
     double wsum[KK_WARPS][8][3];            // per warp: sums of its rows
+    unsigned long long mbar[16];            // one mbarrier per slice of the j-tile (bulk copies)
 };
+
+// ---- TMA bulk copies (cp.async.bulk) and mbarriers: the j-tile of k_kick arrives slice by slice, a warp starts on its slice
+// when that slice has landed instead of after a block-wide barrier over all 88 KB
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    unsigned ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+
+// The packed j-tile of k_kick: records (x, y, z, G m) of the massive bodies and the padding up to a multiple of 128
+// (far away, massless).  Written by the closing k_sun of a map (the positions every full kick acts at) and, for a state
+// that did not come out of a step, by this kernel.
+__global__ void k_pack_kb(DevState d)
+{
+    pdl_sync();
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= d.npm) return;
+    const bool v = j < d.nm;
+    double4 r;
+    r.x = v ? d.x[j] : 1e100; r.y = v ? d.y[j] : 1e100; r.z = v ? d.z[j] : 1e100; r.w = v ? d.G * d.m[j] : 0.0;
+    reinterpret_cast<double4 *>(d.kb)[j] = r;
+    d.hcw[j] = v ? __double2hiint(KK_WIDE2 * d.rc[j] * d.rc[j]) : -1;
+}
 
 __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, int record, int ni, double *aout, int to0, int s2p)
 {
@@ -174,8 +216,22 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
     const int ii = rowbase + 2 * rp, i = i0 + ii;
     const bool ok0 = ii < nib, ok1 = ii + 1 < nib;
 
-    // stage the bodies j: all loads of the (at most 3) rounds in flight together; 9 rc^2 as k_rcrit forms it
-    {
+    // stage the bodies j.  TMA path: the first 16 lanes issue, each for one slice of 8 * iters bodies (what one warp of the first group
+    // covers), three bulk copies (records, precheck words, critical radii) that complete on the slice's mbarrier
+    const bool tma = !(s2p & 4);
+    const int slb = iters << 3;                         // bodies per slice; 16 slices = npad bodies
+    if (tma) {
+        if (tid < 16) {                                 // sixteen lanes, a slice each: the copies are issued side by side
+            const int sl = tid;
+            mbar_init(&S.mbar[sl], 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            mbar_expect_tx(&S.mbar[sl], (unsigned)slb * 32u);
+            bulk_g2s(&S.body[sl * slb], d.kb + 4 * (size_t)sl * slb, (unsigned)slb * 32u, &S.mbar[sl]);
+        }
+        // the precheck words and critical radii (24 KB of the 88) through registers meanwhile; the block barrier below publishes them
+        for (int j = tid; j < npad; j += KK_THREADS) { S.hc[j] = d.hcw[j]; S.rc[j] = d.rc[j]; }
+    } else {
+        // all loads of the (at most 3) rounds in flight together; the precheck word as k_pack_kb forms it
         constexpr int ROUNDS = (KK_MAXN + KK_THREADS - 1) / KK_THREADS;
         double lx[ROUNDS], ly[ROUNDS], lz[ROUNDS], lm[ROUNDS], lr[ROUNDS];
 #pragma unroll
@@ -210,6 +266,10 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
     }
     __syncthreads();
 
+    if (tma) {                                          // my slices of the j-tile (the block barrier above published the mbarriers)
+        const int s0 = wi << (logP - 3), ns = 1 << (logP - 3);
+        for (int sl = s0; sl < s0 + ns; ++sl) mbar_wait(&S.mbar[sl], 0);
+    }
     double ax0 = 0.0, ay0 = 0.0, az0 = 0.0, ax1 = 0.0, ay1 = 0.0, az1 = 0.0;
     unsigned hits = 0u;
     // S2' (L266-274): s2p & 2 = this is the opening kick of a step at the positions of the previous step's closing kick,
@@ -269,6 +329,10 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
         }
         __syncwarp();
 
+        if (tma) {                                      // the exact pass reads any body: all slices
+#pragma unroll 1
+            for (int sl = 0; sl < 16; ++sl) mbar_wait(&S.mbar[sl], 0);
+        }
         // ---- this warp's pairs inside the precheck sphere: exact weight, candidate list.
         // Lane l, bit 2 t + s of its hit mask: row rowbase + 2 (l >> logP) + s, body j = wi L + t P + (l & (P - 1)).  The hits are
         // listed in (lane, bit) order, 32 at a time; lane e evaluates entry e; the row pair's first lane adds its entries in list order.
@@ -985,6 +1049,7 @@ __global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset, do
         d.vx[i] = vx; d.vy[i] = vy; d.vz[i] = vz;
     }
     d.x[i] = x; d.y[i] = y; d.z[i] = z;
+    if (d.kb && hdrift == 0.0) reinterpret_cast<double4 *>(d.kb)[i] = make_double4(x, y, z, d.G * d.m[i]);   // the j-tile of the kick that follows
 }
 // Coordinate maps at the ABI in ONE launch (L69): out = in + f * s / den, s = sum m * in over the massive bodies of the
 // system, den = m0 (+ sum m if divide_by_total).  Every block forms s itself, in a fixed order: modes 0, 1 as k_sun
@@ -1653,6 +1718,7 @@ __device__ inline void remove_body(const DevState &d, int i, int base, int sys, 
     for (int c = 0; c < 3; ++c) d.spin[(size_t)c * d.np + i] = 0.0;
     d.x[i] = Rp; d.y[i] = 0.0; d.z[i] = 0.0;
     d.vx[i] = 0.0; d.vy[i] = sqrt(d.G * d.m0[sys] / Rp); d.vz[i] = 0.0;
+    if (d.kb && i < d.nm) reinterpret_cast<double4 *>(d.kb)[i] = make_double4(Rp, 0.0, 0.0, 0.0);
     d.cnt[CI_S2PMISS] = 1;                                        // positions changed after the closing kick: its stored sums are void
 }
 __global__ void k_end_step(DevState d)

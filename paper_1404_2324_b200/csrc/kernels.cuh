@@ -25,6 +25,7 @@ __global__ void k_reset_counters(DevState d);
 __global__ void k_rcrit(DevState d, double tau, int reset, int check);
 __global__ void k_kick(DevState d, double h, int record, int ni, double *aout, int to0, int s2p);
 size_t kick_smem_bytes();
+__global__ void k_pack_kb(DevState d);
 __global__ void k_tp_kick(DevState d, double h, int record, double *aout);
 __global__ void k_tp_front(DevState d, double h, double tau, int first);
 __global__ void k_tp_back(DevState d, double h);

@@ -31,6 +31,8 @@ struct DevState {
     unsigned *tpmask;            // mode 1: per particle, massive bodies it meets
     int *tplist;                 // mode 1: particles with encounters in this substep
     long long *stat;             // CNT_* accumulators
+    double *kb;                  // mode 0: packed records (x, y, z, G m) of the massive bodies, [npm], padding far away and massless: the j-tile k_kick stages with bulk copies
+    int *hcw;                    // mode 0: high word of the squared precheck radius KK_WIDE2 rc^2 per body (-1 for padding), [npm]
     unsigned *khits;             // mode 0: hit masks of the last closing kick, [blocks][KK_THREADS] (S2', k_kick)
     double *kfar;                // mode 0: its sums over the far pairs, [blocks][KK_THREADS][6]
     int4 *bstrace;               // [BS_TRACE_CAP] one record per group integrated in the last map (bs_trace in kernels.cu)

@@ -577,6 +577,31 @@ def test_opening_kick_from_the_stored_sums_is_the_same_kick(G):
     g.close()
 
 
+def test_kick_tile_by_bulk_copies_is_bit_identical(G):
+    """GENGA_TMA=1 (read at genga_create): the pair kernel stages the partner records with cp.async.bulk + mbarriers,
+    a warp starts when its slices have landed.  Same arithmetic: bit-identical states and lists."""
+    import os
+    w = workloads.config1(n=1333)
+    out = []
+    for env in (None, "1"):
+        if env is None:
+            os.environ.pop("GENGA_TMA", None)
+        else:
+            os.environ["GENGA_TMA"] = env
+        g = G.from_workload(w)
+        a, _ = g.accelerations(w["dt"])
+        g.step(6, w["dt"], 4)
+        x, v = g.get_state_host()
+        pairs, ncand, labels = g.encounters()
+        assert g.status() == 0
+        out.append((a.cpu().numpy(), x, v, pairs, ncand))
+        g.close()
+    os.environ.pop("GENGA_TMA", None)
+    for k in range(4):
+        assert np.array_equal(out[0][k], out[1][k])
+    assert out[0][4] == out[1][4]
+
+
 def test_runs_are_bit_reproducible_with_and_without_dependent_launch(G):
     """No result depends on the order in which blocks or atomics happen to run: two runs of the same steps, and a run with
     programmatic dependent launch switched off (GENGA_NO_PDL=1, read at genga_create), give bit-identical states."""
