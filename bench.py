@@ -126,11 +126,17 @@ def lib_evals(w):
     return maps if (w["mode"] == 0 and w["n_massive"] > 32) else maps + 1
 
 
+def timed_chunk(w):
+    """steps per timed call: 1, except where the library runs all the steps of a call in ONE launch (multi-system mode and
+    massive mode with N <= 16, multi_persist.cuh): there a timed call is 16 steps, L2 flushed between the calls"""
+    return 16 if (w["mode"] == 2 or (w["mode"] == 0 and w["n_massive"] <= 16)) else 1
+
+
 def config_dict(w, name, evals, world=1):
     """the `config` object of the JSON line: the benchmark configuration, the same object on both arms"""
     evals = lib_evals(w)
     return {"workload": name, "n_massive": w["n_massive"], "order": w["order"], "dt_days": w["dt"] / workloads.DAY,
-            "force_evals_per_step": evals, "steps_per_timed_call": 16 if w["mode"] == 2 else 1,
+            "force_evals_per_step": evals, "steps_per_timed_call": timed_chunk(w),
             "l2": "flushed (512 MiB fill) before every timed step",
             "parallelism": ("1 gpu" if world == 1 else "replicas only" if w["mode"] == 0 else
                             "particles sharded, massive bodies replicated, no collective" if w["mode"] == 1
@@ -216,10 +222,8 @@ def measure(torch, G, dev, cfg_id, order, steps, warmup, rank, world, clocks=Non
     assert g.status() == 0
     c0 = g.counters()
 
-    # ---- timed: K steps, timed with events on the library's stream, L2 flushed between the timed calls.  A timed call is
-    # one step; in multi-system mode 16 steps, because there all the steps of a call run in ONE launch in which every
-    # block runs its own systems ahead (a call of one step would time the per-operator pipeline instead)
-    chunk = 16 if w["mode"] == 2 else 1
+    # ---- timed: K steps, timed with events on the library's stream, L2 flushed between the timed calls (timed_chunk)
+    chunk = timed_chunk(w)
     steps = max(chunk, steps // chunk * chunk)
     barrier()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps // chunk)]

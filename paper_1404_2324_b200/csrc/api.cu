@@ -587,7 +587,7 @@ extern "C" __attribute__((visibility("default"))) int genga_step(genga_ctx *c, i
     if (!c || n_steps < 0 || dt == 0.0 || !(dt == dt) || (order != 2 && order != 4 && order != 6)) return GENGA_EINVAL;
     if (n_steps == 0) return GENGA_OK;
     const bool reused_first = c->far_valid;
-    if (c->d.mode == GENGA_MODE_MULTI_SYSTEM && n_steps >= 4 && !c->d.coll && c->d.rcut2 == 0.0 && c->d.rcutsun2 == 0.0 && c->d.nmin == 0 && !(c->cfg.flags & 5)) {
+    if ((c->d.mode == GENGA_MODE_MULTI_SYSTEM || (c->d.mode == GENGA_MODE_MASSIVE && c->d.nm <= MP_LANES)) && n_steps >= 4 && !c->d.coll && c->d.rcut2 == 0.0 && c->d.rcutsun2 == 0.0 && c->d.nmin == 0 && !(c->cfg.flags & 5)) {
         // systems never interact: all the steps of this call (4 or more) in one launch, every block runs its own systems ahead
         // (multi_persist.cuh); collisions / ejections and flags bit 2 keep the per-operator pipeline below
         int64_t left = n_steps;

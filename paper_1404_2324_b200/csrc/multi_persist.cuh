@@ -1,4 +1,5 @@
-// Multi-system mode: ALL the steps of a genga_step call in ONE launch, no grid-wide barrier.
+// Multi-system mode, and massive mode with N <= 16 (one system: the paper's small-N regime, L427-433,
+// where a step is launch latency): ALL the steps of a genga_step call in ONE launch, no grid-wide barrier.
 //
 // Systems never interact.  The launch-per-operator pipeline nevertheless made all 4096 systems of config 3 wait, in
 // every map, for the one system that happened to be in a deep encounter (its Bulirsch-Stoer chain: ~45 us of a 110 us
@@ -73,7 +74,8 @@ __global__ void __launch_bounds__(MP_THREADS) k_multi_persist(DevState d, double
     double x = 1e30 * (1 + t), y = 0.0, z = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, m = 0.0, m0 = 1.0, n1 = 0.0, n2 = 0.0, rc = 0.0;
     if (live) {
         x = d.x[i]; y = d.y[i]; z = d.z[i]; vx = d.vx[i]; vy = d.vy[i]; vz = d.vz[i]; m = d.m[i];
-        m0 = d.m0[sys]; n1 = d.n12[2 * sys]; n2 = d.n12[2 * sys + 1];
+        m0 = d.m0[sys];
+        n1 = d.n12 ? d.n12[2 * sys] : d.n1; n2 = d.n12 ? d.n12[2 * sys + 1] : d.n2;      // per system (L346-354) / the one system of massive mode
     }
     S.m[t] = m; S.gm[t] = d.G * m;
     const double mu = d.G * m0;
