@@ -56,6 +56,7 @@ struct genga_ctx {
     std::map<GraphKey, GraphEntry> graphs;
     long long steps, force_evals, interactions, launches;
     long long acc;              // launches enqueued (or captured) since last reset
+    double tp_pending;          // mode 1, while enqueueing: size of the map whose closing half of the particles is still to come (0: none)
     bool far_valid;             // the stored hit masks / far sums of the last closing kick belong to the current positions (S2')
     // genga_profile_step: events at the phase boundaries of plain (uncaptured) launches
     bool prof;
@@ -116,7 +117,8 @@ static size_t carve(const genga_config *c, char *base, DevState *d, int **exp_la
     t.m0 = (double *)take(sizeof(double) * nsys);
     double **arrs2[] = {&t.vx, &t.vy, &t.vz, &t.rc, &t.c9, &t.x0, &t.y0, &t.z0};
     for (auto a : arrs2) *a = (double *)take(sizeof(double) * np);
-    t.psum = (double *)take(sizeof(double) * 4 * nsys);
+    t.psum = (double *)take(sizeof(double) * 8 * nsys);
+    if (c->mode == GENGA_MODE_TEST_PARTICLE) t.rcprev = (double *)take(sizeof(double) * 32);
     *eout = (double *)take(sizeof(double) * 4 * nsys);
     if (c->mode != GENGA_MODE_MULTI_SYSTEM) {
         t.gstart = (int *)take(sizeof(int) * npm);
@@ -208,7 +210,7 @@ extern "C" __attribute__((visibility("default"))) int genga_create(const genga_c
     c->bs_big_clusters = std::max(1, c->sms / BCB_CS);
     c->steps = c->force_evals = c->interactions = c->launches = 0;
     c->acc = 0;
-    c->prof = false; c->prof_used = 0; c->far_valid = false;
+    c->prof = false; c->prof_used = 0; c->far_valid = false; c->tp_pending = 0.0;
     c->hstage = nullptr; c->hstatus = nullptr; c->ev_stage = nullptr; c->stage_busy = false;
     size_t need = carve(cfg, (char *)cfg->workspace, &c->d, &c->exp_labels, &c->eout, c->sms);
     if (need > cfg->workspace_bytes) { delete c; return GENGA_EINVAL; }
@@ -423,7 +425,7 @@ static cudaError_t launch_bs_cluster(cudaStream_t st, int clusters, const DevSta
 // scheme "applied to each of the substeps"; flags bit 0 keeps them apart).
 static inline bool tiny_mode(const DevState &d) { return d.mode == GENGA_MODE_MASSIVE && d.nm <= 32; }
 
-static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last, double hn, bool opened, bool reuse)
+static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last, double hn, bool opened, bool reuse, bool final_map)
 {
     DevState &d = c->d;
     cudaStream_t st = c->st;
@@ -437,9 +439,12 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
     }
     if (tp) {
         // particles: kick, Sun kick and drift in one pass (k_tp_front); the massive bodies as in mode 0
-        launch_k(c->pdl, k_tpm_kick, 1, 32, 0, st, d, 0.5 * h, 1, 0.0); LAUNCH(c);           // kick + momentum sum, one warp
+        launch_k(c->pdl, k_tpm_kick, 1, 32, 0, st, d, 0.5 * h, 1, 0.0, 0); LAUNCH(c);        // kick + momentum sum, one warp
         launch_k(c->pdl, k_drift, nblk(d.nm, 128), 128, 0, st, dm, h, 0.5 * h); LAUNCH(c);   // Sun kick + drift of the massive bodies
-        launch_k(c->pdl, k_tp_front, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h, tau, first); LAUNCH(c);   // the particles, encounter search included
+        // the particles, encounter search included; the closing half of the map before, if it was put off, in the same pass
+        if (c->tp_pending != 0.0) { launch_k(c->pdl, k_tp_mid, nblk(d.ntot - d.nm, 128), 128, 0, st, d, c->tp_pending, h, tau, first); LAUNCH(c); }
+        else { launch_k(c->pdl, k_tp_front, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h, tau, first); LAUNCH(c); }
+        c->tp_pending = 0.0;
     } else if (tiny_mode(d)) {                                // N <= 32: the opening half map in one warp, one launch
         launch_k(c->pdl, k_tiny_front, 1, 32, 0, st, d, h, tau, first, opened ? 0.0 : 0.5 * h); LAUNCH(c);
     } else if (d.mode == GENGA_MODE_MULTI_SYSTEM) {           // a block holds whole systems: the opening half map in one launch
@@ -497,8 +502,11 @@ static void enqueue_map(genga_ctx *c, double h, double tau, int first, int last,
     }
     mark(c, PH_BACK);
     if (tp) {
-        launch_k(false, k_tpm_kick, 1, 32, 0, st, d, 0.5 * h, 0, 0.5 * h); LAUNCH(c);       // momentum sum, Sun kick, kick of the massive bodies; plain: see enqueue_sun
-        launch_k(c->pdl, k_tp_back, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h); LAUNCH(c);
+        launch_k(false, k_tpm_kick, 1, 32, 0, st, d, 0.5 * h, 0, 0.5 * h, 1); LAUNCH(c);    // momentum sum, Sun kick, kick of the massive bodies; plain: see enqueue_sun
+        // the particles' closing half: with the opening half of the next map in one pass (k_tp_mid), unless this is the last
+        // map this call (or graph) holds
+        if (final_map || d.coll || d.rcut2 > 0.0 || d.rcutsun2 > 0.0 || d.nmin > 0) { launch_k(c->pdl, k_tp_back, nblk(d.ntot - d.nm, 128), 128, 0, st, d, h); LAUNCH(c); }
+        else c->tp_pending = h;
     } else if (tiny_mode(d)) {                                // plain launch: see enqueue_sun
         launch_k(false, k_tiny_back, 1, 32, 0, st, d, h, hn != 0.0 ? 0.5 * (h + hn) : 0.5 * h, hn != 0.0 ? 1 : 0, last ? 0 : 1); LAUNCH(c);
     } else if (d.mode == GENGA_MODE_MULTI_SYSTEM && last) {   // no counter reset after the last map: Sun kick and kick in one launch (plain: see enqueue_sun)
@@ -525,7 +533,7 @@ static long long evals_of(const genga_ctx *c, int order, long long n_steps, bool
 }
 
 // reuse: the positions are those of the previous step's closing kick and its hit masks are stored (S2', L266-274)
-static void enqueue_step(genga_ctx *c, double dt, int order, bool reuse)
+static void enqueue_step(genga_ctx *c, double dt, int order, bool reuse, bool final_step)
 {
     DevState &d = c->d;
     double w[7];
@@ -542,7 +550,7 @@ static void enqueue_step(genga_ctx *c, double dt, int order, bool reuse)
     }
     const bool merge = !(c->cfg.flags & 1) && d.mode != GENGA_MODE_TEST_PARTICLE;
     for (int k = 0; k < nw; ++k)
-        enqueue_map(c, w[k] * dt, dt, k == 0, k == nw - 1, merge && k + 1 < nw ? w[k + 1] * dt : 0.0, merge && k > 0, reuse && k == 0);
+        enqueue_map(c, w[k] * dt, dt, k == 0, k == nw - 1, merge && k + 1 < nw ? w[k + 1] * dt : 0.0, merge && k > 0, reuse && k == 0, final_step && k == nw - 1);
     if (d.coll || d.rcut2 > 0.0 || d.rcutsun2 > 0.0 || d.nmin > 0) {      // ejections, stop of a system, step counter of the events
         k_end_step<<<nblk(d.mode == GENGA_MODE_MULTI_SYSTEM ? d.nsys : d.ntot, 128), 128, 0, c->st>>>(d); LAUNCH(c);
         k_end_step2<<<1, 256, 0, c->st>>>(d); LAUNCH(c);
@@ -565,7 +573,7 @@ static int get_graph(genga_ctx *c, double dt, int order, int nsteps, bool reuse,
         cudaGraph_t g;
         CK(cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal));
         c->acc = 0;
-        for (int s = 0; s < nsteps; ++s) enqueue_step(c, dt, order, s > 0 || reuse);
+        for (int s = 0; s < nsteps; ++s) enqueue_step(c, dt, order, s > 0 || reuse, s == nsteps - 1);
         long long n = c->acc;
         c->acc = 0;
         CK(cudaStreamEndCapture(c->st, &g));
@@ -607,7 +615,7 @@ extern "C" __attribute__((visibility("default"))) int genga_step(genga_ctx *c, i
     }
     if (c->st == nullptr) {                       // legacy stream cannot be captured: plain launches
         c->acc = 0;
-        for (int64_t s = 0; s < n_steps; ++s) enqueue_step(c, dt, order, s > 0 || c->far_valid);
+        for (int64_t s = 0; s < n_steps; ++s) enqueue_step(c, dt, order, s > 0 || c->far_valid, s == n_steps - 1);
         c->launches += c->acc; c->acc = 0;
     } else {
         const int chunk = 16;
@@ -640,7 +648,7 @@ extern "C" __attribute__((visibility("default"))) int genga_profile_step(genga_c
     if (!c || !ms || n_steps < 1 || n_steps > 4096 || dt == 0.0 || !(dt == dt) || (order != 2 && order != 4 && order != 6)) return GENGA_EINVAL;
     const bool reused_first = c->far_valid;
     c->prof = true; c->prof_used = 0; c->acc = 0;
-    for (int64_t s = 0; s < n_steps; ++s) enqueue_step(c, dt, order, s > 0 || c->far_valid);
+    for (int64_t s = 0; s < n_steps; ++s) enqueue_step(c, dt, order, s > 0 || c->far_valid, s == n_steps - 1);
     c->prof = false;
     c->far_valid = true;
     c->launches += c->acc; c->acc = 0;

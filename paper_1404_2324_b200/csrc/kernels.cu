@@ -96,6 +96,7 @@ __global__ void k_rcrit(DevState d, double tau, int reset, int check)
     // S2': the hit masks of the previous closing kick cover r < 3.3 rc_old; they serve the coming opening kick only if
     // 3 rc_new <= 3.3 rc_old for every body
     if (check && rc > KK_GROW * d.rc[i]) d.cnt[CI_S2PMISS] = 1;
+    if (d.rcprev && i < d.nm) d.rcprev[i] = d.rc[i];           // mode 1: the particles' closing kick of the step that ends (k_tp_mid)
     d.rc[i] = rc;
     d.c9[i] = 9.0 * rc * rc;
     if (d.hcw && i < d.nm) d.hcw[i] = __double2hiint(KK_WIDE2 * rc * rc);
@@ -514,6 +515,46 @@ __device__ __forceinline__ unsigned tp_accel(const DevState &d, const TpMassive 
 // Hermite minimum (Eq. 10-12) right here, from registers and shared memory: no candidate list, no gather, and the state
 // before the drift is stored only for the few particles that do have an encounter.
 struct TpMassive2 { double x1[32], y1[32], z1[32], vx0[32], vy0[32], vz0[32], vx1[32], vy1[32], vz1[32]; };
+// Kepler drift of a particle, then its candidates tested by the Hermite minimum (Eq. 10-12) from registers and shared
+// memory; the particle's state is written, the state before the drift only if it has an encounter.
+__device__ __forceinline__ void tp_drift_confirm(const DevState &d, const TpMassive &M, const TpMassive2 &M2, const int i, const bool live,
+                                                 const double h, const unsigned cmask, const double rci,
+                                                 double x, double y, double z, double vx, double vy, double vz)
+{
+    const double x0 = x, y0 = y, z0 = z, vx0 = vx, vy0 = vy, vz0 = vz;
+    if (live && !kepler_drift(d.G * d.m0[0], h, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
+    // candidates of this warp: one atomic
+    {
+        int nc = __popc(cmask);
+        for (int o = 16; o > 0; o >>= 1) nc += __shfl_xor_sync(0xffffffffu, nc, o);
+        if ((threadIdx.x & 31) == 0 && nc) atomicAdd(&d.cnt[CI_NCAND_TP], nc);
+    }
+    if (!live) return;
+    unsigned emask = 0u;
+    for (unsigned cm = cmask; cm; cm &= cm - 1) {
+        const int j = __ffs(cm) - 1;
+        double dx = x0 - M.x[j], dy = y0 - M.y[j], dz = z0 - M.z[j];
+        double dvx = vx0 - M2.vx0[j], dvy = vy0 - M2.vy0[j], dvz = vz0 - M2.vz0[j];
+        const double P0 = dx * dx + dy * dy + dz * dz, Pd0 = 2.0 * (dx * dvx + dy * dvy + dz * dvz);
+        dx = x - M2.x1[j]; dy = y - M2.y1[j]; dz = z - M2.z1[j];
+        dvx = vx - M2.vx1[j]; dvy = vy - M2.vy1[j]; dvz = vz - M2.vz1[j];
+        const double P1 = dx * dx + dy * dy + dz * dz, Pd1 = 2.0 * (dx * dvx + dy * dvy + dz * dvz);
+        const double rcij = fmax(rci, M.rc[j]);
+        // a rigorous lower bound of the interpolant first (bs.cuh pair_collides): most candidates sit between rc and 3 rc
+        if (pair_collides(P0, P1, Pd0, Pd1, h, rcij)) {
+            emask |= 1u << j;
+            const int idx = atomicAdd(&d.cnt[CI_NENC], 1);
+            if (idx < d.cap) d.enc[idx] = make_int2(j, i);
+            else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+        }
+    }
+    if (emask) {                                                // Bulirsch-Stoer needs the state before the drift
+        d.x0[i] = x0; d.y0[i] = y0; d.z0[i] = z0; d.vx0[i] = vx0; d.vy0[i] = vy0; d.vz0[i] = vz0;
+        d.tpmask[i - d.nm] = emask;
+        d.tplist[atomicAdd(&d.cnt[CI_NTP], 1)] = i;
+    }
+    d.x[i] = x; d.y[i] = y; d.z[i] = z; d.vx[i] = vx; d.vy[i] = vy; d.vz[i] = vz;
+}
 __global__ void __launch_bounds__(128) k_tp_front(DevState d, double h, double tau, int first)
 {
     pdl_sync();
@@ -543,38 +584,69 @@ __global__ void __launch_bounds__(128) k_tp_front(DevState d, double h, double t
     double ax, ay, az;
     const unsigned cmask = live ? tp_accel(d, M, x, y, z, rci, ax, ay, az) : 0u;
     if (live) { vx = fma(hh, ax, vx); vy = fma(hh, ay, vy); vz = fma(hh, az, vz); }
-    const double x0 = x, y0 = y, z0 = z, vx0 = vx, vy0 = vy, vz0 = vz;
-    if (live && !kepler_drift(d.G * d.m0[0], h, x, y, z, vx, vy, vz)) atomicOr(&d.cnt[CI_STATUS], ERRBIT_KEPLER);
-    // candidates of this warp: one atomic
-    {
-        int nc = __popc(cmask);
-        for (int o = 16; o > 0; o >>= 1) nc += __shfl_xor_sync(0xffffffffu, nc, o);
-        if ((threadIdx.x & 31) == 0 && nc) atomicAdd(&d.cnt[CI_NCAND_TP], nc);
+    tp_drift_confirm(d, M, M2, i, live, h, cmask, rci, x, y, z, vx, vy, vz);
+}
+// Closing half of a map and opening half of the next one in ONE pass over the particle (the positions are the same):
+//   C(hA/2) B(hA/2) | [new step: rc_i = n2 |tau| |V_i|] B(hB/2) C(hB/2) A(hB) + encounter search.
+// The massive bodies have already gone through the same (k_tpm_kick closing, k_rcrit, k_tpm_kick opening, k_drift): x0..
+// hold them after BOTH Sun kicks, so the particle takes both shifts first and kicks against x0 (B and C commute, R-11);
+// psum + 4 = sum m V of the closing Sun kick, psum = of the opening one; rcprev = the massive bodies' critical radii of
+// the step that ends (newstep).  Within a step (newstep = 0) the two kicks have the same weights: one evaluation.
+__global__ void __launch_bounds__(128) k_tp_mid(DevState d, double hA, double hB, double tau, int newstep)
+{
+    pdl_sync();
+    __shared__ TpMassive M;
+    __shared__ TpMassive2 M2;
+    __shared__ double rcold[32];
+    __shared__ int hcold[32];
+    const int i = d.nm + blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = i < d.ntot;
+    double x = 0.0, y = 0.0, z = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, rci = 0.0;
+    if (live) { x = d.x[i]; y = d.y[i]; z = d.z[i]; vx = d.vx[i]; vy = d.vy[i]; vz = d.vz[i]; rci = d.rc[i]; }
+    if (threadIdx.x < d.nm) {
+        const int j = threadIdx.x;
+        M2.x1[j] = d.x[j]; M2.y1[j] = d.y[j]; M2.z1[j] = d.z[j];
+        M2.vx0[j] = d.vx0[j]; M2.vy0[j] = d.vy0[j]; M2.vz0[j] = d.vz0[j];
+        M2.vx1[j] = d.vx[j]; M2.vy1[j] = d.vy[j]; M2.vz1[j] = d.vz[j];
+        const double ro = newstep ? d.rcprev[j] : d.rc[j];
+        rcold[j] = ro; hcold[j] = __double2hiint(9.0 * ro * ro);
     }
-    if (!live) return;
-    unsigned emask = 0u;
-    for (unsigned cm = cmask; cm; cm &= cm - 1) {
-        const int j = __ffs(cm) - 1;
-        double dx = x0 - M.x[j], dy = y0 - M.y[j], dz = z0 - M.z[j];
-        double dvx = vx0 - M2.vx0[j], dvy = vy0 - M2.vy0[j], dvz = vz0 - M2.vz0[j];
-        const double P0 = dx * dx + dy * dy + dz * dz, Pd0 = 2.0 * (dx * dvx + dy * dvy + dz * dvz);
-        dx = x - M2.x1[j]; dy = y - M2.y1[j]; dz = z - M2.z1[j];
-        dvx = vx - M2.vx1[j]; dvy = vy - M2.vy1[j]; dvz = vz - M2.vz1[j];
-        const double P1 = dx * dx + dy * dy + dz * dz, Pd1 = 2.0 * (dx * dvx + dy * dvy + dz * dvz);
-        const double rcij = fmax(rci, M.rc[j]);
-        if (hermite_min(P0, P1, Pd0, Pd1, h) < rcij * rcij) {
-            emask |= 1u << j;
-            const int idx = atomicAdd(&d.cnt[CI_NENC], 1);
-            if (idx < d.cap) d.enc[idx] = make_int2(j, i);
-            else atomicOr(&d.cnt[CI_STATUS], ERRBIT_CAPACITY);
+    tp_load_massive(d, M, d.x0, d.y0, d.z0);
+    const double gA = 0.5 * hA / d.m0[0], gB = 0.5 * hB / d.m0[0];
+    x = fma(gA, d.psum[4], x); y = fma(gA, d.psum[5], y); z = fma(gA, d.psum[6], z);
+    x = fma(gB, d.psum[0], x); y = fma(gB, d.psum[1], y); z = fma(gB, d.psum[2], z);
+    double ax, ay, az;
+    unsigned cmask = 0u;
+    if (newstep) {
+        // closing kick with the critical radii of the step that ends
+        if (live) {
+            ax = ay = az = 0.0;
+            const int hci = __double2hiint(9.0 * rci * rci);
+            for (int j = 0; j < d.nm; ++j) {
+                double dx = M.x[j] - x, dy = M.y[j] - y, dz = M.z[j] - z;
+                double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                double s3 = M.gm[j] * rinv3_fast(r2);
+                if (__double2hiint(r2) <= max(hci, hcold[j])) {
+                    const double rcij = fmax(rci, rcold[j]);
+                    if (r2 < rcij * rcij) {
+                        double r = sqrt(r2);
+                        s3 = M.gm[j] / (r2 * r) * kick_weight(r, rcij);
+                    }
+                }
+                ax = fma(s3, dx, ax); ay = fma(s3, dy, ay); az = fma(s3, dz, az);
+            }
+            vx = fma(0.5 * hA, ax, vx); vy = fma(0.5 * hA, ay, vy); vz = fma(0.5 * hA, az, vz);
+            rci = fmax(d.n1 * 0.0, d.n2 * fabs(tau) * sqrt(vx * vx + vy * vy + vz * vz));
+            d.rc[i] = rci;
+            cmask = tp_accel(d, M, x, y, z, rci, ax, ay, az);
+            vx = fma(0.5 * hB, ax, vx); vy = fma(0.5 * hB, ay, vy); vz = fma(0.5 * hB, az, vz);
         }
+    } else if (live) {
+        cmask = tp_accel(d, M, x, y, z, rci, ax, ay, az);
+        vx = fma(0.5 * hA, ax, vx); vy = fma(0.5 * hA, ay, vy); vz = fma(0.5 * hA, az, vz);     // two kicks, as k_tp_back and k_tp_front apply them
+        vx = fma(0.5 * hB, ax, vx); vy = fma(0.5 * hB, ay, vy); vz = fma(0.5 * hB, az, vz);
     }
-    if (emask) {                                                // Bulirsch-Stoer needs the state before the drift
-        d.x0[i] = x0; d.y0[i] = y0; d.z0[i] = z0; d.vx0[i] = vx0; d.vy0[i] = vy0; d.vz0[i] = vz0;
-        d.tpmask[i - d.nm] = emask;
-        d.tplist[atomicAdd(&d.cnt[CI_NTP], 1)] = i;
-    }
-    d.x[i] = x; d.y[i] = y; d.z[i] = z; d.vx[i] = vx; d.vy[i] = vy; d.vz[i] = vz;
+    tp_drift_confirm(d, M, M2, i, live, hB, cmask, rci, x, y, z, vx, vy, vz);
 }
 __global__ void __launch_bounds__(128) k_tp_back(DevState d, double h)
 {
@@ -587,7 +659,7 @@ __global__ void __launch_bounds__(128) k_tp_back(DevState d, double h)
     tp_load_massive(d, M, d.x, d.y, d.z);
     if (!live) return;
     const double hh = 0.5 * h, g = hh / d.m0[0];
-    x = fma(g, d.psum[0], x); y = fma(g, d.psum[1], y); z = fma(g, d.psum[2], z);
+    x = fma(g, d.psum[4], x); y = fma(g, d.psum[5], y); z = fma(g, d.psum[6], z);      // the closing k_tpm_kick's sum
     double ax, ay, az;
     tp_accel(d, M, x, y, z, rci, ax, ay, az);
     d.x[i] = x; d.y[i] = y; d.z[i] = z;
@@ -644,7 +716,7 @@ __global__ void __launch_bounds__(128) k_kick_multi(DevState d, double h, int re
 // warp (body = lane).  fshift == 0, opening half: kick, then s = sum m V for the particles' and the massive bodies' Sun kick
 // (k_tp_front, k_drift).  fshift != 0, closing half: s from the velocities as they are, q += fshift s / m0, then the kick at
 // the shifted positions.  Same pair arithmetic as k_kick_multi, same sum order as k_momentum with 32 threads.
-__global__ void __launch_bounds__(32) k_tpm_kick(DevState d, double h, int record, double fshift)
+__global__ void __launch_bounds__(32) k_tpm_kick(DevState d, double h, int record, double fshift, int slot)
 {
     pdl_sync();
     __shared__ double sx[32], sy[32], sz[32], sgm[32], src[32];
@@ -662,7 +734,7 @@ __global__ void __launch_bounds__(32) k_tpm_kick(DevState d, double h, int recor
             s0 += __shfl_xor_sync(0xffffffffu, s0, o); s1 += __shfl_xor_sync(0xffffffffu, s1, o);
             s2 += __shfl_xor_sync(0xffffffffu, s2, o); s3 += __shfl_xor_sync(0xffffffffu, s3, o);
         }
-        if (t == 0) { d.psum[0] = s0; d.psum[1] = s1; d.psum[2] = s2; d.psum[3] = s3; }
+        if (t == 0) { d.psum[4 * slot] = s0; d.psum[4 * slot + 1] = s1; d.psum[4 * slot + 2] = s2; d.psum[4 * slot + 3] = s3; }
     };
     if (fshift != 0.0) {
         double s0, s1, s2;

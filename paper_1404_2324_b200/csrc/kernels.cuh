@@ -36,7 +36,8 @@ __global__ void k_multi_back(DevState d, double h, double hk);
 __global__ void k_coord_map(DevState d, const double *ix, const double *iy, const double *iz, double *ox, double *oy, double *oz, double f, int divide_by_total);
 __global__ void k_tiny_front(DevState d, double h, double tau, int first, double hk);
 __global__ void k_tiny_back(DevState d, double h, double hk, int record, int reset);
-__global__ void k_tpm_kick(DevState d, double h, int record, double fshift);
+__global__ void k_tpm_kick(DevState d, double h, int record, double fshift, int slot);
+__global__ void k_tp_mid(DevState d, double hA, double hB, double tau, int newstep);
 __global__ void k_momentum(DevState d, const double *vx, const double *vy, const double *vz, double fshift);
 __global__ void k_shift(DevState d, double *ax, double *ay, double *az, double f, int divide_by_total);
 __global__ void k_drift(DevState d, double h, double hsun);

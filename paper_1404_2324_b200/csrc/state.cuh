@@ -20,7 +20,8 @@ struct DevState {
     double *rc, *c9;             // critical radius, 9 rc^2 (precheck threshold squared, L142)
     double *x0, *y0, *z0, *vx0, *vy0, *vz0;   // state before the drift (Eq. 10 needs both ends)
     int npm;         // nm padded to 128
-    double *psum;    // [nsys][4]: sum m V (x,y,z) of the massive bodies, and sum m
+    double *psum;    // [nsys][4]: sum m V (x,y,z) of the massive bodies, and sum m; mode 1: [2][4], slot 1 = the closing Sun kick's
+    double *rcprev;  // mode 1: critical radii of the massive bodies in the step before (k_tp_mid)
     int2 *cand, *enc;
     long long cap;
     int *cnt;        // device ints: see CI_* below
