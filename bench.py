@@ -339,20 +339,27 @@ def measure(torch, G, dev, cfg_id, order, steps, warmup, rank, world, clocks=Non
             roof["note"] = ("N <= 32: the step runs k_tiny_front / k_tiny_back (one warp per half map) and is launch-latency "
                             "bound; k_kick and k_drift are timed alone here for reference only")
     elif w["mode"] == 1:
-        # dominant kernels: the fused particle passes.  SURVEY 8(d): 96 algorithmic bytes per particle per STEP
+        # dominant kernel: k_tp_mid, ONE pass over the particle per step (closing half, opening half, drift, encounter search).
+        # It is bound by FP64 issue, as SURVEY 8(d) predicts for a fused particle step; both rooflines are reported.
         nt = w["n_test"]
-        front_ms = g.time_kernel(3, 100, dt)
-        back_ms = g.time_kernel(4, 100, dt)
-        fb = 104.0 * nt
+        mid_ms = g.time_kernel(5, 50, dt)
+        front_ms = g.time_kernel(3, 50, dt)
+        back_ms = g.time_kernel(4, 50, dt)
         step_ms = 1e3 * elapsed / steps
-        roof = {"bound": "hbm", "kernel": "k_tp_back", "achieved": fb / (back_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "frac": fb / (back_ms * 1e-3) / 1e9 / hbm_peak, "traffic": tab.get("k_tp_back"),
-                "peak_source": hbm_src, "ms_per_launch": back_ms, "algorithmic_bytes_per_launch": fb,
-                "front": {"kernel": "k_tp_front", "ms_per_launch": front_ms, "algorithmic_bytes_per_launch": fb,
-                          "gbs": fb / (front_ms * 1e-3) / 1e9, "frac_hbm": fb / (front_ms * 1e-3) / 1e9 / hbm_peak,
-                          "traffic": tab.get("k_tp_front"),
-                          "note": "kick by %d massive bodies + Kepler solve: FP64-issue bound (DESIGN.md section 6)" % w["n_massive"],
-                          "fp64_peak_tflops": peak_probe},
+        FP64_PER_PARTICLE = 528.0          # FP64 instructions per particle of k_tp_mid (profiles/r2_ncu_full_cfg2_cfg3.md: pipe cycles / 2)
+        ach = 2.0 * FP64_PER_PARTICLE * nt / (mid_ms * 1e-3) / 1e12
+        roof = {"bound": "alu", "kernel": "k_tp_mid", "achieved": ach, "peak": peak_probe, "unit": "TFLOP/s",
+                "frac": ach / peak_probe, "traffic": tab.get("k_tp_mid"),
+                "peak_source": "DFMA probe measured in this run (genga_fp64_probe)",
+                "ms_per_launch": mid_ms, "fp64_instructions_per_particle": FP64_PER_PARTICLE,
+                "convention": "achieved = 2 flop x FP64 instructions the kernel issues (528 per particle by ncu's pipe cycles) / time: the share of the FP64 issue slots",
+                "hbm": {"algorithmic_bytes_per_launch": 112.0 * nt, "gbs": 112.0 * nt / (mid_ms * 1e-3) / 1e9, "peak": hbm_peak,
+                        "frac": 112.0 * nt / (mid_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src,
+                        "note": "56 B read + 56 B written per particle (state + rc); not the binding roofline"},
+                "front": {"kernel": "k_tp_front", "ms_per_launch": front_ms, "note": "first map of a call"},
+                "back": {"kernel": "k_tp_back", "ms_per_launch": back_ms, "algorithmic_bytes_per_launch": 104.0 * nt,
+                         "gbs": 104.0 * nt / (back_ms * 1e-3) / 1e9, "frac_hbm": 104.0 * nt / (back_ms * 1e-3) / 1e9 / hbm_peak,
+                         "traffic": tab.get("k_tp_back"), "note": "last map of a call: the HBM-bound one"},
                 # the step as a whole against SURVEY 8(d)'s unit
                 "step": {"algorithmic_bytes_per_step": 96.0 * nt, "unit": "96 B per particle per step",
                          "gbs": 96.0 * nt / (step_ms * 1e-3) / 1e9, "frac_hbm": 96.0 * nt / (step_ms * 1e-3) / 1e9 / hbm_peak,
@@ -374,6 +381,9 @@ def measure(torch, G, dev, cfg_id, order, steps, warmup, rank, world, clocks=Non
     res_max, res_units = reduce_max_and_sum(resident_s, per_step * nres, dev)
     line = {
         "metric": METRIC, "value": units / tmax, "unit": UNIT, "n_gpus": world, "steps": steps,
+        "value_note": "pair interactions EVALUATED per second (force evaluations counted by the library: one per second-order step in "
+                      "massive mode, the opening kick comes from stored sums, PAPER.md L266-274); round 1 counted two per step",
+        "interactions_applied_per_s": units / tmax * ({2: 2, 4: 4, 6: 8}[w["order"]] / evals if w["mode"] != 1 and evals else 1.0),
         "warmup": max(warmup, 3), "ms_per_step": 1e3 * tmax / steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": config_dict(w, name, evals, world),

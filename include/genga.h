@@ -218,6 +218,7 @@ int genga_counters(genga_ctx *ctx, int64_t *out);
  *   which = 2  the whole kick (k_kick [+ k_tp_kick of the test particles]), h = 0
  *   which = 3  mode 1: fused particle pass kick + Sun kick + drift (k_tp_front) over dt and back
  *   which = 4  mode 1: fused particle pass Sun kick + kick (k_tp_back) over dt and back
+ *   which = 5  mode 1: closing half + opening half + drift + encounter search in one pass (k_tp_mid) over dt and back
  * The state is left unchanged up to rounding (3, 4: up to the integration error of the
  * pass and its inverse).  Synchronises. */
 int genga_time_kernel(genga_ctx *ctx, int which, int reps, double dt, double *ms_per_launch);

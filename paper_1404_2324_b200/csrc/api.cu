@@ -293,9 +293,7 @@ static void enqueue_helio_to_demo(genga_ctx *c)
 {
     DevState &d = c->d;
     c->far_valid = false;                                     // new positions: the stored hit masks are void
-    k_init_bodies<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d);   // kinds, spins, internal energy, event list: a new run
-    c->launches += 1;
-    k_coord_map<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx0, d.vy0, d.vz0, d.vx, d.vy, d.vz, -1.0, 1);
+    k_coord_map<<<nblk(std::max(d.ntot, d.nsys), 256), 256, 0, c->st>>>(d, d.vx0, d.vy0, d.vz0, d.vx, d.vy, d.vz, -1.0, 1, 1);   // + kinds, spins, U, event list: a new run
     c->launches += 1;
 }
 
@@ -545,8 +543,8 @@ static void enqueue_step(genga_ctx *c, double dt, int order, bool reuse, bool fi
         dm.ntot = d.nm;
         launch_k(c->pdl, k_rcrit, 1, 128, 0, c->st, dm, dt, 2, 0); LAUNCH(c);    // nm <= 32: one block, which also opens the first map
     } else if (!tiny_mode(d)) {                                   // N <= 32: inside k_tiny_front of the first map
-        launch_k(c->pdl, k_rcrit, nblk(d.ntot, 128), 128, 0, c->st, d, dt, d.mode != GENGA_MODE_TEST_PARTICLE, reuse ? 1 : 0); LAUNCH(c);
-        if (d.kb && !reuse) { launch_k(c->pdl, k_pack_kb, nblk(d.npm, 128), 128, 0, c->st, d); LAUNCH(c); }   // a state that did not come out of a step
+        // check: 1 = the stored hit masks are about to be reused (S2'), 2 = a state that did not come out of a step: pack the kick's j-tile
+        launch_k(c->pdl, k_rcrit, nblk(std::max(d.ntot, d.kb ? d.npm : 0), 128), 128, 0, c->st, d, dt, d.mode != GENGA_MODE_TEST_PARTICLE, reuse ? 1 : 2); LAUNCH(c);
     }
     const bool merge = !(c->cfg.flags & 1) && d.mode != GENGA_MODE_TEST_PARTICLE;
     for (int k = 0; k < nw; ++k)
@@ -695,7 +693,7 @@ static int get_state_impl(genga_ctx *c, double *x, double *v, cudaMemcpyKind kin
     if (!c || !x || !v) return GENGA_EINVAL;
     DevState &d = c->d;
     const size_t n = (size_t)d.ntot, B = sizeof(double);
-    k_coord_map<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0);
+    k_coord_map<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0, 0);
     c->launches += 1;
     const double *src[6] = {d.x, d.y, d.z, d.vx0, d.vy0, d.vz0};
     if ((size_t)d.np == n) {
@@ -719,7 +717,7 @@ extern "C" __attribute__((visibility("default"))) int genga_get_state_host(genga
     if (c && c->hstage && x && v) {                            // small state: one copy, unpack after the latch's sync
         DevState &d = c->d;
         const size_t n = (size_t)d.ntot, np = (size_t)d.np, B = sizeof(double);
-        k_coord_map<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0);
+        k_coord_map<<<nblk(d.ntot, 256), 256, 0, c->st>>>(d, d.vx, d.vy, d.vz, d.vx0, d.vy0, d.vz0, 1.0, 0, 0);
         c->launches += 1;
         CK(cudaMemcpyAsync(c->hstage, d.x, 6 * B * np, cudaMemcpyDeviceToHost, c->st));
         CK(cudaGetLastError());
@@ -914,8 +912,7 @@ extern "C" __attribute__((visibility("default"))) int genga_accelerations(genga_
     if (!c || !a || dt == 0.0) return GENGA_EINVAL;
     DevState &d = c->d;
     c->far_valid = false;
-    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt, 0, 0);
-    if (d.kb) { k_pack_kb<<<nblk(d.npm, 128), 128, 0, c->st>>>(d); c->launches += 1; }
+    k_rcrit<<<nblk(std::max(d.ntot, d.kb ? d.npm : 0), 128), 128, 0, c->st>>>(d, dt, 0, 2);
     if (d.mode == GENGA_MODE_TEST_PARTICLE) { k_begin_map<<<c->sms, 256, 0, c->st>>>(d); c->launches += 1; }
     k_reset_counters<<<1, 32, 0, c->st>>>(d);
     c->launches += 2;
@@ -941,15 +938,14 @@ extern "C" __attribute__((visibility("default"))) int genga_kepler_drift(genga_c
 
 extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ctx *c, int which, int reps, double dt, double *ms)
 {
-    if (!c || !ms || reps < 1 || dt == 0.0 || which < 0 || which > 4) return GENGA_EINVAL;
+    if (!c || !ms || reps < 1 || dt == 0.0 || which < 0 || which > 5) return GENGA_EINVAL;
     DevState &d = c->d;
     if (d.mode == GENGA_MODE_MULTI_SYSTEM && which == 0) return GENGA_EINVAL;
     if (which >= 3 && !(d.mode == GENGA_MODE_TEST_PARTICLE && d.ntot > d.nm)) return GENGA_EINVAL;
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
     c->far_valid = false;
-    k_rcrit<<<nblk(d.ntot, 128), 128, 0, c->st>>>(d, dt, 0, 0);
-    if (d.kb) { k_pack_kb<<<nblk(d.npm, 128), 128, 0, c->st>>>(d); c->launches += 1; }
+    k_rcrit<<<nblk(std::max(d.ntot, d.kb ? d.npm : 0), 128), 128, 0, c->st>>>(d, dt, 0, 2);
     c->launches += 1;
     int per = 1;
     for (int r = -3; r < reps; ++r) {
@@ -966,6 +962,12 @@ extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ct
             k_reset_counters<<<1, 32, 0, c->st>>>(d);
             k_tp_front<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, -dt, dt, 0);
             c->launches += 4; per = 2;
+        } else if (which == 5) {                     // closing + opening half of the particles in one pass, forwards then backwards
+            k_reset_counters<<<1, 32, 0, c->st>>>(d);
+            k_tp_mid<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, dt, dt, dt, 1);
+            k_reset_counters<<<1, 32, 0, c->st>>>(d);
+            k_tp_mid<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, -dt, -dt, dt, 0);
+            c->launches += 4; per = 2;
         } else {
             k_tp_back<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, dt);
             k_tp_back<<<nblk(d.ntot - d.nm, 128), 128, 0, c->st>>>(d, -dt);
@@ -977,7 +979,7 @@ extern "C" __attribute__((visibility("default"))) int genga_time_kernel(genga_ct
     float t = 0.f;
     CK(cudaEventElapsedTime(&t, e0, e1));
     cudaEventDestroy(e0); cudaEventDestroy(e1);
-    *ms = (double)t / reps / (which == 1 || which >= 3 ? per : 1);
+    *ms = (double)t / reps / (which == 1 || which >= 3 ? per : 1);   // (the k_reset_counters launches of 3 and 5 are inside the time: ~2 us each)
     CK(cudaGetLastError());
     return GENGA_OK;
 }

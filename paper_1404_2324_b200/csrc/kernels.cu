@@ -87,15 +87,23 @@ __global__ void k_rcrit(DevState d, double tau, int reset, int check)
     if (reset && i == 0) {                                // start of a step: forget the previous step's lists
         reset_map_counters(d);
     }
+    // check & 2: the state did not come out of a step (set_state, an operator call): the packed j-tile of the kick is
+    // written here too ; its padding up to a multiple of 128 sits far away and is massless
+    const bool pack = (check & 2) && d.kb != nullptr;
+    if (pack && i >= d.nm && i < d.npm) {
+        reinterpret_cast<double4 *>(d.kb)[i] = make_double4(1e100, 1e100, 1e100, 0.0);
+        d.hcw[i] = -1;
+    }
     if (i >= d.ntot) return;
     double x = d.x[i], y = d.y[i], z = d.z[i], vx = d.vx[i], vy = d.vy[i], vz = d.vz[i], m = d.m[i];
+    if (pack && i < d.nm) reinterpret_cast<double4 *>(d.kb)[i] = make_double4(x, y, z, d.G * m);
     double m0 = d.m0[system_of(d, i)];
     double n1 = d.n1, n2 = d.n2;
     if (d.mode == 2) { n1 = d.n12[2 * (i / d.nm)]; n2 = d.n12[2 * (i / d.nm) + 1]; }   // per system (L346-354)
     double rc = rcrit_of(d.G, m0, n1, n2, tau, x, y, z, vx, vy, vz, m);
     // S2': the hit masks of the previous closing kick cover r < 3.3 rc_old; they serve the coming opening kick only if
     // 3 rc_new <= 3.3 rc_old for every body
-    if (check && rc > KK_GROW * d.rc[i]) d.cnt[CI_S2PMISS] = 1;
+    if ((check & 1) && rc > KK_GROW * d.rc[i]) d.cnt[CI_S2PMISS] = 1;
     if (d.rcprev && i < d.nm) d.rcprev[i] = d.rc[i];           // mode 1: the particles' closing kick of the step that ends (k_tp_mid)
     d.rc[i] = rc;
     d.c9[i] = 9.0 * rc * rc;
@@ -183,21 +191,6 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
     } while (!ok);
 }
 
-// The packed j-tile of k_kick: records (x, y, z, G m) of the massive bodies and the padding up to a multiple of 128
-// (far away, massless).  Written by the closing k_sun of a map (the positions every full kick acts at) and, for a state
-// that did not come out of a step, by this kernel.
-__global__ void k_pack_kb(DevState d)
-{
-    pdl_sync();
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= d.npm) return;
-    const bool v = j < d.nm;
-    double4 r;
-    r.x = v ? d.x[j] : 1e100; r.y = v ? d.y[j] : 1e100; r.z = v ? d.z[j] : 1e100; r.w = v ? d.G * d.m[j] : 0.0;
-    reinterpret_cast<double4 *>(d.kb)[j] = r;
-    d.hcw[j] = v ? __double2hiint(KK_WIDE2 * d.rc[j] * d.rc[j]) : -1;
-}
-
 __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, int record, int ni, double *aout, int to0, int s2p)
 {
     pdl_sync();
@@ -219,9 +212,15 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
 
     // stage the bodies j.  TMA path: the first 16 lanes issue, each for one slice of 8 * iters bodies (what one warp of the first group
     // covers), three bulk copies (records, precheck words, critical radii) that complete on the slice's mbarrier
-    const bool tma = !(s2p & 4);
+    // S2' (L266-274): s2p & 2 = this is the opening kick of a step at the positions of the previous step's closing kick,
+    // whose hit masks and far-pair sums are stored (s2p & 1 there); they hold as long as no critical radius grew past the
+    // margin of the wide precheck (k_rcrit latches that in CI_S2PMISS, then the pair loop runs again).  With the stored
+    // sums nothing is staged: the exact pass fetches the few bodies it needs from the packed records in L2.
+    const bool stored = (s2p & 2) && d.cnt[CI_S2PMISS] == 0;
+    const bool tma = !(s2p & 4) && !stored;
     const int slb = iters << 3;                         // bodies per slice; 16 slices = npad bodies
-    if (tma) {
+    if (stored) {
+    } else if (tma) {
         if (tid < 16) {                                 // sixteen lanes, a slice each: the copies are issued side by side
             const int sl = tid;
             mbar_init(&S.mbar[sl], 1);
@@ -232,7 +231,7 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
         // the precheck words and critical radii (24 KB of the 88) through registers meanwhile; the block barrier below publishes them
         for (int j = tid; j < npad; j += KK_THREADS) { S.hc[j] = d.hcw[j]; S.rc[j] = d.rc[j]; }
     } else {
-        // all loads of the (at most 3) rounds in flight together; the precheck word as k_pack_kb forms it
+        // all loads of the (at most 3) rounds in flight together; the precheck word as k_rcrit forms it
         constexpr int ROUNDS = (KK_MAXN + KK_THREADS - 1) / KK_THREADS;
         double lx[ROUNDS], ly[ROUNDS], lz[ROUNDS], lm[ROUNDS], lr[ROUNDS];
 #pragma unroll
@@ -273,10 +272,6 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
     }
     double ax0 = 0.0, ay0 = 0.0, az0 = 0.0, ax1 = 0.0, ay1 = 0.0, az1 = 0.0;
     unsigned hits = 0u;
-    // S2' (L266-274): s2p & 2 = this is the opening kick of a step at the positions of the previous step's closing kick,
-    // whose hit masks and far-pair sums are stored (s2p & 1 there); they hold as long as no critical radius grew past the
-    // margin of the wide precheck (k_rcrit latches that in CI_S2PMISS, then the pair loop runs again)
-    const bool stored = (s2p & 2) && d.cnt[CI_S2PMISS] == 0;
     if ((s2p & 1) && blockIdx.x == 0 && tid == 0) d.cnt[CI_S2PMISS] = 0;      // read by the k_rcrit of the next step
     if (rowbase < nib) {                                // warp-uniform: the group has rows in this block
         const int L = iters << logP;
@@ -363,10 +358,14 @@ __global__ void __launch_bounds__(KK_THREADS, 1) k_kick(DevState d, double h, in
                 ci = i0 + rowbase + 2 * (b >> logP) + (wd & 1); cj = wi * L + ((wd >> 1) << logP) + (b & (P - 1));
                 double cx = 0.0, cy = 0.0, cz = 0.0;
                 if (cj != ci) {
-                    const KickBody bj = S.body[cj], bi = S.body[ci];
+                    KickBody bj, bi;
+                    if (stored) {
+                        const double4 rj = reinterpret_cast<const double4 *>(d.kb)[cj], ri = reinterpret_cast<const double4 *>(d.kb)[ci];
+                        bj.x = rj.x; bj.y = rj.y; bj.z = rj.z; bj.gm = rj.w; bi.x = ri.x; bi.y = ri.y; bi.z = ri.z; bi.gm = ri.w;
+                    } else { bj = S.body[cj]; bi = S.body[ci]; }
                     double dx = bj.x - bi.x, dy = bj.y - bi.y, dz = bj.z - bi.z;
                     double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                    const double rcij = fmax(S.rc[ci], S.rc[cj]);
+                    const double rcij = stored ? fmax(d.rc[ci], d.rc[cj]) : fmax(S.rc[ci], S.rc[cj]);
                     double s3 = kick_scale_exact(r2, rcij, bj.gm);
                     cand = record && ci < cj && r2 < 9.0 * rcij * rcij;      // = max(9 rc_i^2, 9 rc_j^2) as k_rcrit rounds it
                     cx = s3 * dx; cy = s3 * dy; cz = s3 * dz;
@@ -1127,11 +1126,19 @@ __global__ void __launch_bounds__(256) k_sun(DevState d, double h, int reset, do
 // system, den = m0 (+ sum m if divide_by_total).  Every block forms s itself, in a fixed order: modes 0, 1 as k_sun
 // (at most 8 bodies per thread, then a tree), mode 2 a thread sums the bodies of its own system.
 __global__ void __launch_bounds__(256) k_coord_map(DevState d, const double *ix, const double *iy, const double *iz,
-                                                   double *ox, double *oy, double *oz, double f, int divide_by_total)
+                                                   double *ox, double *oy, double *oz, double f, int divide_by_total, int init)
 {
     pdl_sync();
     __shared__ double red[4][8];
     const int i = blockIdx.x * 256 + threadIdx.x;
+    if (init) {                                           // a new state has been loaded (genga_set_state*): every body is what its slot
+        if (i == 0) { d.stat[CNT_NEV] = 0; d.stat[CNT_STEPID] = 0; }   // says, no spin, no internal energy, no events, step 0
+        if (i < d.nsys) d.U[i] = 0.0;
+        if (i < d.ntot) {
+            d.kind[i] = (d.mode == 1 && i >= d.nm) ? 1 : 0;
+            for (int c = 0; c < 3; ++c) d.spin[(size_t)c * d.np + i] = 0.0;
+        }
+    }
     double sx = 0.0, sy = 0.0, sz = 0.0, sm = 0.0, m0;
     if (d.mode == 2) {
         if (i >= d.ntot) return;
@@ -1960,18 +1967,6 @@ __global__ void k_eval_fast(int which, long long n, const double *in, double *ou
     if (i >= n) return;
     const double x = in[i];
     out[i] = which == 0 ? rsqrt_fast(x) : which == 1 ? rinv3_fast(x) : rcp_fast(x);
-}
-
-// A new state has been loaded: every body is what its slot says (massive / test particle), no spin, no internal
-// energy, no events, step 0 (genga_set_state*).
-__global__ void k_init_bodies(DevState d)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i == 0) { d.stat[CNT_NEV] = 0; d.stat[CNT_STEPID] = 0; }
-    if (i < d.nsys) d.U[i] = 0.0;
-    if (i >= d.ntot) return;
-    d.kind[i] = (d.mode == 1 && i >= d.nm) ? 1 : 0;
-    for (int c = 0; c < 3; ++c) d.spin[(size_t)c * d.np + i] = 0.0;
 }
 
 // labels for genga_encounters: body's own index unless it is in a group

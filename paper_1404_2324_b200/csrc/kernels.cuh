@@ -25,7 +25,6 @@ __global__ void k_reset_counters(DevState d);
 __global__ void k_rcrit(DevState d, double tau, int reset, int check);
 __global__ void k_kick(DevState d, double h, int record, int ni, double *aout, int to0, int s2p);
 size_t kick_smem_bytes();
-__global__ void k_pack_kb(DevState d);
 __global__ void k_tp_kick(DevState d, double h, int record, double *aout);
 __global__ void k_tp_front(DevState d, double h, double tau, int first);
 __global__ void k_tp_back(DevState d, double h);
@@ -33,7 +32,7 @@ __global__ void k_kick_multi(DevState d, double h, int record, double *aout);
 __global__ void k_sun(DevState d, double h, int reset, double hdrift);
 __global__ void k_multi_front(DevState d, double h, double hk);
 __global__ void k_multi_back(DevState d, double h, double hk);
-__global__ void k_coord_map(DevState d, const double *ix, const double *iy, const double *iz, double *ox, double *oy, double *oz, double f, int divide_by_total);
+__global__ void k_coord_map(DevState d, const double *ix, const double *iy, const double *iz, double *ox, double *oy, double *oz, double f, int divide_by_total, int init);
 __global__ void k_tiny_front(DevState d, double h, double tau, int first, double hk);
 __global__ void k_tiny_back(DevState d, double h, double hk, int record, int reset);
 __global__ void k_tpm_kick(DevState d, double h, int record, double fshift, int slot);
@@ -55,7 +54,6 @@ __global__ void k_bs_multi(DevState d, double h);
 __global__ void k_bs_generic(DevState d, double h, int pass);
 __global__ void k_end_step(DevState d);
 __global__ void k_end_step2(DevState d);
-__global__ void k_init_bodies(DevState d);
 __global__ void k_energy(DevState d, double *out);
 __global__ void k_export_labels(DevState d, int *out);
 __global__ void k_fp64_probe(double *out, int iters);
