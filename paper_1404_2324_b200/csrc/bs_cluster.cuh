@@ -21,6 +21,9 @@
 // body's midpoint state in registers.  Positions are exchanged through a double-buffered shared array: one
 // __syncthreads per force evaluation.
 #pragma once
+#ifndef GENGA_MB
+#define GENGA_MB 0
+#endif
 #include <cooperative_groups.h>
 #include <cstdio>
 
@@ -45,9 +48,18 @@ struct BcSmem {
     double diag[6][MAXN];           // checker: T[k][k] of the row tested last
     double red[THREADS / 32];
     // ---- close pairs of the current evaluation (bc_rhs2, list path)
-    int2 plist[BC_MAXP];            // ordered pairs (i, j) that passed the FP32 pretest at either point, body by body
-    double pres[BC_MAXP][6];        // their geometric factors times the separation at the two points (without G m_j)
-    int wtot[THREADS / 32];         // pairs found by each warp
+    int part[BC_MAXP];              // entry (k + 1) npad + i: the k-th partner of body i that passed the FP32 pretest at either point
+    alignas(16) double pres[BC_MAXP][6];        // same entries: the acceleration of i by that partner at the two points; entry i (row 0): by the star
+    int kmax[2];                    // most partners of one body (double-buffered like pos)
+    int stale[2];                   // an owner found the list outdated (double-buffered like pos)
+    int refbody;                    // the body nearest the group's centre
+    int ok;                         // block-local broadcast: the record just read is consistent
+#ifdef GENGA_BC_PROF
+    int dbg_rebuild, dbg_total;
+#endif
+    float4 ref[MAXN];               // positions (FP32) at the evaluation the list was built from
+    int cnt[MAXN];                  // partners of body i in the list
+    float skin2;                    // the list stays valid while every |(q_i - q_0) - ref_i|^2 < skin2 (0: never)
     // ---- round record, written by the master under a sequence lock (seq_begin first, seq_end last).  Round numbers
     // run on from group to group, so a flag of an older round never equals a current one.
     volatile int seq_begin, seq_end;
@@ -60,9 +72,27 @@ struct BcSmem {
 };
 
 struct BcLane {
-    int n, L, i, s;
+    int n, L;
+    int i;              // the body this thread OWNS (integrates, sums the forces of): thread i < n owns body i
     bool owner;
+    int pi, s;          // lane s of the L lanes that examine the pairs of body pi (the n^2 distance tests)
 };
+
+// The list of close pairs the block carries from one evaluation to the next (bc_rhs2).
+struct BcList {
+    int rows, npad;     // S.part / S.pres: rows of npad entries (row 0 the star, row k + 1 the k-th partner of every body)
+    unsigned magic;     // ceil(2^32 / npad): entry / npad without a division
+    bool valid;
+    int age;            // evaluations the current list has served
+    int early;          // lists of this round that were outdated at their first check: after two of them the round stops
+                        // checking (steps this long move the bodies by more than the skin every time) and makes a new one each time
+    int ref;            // the body the rigid motion is taken from: the one nearest the group's centre
+};
+
+#ifndef GENGA_BC_SKIN
+#define GENGA_BC_SKIN 0.3
+#endif
+constexpr double BC_SKIN = GENGA_BC_SKIN;      // the list takes pairs out to (1 + BC_SKIN) rc_ij
 
 template <int THREADS>
 __device__ __forceinline__ BcLane bc_lanes(int n)
@@ -70,36 +100,84 @@ __device__ __forceinline__ BcLane bc_lanes(int n)
     int P = 2;
     while (P < n) P <<= 1;              // bodies, rounded up to a power of two
     BcLane t;
-    t.n = n; t.L = min(8, THREADS / P);  // lanes per body: they only pretest and gather (bc_rhs2)
-    t.i = threadIdx.x / t.L; t.s = threadIdx.x % t.L;
-    t.owner = t.s == 0 && t.i < n;
+    t.n = n; t.L = min(8, THREADS / P);
+    t.i = threadIdx.x; t.owner = threadIdx.x < n;
+    t.pi = threadIdx.x / t.L; t.s = threadIdx.x % t.L;
     return t;
+}
+
+// The list path of bc_rhs2: one thread per entry of the table S.part (rows x npad; threads first, first + 1, ..,
+// THREADS - 1 share them): row 0, column i the star's acceleration of body i; row k + 1, column i the acceleration of i by
+// its k-th listed partner at the two points (zero where the pair is outside rc_ij).  Results go to the same entry of
+// S.pres: npad is odd and an entry 48 bytes, so the LDS.128 of eight neighbouring owners walking down their columns fall
+// into eight different groups of four banks (a compact list walked a lane every few entries measured 16-way conflicts:
+// ~100 cycles per entry).
+template <int MAXN, int THREADS>
+__device__ __forceinline__ void bc_pairs(BcSmem<MAXN, THREADS> &S, const double (*pA)[MAXN], const double (*pB)[MAXN], double G, double m0,
+                                         const BcList &lst, const int n, const int first)
+{
+    const int npad = lst.npad, entries = lst.rows * npad;
+    for (int p = (int)threadIdx.x - first; p >= 0 && p < entries; p += THREADS - first) {
+        const int row = (int)__umulhi((unsigned)p, lst.magic), i = p - row * npad;
+        if (i >= n) continue;
+        double *o = S.pres[p];
+        if (row == 0) {
+            const double xA = pA[0][i], yA = pA[1][i], zA = pA[2][i], xB = pB[0][i], yB = pB[1][i], zB = pB[2][i];
+            const double sA = -G * m0 * rinv3_fast(xA * xA + yA * yA + zA * zA), sB = -G * m0 * rinv3_fast(xB * xB + yB * yB + zB * zB);
+            *reinterpret_cast<double2 *>(o) = make_double2(sA * xA, sA * yA);
+            *reinterpret_cast<double2 *>(o + 2) = make_double2(sA * zA, sB * xB);
+            *reinterpret_cast<double2 *>(o + 4) = make_double2(sB * yB, sB * zB);
+            continue;
+        }
+        if (row > S.cnt[i]) continue;
+        const int j = S.part[p];
+        const double rci = S.rc[i], rcj = S.rc[j];
+        const bool big = rci >= rcj;
+        const double rcij = big ? rci : rcj, rc2 = rcij * rcij;
+        const double dx = pA[0][j] - pA[0][i], dy = pA[1][j] - pA[1][i], dz = pA[2][j] - pA[2][i];
+        const double ex = pB[0][j] - pB[0][i], ey = pB[1][j] - pB[1][i], ez = pB[2][j] - pB[2][i];
+        const double dA = dx * dx + dy * dy + dz * dz, dB = ex * ex + ey * ey + ez * ez;
+        const bool inA = dA < rc2, inB = dB < rc2;
+        const double ir = big ? S.irc[i] : S.irc[j];
+        const double gmj = G * S.m[j];
+        double wA = direct_scale_nb(inA ? dA : rc2, rcij, ir, gmj);
+        double wB = direct_scale_nb(inB ? dB : rc2, rcij, ir, gmj);
+        wA = inA ? wA : 0.0; wB = inB ? wB : 0.0;
+        *reinterpret_cast<double2 *>(o) = make_double2(wA * dx, wA * dy);
+        *reinterpret_cast<double2 *>(o + 2) = make_double2(wA * dz, wB * ex);
+        *reinterpret_cast<double2 *>(o + 4) = make_double2(wB * ey, wB * ez);
+    }
 }
 
 // Forces on body t.i at TWO sets of positions (qA, qB of the owners) at once (Eq. 1 L73-74 through Eq. 8
 // L104; star fixed at the origin, L314; every pair of the group is examined at every evaluation, L505).
-// Two at once because a(q_k) and a(q_{k+1}) of Gragg's rule are independent (bs_warp.cuh): one barrier and
-// one segment reduction serve both, and their dependent chains overlap.  The n^2 examinations are done
-// first in FP32 against a threshold widened by more than the FP32 rounding, so the test can only err
-// towards "inside"; pairs that pass take the exact FP64 test and weight.
+// Two at once because a(q_k) and a(q_{k+1}) of Gragg's rule are independent (bs_warp.cuh): one set of barriers
+// serves both, and their dependent chains overlap.
 //
-// What that costs is the exact pass: ~110 FP64 instructions per close pair, and a warp runs them as long as ANY of its
-// lanes has a pair left, so with 16 warps on one SM the FP64 pipe was busy ~2.6 k of the 6.5 k cycles of an evaluation
-// of a 55-body group, most of it on idle lanes.  LIST PATH (all partners of a lane in one 32-bit mask, at most BC_MAXP
-// close ordered pairs: the sparse chains of a planetesimal disc): the lanes only pretest; their hits are compacted into
-// one list (block-wide prefix sum, body by body, fixed order), ONE thread per listed pair evaluates the exact weights
-// of both points, and body i adds up its own contiguous range of the list: the exact pass shrinks to total / 32 warps.
-// Dense or very large groups keep the direct loop.
-// Thread 0 copies *watch (the master's round number) into S.bc[buf] before the barrier of this evaluation; the value
-// every thread finds there afterwards is returned.
+// What an evaluation costs is latency and issue slots, not arithmetic (measured on B200, one warp per scheduler: DFMA
+// 8.8 cycles dependent / 2.1 issue, SHFL 26 / 4.5 and one per cycle for the whole SM, F2F ~10 issue, a barrier of 16 warps
+// ~50): so the owners are the first n threads (few warps convert and integrate, the others only help with the pairs), and
+// nothing on the per-evaluation path is reduced by shuffles.
+//
+// LIST PATH (n <= 32 L, at most BC_MAXP entries: the sparse chains of a planetesimal disc).  The n^2 examinations are
+// done in FP32 against a threshold widened by more than the FP32 rounding AND by the skin BC_SKIN rc, L lanes per body;
+// the hits are compacted into one list (block-wide prefix sum, body by body, fixed order).  The list is then KEPT: an
+// evaluation first checks that no body has moved, after the rigid motion that takes body 0 back to where it was (a rigid
+// motion keeps every distance), by more than half the skin; if so no pair outside the list can have come inside rc_ij,
+// and the n^2 pass is skipped.  One thread per listed ordered pair evaluates the exact FP64 test and both changeover
+// weights (a listed pair outside rc_ij gives zero), one thread per body the star; the owner adds up its own contiguous
+// range of the list, in list order.
+// Dense or very large groups keep the direct loop: the lanes of a body evaluate their own hits and reduce by shuffles.
+// One thread copies *watch (the master's round number) into S.bc[buf] before the first barrier of this evaluation; the
+// value every thread finds there afterwards is returned.
 template <int MAXN, int THREADS>
 __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t, int &buf, double G, double m0,
                                        const double qA[3], const double qB[3], double aA[3], double aB[3],
-                                       const volatile int *watch)
+                                       const volatile int *watch, BcList &lst)
 {
     GENGA_BS_RHS_HOOK();
-#ifdef GENGA_BC_PROF
-    long long ph_[8]; int phn_ = 0;
+#ifdef GENGA_BC_PROF_RHS
+    long long ph_[10]; int phn_ = 0;
 #define RHS_PROF() ph_[phn_++] = clock64();
 #else
 #define RHS_PROF()
@@ -115,107 +193,164 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
             pA[c][t.i] = qA[c]; pB[c][t.i] = qB[c];
         }
         const float th = S.thr2[t.i];
+        if (!(GENGA_MB & 2)) {
         fA[t.i] = make_float4((float)qA[0], (float)qA[1], (float)qA[2], th);
         fB[t.i] = make_float4((float)qB[0], (float)qB[1], (float)qB[2], th);
+        }
     }
-    if (threadIdx.x == 0) S.bc[buf] = *watch;
+    if (threadIdx.x == THREADS - 32 && !(GENGA_MB & 16)) S.bc[buf] = *watch;     // a thread that owns nothing: the owners' warp does not wait for this
     __syncthreads();
-    const int seen = S.bc[buf];
+    const int seen = (GENGA_MB & 16) ? 1 : S.bc[buf];
+    const int sb = buf;
+    if (threadIdx.x == THREADS - 32 && !(GENGA_MB & 32)) { S.stale[buf ^ 1] = 0; S.kmax[buf ^ 1] = 0; }                  // read last in the evaluation before this one
     RHS_PROF()
     buf ^= 1;
     double ax = 0.0, ay = 0.0, az = 0.0, bx = 0.0, by = 0.0, bz = 0.0;
-    const int n = t.n, L = t.L, i = t.i;
+    const int n = t.n, L = t.L, i = t.pi;                         // below, i is the body whose pairs this lane examines
     const bool live = i < n;
     const bool one_chunk = n <= 32 * L;                           // every partner of a lane fits one mask (uniform)
+    bool summed = false;                                          // the owners already hold their sums
     if (one_chunk) {
-        // ---- pretest: bit kk = partner j = s + kk L passed at point A or B
-        unsigned mask = 0u;
-        if (live) {
-            const float4 mA = fA[i], mB = fB[i];
-            const float ft = mA.w;
-#pragma unroll 4
-            for (int kk = 0; kk < 32; ++kk) {
-                const int j = t.s + kk * L;
-                if (j >= n) break;
-                const float4 pa = fA[j], pb = fB[j];
-                float dx = pa.x - mA.x, dy = pa.y - mA.y, dz = pa.z - mA.z;
-                float ex = pb.x - mB.x, ey = pb.y - mB.y, ez = pb.z - mB.z;
-                float d2 = fminf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), fmaf(ez, ez, fmaf(ey, ey, ex * ex)));
-                const bool in = d2 < fmaxf(ft, pa.w) && j != i;
-                mask |= (in ? 1u : 0u) << kk;
+        bool listed = false;
+        if (lst.valid) {
+            // optimistic: the warps that own no body evaluate the listed pairs while the owners check the list; if the
+            // check fails (rare), what they wrote is thrown away
+            const int ow = (n + 31) & ~31;                        // threads of the owners' warps
+            bool still = true;
+            if (t.owner && !(GENGA_MB & 1)) {
+                // rigid motion taken out first: the rotation about z that puts the central body back on its old azimuth, then its shift
+                const float4 oA = fA[lst.ref], oB = fB[lst.ref], o = S.ref[lst.ref], r = S.ref[t.i], mA = fA[t.i], mB = fB[t.i];
+                const float on = o.x * o.x + o.y * o.y;
+                const float nA = rsqrtf((oA.x * oA.x + oA.y * oA.y) * on), nB = rsqrtf((oB.x * oB.x + oB.y * oB.y) * on);
+                const float cA = (oA.x * o.x + oA.y * o.y) * nA, sA = (oA.x * o.y - oA.y * o.x) * nA;
+                const float cB = (oB.x * o.x + oB.y * o.y) * nB, sB = (oB.x * o.y - oB.y * o.x) * nB;
+                const float ux = mA.x - oA.x, uy = mA.y - oA.y, wx = mB.x - oB.x, wy = mB.y - oB.y;
+                const float rx = r.x - o.x, ry = r.y - o.y, rz = r.z - o.z;
+                const float dx = (cA * ux - sA * uy) - rx, dy = (sA * ux + cA * uy) - ry, dz = (mA.z - oA.z) - rz;
+                const float ex = (cB * wx - sB * wy) - rx, ey = (sB * wx + cB * wy) - ry, ez = (mB.z - oB.z) - rz;
+                const float moved = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), fmaf(ez, ez, fmaf(ey, ey, ex * ex)));
+                still = moved < S.skin2;
+                if (!(moved < 0.5f * S.skin2)) atomicOr(&S.stale[sb], still ? 2 : 3);     // 2: 70 % of the way: a new list next time
+            }
+            if (ow < THREADS && !(GENGA_MB & 8)) bc_pairs(S, pA, pB, G, m0, lst, n, ow);
+            RHS_PROF()
+            if (!(GENGA_MB & 64)) __syncthreads();                                      // a plain barrier and a flag: half the price of a voting barrier
+            const int st = (GENGA_MB & 32) ? 0 : S.stale[sb];
+            listed = !(st & 1);
+            if (st) lst.valid = false;                            // this list was used for the last time
+            if (!listed && lst.age == 0) ++lst.early;
+            ++lst.age;
+            if (listed && ow >= THREADS) {                        // no warp to spare: the pairs after the check
+                bc_pairs(S, pA, pB, G, m0, lst, n, 0);
+                __syncthreads();
+            }
+            RHS_PROF()
+        }
+        if (!listed) {
+            // ---- pretest: bit kk = partner j = s + kk L passed at point A or B.  Four partners per trip, no early exit:
+            // their loads and short FP32 chains overlap (one at a time this loop was most of what a new list costs)
+            unsigned mask = 0u;
+            if (live) {
+                const float4 mA = fA[i], mB = fB[i];
+                const float ft = mA.w;
+                if (t.s == 0) S.ref[i] = mA;
+                const int trips = (n - t.s + 4 * L - 1) / (4 * L);    // t.s < L <= n
+#pragma unroll 1
+                for (int q4 = 0; q4 < trips && !(GENGA_MB & 128); ++q4) {
+                    unsigned bits = 0u;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int j = t.s + (4 * q4 + u) * L, jj = min(j, n - 1);
+                        const float4 pa = fA[jj], pb = fB[jj];
+                        const float dx = pa.x - mA.x, dy = pa.y - mA.y, dz = pa.z - mA.z;
+                        const float ex = pb.x - mB.x, ey = pb.y - mB.y, ez = pb.z - mB.z;
+                        const float d2 = fminf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), fmaf(ez, ez, fmaf(ey, ey, ex * ex)));
+                        bits |= (d2 < fmaxf(ft, pa.w) && j != i && j < n) ? 1u << u : 0u;
+                    }
+                    mask |= bits << (4 * q4);
+                }
+            }
+            // ---- the k-th hit of body i goes to entry (k + 1) npad + i: k from a prefix sum over the body's L lanes only, so
+            // the table is complete after ONE barrier (no block-wide compaction)
+            const int lane = threadIdx.x & 31;
+            const int cnt = __popc(mask);
+            int pre = cnt;
+            if (!(GENGA_MB & 256)) for (int o = 1; o < L; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o, L); if (t.s >= o) pre += v; }
+            const int cseg = __shfl_sync(0xffffffffu, pre, L - 1, L);           // the body's partners
+            const int wmax = __reduce_max_sync(0xffffffffu, cseg);
+            if (lane == 0 && wmax > 0 && !(GENGA_MB & 512)) atomicMax(&S.kmax[sb], wmax);
+            const int npad = lst.npad;
+            if (live) {
+                if (t.s == 0) S.cnt[i] = cseg;
+                int slot = (pre - cnt + 1) * npad + i;
+                for (unsigned mm = mask; mm && slot < BC_MAXP; mm &= mm - 1, slot += npad) S.part[slot] = t.s + (__ffs(mm) - 1) * L;
+            }
+            RHS_PROF()
+            __syncthreads();
+            RHS_PROF()
+            const int kmax = S.kmax[sb];
+            listed = (kmax + 1) * npad <= BC_MAXP;
+            lst.valid = listed && S.skin2 > 0.f && lst.early < 2;
+            lst.age = 0;
+            lst.rows = kmax + 1;
+#ifdef GENGA_BC_PROF
+            if (threadIdx.x == 0) { ++S.dbg_rebuild; S.dbg_total = lst.rows * npad; }
+#endif
+            if (listed) {
+                bc_pairs(S, pA, pB, G, m0, lst, n, 0);
+                __syncthreads();
+            } else if (live) {
+                // ---- dense group: the lanes evaluate their own hits
+                const double xA = pA[0][i], yA = pA[1][i], zA = pA[2][i], xB = pB[0][i], yB = pB[1][i], zB = pB[2][i];
+                const double my_rc = S.rc[i], my_irc = S.irc[i];
+                while (mask) {
+                    const int j = t.s + (__ffs(mask) - 1) * L;
+                    mask &= mask - 1;
+                    double rcj = S.rc[j];
+                    double rcij = fmax(my_rc, rcj), rc2 = rcij * rcij;
+                    double dx = pA[0][j] - xA, dy = pA[1][j] - yA, dz = pA[2][j] - zA;
+                    double ex = pB[0][j] - xB, ey = pB[1][j] - yB, ez = pB[2][j] - zB;
+                    double dA = dx * dx + dy * dy + dz * dz, dB = ex * ex + ey * ey + ez * ez;
+                    const bool inA = dA < rc2, inB = dB < rc2;
+                    if (inA || inB) {
+                        const double ir = my_rc >= rcj ? my_irc : S.irc[j], gmj = G * S.m[j];
+                        double scA = direct_scale_nb(inA ? dA : rc2, rcij, ir, gmj);
+                        double scB = direct_scale_nb(inB ? dB : rc2, rcij, ir, gmj);
+                        scA = inA ? scA : 0.0; scB = inB ? scB : 0.0;
+                        ax += scA * dx; ay += scA * dy; az += scA * dz;
+                        bx += scB * ex; by += scB * ey; bz += scB * ez;
+                    }
+                }
             }
         }
-        // ---- block-wide exclusive prefix sum of the hit counts, in thread order (= body by body)
-        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-        const int cnt = __popc(mask);
-        int inc = cnt;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-        if (lane == 31) S.wtot[warp] = inc;
-        RHS_PROF()
-        __syncthreads();
-        RHS_PROF()
-        int base = 0, total = 0;
-#pragma unroll
-        for (int w = 0; w < THREADS / 32; ++w) { const int v = S.wtot[w]; base += w < warp ? v : 0; total += v; }
-        if (total <= BC_MAXP) {
-            int at = base + inc - cnt;
-            // my body's range of the list: [start of its first lane, + the counts of its L lanes)
-            int cseg = cnt;
-            for (int o = L >> 1; o > 0; o >>= 1) cseg += __shfl_xor_sync(0xffffffffu, cseg, o);
-            const int start = __shfl_sync(0xffffffffu, at, lane & ~(L - 1));
-            for (unsigned mm = mask; mm; mm &= mm - 1) S.plist[at++] = make_int2(i, t.s + (__ffs(mm) - 1) * L);
-            __syncthreads();
-            RHS_PROF()
-            // ---- one thread per listed pair: exact test and both changeover weights, without the partner's mass
-            for (int p = threadIdx.x; p < total; p += THREADS) {
-                const int2 pr = S.plist[p];
-                const double rci = S.rc[pr.x], rcj = S.rc[pr.y];
-                const double rcij = fmax(rci, rcj), rc2 = rcij * rcij;
-                const double dx = pA[0][pr.y] - pA[0][pr.x], dy = pA[1][pr.y] - pA[1][pr.x], dz = pA[2][pr.y] - pA[2][pr.x];
-                const double ex = pB[0][pr.y] - pB[0][pr.x], ey = pB[1][pr.y] - pB[1][pr.x], ez = pB[2][pr.y] - pB[2][pr.x];
-                const double dA = dx * dx + dy * dy + dz * dz, dB = ex * ex + ey * ey + ez * ez;
-                const bool inA = dA < rc2, inB = dB < rc2;
-                const double ir = rci >= rcj ? S.irc[pr.x] : S.irc[pr.y];
-                double wA = direct_scale_nb(inA ? dA : rc2, rcij, ir, 1.0);
-                double wB = direct_scale_nb(inB ? dB : rc2, rcij, ir, 1.0);
-                wA = inA ? wA : 0.0; wB = inB ? wB : 0.0;
-                S.pres[p][0] = wA * dx; S.pres[p][1] = wA * dy; S.pres[p][2] = wA * dz;
-                S.pres[p][3] = wB * ex; S.pres[p][4] = wB * ey; S.pres[p][5] = wB * ez;
-            }
-            RHS_PROF()
-            __syncthreads();
-            RHS_PROF()
-            // ---- body i: its own range, lane s takes every L-th entry
-            if (live) {
-                for (int p = start + t.s; p < start + cseg; p += L) {
-                    const double gmj = G * S.m[S.plist[p].y];
-                    ax = fma(gmj, S.pres[p][0], ax); ay = fma(gmj, S.pres[p][1], ay); az = fma(gmj, S.pres[p][2], az);
-                    bx = fma(gmj, S.pres[p][3], bx); by = fma(gmj, S.pres[p][4], by); bz = fma(gmj, S.pres[p][5], bz);
+        if (listed) {
+            // ---- the owner: the star, then its own range in list order; four entries per trip (their loads in flight
+            // together), then one by one: as few instructions as possible, the owners' warp is alone on this stretch
+            if (t.owner && !(GENGA_MB & 4)) {
+                const int row = 6 * lst.npad;
+                const double *e = S.pres[t.i];
+                int left = S.cnt[t.i];
+                double2 v0 = *reinterpret_cast<const double2 *>(e), v1 = *reinterpret_cast<const double2 *>(e + 2), v2 = *reinterpret_cast<const double2 *>(e + 4);
+                ax = v0.x; ay = v0.y; az = v1.x; bx = v1.y; by = v2.x; bz = v2.y;
+                e += row;
+#pragma unroll 1
+                for (; left >= 4; left -= 4, e += 4 * row) {
+                    const double *f = e + row, *g = f + row, *h = g + row;
+                    const double2 a0 = *reinterpret_cast<const double2 *>(e), a1 = *reinterpret_cast<const double2 *>(e + 2), a2 = *reinterpret_cast<const double2 *>(e + 4);
+                    const double2 b0 = *reinterpret_cast<const double2 *>(f), b1 = *reinterpret_cast<const double2 *>(f + 2), b2 = *reinterpret_cast<const double2 *>(f + 4);
+                    const double2 c0 = *reinterpret_cast<const double2 *>(g), c1 = *reinterpret_cast<const double2 *>(g + 2), c2 = *reinterpret_cast<const double2 *>(g + 4);
+                    const double2 d0 = *reinterpret_cast<const double2 *>(h), d1 = *reinterpret_cast<const double2 *>(h + 2), d2 = *reinterpret_cast<const double2 *>(h + 4);
+                    ax += (a0.x + b0.x) + (c0.x + d0.x); ay += (a0.y + b0.y) + (c0.y + d0.y); az += (a1.x + b1.x) + (c1.x + d1.x);
+                    bx += (a1.y + b1.y) + (c1.y + d1.y); by += (a2.x + b2.x) + (c2.x + d2.x); bz += (a2.y + b2.y) + (c2.y + d2.y);
+                }
+#pragma unroll 1
+                for (; left > 0; --left, e += row) {
+                    v0 = *reinterpret_cast<const double2 *>(e); v1 = *reinterpret_cast<const double2 *>(e + 2); v2 = *reinterpret_cast<const double2 *>(e + 4);
+                    ax += v0.x; ay += v0.y; az += v1.x; bx += v1.y; by += v2.x; bz += v2.y;
                 }
             }
-        } else if (live) {
-            // ---- dense group: the lanes evaluate their own hits
-            const double xA = pA[0][i], yA = pA[1][i], zA = pA[2][i], xB = pB[0][i], yB = pB[1][i], zB = pB[2][i];
-            const double my_rc = S.rc[i], my_irc = S.irc[i];
-            while (mask) {
-                const int j = t.s + (__ffs(mask) - 1) * L;
-                mask &= mask - 1;
-                double rcj = S.rc[j];
-                double rcij = fmax(my_rc, rcj), rc2 = rcij * rcij;
-                double dx = pA[0][j] - xA, dy = pA[1][j] - yA, dz = pA[2][j] - zA;
-                double ex = pB[0][j] - xB, ey = pB[1][j] - yB, ez = pB[2][j] - zB;
-                double dA = dx * dx + dy * dy + dz * dz, dB = ex * ex + ey * ey + ez * ez;
-                const bool inA = dA < rc2, inB = dB < rc2;
-                if (inA || inB) {
-                    const double ir = my_rc >= rcj ? my_irc : S.irc[j], gmj = G * S.m[j];
-                    double scA = direct_scale_nb(inA ? dA : rc2, rcij, ir, gmj);
-                    double scB = direct_scale_nb(inB ? dB : rc2, rcij, ir, gmj);
-                    scA = inA ? scA : 0.0; scB = inB ? scB : 0.0;
-                    ax += scA * dx; ay += scA * dy; az += scA * dz;
-                    bx += scB * ex; by += scB * ey; bz += scB * ez;
-                }
-            }
+            RHS_PROF()
+            summed = true;
         }
     } else if (live) {
         const float4 mA = fA[i], mB = fB[i];
@@ -257,31 +392,47 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
             }
         }
     }
-    if (live) {
-        // the star (fixed at the origin): every lane of the body computes it, lane 0 keeps it (no split of the warp)
-        const double xA = pA[0][i], yA = pA[1][i], zA = pA[2][i], xB = pB[0][i], yB = pB[1][i], zB = pB[2][i];
-        double rA = xA * xA + yA * yA + zA * zA, rB = xB * xB + yB * yB + zB * zB;
-        double sA = -G * m0 * rinv3_fast(rA), sB = -G * m0 * rinv3_fast(rB);
-        sA = t.s == 0 ? sA : 0.0; sB = t.s == 0 ? sB : 0.0;
-        ax += sA * xA; ay += sA * yA; az += sA * zA;
-        bx += sB * xB; by += sB * yB; bz += sB * zB;
-    }
-    for (int o = t.L >> 1; o > 0; o >>= 1) {
-        ax += __shfl_xor_sync(0xffffffffu, ax, o); ay += __shfl_xor_sync(0xffffffffu, ay, o); az += __shfl_xor_sync(0xffffffffu, az, o);
-        bx += __shfl_xor_sync(0xffffffffu, bx, o); by += __shfl_xor_sync(0xffffffffu, by, o); bz += __shfl_xor_sync(0xffffffffu, bz, o);
+    if (!summed) {
+        // ---- direct loops: lane 0 of the body adds the star; the L partial sums are reduced by an xor-butterfly (fixed
+        // order) and handed to the owner thread through S.pres
+        if (live) {
+            const double xA = pA[0][i], yA = pA[1][i], zA = pA[2][i], xB = pB[0][i], yB = pB[1][i], zB = pB[2][i];
+            double rA = xA * xA + yA * yA + zA * zA, rB = xB * xB + yB * yB + zB * zB;
+            double sA = -G * m0 * rinv3_fast(rA), sB = -G * m0 * rinv3_fast(rB);
+            sA = t.s == 0 ? sA : 0.0; sB = t.s == 0 ? sB : 0.0;
+            ax += sA * xA; ay += sA * yA; az += sA * zA;
+            bx += sB * xB; by += sB * yB; bz += sB * zB;
+        }
+        for (int o = L >> 1; o > 0; o >>= 1) {
+            ax += __shfl_xor_sync(0xffffffffu, ax, o); ay += __shfl_xor_sync(0xffffffffu, ay, o); az += __shfl_xor_sync(0xffffffffu, az, o);
+            bx += __shfl_xor_sync(0xffffffffu, bx, o); by += __shfl_xor_sync(0xffffffffu, by, o); bz += __shfl_xor_sync(0xffffffffu, bz, o);
+        }
+        if (live && t.s == 0) {
+            double *o = S.pres[i];
+            o[0] = ax; o[1] = ay; o[2] = az; o[3] = bx; o[4] = by; o[5] = bz;
+        }
+        __syncthreads();
+        if (t.owner) {
+            const double *o = S.pres[t.i];
+            ax = o[0]; ay = o[1]; az = o[2]; bx = o[3]; by = o[4]; bz = o[5];
+        }
     }
     aA[0] = ax; aA[1] = ay; aA[2] = az;
     aB[0] = bx; aB[1] = by; aB[2] = bz;
-#ifdef GENGA_BC_PROF
+#ifdef GENGA_BC_PROF_RHS
     RHS_PROF()
-    if (threadIdx.x == 0 && t.n == 55 && (blockIdx.x & 7) < 2 && seen < 4) {
-        printf("rhs n=%d blk=%d seq=%d phases:", t.n, blockIdx.x & 7, seen);
+    if (threadIdx.x == 0 && t.n == 10 && (blockIdx.x & 15) == 3 && (seen & 15) == 3) {
+        printf("rhs n=%d blk=%d seq=%d rows=%d phases:", t.n, blockIdx.x & 7, seen, lst.rows);
         for (int k = 1; k < phn_; ++k) printf(" %d", (int)(ph_[k] - ph_[k - 1]));
         printf("\n");
     }
 #endif
     return seen;
 }
+
+// Orders this thread's accesses to the shared memory of the cluster's CTAs (the round record, the column results, the
+// flags): cluster scope is enough, and far cheaper than the device-wide fence with its L1 invalidation.
+__device__ __forceinline__ void bc_fence() { asm volatile("fence.acq_rel.cluster;" ::: "memory"); }
 
 template <int MAXN, int THREADS>
 __device__ __forceinline__ double bc_block_max(BcSmem<MAXN, THREADS> &S, double v)
@@ -304,6 +455,7 @@ __device__ __forceinline__ int bc_wait_change(BcSmem<MAXN, THREADS> &S, const vo
     if (threadIdx.x == 0) {
         int v;
         while ((v = *flag) == old) __nanosleep(20);
+        bc_fence();                 // what the writer stored before the flag is visible to this thread, and after the barrier to the block
         S.bc[0] = v;
     }
     __syncthreads();
@@ -411,26 +563,51 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
                  fabs(h) * fmax(fmax(fabs(S.Y[3][i]), fabs(S.Y[4][i])), fabs(S.Y[5][i]));
         }
         const double Q = 2.0 * bc_block_max(S, qm);
+        // List path of bc_rhs2 (n <= 32 L): the pretest reaches out to (1 + BC_SKIN) rc, and the list is kept while every
+        // body stays within skin = BC_SKIN min_i rc_i / 2 of where it was, relative to body 0, when the list was made
+        // (less 2^-19 Q for the FP32 roundings of that difference): a pair left out cannot have come inside rc_ij.
+        const bool wide = n <= 32 * t.L;
+        const double rcmin = -bc_block_max(S, t.owner ? -S.rc[i] : -1.0e300);
         if (t.owner) {
-            double w = S.rc[i] + 0x1.0p-20 * Q;
+            double w = S.rc[i] * (wide ? 1.0 + BC_SKIN : 1.0) + 0x1.0p-20 * Q;
             S.thr2[i] = __double2float_ru(w * w * (1.0 + 0x1.0p-18));
+        }
+        if (tid == 0) {
+            const double sk = 0.5 * BC_SKIN * rcmin - 0x1.0p-19 * Q;
+            S.skin2 = wide && sk > 0.0 ? __double2float_rd(sk * sk * (1.0 - 0x1.0p-18)) : 0.f;
+            S.stale[0] = 0; S.stale[1] = 0; S.kmax[0] = 0; S.kmax[1] = 0;
+            // the body nearest the centre of the group: differential rotation moves the others least against its frame
+            double cx = 0.0, cy = 0.0, cz = 0.0;
+            for (int b = 0; b < n; ++b) { cx += S.Y[0][b]; cy += S.Y[1][b]; cz += S.Y[2][b]; }
+            cx /= n; cy /= n; cz /= n;
+            int best = 0;
+            double bd = 1.0e300;
+            for (int b = 0; b < n; ++b) {
+                const double dx = S.Y[0][b] - cx, dy = S.Y[1][b] - cy, dz = S.Y[2][b] - cz, dd = dx * dx + dy * dy + dz * dz;
+                if (dd < bd) { bd = dd; best = b; }
+            }
+            S.refbody = best;
+#ifdef GENGA_BC_PROF
+            S.dbg_rebuild = 0; S.dbg_total = 0;
+#endif
         }
         __syncthreads();
     }
+    BcList lst;
+    lst.rows = 1; lst.npad = n | 1; lst.magic = 0xffffffffu / (unsigned)(n | 1) + 1u; lst.valid = false;
+    lst.age = 0; lst.early = 0; lst.ref = S.refbody;
     // ---- master: the step-size control of the sequential algorithm; everybody: rounds as they are published
     double done = 0.0, H = h;
     bool last = true;                             // the first trial step is the whole interval
-    if (master && tid == 0) {                     // first round of this group: the state is already in every CTA
-        for (int r = 0; r < NCTA; ++r) {
-            Smem *R = cluster.map_shared_rank(&S, r);
-            R->seq_begin = seq + 1; R->rec_H = H; R->rec_state = 0;
-        }
-        __threadfence();
-        for (int r = 0; r < NCTA; ++r) cluster.map_shared_rank(&S, r)->seq_end = seq + 1;
+    if (master && tid < NCTA) {                   // first round of this group: the state is already in every CTA
+        Smem *R = cluster.map_shared_rank(&S, tid);
+        R->seq_begin = seq + 1; R->rec_H = H; R->rec_state = 0;
+        bc_fence();
+        R->seq_end = seq + 1;
     }
     int ok = 1;
 #ifdef GENGA_BC_PROF
-    long long pf_t = clock64(), pf_acc[6] = {0, 0, 0, 0, 0, 0};   // record, rhs, wait, check, publish, calls
+    long long pf_t = clock64(), pf_acc[6] = {0, 0, 0, 0, 0, 0}, pc_cyc = 0; int pc_calls = 0;   // record, rhs, wait, check, publish, calls
 #define BC_PROF(k) { const long long now_ = clock64(); pf_acc[k] += now_ - pf_t; pf_t = now_; }
 #else
 #define BC_PROF(k)
@@ -443,7 +620,6 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
         double q[3] = {1.0, 0.0, 0.0}, V[3] = {0.0, 1.0, 0.0};
         do {
             e = bc_wait_change(S, &S.seq_end, seq);
-            __threadfence();
             Hr = S.rec_H; state = S.rec_state;
             if (t.owner) {
 #pragma unroll
@@ -452,15 +628,21 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
             if (checker && state == 0) {
                 for (int b = tid; b < n; b += THREADS) {
                     const double x = S.Y[0][b], y = S.Y[1][b], z = S.Y[2][b], vx = S.Y[3][b], vy = S.Y[4][b], vz = S.Y[5][b];
-                    S.isq[b] = 1.0 / (x * x + y * y + z * z);
-                    S.isv[b] = 1.0 / (vx * vx + vy * vy + vz * vz);
+                    S.isq[b] = rcp_fast(x * x + y * y + z * z);
+                    S.isv[b] = rcp_fast(vx * vx + vy * vy + vz * vz);
                 }
             }
-            __threadfence();
-            consistent = __syncthreads_and(S.seq_begin == e) != 0;
+            __syncthreads();                      // every thread has read its part of the record
+            if (tid == 0) { bc_fence(); S.ok = S.seq_begin == e ? 1 : 0; }
+            __syncthreads();
+            consistent = S.ok != 0;
         } while (!consistent);
         seq = e;
+        lst.early = 0;
         BC_PROF(0)
+#ifdef GENGA_BC_TL
+        long long tl_[20]; for (int z = 0; z < 20; ++z) tl_[z] = 0; const long long tl0_ = clock64();
+#endif
         if (state != 0) { ok = state == 1 ? 1 : state == 3 ? 2 : 0; break; }
         const double Hl = ldexp(Hr, -lev);
         const bool under = lev > 0 && fabs(Hl) < BS_HMIN * fabs(h);
@@ -469,39 +651,65 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
             // ---- force at the starting state, then my column: Gragg's modified midpoint rule with 2 (col + 1) substeps,
             // two per evaluation (bc_rhs2): q_{k+1} = q_{k-1} + 2 eta V_k does not need a(q_k)
             double acc0[3], dummy[3];
-            dropped = bc_rhs2(S, t, buf, G, m0, q, q, acc0, dummy, &S.seq_end) != seq;
+#ifdef GENGA_BC_PROF
+            const long long c0_ = clock64();
+#endif
+#ifdef GENGA_BC_TL
+            long long tc_[10]; for (int z = 0; z < 10; ++z) tc_[z] = 0; const long long tc0_ = clock64(); int tcv_[10]; for (int z = 0; z < 10; ++z) tcv_[z] = 0;
+#endif
+            dropped = bc_rhs2(S, t, buf, G, m0, q, q, acc0, dummy, &S.seq_end, lst) != seq;
+#ifdef GENGA_BC_TL
+            tc_[0] = clock64() - tc0_; tcv_[0] = lst.valid;
+#endif
             const double eta = Hl / (2 * (col + 1));
-            double qa[3], Va[3], qb[3], Vb[3];
+            double qa[3] = {1.0, 0.0, 0.0}, Va[3] = {0.0, 0.0, 0.0}, qb[3] = {1.0, 0.0, 0.0}, Vb[3] = {0.0, 0.0, 0.0};
+            if (t.owner) {                        // the other warps only help with the pairs (bc_rhs2)
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                qa[c] = q[c]; Va[c] = V[c];
-                qb[c] = q[c] + eta * V[c]; Vb[c] = V[c] + eta * acc0[c];
+                for (int c = 0; c < 3; ++c) {
+                    qa[c] = q[c]; Va[c] = V[c];
+                    qb[c] = q[c] + eta * V[c]; Vb[c] = V[c] + eta * acc0[c];
+                }
             }
 #pragma unroll 1
             for (int it = 0; it <= col && !dropped; ++it) {
-                double qc[3], A[3], C[3];
+                double qc[3] = {1.0, 0.0, 0.0}, A[3], C[3];
+                if (t.owner) {
 #pragma unroll
-                for (int c = 0; c < 3; ++c) qc[c] = qa[c] + 2.0 * eta * Vb[c];
-                dropped = bc_rhs2(S, t, buf, G, m0, qb, qc, A, C, &S.seq_end) != seq;    // a newer round: drop this one
+                    for (int c = 0; c < 3; ++c) qc[c] = qa[c] + 2.0 * eta * Vb[c];
+                }
+                dropped = bc_rhs2(S, t, buf, G, m0, qb, qc, A, C, &S.seq_end, lst) != seq;    // a newer round: drop this one
+#ifdef GENGA_BC_TL
+                tc_[it + 1] = clock64() - tc0_; tcv_[it + 1] = lst.valid;
+#endif
+                if (t.owner) {
 #pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    double vc = Va[c] + 2.0 * eta * A[c];
-                    if (it == col && t.owner && !dropped) {
-                        SC->tab[col][c][i] = 0.5 * (qc[c] + qb[c] + eta * vc);
-                        SC->tab[col][3 + c][i] = 0.5 * (vc + Vb[c] + eta * C[c]);
+                    for (int c = 0; c < 3; ++c) {
+                        double vc = Va[c] + 2.0 * eta * A[c];
+                        if (it == col && !dropped) {
+                            SC->tab[col][c][i] = 0.5 * (qc[c] + qb[c] + eta * vc);
+                            SC->tab[col][3 + c][i] = 0.5 * (vc + Vb[c] + eta * C[c]);
+                        }
+                        double qd = qb[c] + 2.0 * eta * vc, vd = Vb[c] + 2.0 * eta * C[c];
+                        qa[c] = qc[c]; Va[c] = vc; qb[c] = qd; Vb[c] = vd;
                     }
-                    double qd = qb[c] + 2.0 * eta * vc, vd = Vb[c] + 2.0 * eta * C[c];
-                    qa[c] = qc[c]; Va[c] = vc; qb[c] = qd; Vb[c] = vd;
                 }
             }
+#ifdef GENGA_BC_PROF
+            if (!dropped) { pc_cyc += clock64() - c0_; pc_calls += col + 2; }
+#endif
             if (!dropped) {
-                __threadfence();
-                __syncthreads();
-                if (tid == 0) SC->ready[col] = seq;
+                __syncthreads();                  // the owners' column results are on their way to the checker
+                if (tid == 0) { bc_fence(); SC->ready[col] = seq; }
             }
+#ifdef GENGA_BC_TL
+            if (tid == 0 && rank == 7 && n >= 30 && n <= 40 && GENGA_BC_TL == 1) { printf("TC n %d dropped %d H %.3f:", n, (int)dropped, Hl); for (int z = 0; z < 9; ++z) printf(" %lld%c", tc_[z], tcv_[z] ? ' ' : '*'); printf("\n"); }
+#endif
         }
         BC_PROF(1)
         if (!checker) continue;
+#ifdef GENGA_BC_TL
+        tl_[0] = clock64() - tl0_;
+#endif
         // ---- checker of this level: rows 1.. as their columns arrive; first row whose error passes
         int code = under ? 0 : 1;                 // 0 underflow, 1 rejected, 2 + k passed at row k
         if (!under && !dropped) {
@@ -511,22 +719,27 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
                 if (tid == 0) {
                     int a;
                     while ((a = S.ready[k]) != seq && S.seq_end == seq) __nanosleep(20);
+                    bc_fence();
                     S.bc[0] = a == seq ? 1 : 0;
                 }
                 __syncthreads();
                 if (S.bc[0] == 0) { dropped = true; break; }
-                __threadfence();
                 BC_PROF(2)
+#ifdef GENGA_BC_TL
+                tl_[2 * k] = clock64() - tl0_;
+#endif
                 const double err = bc_check_row(S, n, k);
+#ifdef GENGA_BC_TL
+                tl_[2 * k + 1] = clock64() - tl0_;
+#endif
                 BC_PROF(3)
                 if (err <= eps2) { code = 2 + k; break; }
             }
         }
         if (dropped) continue;
         if (!master) {                            // report; T[k][k] stays in S.diag for the master
-            __threadfence();
             __syncthreads();
-            if (tid == 0) S0->lev_result[lev] = (seq << 8) | code;
+            if (tid == 0) { bc_fence(); S0->lev_result[lev] = (seq << 8) | code; }
             continue;
         }
         // ---- master: the first level, in the order H, H/2, .., that passed
@@ -540,6 +753,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
                 if (tid == 0) {
                     int v;
                     while (((v = S.lev_result[l]) >> 8) != seq) __nanosleep(20);
+                    bc_fence();
                     S.bc[0] = v & 255;
                 }
                 __syncthreads();
@@ -548,15 +762,15 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
                 if (cl == 0) { fail = true; break; }
             }
         }
-        __threadfence();
         int next_state = 0;
         if (fail) next_state = 2;
         else if (winner >= 0 && coll && bc_any_collision(S, cluster.map_shared_rank(&S, winner * BS_KMAX), n, ldexp(Hr, -winner))) next_state = 3;
         else if (winner >= 0) {
+            // the accepted state T[k][k] of the winning level becomes the master's Y (pushed to the others below)
             const Smem *SW = cluster.map_shared_rank(&S, winner * BS_KMAX);
-            for (int b = tid; b < 6 * n; b += THREADS) {
-                const int c = b / n, k = b - c * n;
-                S.Y[c][k] = SW->diag[c][k];
+            for (int k = tid; k < n; k += THREADS) {
+#pragma unroll
+                for (int c = 0; c < 6; ++c) S.Y[c][k] = SW->diag[c][k];
             }
             const double Hw = ldexp(Hr, -winner);
             done += Hw; H = Hw;
@@ -574,37 +788,39 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
             if (fabs(rem) <= 8.0 * 2.220446049250313e-16 * fabs(h)) next_state = 1;     // a remainder of a few ulp of h: done
             else if (fabs(H) >= fabs(rem)) { H = rem; last = true; }
         }
-        // ---- publish the next record (and the new state) to every CTA of the cluster
+        // ---- publish the next record (and the new state) to every CTA of the cluster: sequence number first, then the
+        // data, then the sequence number again (a reader that finds the two equal has a consistent record).  Lane r of the
+        // first warp writes the words of CTA r; (body, CTA) pairs are spread over the block for the state.
         const int ns = seq + 1;
         __syncthreads();
-        if (tid == 0) {
-            for (int r = 0; r < NCTA; ++r) cluster.map_shared_rank(&S, r)->seq_begin = ns;
-            __threadfence();
+        if (tid < NCTA) {
+            cluster.map_shared_rank(&S, tid)->seq_begin = ns;
+            bc_fence();
         }
         __syncthreads();
         if (winner >= 0 && next_state == 0) {
-            for (int r = 1; r < NCTA; ++r) {
+            for (int idx = tid; idx < n * NCTA; idx += THREADS) {
+                const int r = idx % NCTA, k = idx / NCTA;
+                if (r == 0) continue;
                 Smem *R = cluster.map_shared_rank(&S, r);
-                for (int b = tid; b < 6 * n; b += THREADS) {
-                    const int c = b / n, k = b - c * n;
-                    R->Y[c][k] = S.Y[c][k];
-                }
+#pragma unroll
+                for (int c = 0; c < 6; ++c) R->Y[c][k] = S.Y[c][k];
             }
         }
-        __threadfence();
+        if (tid < NCTA) {
+            Smem *R = cluster.map_shared_rank(&S, tid);
+            R->rec_H = H; R->rec_state = next_state;
+        }
         __syncthreads();
-        if (tid == 0) {
-            for (int r = 0; r < NCTA; ++r) {
-                Smem *R = cluster.map_shared_rank(&S, r);
-                R->rec_H = H; R->rec_state = next_state;
-            }
-            __threadfence();
-            for (int r = 0; r < NCTA; ++r) cluster.map_shared_rank(&S, r)->seq_end = ns;
-        }
+        if (tid < NCTA) { bc_fence(); cluster.map_shared_rank(&S, tid)->seq_end = ns; }
         BC_PROF(4)
+#ifdef GENGA_BC_TL
+        if (tid == 0 && n >= 30 && n <= 40 && GENGA_BC_TL == 2) { tl_[16] = clock64() - tl0_; printf("TL n %d winner %d row %d col0 %lld |", n, winner, wrow, tl_[0]); for (int z = 1; z < 8; ++z) printf(" %lld-%lld", tl_[2 * z], tl_[2 * z + 1]); printf(" | pub %lld\n", tl_[16]); }
+#endif
     }
 #ifdef GENGA_BC_PROF
     if (master && tid == 0 && nsteps) { for (int k = 0; k < 5; ++k) nsteps[2 + k] = (int)(pf_acc[k] >> 4); }
+    if (tid == 0 && (rank == 7 || rank == 3 || rank == 0) && pc_calls) printf("col %d n %d calls %d cycles/call %d rebuilds %d list %d\n", rank, n, pc_calls, (int)(pc_cyc / pc_calls), S.dbg_rebuild, S.dbg_total);
 #endif
     return ok;
 }
