@@ -433,6 +433,15 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
 // Orders this thread's accesses to the shared memory of the cluster's CTAs (the round record, the column results, the
 // flags): cluster scope is enough, and far cheaper than the device-wide fence with its L1 invalidation.
 __device__ __forceinline__ void bc_fence() { asm volatile("fence.acq_rel.cluster;" ::: "memory"); }
+// Polling a flag another CTA of the cluster sets after it has fenced its data: an acquire load (measured ~30 cycles; a
+// fence after a plain load ~290, it is a device-wide MEMBAR with an L1 invalidation whatever scope is asked for).
+__device__ __forceinline__ int bc_ld_acquire(const volatile int *flag)
+{
+    int v;
+    const unsigned a = (unsigned)__cvta_generic_to_shared(const_cast<const int *>(flag));
+    asm volatile("ld.acquire.cluster.shared::cta.b32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
 
 template <int MAXN, int THREADS>
 __device__ __forceinline__ double bc_block_max(BcSmem<MAXN, THREADS> &S, double v)
@@ -454,8 +463,7 @@ __device__ __forceinline__ int bc_wait_change(BcSmem<MAXN, THREADS> &S, const vo
     __syncthreads();
     if (threadIdx.x == 0) {
         int v;
-        while ((v = *flag) == old) __nanosleep(20);
-        bc_fence();                 // what the writer stored before the flag is visible to this thread, and after the barrier to the block
+        while ((v = bc_ld_acquire(flag)) == old) __nanosleep(20);      // what the writer stored before the flag is visible to this thread, and after the barrier to the block
         S.bc[0] = v;
     }
     __syncthreads();
@@ -505,6 +513,39 @@ __device__ __forceinline__ double bc_check_row(BcSmem<MAXN, THREADS> &S, const i
         e = fmax(e, fmax(dq * isq, dv * isv));
     }
     return bc_block_max(S, e);
+}
+
+// The same for groups of at most THREADS / 8 bodies (one tableau entry per thread), row after row: the thread keeps the
+// previous row T[k-1][0..k-1] of its entry in prow, so row k costs k steps of the recurrence instead of the whole
+// triangle, with the same operands in the same order (the result is bit for bit the one of bc_check_row).
+template <int MAXN, int THREADS>
+__device__ __forceinline__ double bc_check_row_inc(BcSmem<MAXN, THREADS> &S, const int n, const int k, double (&prow)[BS_KMAX])
+{
+    const int i8 = threadIdx.x >> 3, c = threadIdx.x & 7;
+    double d2 = 0.0;
+    if (c < 6 && i8 < n) {
+        if (k == 1) prow[0] = S.tab[0][c][i8];
+        double cur = S.tab[k][c][i8], prev = prow[0], diff = 0.0;
+        prow[0] = cur;
+#pragma unroll
+        for (int j = 1; j < BS_KMAX; ++j) {
+            if (j <= k) {
+                const double tmp = prow[j];
+                const double nxt = cur + (cur - prev) * c_bs_iden.v[k][j];
+                diff = nxt - cur;
+                cur = nxt;
+                prow[j] = cur;
+                prev = tmp;
+            }
+        }
+        S.diag[c][i8] = cur;
+        d2 = diff * diff;
+    }
+    const int base = (threadIdx.x & 31) & ~7;
+    const double isq = i8 < n ? S.isq[i8] : 0.0, isv = i8 < n ? S.isv[i8] : 0.0;
+    const double dq = __shfl_sync(0xffffffffu, d2, base) + __shfl_sync(0xffffffffu, d2, base + 1) + __shfl_sync(0xffffffffu, d2, base + 2);
+    const double dv = __shfl_sync(0xffffffffu, d2, base + 3) + __shfl_sync(0xffffffffu, d2, base + 4) + __shfl_sync(0xffffffffu, d2, base + 5);
+    return bc_block_max(S, fmax(dq * isq, dv * isv));
 }
 
 // Master: does a pair of the group collide in the step just accepted (L328: the Hermite minimum of Eq. 10-12 over the
@@ -639,6 +680,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
         } while (!consistent);
         seq = e;
         lst.early = 0;
+        lst.valid = false;                        // the state has jumped: the old list fails its check more often than not
         BC_PROF(0)
 #ifdef GENGA_BC_TL
         long long tl_[20]; for (int z = 0; z < 20; ++z) tl_[z] = 0; const long long tl0_ = clock64();
@@ -712,14 +754,14 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
 #endif
         // ---- checker of this level: rows 1.. as their columns arrive; first row whose error passes
         int code = under ? 0 : 1;                 // 0 underflow, 1 rejected, 2 + k passed at row k
+        double prow[BS_KMAX] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
         if (!under && !dropped) {
             for (int k = 1; k < BS_KMAX; ++k) {
                 // wait for column k of this round (or for a newer round: checkers of the levels behind the first)
                 __syncthreads();
                 if (tid == 0) {
                     int a;
-                    while ((a = S.ready[k]) != seq && S.seq_end == seq) __nanosleep(20);
-                    bc_fence();
+                    while ((a = bc_ld_acquire(&S.ready[k])) != seq && S.seq_end == seq) __nanosleep(20);
                     S.bc[0] = a == seq ? 1 : 0;
                 }
                 __syncthreads();
@@ -728,7 +770,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
 #ifdef GENGA_BC_TL
                 tl_[2 * k] = clock64() - tl0_;
 #endif
-                const double err = bc_check_row(S, n, k);
+                const double err = n <= THREADS / 8 ? bc_check_row_inc(S, n, k, prow) : bc_check_row(S, n, k);
 #ifdef GENGA_BC_TL
                 tl_[2 * k + 1] = clock64() - tl0_;
 #endif
@@ -752,8 +794,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
                 __syncthreads();
                 if (tid == 0) {
                     int v;
-                    while (((v = S.lev_result[l]) >> 8) != seq) __nanosleep(20);
-                    bc_fence();
+                    while (((v = bc_ld_acquire(&S.lev_result[l])) >> 8) != seq) __nanosleep(20);
                     S.bc[0] = v & 255;
                 }
                 __syncthreads();
