@@ -43,7 +43,7 @@ struct BcSmem {
     float thr2[MAXN];               // (rc_i + margin)^2 rounded up
     double m[MAXN], rc[MAXN], irc[MAXN];
     double R[MAXN];                 // physical radii (collision test; < 0: none)
-    double Y[6][MAXN];              // state the current round starts from (pushed by the master)
+    alignas(16) double Y[6][MAXN];  // state the current round starts from (pushed by the master)
     double tab[BS_KMAX][6][MAXN];   // checker: column results T[k][0] of its level
     double diag[6][MAXN];           // checker: T[k][k] of the row tested last
     double red[THREADS / 32];
@@ -84,8 +84,9 @@ struct BcList {
     unsigned magic;     // ceil(2^32 / npad): entry / npad without a division
     bool valid;
     int age;            // evaluations the current list has served
-    int early;          // lists of this round that were outdated at their first check: after two of them the round stops
-                        // checking (steps this long move the bodies by more than the skin every time) and makes a new one each time
+    double span, span_fail;   // time between this evaluation and the one before (set by the caller); the shortest one after
+                        // which a list was found outdated at its first check: from there on (long trial steps, few
+                        // substeps) a new list is made every time without trying the old one first
     int ref;            // the body the rigid motion is taken from: the one nearest the group's centre
 };
 
@@ -238,7 +239,7 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
             const int st = (GENGA_MB & 32) ? 0 : S.stale[sb];
             listed = !(st & 1);
             if (st) lst.valid = false;                            // this list was used for the last time
-            if (!listed && lst.age == 0) ++lst.early;
+            if (!listed && lst.age == 0) lst.span_fail = fmin(lst.span_fail, lst.span);
             ++lst.age;
             if (listed && ow >= THREADS) {                        // no warp to spare: the pairs after the check
                 bc_pairs(S, pA, pB, G, m0, lst, n, 0);
@@ -290,7 +291,7 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
             RHS_PROF()
             const int kmax = S.kmax[sb];
             listed = (kmax + 1) * npad <= BC_MAXP;
-            lst.valid = listed && S.skin2 > 0.f && lst.early < 2;
+            lst.valid = listed && S.skin2 > 0.f && lst.span < lst.span_fail;
             lst.age = 0;
             lst.rows = kmax + 1;
 #ifdef GENGA_BC_PROF
@@ -636,7 +637,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
     }
     BcList lst;
     lst.rows = 1; lst.npad = n | 1; lst.magic = 0xffffffffu / (unsigned)(n | 1) + 1u; lst.valid = false;
-    lst.age = 0; lst.early = 0; lst.ref = S.refbody;
+    lst.age = 0; lst.span = 0.0; lst.span_fail = 1.0e300; lst.ref = S.refbody;
     // ---- master: the step-size control of the sequential algorithm; everybody: rounds as they are published
     double done = 0.0, H = h;
     bool last = true;                             // the first trial step is the whole interval
@@ -679,7 +680,6 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
             consistent = S.ok != 0;
         } while (!consistent);
         seq = e;
-        lst.early = 0;
         lst.valid = false;                        // the state has jumped: the old list fails its check more often than not
         BC_PROF(0)
 #ifdef GENGA_BC_TL
@@ -704,6 +704,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
             tc_[0] = clock64() - tc0_; tcv_[0] = lst.valid;
 #endif
             const double eta = Hl / (2 * (col + 1));
+            lst.span = fabs(2.0 * eta);
             double qa[3] = {1.0, 0.0, 0.0}, Va[3] = {0.0, 0.0, 0.0}, qb[3] = {1.0, 0.0, 0.0}, Vb[3] = {0.0, 0.0, 0.0};
             if (t.owner) {                        // the other warps only help with the pairs (bc_rhs2)
 #pragma unroll
@@ -744,7 +745,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
                 if (tid == 0) { bc_fence(); SC->ready[col] = seq; }
             }
 #ifdef GENGA_BC_TL
-            if (tid == 0 && rank == 7 && n >= 30 && n <= 40 && GENGA_BC_TL == 1) { printf("TC n %d dropped %d H %.3f:", n, (int)dropped, Hl); for (int z = 0; z < 9; ++z) printf(" %lld%c", tc_[z], tcv_[z] ? ' ' : '*'); printf("\n"); }
+            if (tid == 0 && rank == GENGA_BC_TLR && n >= 30 && n <= 40 && GENGA_BC_TL == 1) { printf("TC n %d dropped %d H %.3f:", n, (int)dropped, Hl); for (int z = 0; z < 9; ++z) printf(" %lld%c", tc_[z], tcv_[z] ? ' ' : '*'); printf("\n"); }
 #endif
         }
         BC_PROF(1)
@@ -785,6 +786,9 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
             continue;
         }
         // ---- master: the first level, in the order H, H/2, .., that passed
+#ifdef GENGA_BC_TL
+        tl_[15] = clock64() - tl0_;
+#endif
         int winner = -1, wrow = 0;
         bool fail = false;
         if (code >= 2) { winner = 0; wrow = code - 2; }
@@ -802,6 +806,14 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
                 if (cl >= 2) { winner = l; wrow = cl - 2; break; }
                 if (cl == 0) { fail = true; break; }
             }
+        }
+        // a record will be published whatever the outcome: its sequence number goes out first (a reader that finds
+        // seq_begin != seq_end knows the record is being rewritten), now, so that its fence overlaps the work below
+        const int ns = seq + 1;
+        __syncthreads();
+        if (tid < NCTA) {
+            cluster.map_shared_rank(&S, tid)->seq_begin = ns;
+            bc_fence();
         }
         int next_state = 0;
         if (fail) next_state = 2;
@@ -829,23 +841,21 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
             if (fabs(rem) <= 8.0 * 2.220446049250313e-16 * fabs(h)) next_state = 1;     // a remainder of a few ulp of h: done
             else if (fabs(H) >= fabs(rem)) { H = rem; last = true; }
         }
-        // ---- publish the next record (and the new state) to every CTA of the cluster: sequence number first, then the
-        // data, then the sequence number again (a reader that finds the two equal has a consistent record).  Lane r of the
-        // first warp writes the words of CTA r; (body, CTA) pairs are spread over the block for the state.
-        const int ns = seq + 1;
-        __syncthreads();
-        if (tid < NCTA) {
-            cluster.map_shared_rank(&S, tid)->seq_begin = ns;
-            bc_fence();
-        }
-        __syncthreads();
+        // ---- publish the next record (and the new state) to every CTA of the cluster, then the sequence number again.
+        // Lane r of the first warp writes the words of CTA r; the state goes out in 16-byte stores (two bodies of one
+        // component), spread over the block: what a store to another CTA's shared memory costs is the packet, not its size
+        // (8-byte stores: 2.9 k cycles for 30 bodies, measured).
+        __syncthreads();                          // seq_begin is out (fenced), the master's Y is complete
+#ifdef GENGA_BC_TL
+        tl_[18] = clock64() - tl0_;
+#endif
         if (winner >= 0 && next_state == 0) {
-            for (int idx = tid; idx < n * NCTA; idx += THREADS) {
-                const int r = idx % NCTA, k = idx / NCTA;
+            const int np2 = (n + 1) >> 1;         // pairs of bodies (Y rows are MAXN long, MAXN even: the odd one out copies a spare)
+            for (int idx = tid; idx < 6 * np2 * NCTA; idx += THREADS) {
+                const int r = idx % NCTA, w = idx / NCTA, c = w / np2, kp = w - c * np2;
                 if (r == 0) continue;
                 Smem *R = cluster.map_shared_rank(&S, r);
-#pragma unroll
-                for (int c = 0; c < 6; ++c) R->Y[c][k] = S.Y[c][k];
+                *reinterpret_cast<double2 *>(&R->Y[c][2 * kp]) = *reinterpret_cast<const double2 *>(&S.Y[c][2 * kp]);
             }
         }
         if (tid < NCTA) {
@@ -853,10 +863,13 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
             R->rec_H = H; R->rec_state = next_state;
         }
         __syncthreads();
+#ifdef GENGA_BC_TL
+        tl_[19] = clock64() - tl0_;
+#endif
         if (tid < NCTA) { bc_fence(); cluster.map_shared_rank(&S, tid)->seq_end = ns; }
         BC_PROF(4)
 #ifdef GENGA_BC_TL
-        if (tid == 0 && n >= 30 && n <= 40 && GENGA_BC_TL == 2) { tl_[16] = clock64() - tl0_; printf("TL n %d winner %d row %d col0 %lld |", n, winner, wrow, tl_[0]); for (int z = 1; z < 8; ++z) printf(" %lld-%lld", tl_[2 * z], tl_[2 * z + 1]); printf(" | pub %lld\n", tl_[16]); }
+        if (tid == 0 && n >= 30 && n <= 40 && GENGA_BC_TL == 2) { tl_[16] = clock64() - tl0_; printf("TL n %d winner %d row %d col0 %lld |", n, winner, wrow, tl_[0]); for (int z = 1; z < 8; ++z) printf(" %lld-%lld", tl_[2 * z], tl_[2 * z + 1]); printf(" | dec %lld copy %lld seqb %lld push %lld pub %lld\n", tl_[15], tl_[17], tl_[18], tl_[19], tl_[16]); }
 #endif
     }
 #ifdef GENGA_BC_PROF
