@@ -851,11 +851,12 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
 #endif
         if (winner >= 0 && next_state == 0) {
             const int np2 = (n + 1) >> 1;         // pairs of bodies (Y rows are MAXN long, MAXN even: the odd one out copies a spare)
-            for (int idx = tid; idx < 6 * np2 * NCTA; idx += THREADS) {
-                const int r = idx % NCTA, w = idx / NCTA, c = w / np2, kp = w - c * np2;
+            for (int idx = tid; idx < np2 * NCTA; idx += THREADS) {
+                const int r = idx % NCTA, kp = idx / NCTA;
                 if (r == 0) continue;
                 Smem *R = cluster.map_shared_rank(&S, r);
-                *reinterpret_cast<double2 *>(&R->Y[c][2 * kp]) = *reinterpret_cast<const double2 *>(&S.Y[c][2 * kp]);
+#pragma unroll
+                for (int c = 0; c < 6; ++c) *reinterpret_cast<double2 *>(&R->Y[c][2 * kp]) = *reinterpret_cast<const double2 *>(&S.Y[c][2 * kp]);
             }
         }
         if (tid < NCTA) {

@@ -36,6 +36,8 @@ struct BsmSmem {
     int status[BSM_MAXL];                        // 0 running, 1 + k accepted at row k, -1 rejected, -2 step size underflow
     double R[BW_MAXN];                           // physical radii (collision test; < 0: none)
     int coll;                                    // look for collisions in every accepted step (L328)
+    BwGroup8 grp;                                // S = 8: (rc, G m) of the bodies
+    BwSlot8 slot[BSM_SLOTS];                     // S = 8: positions of each column segment (bw_rhs2_seg8)
 };
 
 // Does a pair of the group collide in the step just accepted (L328: the Hermite minimum of Eq. 10-12 over the step
@@ -111,6 +113,25 @@ __device__ __forceinline__ int bsm_integrate(BsmSmem &W, const int n, const doub
         gm[t] = valid ? G * mj : 0.0;
     }
 
+    // S = 8: FP32 pretest threshold of this body: positions stay within Q = 2 max_b(|q_b| + |h| |V_b|) (max norms) of the
+    // origin during the step, so rounding them to FP32 moves a separation by < 2^-22 Q and the FP32 evaluation of its
+    // square adds < 2^-21 relative: thr = (rc + 2^-20 Q)^2 (1 + 2^-18) (as bs_cluster.cuh); bodies without mass exert no
+    // force and are left out of everybody's partner mask.
+    float thr = 0.f;
+    unsigned massive = 0u;
+    BwSlot8 &myslot = W.slot[slot % BSM_SLOTS];
+    if constexpr (S == 8) {
+        double qm = body ? fmax(fmax(fabs(Y[0]), fabs(Y[1])), fabs(Y[2])) + fabs(h) * fmax(fmax(fabs(Y[3]), fabs(Y[4])), fabs(Y[5])) : 0.0;
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) qm = fmax(qm, __shfl_xor_sync(full, qm, o, 8));
+        const double w = my_rc + 0x1.0p-20 * 2.0 * qm;
+        thr = body ? __double2float_ru(w * w * (1.0 + 0x1.0p-18)) : 0.f;
+        massive = __ballot_sync(full, body && my_m != 0.0);
+        massive = (massive >> (lane & 24)) & 0xffu;               // the eight lanes of my segment
+        if (warp == 0 && lane < 8) W.grp.rcm[lane] = make_double2(body ? my_rc : 0.0, body ? G * my_m : 0.0);
+        __syncthreads();
+    }
+
     double done = 0.0, H = h;
     bool last = false, fresh = true;
     const double eps2 = eps * eps;
@@ -129,8 +150,8 @@ __device__ __forceinline__ int bsm_integrate(BsmSmem &W, const int n, const doub
                 for (int c = 0; c < 6; ++c) W.Y[c][b] = Y[c];
             }
             double dummy[3];
-            if constexpr (S == 8) bw_rhs2_seg8(q, q, n, b, Gm0, G, my_rc, my_m, rcij, acc0, dummy);
-            else bw_rhs2<S>(q, q, Gm0, src, rcij, irc, gm, acc0, dummy);
+            if constexpr (S == 8) bw_rhs2_seg8(W.grp, myslot, q, q, n, b, Gm0, my_rc, thr, massive, acc0, dummy);
+            else bw_rhs2<S>(q, q, Gm0, src, rcij, irc, gm, n, acc0, dummy);
             __syncthreads();
             if (checker) {
 #pragma unroll
@@ -173,8 +194,8 @@ __device__ __forceinline__ int bsm_integrate(BsmSmem &W, const int n, const doub
                 double qc[3], A[3], C[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) qc[c] = qa[c] + 2.0 * eta * Vb[c];
-                if constexpr (S == 8) bw_rhs2_seg8(qb, qc, n, b, Gm0, G, my_rc, my_m, rcij, A, C);
-                else bw_rhs2<S>(qb, qc, Gm0, src, rcij, irc, gm, A, C);
+                if constexpr (S == 8) bw_rhs2_seg8(W.grp, myslot, qb, qc, n, b, Gm0, my_rc, thr, massive, A, C);
+                else bw_rhs2<S>(qb, qc, Gm0, src, rcij, irc, gm, n, A, C);
                 const bool fin = it == col;
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
