@@ -16,16 +16,14 @@
 // works on the round it finds, drops it as soon as a newer record appears (it looks once per evaluation), and signals
 // its finished column with one remote flag store.  A CTA that lags simply joins the current round.
 //
-// Inside a CTA, body i owns L adjacent lanes (a power of two, at most a warp); lane s of the segment takes partners
-// j = s, s+L, ...; the segment sum is an xor-butterfly (fixed order); lane 0 of the segment ("owner") carries the
-// body's midpoint state in registers.  Positions are exchanged through a double-buffered shared array: one
-// __syncthreads per force evaluation.
+// Inside a CTA, thread i < n OWNS body i: it carries the body's midpoint state in registers, writes its positions to
+// a double-buffered shared array before every force evaluation and adds up the forces on it afterwards (bc_rhs2); the
+// other warps only evaluate pairs.  What an evaluation costs is the owners' dependent chain, counted in instructions
+// (one warp per scheduler issues a dependent instruction every 5-9 cycles) and barriers (44 cycles each for 16 warps),
+// and what a round costs beyond its evaluations is the master's own chain (its column, the tableau rows one after the
+// other, the publication): both were measured with clock64 traces and shortened step by step (profiles/r2_bs_chain.md).
 #pragma once
-#ifndef GENGA_MB
-#define GENGA_MB 0
-#endif
 #include <cooperative_groups.h>
-#include <cstdio>
 
 #include "bs.cuh"
 
@@ -33,7 +31,7 @@ namespace genga {
 
 namespace cg = cooperative_groups;
 
-constexpr int BC_MAXP = 768;         // ordered close pairs the list path of bc_rhs2 takes (sparse groups: a few per body)
+constexpr int BC_MAXP = 768;         // entries of the pair table of bc_rhs2: (most partners of one body + 1) x (n | 1) must fit
 
 template <int MAXN, int THREADS>
 struct BcSmem {
@@ -54,12 +52,9 @@ struct BcSmem {
     int stale[2];                   // an owner found the list outdated (double-buffered like pos)
     int refbody;                    // the body nearest the group's centre
     int ok;                         // block-local broadcast: the record just read is consistent
-#ifdef GENGA_BC_PROF
-    int dbg_rebuild, dbg_total;
-#endif
     float4 ref[MAXN];               // positions (FP32) at the evaluation the list was built from
     int cnt[MAXN];                  // partners of body i in the list
-    float skin2;                    // the list stays valid while every |(q_i - q_0) - ref_i|^2 < skin2 (0: never)
+    float skin2;                    // the list stays valid while every body has moved, in the central body's frame, by less than sqrt(skin2) (0: never)
     // ---- round record, written by the master under a sequence lock (seq_begin first, seq_end last).  Round numbers
     // run on from group to group, so a flag of an older round never equals a current one.
     volatile int seq_begin, seq_end;
@@ -160,14 +155,18 @@ __device__ __forceinline__ void bc_pairs(BcSmem<MAXN, THREADS> &S, const double 
 // ~50): so the owners are the first n threads (few warps convert and integrate, the others only help with the pairs), and
 // nothing on the per-evaluation path is reduced by shuffles.
 //
-// LIST PATH (n <= 32 L, at most BC_MAXP entries: the sparse chains of a planetesimal disc).  The n^2 examinations are
-// done in FP32 against a threshold widened by more than the FP32 rounding AND by the skin BC_SKIN rc, L lanes per body;
-// the hits are compacted into one list (block-wide prefix sum, body by body, fixed order).  The list is then KEPT: an
-// evaluation first checks that no body has moved, after the rigid motion that takes body 0 back to where it was (a rigid
-// motion keeps every distance), by more than half the skin; if so no pair outside the list can have come inside rc_ij,
-// and the n^2 pass is skipped.  One thread per listed ordered pair evaluates the exact FP64 test and both changeover
-// weights (a listed pair outside rc_ij gives zero), one thread per body the star; the owner adds up its own contiguous
-// range of the list, in list order.
+// LIST PATH (n <= 32 L and the table fits: the sparse chains of a planetesimal disc).  The n^2 examinations are done in
+// FP32 against a threshold widened by more than the FP32 rounding AND by the skin BC_SKIN rc, L lanes per body; the k-th
+// hit of body i goes to entry (k + 1) npad + i of the table S.part (k from a prefix sum over the body's L lanes: one
+// barrier, no block-wide compaction).  The table is then KEPT: the owners check that no body has moved, after the rigid
+// motion that takes the central body back to where it was (a rigid motion keeps every distance), by more than half the
+// skin; if so no pair outside the table can have come inside rc_ij and the n^2 pass is skipped.  While they check, the
+// warps that own nothing already evaluate the table (bc_pairs: exact FP64 test and both changeover weights of every
+// listed ordered pair, zero where it is outside rc_ij; row 0: the star); if the check fails their work is thrown
+// away and a new table is made.  At 70 % of the skin the table is used once more and dropped; a round starts with a new
+// one (the state has jumped), and trial steps so long that a table never survives to its first check (lst.span_fail:
+// differential rotation moves the members of a group against each other by more than the skin) make a new one every time
+// without trying.  The owner adds up its own column of the table, top to bottom.
 // Dense or very large groups keep the direct loop: the lanes of a body evaluate their own hits and reduce by shuffles.
 // One thread copies *watch (the master's round number) into S.bc[buf] before the first barrier of this evaluation; the
 // value every thread finds there afterwards is returned.
@@ -177,13 +176,6 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
                                        const volatile int *watch, BcList &lst)
 {
     GENGA_BS_RHS_HOOK();
-#ifdef GENGA_BC_PROF_RHS
-    long long ph_[10]; int phn_ = 0;
-#define RHS_PROF() ph_[phn_++] = clock64();
-#else
-#define RHS_PROF()
-#endif
-    RHS_PROF()
     double(*pA)[MAXN] = S.pos[buf][0];
     double(*pB)[MAXN] = S.pos[buf][1];
     float4 *fA = S.pf[buf][0];
@@ -194,17 +186,14 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
             pA[c][t.i] = qA[c]; pB[c][t.i] = qB[c];
         }
         const float th = S.thr2[t.i];
-        if (!(GENGA_MB & 2)) {
         fA[t.i] = make_float4((float)qA[0], (float)qA[1], (float)qA[2], th);
         fB[t.i] = make_float4((float)qB[0], (float)qB[1], (float)qB[2], th);
-        }
     }
-    if (threadIdx.x == THREADS - 32 && !(GENGA_MB & 16)) S.bc[buf] = *watch;     // a thread that owns nothing: the owners' warp does not wait for this
+    if (threadIdx.x == THREADS - 32) S.bc[buf] = *watch;     // a thread that owns nothing: the owners' warp does not wait for this
     __syncthreads();
-    const int seen = (GENGA_MB & 16) ? 1 : S.bc[buf];
+    const int seen = S.bc[buf];
     const int sb = buf;
-    if (threadIdx.x == THREADS - 32 && !(GENGA_MB & 32)) { S.stale[buf ^ 1] = 0; S.kmax[buf ^ 1] = 0; }                  // read last in the evaluation before this one
-    RHS_PROF()
+    if (threadIdx.x == THREADS - 32) { S.stale[buf ^ 1] = 0; S.kmax[buf ^ 1] = 0; }                  // read last in the evaluation before this one
     buf ^= 1;
     double ax = 0.0, ay = 0.0, az = 0.0, bx = 0.0, by = 0.0, bz = 0.0;
     const int n = t.n, L = t.L, i = t.pi;                         // below, i is the body whose pairs this lane examines
@@ -218,7 +207,7 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
             // check fails (rare), what they wrote is thrown away
             const int ow = (n + 31) & ~31;                        // threads of the owners' warps
             bool still = true;
-            if (t.owner && !(GENGA_MB & 1)) {
+            if (t.owner) {
                 // rigid motion taken out first: the rotation about z that puts the central body back on its old azimuth, then its shift
                 const float4 oA = fA[lst.ref], oB = fB[lst.ref], o = S.ref[lst.ref], r = S.ref[t.i], mA = fA[t.i], mB = fB[t.i];
                 const float on = o.x * o.x + o.y * o.y;
@@ -233,10 +222,9 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
                 still = moved < S.skin2;
                 if (!(moved < 0.5f * S.skin2)) atomicOr(&S.stale[sb], still ? 2 : 3);     // 2: 70 % of the way: a new list next time
             }
-            if (ow < THREADS && !(GENGA_MB & 8)) bc_pairs(S, pA, pB, G, m0, lst, n, ow);
-            RHS_PROF()
-            if (!(GENGA_MB & 64)) __syncthreads();                                      // a plain barrier and a flag: half the price of a voting barrier
-            const int st = (GENGA_MB & 32) ? 0 : S.stale[sb];
+            if (ow < THREADS) bc_pairs(S, pA, pB, G, m0, lst, n, ow);
+            __syncthreads();                                      // a plain barrier and a flag: half the price of a voting barrier
+            const int st = S.stale[sb];
             listed = !(st & 1);
             if (st) lst.valid = false;                            // this list was used for the last time
             if (!listed && lst.age == 0) lst.span_fail = fmin(lst.span_fail, lst.span);
@@ -245,7 +233,6 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
                 bc_pairs(S, pA, pB, G, m0, lst, n, 0);
                 __syncthreads();
             }
-            RHS_PROF()
         }
         if (!listed) {
             // ---- pretest: bit kk = partner j = s + kk L passed at point A or B.  Four partners per trip, no early exit:
@@ -257,7 +244,7 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
                 if (t.s == 0) S.ref[i] = mA;
                 const int trips = (n - t.s + 4 * L - 1) / (4 * L);    // t.s < L <= n
 #pragma unroll 1
-                for (int q4 = 0; q4 < trips && !(GENGA_MB & 128); ++q4) {
+                for (int q4 = 0; q4 < trips; ++q4) {
                     unsigned bits = 0u;
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
@@ -276,27 +263,22 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
             const int lane = threadIdx.x & 31;
             const int cnt = __popc(mask);
             int pre = cnt;
-            if (!(GENGA_MB & 256)) for (int o = 1; o < L; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o, L); if (t.s >= o) pre += v; }
+            for (int o = 1; o < L; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o, L); if (t.s >= o) pre += v; }
             const int cseg = __shfl_sync(0xffffffffu, pre, L - 1, L);           // the body's partners
             const int wmax = __reduce_max_sync(0xffffffffu, cseg);
-            if (lane == 0 && wmax > 0 && !(GENGA_MB & 512)) atomicMax(&S.kmax[sb], wmax);
+            if (lane == 0 && wmax > 0) atomicMax(&S.kmax[sb], wmax);
             const int npad = lst.npad;
             if (live) {
                 if (t.s == 0) S.cnt[i] = cseg;
                 int slot = (pre - cnt + 1) * npad + i;
                 for (unsigned mm = mask; mm && slot < BC_MAXP; mm &= mm - 1, slot += npad) S.part[slot] = t.s + (__ffs(mm) - 1) * L;
             }
-            RHS_PROF()
             __syncthreads();
-            RHS_PROF()
             const int kmax = S.kmax[sb];
             listed = (kmax + 1) * npad <= BC_MAXP;
             lst.valid = listed && S.skin2 > 0.f && lst.span < lst.span_fail;
             lst.age = 0;
             lst.rows = kmax + 1;
-#ifdef GENGA_BC_PROF
-            if (threadIdx.x == 0) { ++S.dbg_rebuild; S.dbg_total = lst.rows * npad; }
-#endif
             if (listed) {
                 bc_pairs(S, pA, pB, G, m0, lst, n, 0);
                 __syncthreads();
@@ -327,7 +309,7 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
         if (listed) {
             // ---- the owner: the star, then its own range in list order; four entries per trip (their loads in flight
             // together), then one by one: as few instructions as possible, the owners' warp is alone on this stretch
-            if (t.owner && !(GENGA_MB & 4)) {
+            if (t.owner) {
                 const int row = 6 * lst.npad;
                 const double *e = S.pres[t.i];
                 int left = S.cnt[t.i];
@@ -350,7 +332,6 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
                     ax += v0.x; ay += v0.y; az += v1.x; bx += v1.y; by += v2.x; bz += v2.y;
                 }
             }
-            RHS_PROF()
             summed = true;
         }
     } else if (live) {
@@ -420,14 +401,6 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
     }
     aA[0] = ax; aA[1] = ay; aA[2] = az;
     aB[0] = bx; aB[1] = by; aB[2] = bz;
-#ifdef GENGA_BC_PROF_RHS
-    RHS_PROF()
-    if (threadIdx.x == 0 && t.n == 10 && (blockIdx.x & 15) == 3 && (seen & 15) == 3) {
-        printf("rhs n=%d blk=%d seq=%d rows=%d phases:", t.n, blockIdx.x & 7, seen, lst.rows);
-        for (int k = 1; k < phn_; ++k) printf(" %d", (int)(ph_[k] - ph_[k - 1]));
-        printf("\n");
-    }
-#endif
     return seen;
 }
 
@@ -606,7 +579,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
         }
         const double Q = 2.0 * bc_block_max(S, qm);
         // List path of bc_rhs2 (n <= 32 L): the pretest reaches out to (1 + BC_SKIN) rc, and the list is kept while every
-        // body stays within skin = BC_SKIN min_i rc_i / 2 of where it was, relative to body 0, when the list was made
+        // body stays within skin = BC_SKIN min_i rc_i / 2 of where it was, in the frame of the central body, when the list was made
         // (less 2^-19 Q for the FP32 roundings of that difference): a pair left out cannot have come inside rc_ij.
         const bool wide = n <= 32 * t.L;
         const double rcmin = -bc_block_max(S, t.owner ? -S.rc[i] : -1.0e300);
@@ -629,9 +602,6 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
                 if (dd < bd) { bd = dd; best = b; }
             }
             S.refbody = best;
-#ifdef GENGA_BC_PROF
-            S.dbg_rebuild = 0; S.dbg_total = 0;
-#endif
         }
         __syncthreads();
     }
@@ -649,7 +619,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
     }
     int ok = 1;
 #ifdef GENGA_BC_PROF
-    long long pf_t = clock64(), pf_acc[6] = {0, 0, 0, 0, 0, 0}, pc_cyc = 0; int pc_calls = 0;   // record, rhs, wait, check, publish, calls
+    long long pf_t = clock64(), pf_acc[6] = {0, 0, 0, 0, 0, 0};   // record, rhs, wait, check, publish, calls
 #define BC_PROF(k) { const long long now_ = clock64(); pf_acc[k] += now_ - pf_t; pf_t = now_; }
 #else
 #define BC_PROF(k)
@@ -682,9 +652,6 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
         seq = e;
         lst.valid = false;                        // the state has jumped: the old list fails its check more often than not
         BC_PROF(0)
-#ifdef GENGA_BC_TL
-        long long tl_[20]; for (int z = 0; z < 20; ++z) tl_[z] = 0; const long long tl0_ = clock64();
-#endif
         if (state != 0) { ok = state == 1 ? 1 : state == 3 ? 2 : 0; break; }
         const double Hl = ldexp(Hr, -lev);
         const bool under = lev > 0 && fabs(Hl) < BS_HMIN * fabs(h);
@@ -693,16 +660,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
             // ---- force at the starting state, then my column: Gragg's modified midpoint rule with 2 (col + 1) substeps,
             // two per evaluation (bc_rhs2): q_{k+1} = q_{k-1} + 2 eta V_k does not need a(q_k)
             double acc0[3], dummy[3];
-#ifdef GENGA_BC_PROF
-            const long long c0_ = clock64();
-#endif
-#ifdef GENGA_BC_TL
-            long long tc_[10]; for (int z = 0; z < 10; ++z) tc_[z] = 0; const long long tc0_ = clock64(); int tcv_[10]; for (int z = 0; z < 10; ++z) tcv_[z] = 0;
-#endif
             dropped = bc_rhs2(S, t, buf, G, m0, q, q, acc0, dummy, &S.seq_end, lst) != seq;
-#ifdef GENGA_BC_TL
-            tc_[0] = clock64() - tc0_; tcv_[0] = lst.valid;
-#endif
             const double eta = Hl / (2 * (col + 1));
             lst.span = fabs(2.0 * eta);
             double qa[3] = {1.0, 0.0, 0.0}, Va[3] = {0.0, 0.0, 0.0}, qb[3] = {1.0, 0.0, 0.0}, Vb[3] = {0.0, 0.0, 0.0};
@@ -721,9 +679,6 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
                     for (int c = 0; c < 3; ++c) qc[c] = qa[c] + 2.0 * eta * Vb[c];
                 }
                 dropped = bc_rhs2(S, t, buf, G, m0, qb, qc, A, C, &S.seq_end, lst) != seq;    // a newer round: drop this one
-#ifdef GENGA_BC_TL
-                tc_[it + 1] = clock64() - tc0_; tcv_[it + 1] = lst.valid;
-#endif
                 if (t.owner) {
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
@@ -737,22 +692,13 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
                     }
                 }
             }
-#ifdef GENGA_BC_PROF
-            if (!dropped) { pc_cyc += clock64() - c0_; pc_calls += col + 2; }
-#endif
             if (!dropped) {
                 __syncthreads();                  // the owners' column results are on their way to the checker
                 if (tid == 0) { bc_fence(); SC->ready[col] = seq; }
             }
-#ifdef GENGA_BC_TL
-            if (tid == 0 && rank == GENGA_BC_TLR && n >= 30 && n <= 40 && GENGA_BC_TL == 1) { printf("TC n %d dropped %d H %.3f:", n, (int)dropped, Hl); for (int z = 0; z < 9; ++z) printf(" %lld%c", tc_[z], tcv_[z] ? ' ' : '*'); printf("\n"); }
-#endif
         }
         BC_PROF(1)
         if (!checker) continue;
-#ifdef GENGA_BC_TL
-        tl_[0] = clock64() - tl0_;
-#endif
         // ---- checker of this level: rows 1.. as their columns arrive; first row whose error passes
         int code = under ? 0 : 1;                 // 0 underflow, 1 rejected, 2 + k passed at row k
         double prow[BS_KMAX] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
@@ -768,13 +714,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
                 __syncthreads();
                 if (S.bc[0] == 0) { dropped = true; break; }
                 BC_PROF(2)
-#ifdef GENGA_BC_TL
-                tl_[2 * k] = clock64() - tl0_;
-#endif
                 const double err = n <= THREADS / 8 ? bc_check_row_inc(S, n, k, prow) : bc_check_row(S, n, k);
-#ifdef GENGA_BC_TL
-                tl_[2 * k + 1] = clock64() - tl0_;
-#endif
                 BC_PROF(3)
                 if (err <= eps2) { code = 2 + k; break; }
             }
@@ -786,9 +726,6 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
             continue;
         }
         // ---- master: the first level, in the order H, H/2, .., that passed
-#ifdef GENGA_BC_TL
-        tl_[15] = clock64() - tl0_;
-#endif
         int winner = -1, wrow = 0;
         bool fail = false;
         if (code >= 2) { winner = 0; wrow = code - 2; }
@@ -846,9 +783,6 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
         // component), spread over the block: what a store to another CTA's shared memory costs is the packet, not its size
         // (8-byte stores: 2.9 k cycles for 30 bodies, measured).
         __syncthreads();                          // seq_begin is out (fenced), the master's Y is complete
-#ifdef GENGA_BC_TL
-        tl_[18] = clock64() - tl0_;
-#endif
         if (winner >= 0 && next_state == 0) {
             const int np2 = (n + 1) >> 1;         // pairs of bodies (Y rows are MAXN long, MAXN even: the odd one out copies a spare)
             for (int idx = tid; idx < np2 * NCTA; idx += THREADS) {
@@ -864,18 +798,11 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
             R->rec_H = H; R->rec_state = next_state;
         }
         __syncthreads();
-#ifdef GENGA_BC_TL
-        tl_[19] = clock64() - tl0_;
-#endif
         if (tid < NCTA) { bc_fence(); cluster.map_shared_rank(&S, tid)->seq_end = ns; }
         BC_PROF(4)
-#ifdef GENGA_BC_TL
-        if (tid == 0 && n >= 30 && n <= 40 && GENGA_BC_TL == 2) { tl_[16] = clock64() - tl0_; printf("TL n %d winner %d row %d col0 %lld |", n, winner, wrow, tl_[0]); for (int z = 1; z < 8; ++z) printf(" %lld-%lld", tl_[2 * z], tl_[2 * z + 1]); printf(" | dec %lld copy %lld seqb %lld push %lld pub %lld\n", tl_[15], tl_[17], tl_[18], tl_[19], tl_[16]); }
-#endif
     }
 #ifdef GENGA_BC_PROF
     if (master && tid == 0 && nsteps) { for (int k = 0; k < 5; ++k) nsteps[2 + k] = (int)(pf_acc[k] >> 4); }
-    if (tid == 0 && (rank == 7 || rank == 3 || rank == 0) && pc_calls) printf("col %d n %d calls %d cycles/call %d rebuilds %d list %d\n", rank, n, pc_calls, (int)(pc_cyc / pc_calls), S.dbg_rebuild, S.dbg_total);
 #endif
     return ok;
 }
