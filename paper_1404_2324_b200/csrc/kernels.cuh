@@ -18,7 +18,7 @@ constexpr double KK_WIDE2 = 10.89, KK_GROW = 1.0999;
 
 // Bulirsch-Stoer layouts: groups of 2..8 bodies on one warp (bs_warp.cuh), of 9..256 bodies on a
 // cluster of 8 CTAs (bs_cluster.cuh), larger ones on one block with a global-memory tableau (bs.cuh)
-constexpr int BCB_MAXN = 256, BCB_THREADS = 512, BCB_LV = 2, BCB_CS = 8 * BCB_LV;   // BCB_LV trial step sizes side by side, 8 CTAs each
+constexpr int BCB_MAXN = 256, BCB_THREADS = 256, BCB_LV = 2, BCB_CS = 8 * BCB_LV;   // BCB_LV trial step sizes side by side, 8 CTAs each
 
 __global__ void k_begin_map(DevState d);
 __global__ void k_reset_counters(DevState d);
