@@ -155,7 +155,7 @@ __device__ __forceinline__ void bc_pairs(BcSmem<MAXN, THREADS> &S, const double 
 // ~50): so the owners are the first n threads (few warps convert and integrate, the others only help with the pairs), and
 // nothing on the per-evaluation path is reduced by shuffles.
 //
-// LIST PATH (n <= 32 L and the table fits: the sparse chains of a planetesimal disc).  The n^2 examinations are done in
+// LIST PATH (n <= 64 L and the table fits: the sparse chains of a planetesimal disc).  The n^2 examinations are done in
 // FP32 against a threshold widened by more than the FP32 rounding AND by the skin BC_SKIN rc, L lanes per body; the k-th
 // hit of body i goes to entry (k + 1) npad + i of the table S.part (k from a prefix sum over the body's L lanes: one
 // barrier, no block-wide compaction).  The table is then KEPT: the owners check that no body has moved, after the rigid
@@ -198,7 +198,7 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
     double ax = 0.0, ay = 0.0, az = 0.0, bx = 0.0, by = 0.0, bz = 0.0;
     const int n = t.n, L = t.L, i = t.pi;                         // below, i is the body whose pairs this lane examines
     const bool live = i < n;
-    const bool one_chunk = n <= 32 * L;                           // every partner of a lane fits one mask (uniform)
+    const bool one_chunk = n <= 64 * L;                           // every partner of a lane fits one 64-bit mask (uniform)
     bool summed = false;                                          // the owners already hold their sums
     if (one_chunk) {
         bool listed = false;
@@ -237,7 +237,7 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
         if (!listed) {
             // ---- pretest: bit kk = partner j = s + kk L passed at point A or B.  Four partners per trip, no early exit:
             // their loads and short FP32 chains overlap (one at a time this loop was most of what a new list costs)
-            unsigned mask = 0u;
+            unsigned long long mask = 0ull;
             if (live) {
                 const float4 mA = fA[i], mB = fB[i];
                 const float ft = mA.w;
@@ -255,13 +255,13 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
                         const float d2 = fminf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), fmaf(ez, ez, fmaf(ey, ey, ex * ex)));
                         bits |= (d2 < fmaxf(ft, pa.w) && j != i && j < n) ? 1u << u : 0u;
                     }
-                    mask |= bits << (4 * q4);
+                    mask |= (unsigned long long)bits << (4 * q4);
                 }
             }
             // ---- the k-th hit of body i goes to entry (k + 1) npad + i: k from a prefix sum over the body's L lanes only, so
             // the table is complete after ONE barrier (no block-wide compaction)
             const int lane = threadIdx.x & 31;
-            const int cnt = __popc(mask);
+            const int cnt = __popcll(mask);
             int pre = cnt;
             for (int o = 1; o < L; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o, L); if (t.s >= o) pre += v; }
             const int cseg = __shfl_sync(0xffffffffu, pre, L - 1, L);           // the body's partners
@@ -271,7 +271,7 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
             if (live) {
                 if (t.s == 0) S.cnt[i] = cseg;
                 int slot = (pre - cnt + 1) * npad + i;
-                for (unsigned mm = mask; mm && slot < BC_MAXP; mm &= mm - 1, slot += npad) S.part[slot] = t.s + (__ffs(mm) - 1) * L;
+                for (unsigned long long mm = mask; mm && slot < BC_MAXP; mm &= mm - 1, slot += npad) S.part[slot] = t.s + (__ffsll((long long)mm) - 1) * L;
             }
             __syncthreads();
             const int kmax = S.kmax[sb];
@@ -287,7 +287,7 @@ __device__ __forceinline__ int bc_rhs2(BcSmem<MAXN, THREADS> &S, const BcLane &t
                 const double xA = pA[0][i], yA = pA[1][i], zA = pA[2][i], xB = pB[0][i], yB = pB[1][i], zB = pB[2][i];
                 const double my_rc = S.rc[i], my_irc = S.irc[i];
                 while (mask) {
-                    const int j = t.s + (__ffs(mask) - 1) * L;
+                    const int j = t.s + (__ffsll((long long)mask) - 1) * L;
                     mask &= mask - 1;
                     double rcj = S.rc[j];
                     double rcij = fmax(my_rc, rcj), rc2 = rcij * rcij;
@@ -581,7 +581,7 @@ __device__ __forceinline__ int bc_integrate(BcSmem<MAXN, THREADS> &S, const int 
         // List path of bc_rhs2 (n <= 32 L): the pretest reaches out to (1 + BC_SKIN) rc, and the list is kept while every
         // body stays within skin = BC_SKIN min_i rc_i / 2 of where it was, in the frame of the central body, when the list was made
         // (less 2^-19 Q for the FP32 roundings of that difference): a pair left out cannot have come inside rc_ij.
-        const bool wide = n <= 32 * t.L;
+        const bool wide = n <= 64 * t.L;
         const double rcmin = -bc_block_max(S, t.owner ? -S.rc[i] : -1.0e300);
         if (t.owner) {
             double w = S.rc[i] * (wide ? 1.0 + BC_SKIN : 1.0) + 0x1.0p-20 * Q;
