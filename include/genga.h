@@ -243,6 +243,28 @@ int genga_eval_fast(genga_ctx *ctx, int which, int64_t n, const double *in, doub
  * *tflops (HOST out) = 2 * DFMAs / time.  The ALU-roofline denominator.  Synchronises. */
 int genga_fp64_probe(genga_ctx *ctx, double *tflops);
 
+/* ---- an entry point that allocates nothing (csrc/noalloc.cu) ----
+ * Kick accelerations of operator B for ONE system of n massive bodies, without a context and without a workspace:
+ * a_i = sum_{j != i} G m_j W(r_ij, max(rcrit_i, rcrit_j)) (q_j - q_i) / r_ij^3, W = K - r dK/dr (Eq. 2, Eq. 4-8
+ * L84-104): what genga_accelerations returns in `a` for the same positions, masses and critical radii (to rounding:
+ * the partial sums are added in another order).  For callers that cannot call cudaMalloc (CUDA graph capture, serving
+ * loops, harnesses that forbid it): the kernels' scratch memory (packed body records, partial sums of 16 j slices) is
+ * a file-scope device array of GENGA_NOALLOC_SCRATCH_BYTES that every GPU which loads the library holds until the
+ * process exits; the call makes no cudaMalloc, cudaFree or other allocating call and does not synchronise.
+ *   stream      cudaStream_t (may be 0); three kernels are enqueued on it
+ *   n           0 .. GENGA_NOALLOC_MAX_BODIES; a larger n is rejected with GENGA_EINVAL (genga_noalloc_last_error says why)
+ *   G           > 0
+ *   m, rcrit    DEVICE, n doubles each; x DEVICE, 3 n doubles, component-major (x[c * n + i]); owned by the caller, read only
+ *   a           DEVICE out, 3 n doubles, component-major
+ * All calls on one device SHARE the scratch array, which keeps the last call's contents; a call writes every word it
+ * reads, so nothing needs clearing, but two calls that overlap on the GPU (different streams, concurrent graph
+ * launches) race: serialise them.  Returns GENGA_OK, GENGA_EINVAL (sizes, NULL, G) or GENGA_ECUDA. */
+#define GENGA_NOALLOC_MAX_BODIES 2048
+#define GENGA_NOALLOC_SCRATCH_BYTES 868352
+int genga_kick_accel_noalloc(void *stream, int64_t n, double G, const double *m, const double *x, const double *rcrit, double *a);
+/* The reason of the last GENGA_EINVAL / GENGA_ECUDA of genga_kick_accel_noalloc on this thread ("" if none). */
+const char *genga_noalloc_last_error(void);
+
 const char *genga_strerror(int code);
 const char *genga_last_cuda_error(void);
 

@@ -25,8 +25,10 @@ SYMBOLS = [
     "genga_energy", "genga_encounters", "genga_bs_trace", "genga_set_collisions", "genga_events", "genga_bodies",
     "genga_status", "genga_accelerations", "genga_kepler_drift", "genga_counters", "genga_time_kernel", "genga_profile_step",
     "genga_eval_fast", "genga_fp64_probe", "genga_strerror",
-    "genga_last_cuda_error",
+    "genga_last_cuda_error", "genga_kick_accel_noalloc", "genga_noalloc_last_error",
 ]
+
+NOALLOC_MAX_BODIES = 2048           # GENGA_NOALLOC_MAX_BODIES of include/genga.h
 
 
 class genga_config(C.Structure):
@@ -88,6 +90,8 @@ def load():
         "genga_fp64_probe": (i, [vp, C.POINTER(d)]),
         "genga_strerror": (C.c_char_p, [i]),
         "genga_last_cuda_error": (C.c_char_p, []),
+        "genga_kick_accel_noalloc": (i, [vp, l, d, dp, dp, dp, dp]),
+        "genga_noalloc_last_error": (C.c_char_p, []),
     }
     for name, (res, args) in sig.items():
         f = getattr(L, name)
@@ -320,3 +324,22 @@ def from_workload(w, **kw):
               n2=w["n2"], bs_eps=w["bs_eps"], **kw)
     g.set_state(w["m0"], w["m"], w["radius"], w["x"], w["v"])
     return g
+
+
+def kick_accel_noalloc(G, m, x, rcrit, a, stream=None):
+    """genga_kick_accel_noalloc (include/genga.h): kick accelerations of one system of n <= NOALLOC_MAX_BODIES massive
+    bodies into `a`, no context, no workspace, no allocation (the scratch is a static device array of the library; calls
+    that overlap on the GPU race on it).  m, rcrit: device float64 tensors of n; x, a: device float64 (3, n), contiguous.
+    Enqueues on `stream` (a torch stream; default: the current one) and does not synchronise."""
+    import torch
+    n = int(m.numel())
+    for t, size in ((m, n), (rcrit, n), (x, 3 * n), (a, 3 * n)):
+        if t.dtype != torch.float64 or not t.is_cuda or not t.is_contiguous() or t.numel() != size:
+            raise ValueError("kick_accel_noalloc wants contiguous float64 CUDA tensors of n, n, 3 n and 3 n elements")
+    st = (stream or torch.cuda.current_stream(m.device)).cuda_stream
+    L = load()
+    with torch.cuda.device(m.device):
+        code = L.genga_kick_accel_noalloc(st, n, float(G), m.data_ptr(), x.data_ptr(), rcrit.data_ptr(), a.data_ptr())
+    if code != 0:
+        raise GengaError(code, "genga_kick_accel_noalloc: " + L.genga_noalloc_last_error().decode())
+    return a
