@@ -187,6 +187,17 @@ def test_bulirsch_stoer_layouts_reached_by_large_groups(G, name, make, nsteps, m
     assert min_group <= c["max_group"] <= max_group, c["max_group"]
 
 
+@pytest.mark.parametrize("seed", [2, 5])
+def test_other_seeds_same_parity(G, seed):
+    """The group structure (sizes 2..50 on the cluster and block layouts, 400+ on k_bs_block with n2 = 0.8) changes with the
+    seed of the disc; parity must not."""
+    for w, nwin, win, order in ((workloads.config1(seed=seed), 2, 5, 2),
+                                (dict(workloads.config1(seed=seed), n2=0.8), 1, 3, 2),
+                                (workloads.config4(seed=seed, order=4), 1, 2, 4)):
+        sg, so, E0, c = windowed_parity(G, w, nwin, win, order)
+        assert c["groups"] > 0
+
+
 @pytest.mark.parametrize("order", [2, 4])
 def test_1e4_steps_energy_with_encounters(G, order):
     """north_star: |dE/E| after 10^4 steps within 2x of the oracle's -- on a run WITH encounters (config 4's annulus,
